@@ -1,0 +1,403 @@
+"""Pins for the oracle's lattice arithmetic against what physics / mathematics fix (CPU only).
+
+Each test names the SURVEY.md sec 8(c)-5 row it implements.  None of the expected values comes from the oracle
+or from the CUDA path: they are closed forms, invariants, brute force, or an independent numpy implementation.
+"""
+import numpy as np
+import pytest
+from scipy import integrate, special
+
+import oracle
+from tests import np_lattice as npl
+from tests.inputs import random_links, random_sun
+
+
+def make(dims, N, links=None):
+    L = oracle.OracleLattice(dims, N)
+    if links is not None:
+        L.set_links(links)
+    return L
+
+
+# ----------------------------------------------------------------------------- cold start / closed forms
+@pytest.mark.parametrize("dims,N", [((4, 6), 2), ((4, 4, 2), 3), ((4, 2, 6, 4), 3), ((2, 2, 2, 2), 2)])
+def test_cold_start_observables(dims, N):
+    L = make(dims, N)
+    L.init(oracle.COLD, 1)
+    tot, planes, poly = L.measure()
+    assert tot == 1.0 and np.all(planes == 1.0) and poly == 1.0 + 0j
+    links = L.get_links()
+    assert np.array_equal(links, np.broadcast_to(np.eye(N), links.shape))
+
+
+def test_cold_field_plane_plaquette():
+    # row "Field factor": cold start => field-plane plaquette = (1/N) sum cos(theta_c); SU(2): cos(phi/2); others 1
+    dims = (6, 4, 4, 2)
+    phi = 2 * np.pi * 4 / (6 * 4)
+    L = make(dims, 2)
+    L.init(oracle.COLD, 1)
+    f = oracle.make_field(0, 1, [phi / 2, -phi / 2])
+    tot, planes, _ = L.measure(f)
+    assert abs(planes[0] - np.cos(phi / 2)) < 1e-15 and np.all(planes[1:] == 1.0)
+    assert abs(tot - (np.cos(phi / 2) + 5) / 6) < 1e-15
+    th = [0.3, -0.1, -0.2]
+    L3 = make(dims, 3)
+    L3.init(oracle.COLD, 1)
+    tot, planes, _ = L3.measure(oracle.make_field(1, 3, th))
+    # plane order (0,1),(0,2),(0,3),(1,2),(1,3),(2,3) -> index 4
+    assert abs(planes[4] - np.mean(np.cos(th))) < 1e-15
+    assert np.all(np.delete(planes, 4) == 1.0)
+
+
+# ----------------------------------------------------------------------------- observables vs independent numpy
+@pytest.mark.parametrize("dims,N", [((4, 6), 2), ((4, 2, 6), 3), ((4, 6, 2, 4), 3), ((6, 4, 4, 2), 2)])
+def test_observables_match_numpy_roll_implementation(dims, N):
+    links = random_links(dims, N, seed=11)
+    L = make(dims, N, links)
+    tot, planes, poly = L.measure()
+    ref = npl.plaquettes(links, dims)
+    assert np.max(np.abs(planes - ref)) < 1e-14
+    assert abs(tot - ref.mean()) < 1e-14
+    assert abs(poly - npl.polyakov(links, dims)) < 1e-14
+    # dressed plaquette with a field in plane (0, D-1)
+    D = len(dims)
+    th = [0.7, -0.7] if N == 2 else [0.5, 0.2, -0.7]
+    f = oracle.make_field(0, D - 1, th)
+    _, planes_f, _ = L.measure(f)
+    ref_f = npl.plaquettes(links, dims, field=(0, D - 1, th))
+    assert np.max(np.abs(planes_f - ref_f)) < 1e-14
+    assert abs(planes_f[D - 2] - planes[D - 2]) > 1e-4        # the field does change that plane
+
+
+@pytest.mark.parametrize("dims,N", [((4, 6, 2, 4), 3), ((4, 6, 4), 2)])
+def test_gauge_and_translation_invariance(dims, N):
+    # row "Layout / neighbour indexing / wrap"
+    links = random_links(dims, N, seed=5)
+    L = make(dims, N, links)
+    tot, planes, poly = L.measure()
+    rng = np.random.Generator(np.random.PCG64(77))
+    omega = random_sun(rng, int(np.prod(dims)), N)
+    L.set_links(npl.gauge_transform(links, dims, omega))
+    tot2, planes2, poly2 = L.measure()
+    assert np.max(np.abs(planes2 - planes)) < 1e-13 and abs(poly2 - poly) < 1e-13
+    for mu in range(len(dims)):
+        L.set_links(npl.translate(links, dims, mu))
+        tot3, planes3, poly3 = L.measure()
+        assert np.max(np.abs(planes3 - planes)) < 1e-13 and abs(poly3 - poly) < 1e-13
+
+
+@pytest.mark.parametrize("N", [2, 3])
+def test_polyakov_centre_transformation(N):
+    # row "Polyakov loop": multiply all U_{D-1} on one time slice by the centre element z: plaquette same, L -> z L
+    dims = (4, 4, 2, 6)
+    links = random_links(dims, N, seed=3)
+    L = make(dims, N, links)
+    tot, planes, poly = L.measure()
+    z = np.exp(2j * np.pi / N)
+    g = npl.to_grid(links, dims).copy()
+    g[2, ..., 3, :, :] *= z            # time slice t=2, direction D-1=3
+    L.set_links(npl.from_grid(g, dims))
+    tot2, planes2, poly2 = L.measure()
+    assert np.max(np.abs(planes2 - planes)) < 1e-13
+    assert abs(poly2 - z * poly) < 1e-13
+
+
+# ----------------------------------------------------------------------------- staples: brute force
+def _total_trace_sum(L, field, N):
+    """sum over all plaquettes of Re Tr P (dressed), from the per-plane means"""
+    _, planes, _ = L.measure(field)
+    return float(np.sum(planes)) * L.V * N
+
+
+@pytest.mark.parametrize("dims,N,fld", [
+    ((4, 4, 2), 3, None), ((4, 4, 2), 2, None), ((4, 6), 2, None), ((2, 2, 4, 4), 3, None),
+    ((4, 4, 2), 3, (0, 1, [0.4, 0.3, -0.7])), ((4, 4, 2), 3, (0, 2, [0.4, 0.3, -0.7])), ((4, 4, 2), 3, (1, 2, [0.4, 0.3, -0.7])),
+    ((4, 2, 4, 2), 2, (0, 1, [0.6, -0.6])), ((4, 2, 4, 2), 2, (1, 3, [0.6, -0.6])),
+])
+def test_staples_brute_force(dims, N, fld):
+    # row "Staples": replace one link; Delta(sum_P Re Tr P) == Re Tr[(U' - U) A] for every direction / plane role
+    links = random_links(dims, N, seed=21)
+    field = oracle.make_field(*fld) if fld else None
+    L = make(dims, N, links)
+    base = _total_trace_sum(L, field, N)
+    rng = np.random.Generator(np.random.PCG64(8))
+    V, D = L.V, L.D
+    for mu in range(D):
+        for lex in rng.choice(V, size=3, replace=False):
+            A = L.staple(lex, mu, field)
+            Unew = random_sun(rng, 1, N)[0]
+            mod = links.copy()
+            mod[lex, mu] = Unew
+            L.set_links(mod)
+            delta = _total_trace_sum(L, field, N) - base
+            L.set_links(links)
+            assert abs(delta - np.trace((Unew - links[lex, mu]) @ A).real) < 1e-11, (mu, lex)
+
+
+def test_staple_count_cold():
+    # cold lattice: A = 2(D-1) * identity
+    for dims, N in [((4, 4), 2), ((4, 4, 4), 3), ((4, 4, 2, 2), 3)]:
+        L = make(dims, N)
+        L.init(oracle.COLD, 0)
+        A = L.staple(5, 1)
+        assert np.array_equal(A, 2 * (len(dims) - 1) * np.eye(N))
+
+
+# ----------------------------------------------------------------------------- overrelaxation
+@pytest.mark.parametrize("dims,N,fld", [((4, 4), 2, None), ((4, 4, 4), 3, None), ((4, 2, 4, 2), 3, None),
+                                        ((4, 2, 4, 2), 2, (0, 1, [0.5, -0.5])), ((4, 4, 2), 3, (0, 2, [0.2, 0.5, -0.7]))])
+def test_overrelaxation_conserves_action(dims, N, fld):
+    # row "OR": total action unchanged by OR-only sweeps; links do change; group property kept
+    links = random_links(dims, N, seed=31)
+    field = oracle.make_field(*fld) if fld else None
+    L = make(dims, N, links)
+    tot0, _, _ = L.measure(field)
+    for _ in range(3):
+        L.sweep(2.3, 0, 2, field)
+    tot1, _, _ = L.measure(field)
+    assert abs(tot1 - tot0) < 2e-13
+    new = L.get_links()
+    assert np.max(np.abs(new - links)) > 0.1
+    uni, det = npl.unitarity_defect(new)
+    assert uni < 1e-12 and det < 1e-12
+
+
+def test_su2_overrelaxation_is_involution():
+    dims = (4, 4, 2, 2)
+    links = random_links(dims, 2, seed=41)
+    L = make(dims, 2, links)
+    L.substep(1.0, oracle.KIND_OR, 0, 1, 2)
+    once = L.get_links()
+    assert np.max(np.abs(once - links)) > 0.1
+    L.substep(1.0, oracle.KIND_OR, 0, 1, 2)
+    assert np.max(np.abs(L.get_links() - links)) < 1e-13
+
+
+def test_substep_touches_only_its_links():
+    dims = (4, 4, 4)
+    links = random_links(dims, 3, seed=51)
+    L = make(dims, 3, links)
+    L.set_seed(9)
+    L.substep(5.0, oracle.KIND_HB, 0, 1, 2)
+    new = L.get_links()
+    g_old, g_new = npl.to_grid(links, dims), npl.to_grid(new, dims)
+    z, y, x = np.meshgrid(range(4), range(4), range(4), indexing="ij")
+    par = (x + y + z) & 1
+    changed = np.max(np.abs(g_new - g_old), axis=(-1, -2)) > 0
+    assert np.all(changed[..., 2] == (par == 1))
+    assert not changed[..., 0].any() and not changed[..., 1].any()
+
+
+# ----------------------------------------------------------------------------- Kennedy-Pendleton sampler
+@pytest.mark.parametrize("alpha,mode", [(1.0, 0), (4.0, 0), (10.0, 0), (4.0, 1), (16.0, 1)])
+def test_kennedy_pendleton_density(alpha, mode):
+    # row "KP sampler": chi-square against sqrt(1-x^2) exp(alpha x) and <g0> = I2(alpha)/I1(alpha)
+    n = 200000
+    g0, codes = oracle.kp_samples(alpha, seed=1234 + mode, n=n, max_trials=100, uniform_mode=mode)
+    assert not np.isnan(g0).any() and np.all(codes < 0x80)
+    assert np.all(g0 >= -1.0) and np.all(g0 <= 1.0)
+    dens = lambda x: np.sqrt(1 - x * x) * np.exp(alpha * (x - 1))
+    norm = integrate.quad(dens, -1, 1)[0]
+    edges = np.linspace(-1, 1, 41)
+    # merge sparse bins on the left so every expected count is >= 20
+    expected = np.array([integrate.quad(dens, a, b)[0] for a, b in zip(edges[:-1], edges[1:])]) / norm * n
+    observed = np.histogram(g0, bins=edges)[0].astype(float)
+    while expected[0] < 20:
+        expected = np.concatenate([[expected[0] + expected[1]], expected[2:]])
+        observed = np.concatenate([[observed[0] + observed[1]], observed[2:]])
+    chi2 = np.sum((observed - expected) ** 2 / expected)
+    dof = len(expected) - 1
+    assert chi2 < dof + 5 * np.sqrt(2 * dof), (chi2, dof)
+    exact_mean = special.iv(2, alpha) / special.iv(1, alpha)
+    var = integrate.quad(lambda x: x * x * dens(x), -1, 1)[0] / norm - exact_mean ** 2
+    assert abs(g0.mean() - exact_mean) < 4 * np.sqrt(var / n)
+
+
+def test_kennedy_pendleton_trial_cap_and_acceptance():
+    # acceptance per trial: alpha=1 -> ~0.52, alpha=8 -> ~0.95; exhaustion code when the cap is hit
+    for alpha, acc in [(1.0, 0.52), (8.0, 0.951)]:
+        g0, codes = oracle.kp_samples(alpha, seed=5, n=50000, max_trials=1)
+        frac = np.mean(codes == 1)
+        assert abs(frac - acc) < 0.01
+        assert np.all(codes[np.isnan(g0)] == (0x80 | 1))
+    g0, codes = oracle.kp_samples(1.0, seed=5, n=50000, max_trials=10)
+    assert np.mean(codes >= 0x80) < 5e-3 and codes[codes < 0x80].max() <= 10
+
+
+# ----------------------------------------------------------------------------- hot start
+@pytest.mark.parametrize("N", [2, 3])
+def test_hot_start_haar_moments(N):
+    # row "Hot start": unitarity, det 1, <tr U>=0, <|tr U|^2>=1, <|tr U|^4>=2, SU(3): <(tr U)^3>=1
+    dims = (8, 8, 8, 4)
+    L = make(dims, N)
+    L.init(oracle.HOT, 7)
+    links = L.get_links()
+    uni, det = npl.unitarity_defect(links)
+    assert uni < 1e-14 and det < 1e-14
+    tr = np.trace(links, axis1=-2, axis2=-1).ravel()
+    n = tr.size
+    assert abs(tr.mean()) < 5 / np.sqrt(n)
+    assert abs(np.mean(np.abs(tr) ** 2) - 1.0) < 5 * np.sqrt(1.0 / n)          # var(|tr|^2) = <|tr|^4> - 1 = 1
+    assert abs(np.mean(np.abs(tr) ** 4) - 2.0) < 0.05
+    retr = tr.real / N
+    assert abs(retr.var() - (1 / 4 if N == 2 else 1 / 18)) < 0.01 * (1 / 4 if N == 2 else 1 / 18) * 5
+    if N == 3:
+        assert abs(np.mean(tr ** 3) - 1.0) < 0.05
+    # first-row entries: <|U_00|^2> = 1/N (uniform on the sphere), directions independent
+    assert abs(np.mean(np.abs(links[..., 0, 0]) ** 2) - 1 / N) < 0.005
+    tot, _, poly = L.measure()
+    assert abs(tot) < 5 / np.sqrt(6 * L.V) and abs(poly) < 0.05
+    # different links are different, same (seed) reproduces bit-for-bit, other seed differs
+    L2 = make(dims, N)
+    L2.init(oracle.HOT, 7)
+    assert np.array_equal(L2.get_links(), links)
+    L2.init(oracle.HOT, 8)
+    assert np.max(np.abs(L2.get_links() - links)) > 0.5
+
+
+# ----------------------------------------------------------------------------- whole sampler, exact results
+def _binned_error(x, nbins=10):
+    x = np.asarray(x)
+    b = x[: len(x) // nbins * nbins].reshape(nbins, -1).mean(axis=1)
+    return b.std(ddof=1) / np.sqrt(nbins)
+
+
+def _run_plaquettes(dims, N, beta, seed, sweeps, n_hb, n_or, start, max_trials=10, fp32=False):
+    L = make(dims, N)
+    L.set_max_trials(max_trials)
+    if fp32:
+        L.set_fp32_shadow(True)
+    L.init(start, seed)
+    ps = []
+    for _ in range(sweeps):
+        L.sweep(beta, n_hb, n_or)
+        ps.append(L.measure()[0])
+    return L, np.array(ps)
+
+
+def test_config1_su2_2d_exact_plaquette():
+    # BASELINE.json configs[0]: SU(2) D=2 16x16 beta=2.0 cold 200 x (1 HB + 1 OR), seed 1234: <P> = I2(2)/I1(2)
+    exact = special.iv(2, 2.0) / special.iv(1, 2.0)
+    assert abs(exact - 0.433127426722) < 1e-11
+    L, ps = _run_plaquettes((16, 16), 2, 2.0, 1234, 200, 1, 1, oracle.COLD)
+    meas = ps[20:]
+    sigma_indep = np.sqrt(0.162709 / 256 / len(meas))            # plaquettes are independent in 2-D
+    err = max(_binned_error(meas), sigma_indep)
+    assert abs(meas.mean() - exact) < 3 * err, (meas.mean(), exact, err)
+    uni, det = npl.unitarity_defect(L.get_links())
+    assert uni < 1e-12 and det < 1e-12
+
+
+@pytest.mark.parametrize("max_trials", [1, 100])
+def test_capped_heatbath_is_exact(max_trials):
+    # row "Capped KP is exact": with T_max = 1 the pseudo-heatbath still samples the exact distribution
+    exact = special.iv(2, 2.0) / special.iv(1, 2.0)
+    L, ps = _run_plaquettes((16, 16), 2, 2.0, 4321 + max_trials, 300, 1, 1, oracle.COLD, max_trials=max_trials)
+    meas = ps[40:]
+    err = max(_binned_error(meas), np.sqrt(0.162709 / 256 / len(meas)))
+    assert abs(meas.mean() - exact) < 3.5 * err, (meas.mean(), exact, err)
+
+
+def _su3_weyl_plaquette(beta):
+    """<(1/3) Re tr U> under dU exp((beta/3) Re tr U) on SU(3): 2-D quadrature over the maximal torus (Weyl formula)."""
+    def vand2(a, b):
+        c = -a - b
+        return (np.abs(np.exp(1j * a) - np.exp(1j * b)) * np.abs(np.exp(1j * a) - np.exp(1j * c)) *
+                np.abs(np.exp(1j * b) - np.exp(1j * c))) ** 2
+
+    def retr(a, b):
+        return np.cos(a) + np.cos(b) + np.cos(a + b)
+
+    n = 400
+    t = (np.arange(n) + 0.5) * 2 * np.pi / n           # periodic integrand: midpoint rule is spectrally accurate
+    a, b = np.meshgrid(t, t, indexing="ij")
+    w = vand2(a, b) * np.exp(beta / 3 * retr(a, b))
+    return float(np.sum(w * retr(a, b) / 3) / np.sum(w))
+
+
+def test_su3_weyl_reference_values():
+    # row "Whole sampler, SU(3)" and "Strong coupling": the closed-form integral reproduces the survey's digits
+    assert abs(_su3_weyl_plaquette(1.0) - 0.0601265548) < 1e-9
+    assert abs(_su3_weyl_plaquette(2.0) - 0.1286277853) < 1e-9
+    assert abs(_su3_weyl_plaquette(0.3) - 0.0170829) < 1e-6
+    assert abs(_su3_weyl_plaquette(0.3) - (0.3 / 18 + 0.3 ** 2 / 216)) < 1e-5
+
+
+def test_su3_2d_exact_plaquette():
+    beta = 2.0
+    exact = _su3_weyl_plaquette(beta)
+    L, ps = _run_plaquettes((12, 12), 3, beta, 99, 260, 1, 1, oracle.HOT)
+    meas = ps[30:]
+    err = _binned_error(meas)
+    assert abs(meas.mean() - exact) < 3.5 * err + 1e-4, (meas.mean(), exact, err)
+    uni, det = npl.unitarity_defect(L.get_links())
+    assert uni < 1e-12 and det < 1e-12
+
+
+@pytest.mark.parametrize("N,beta,dims", [(3, 0.3, (4, 4, 4, 4)), (2, 0.2, (4, 4, 4, 4)), (3, 0.5, (4, 4, 4))])
+def test_strong_coupling_plaquette(N, beta, dims):
+    # row "Strong coupling, any D": <P> = single-plaquette value up to O((beta/2N^2)^5)
+    exact = _su3_weyl_plaquette(beta) if N == 3 else special.iv(2, beta) / special.iv(1, beta)
+    L, ps = _run_plaquettes(dims, N, beta, 17, 160, 1, 1, oracle.HOT)
+    meas = ps[10:]
+    err = _binned_error(meas)
+    assert abs(meas.mean() - exact) < 3.5 * err + 2e-4, (meas.mean(), exact, err)
+    assert exact > 5 * err                     # the signal is resolved: a wrong 1/N or beta normalisation would fail
+
+
+def test_group_property_every_sweep_su3_4d():
+    # north_star: unitarity |UU^+ - 1| < 1e-12 and det U = 1 after every sweep (fp64)
+    L = make((4, 4, 4, 2), 3)
+    L.init(oracle.HOT, 3)
+    for _ in range(5):
+        L.sweep(5.7, 1, 4)
+        uni, det = npl.unitarity_defect(L.get_links())
+        assert uni < 1e-12 and det < 1e-12
+
+
+# ----------------------------------------------------------------------------- bookkeeping
+def test_resume_is_bit_identical():
+    # row "Resume": 2k sweeps == k sweeps + get/set links + set counter + k sweeps
+    dims, N, beta = (4, 4, 2, 2), 3, 5.5
+    A = make(dims, N)
+    A.init(oracle.HOT, 11)
+    for _ in range(4):
+        A.sweep(beta, 1, 2)
+    B = make(dims, N)
+    B.init(oracle.HOT, 11)
+    for _ in range(2):
+        B.sweep(beta, 1, 2)
+    C2 = make(dims, N, B.get_links())
+    C2.set_seed(11)
+    C2.sweep_counter = B.sweep_counter
+    for _ in range(2):
+        C2.sweep(beta, 1, 2)
+    assert np.array_equal(A.get_links(), C2.get_links())
+    # and without restoring the counter the stream differs
+    D2 = make(dims, N, B.get_links())
+    D2.set_seed(11)
+    for _ in range(2):
+        D2.sweep(beta, 1, 2)
+    assert not np.array_equal(A.get_links(), D2.get_links())
+
+
+def test_fp32_shadow_mode_rounds_storage():
+    L = make((4, 4, 4, 2), 3)
+    L.set_fp32_shadow(True)
+    L.init(oracle.HOT, 3)
+    L.sweep(5.7, 1, 1)
+    links = L.get_links()
+    assert np.array_equal(links, links.astype(np.complex64).astype(np.complex128))
+    uni, det = npl.unitarity_defect(links)
+    assert uni < 5e-7 and det < 5e-7
+
+
+def test_single_link_update_matches_substep():
+    dims, N = (4, 4, 4, 2), 3
+    links = random_links(dims, N, seed=61)
+    L = make(dims, N, links)
+    L.set_seed(77)
+    one, codes = L.update_one_link(5.7, oracle.KIND_HB, 0, lex=9, mu=1)      # lex 9 = (1,2,0,0): parity 1
+    trials = L.substep(5.7, oracle.KIND_HB, 0, 1, 1, want_trials=True)
+    assert np.array_equal(L.get_links()[9, 1], one)
+    assert np.array_equal(trials[9], codes) and np.all(codes >= 1)
