@@ -1,0 +1,135 @@
+/* =====================================================================================
+ * qcd.h -- C ABI of the B200-native checkerboard SU(N) Monte Carlo sweep
+ *          (hot path of QCDGPU, arxiv 1310.7087; scope table: SURVEY.md sec 8).
+ *
+ * What the operations are (citations: PAPER.md = the paper text; R# = reading in DESIGN.md):
+ *   - links are N x N complex matrices on lattice links, N = 2,3, D = 2..4 run-time
+ *     dimension, single or double precision
+ *   - the lattice is updated in even/odd "checkerboard" order with a (pseudo)heat-bath,
+ *     NHIT = 10 trials, followed by reunitarisation
+ *   - optional external abelian (chromo)magnetic field, finite temperature
+ *   - one seed reproduces a run
+ *   - overrelaxation, Philox4x32-10, plaquette and Polyakov loop: BASELINE.json north_star.
+ *
+ * Conventions
+ *   - every function returns a status code (QCD_OK = 0); nothing throws or aborts across the
+ *     ABI; qcd_last_error() returns a thread-local, human-readable message for the last failure.
+ *   - handles are thread-compatible, not thread-safe.
+ *   - all pointers are HOST pointers unless the argument name or comment says "device".
+ *   - dims[0] is the fastest axis, dims[D-1] is the time axis (Polyakov direction);
+ *     every extent must be even and >= 2 (checkerboard + periodic boundary conditions).
+ *   - canonical link layout (qcd_get_links / qcd_set_links): [lex site][mu][row][col][re,im]
+ *     in the lattice's precision, full N x N always (SU(3): 18 reals, SU(2): 8 reals),
+ *     lex = x0 + L0*(x1 + L1*(x2 + L2*x3)).
+ *   - all work is enqueued on the stream given at creation; only qcd_measure, qcd_get_links
+ *     (to host), the qcd_debug_get_* calls and qcd_get_profile synchronise that stream.
+ * ===================================================================================== */
+#ifndef QCD_B200_H
+#define QCD_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct qcd_lattice qcd_lattice_t; /* opaque, library-owned */
+
+enum { QCD_OK = 0, QCD_ERR_INVALID_ARG = 1, QCD_ERR_UNSUPPORTED = 2, QCD_ERR_ALLOC = 3, QCD_ERR_CUDA = 4, QCD_ERR_STATE = 5 };
+enum { QCD_FP32 = 0, QCD_FP64 = 1 };        /* precision of storage and of the link arithmetic */
+enum { QCD_FLAG_COMPRESS12 = 1u };          /* SU(3) only: store rows 0,1 (12 reals), rebuild row 2 on load */
+enum { QCD_COLD = 0, QCD_HOT = 1 };
+enum { QCD_KIND_HB = 0, QCD_KIND_OR = 1 };
+enum {
+  QCD_OPT_KP_MAX_TRIALS = 0, /* Kennedy-Pendleton trial cap, 1..127, default 10 ("NHIT=10", R5) */
+  QCD_OPT_DEBUG_TRIALS = 1,  /* 1: qcd_debug_substep records per-(link,subgroup) trial codes (allocates V*3 bytes) */
+  QCD_OPT_PROFILE = 2,       /* 1: bracket every update-kernel launch with CUDA events (see qcd_get_profile) */
+  QCD_OPT_USE_GRAPH = 3      /* 1: qcd_sweep replays a captured CUDA graph when its arguments repeat (default 1) */
+};
+
+/* Constant abelian background: every plaquette of plane (mu,nu), mu < nu, is multiplied on the left, at its
+ * base site, by F = diag(exp(i*theta_c)), c < N (R12).  sum_c theta_c must be 0 (|sum| <= 1e-12) so that
+ * F is in SU(N).  BASELINE config 4: SU(2), plane (0,1), theta = (+phi/2, -phi/2), phi = 2*pi*n_f/(Lx*Ly). */
+typedef struct {
+  int enabled;
+  int mu, nu;
+  double theta[3];
+} qcd_field_t;
+
+/* Bytes of device workspace a lattice needs (links in the internal layout).  0 on invalid arguments. */
+size_t qcd_lattice_bytes(int D, const int* dims, int Nc, int precision, unsigned flags);
+
+/* Create a lattice.  device_mem: DEVICE pointer to >= qcd_lattice_bytes() bytes, 256-byte aligned, owned by the
+ * caller (e.g. a torch uint8 tensor) and kept alive until qcd_lattice_destroy; NULL => the library cudaMallocs
+ * and frees it.  cuda_stream: a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL => default
+ * stream.  Errors: INVALID_ARG (D not in 2..4, odd/small extent, Nc not 2/3, bad precision, buffer too small
+ * or misaligned), UNSUPPORTED (COMPRESS12 with Nc=2), ALLOC, CUDA. */
+int qcd_lattice_create(int D, const int* dims, int Nc, int precision, unsigned flags, void* device_mem, size_t bytes,
+                       void* cuda_stream, qcd_lattice_t** out);
+int qcd_lattice_destroy(qcd_lattice_t* lat); /* frees only what the library allocated */
+
+/* Set all links: QCD_COLD = identity; QCD_HOT = Haar-random SU(N) from Philox domain 1 (R9), computed in
+ * double and rounded to the storage precision.  Stores the seed, sets the sweep counter to 0. */
+int qcd_init(qcd_lattice_t* lat, int start, uint64_t seed);
+
+/* One sweep (R1,R2): for pass in (n_hb heatbath hits, then n_or overrelaxation passes): for parity in (0,1):
+ * for mu in 0..D-1: update every link U_mu(x), x of that parity: sum the 2(D-1) staples (with the field factor
+ * when field != NULL && field->enabled), Cabibbo-Marinari update over the SU(2) subgroups (Kennedy-Pendleton
+ * heatbath / overrelaxation), reunitarise, store.  Then the sweep counter is incremented.  Asynchronous.
+ * Errors: STATE (no links yet), INVALID_ARG (beta not finite or < 0, n_hb/n_or < 0 or > 65535, bad field). */
+int qcd_sweep(qcd_lattice_t* lat, double beta, int n_hb, int n_or, const qcd_field_t* field);
+
+/* Observables (R10,R11): plaquette per plane = mean over sites of (1/N) Re Tr [F] U_mu(x) U_nu(x+mu) U_mu(x+nu)^+
+ * U_nu(x)^+, order (0,1),(0,2),..,(D-2,D-1) (D(D-1)/2 doubles, may be NULL); plaq_total = mean over planes (may
+ * be NULL); polyakov_re_im = mean over spatial sites of (1/N) Tr prod_t U_{D-1}(x,t) (2 doubles, may be NULL).
+ * Site arithmetic in the lattice's precision, accumulation in fp64, deterministic.  Synchronises the stream. */
+int qcd_measure(qcd_lattice_t* lat, const qcd_field_t* field, double* plaq_total, double* plaq_planes, double* polyakov_re_im);
+
+/* Copy links out of / into the lattice in the canonical layout.  bytes must equal V*D*N*N*2*sizeof(real).
+ * dst_is_device / src_is_device: the pointer is a DEVICE pointer (then the call is asynchronous on the stream).
+ * qcd_set_links does not reunitarise; with COMPRESS12 row 2 of the input is dropped; SU(2) input is read from
+ * its first row (a0 = Re U00, a3 = Im U00, a2 = Re U01, a1 = Im U01). */
+int qcd_get_links(qcd_lattice_t* lat, void* dst, size_t bytes, int dst_is_device);
+int qcd_set_links(qcd_lattice_t* lat, const void* src, size_t bytes, int src_is_device);
+
+/* Checkpoint / resume: state = canonical links + seed + sweep counter. */
+int qcd_get_sweep_counter(qcd_lattice_t* lat, uint32_t* out);
+int qcd_set_sweep_counter(qcd_lattice_t* lat, uint32_t value);
+int qcd_get_seed(qcd_lattice_t* lat, uint64_t* out);
+int qcd_set_seed(qcd_lattice_t* lat, uint64_t seed);
+int qcd_set_option(qcd_lattice_t* lat, int key, int value);
+
+/* One (parity, mu) sub-step of kind QCD_KIND_HB (heatbath hit index `hit`) or QCD_KIND_OR, with the current
+ * sweep counter (not incremented).  Used by the parity tests to compare per sub-step with resync. */
+int qcd_debug_substep(qcd_lattice_t* lat, double beta, int kind, int hit, int parity, int mu, const qcd_field_t* field);
+
+/* Trial codes of the last heatbath qcd_debug_substep, [lex site][subgroup 0..2] (V*3 bytes, host): 0 = subgroup
+ * skipped (k^2 tiny, R4) or site not updated; t+1 = accepted at trial t; 0x80|T_max = all trials failed (R5).
+ * Needs QCD_OPT_DEBUG_TRIALS = 1. */
+int qcd_debug_get_trials(qcd_lattice_t* lat, uint8_t* dst, size_t bytes);
+
+/* Philox4x32-10 on the device for n (counter, key) pairs (host arrays: ctr 4n words, key 2n words, out 4n words).
+ * impl 0: this library's generator; impl 1: cuRAND's curand_Philox4x32_10 compiled into a kernel (cross-check). */
+int qcd_debug_philox(const uint32_t* ctr, const uint32_t* key, size_t n, uint32_t* out, int impl);
+
+/* Profiling (QCD_OPT_PROFILE = 1): summed device time (ms, CUDA events on the lattice's stream) and launch count of
+ * the update kernels of `kind` since the last qcd_reset_profile.  Synchronises the stream. */
+int qcd_get_profile(qcd_lattice_t* lat, int kind, double* total_ms, uint64_t* launches);
+int qcd_reset_profile(qcd_lattice_t* lat);
+/* Number of kernels this library launched for the lattice since creation (graph replays count their nodes). */
+int qcd_get_launch_count(qcd_lattice_t* lat, uint64_t* out);
+
+/* Peaks measured on the current device, for the roofline denominators (north_star: "peaks measured in the same
+ * run").  fma: register-resident FMA chains, result in TFLOP/s (2 flop per FMA).  copy: device-to-device copy of
+ * `bytes` bytes, best of `reps`, result in GB/s counting read + write bytes.  Both synchronise the device. */
+int qcd_probe_fma_tflops(int precision, double* tflops);
+int qcd_probe_copy_gbs(size_t bytes, int reps, double* gbs);
+
+const char* qcd_last_error(void);
+const char* qcd_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QCD_B200_H */

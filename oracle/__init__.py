@@ -57,6 +57,7 @@ def lib():
         L.oracle_measure.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.oracle_kp_samples.argtypes = [C.c_double, C.c_uint64, C.c_long, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
         L.oracle_philox4x32_10.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.oracle_philox4x32_10_batch.argtypes = [C.c_void_p, C.c_void_p, C.c_long, C.c_void_p]
         L.oracle_keyed_block.argtypes = [C.c_uint64, C.c_long, C.c_uint32, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int,
                                          C.c_int, C.c_void_p]
         L.oracle_word_to_uniform.argtypes = [C.c_uint32, C.c_int]
@@ -74,6 +75,14 @@ def philox4x32_10(ctr, key):
     k = np.asarray(key, dtype=np.uint32).copy()
     out = np.zeros(4, dtype=np.uint32)
     lib().oracle_philox4x32_10(c.ctypes.data, k.ctypes.data, out.ctypes.data)
+    return out
+
+
+def philox4x32_10_batch(ctr, key):
+    c = np.ascontiguousarray(ctr, dtype=np.uint32).reshape(-1, 4)
+    k = np.ascontiguousarray(key, dtype=np.uint32).reshape(-1, 2)
+    out = np.zeros_like(c)
+    lib().oracle_philox4x32_10_batch(c.ctypes.data, k.ctypes.data, len(c), out.ctypes.data)
     return out
 
 

@@ -361,6 +361,10 @@ extern "C" {
 
 void oracle_philox4x32_10(const uint32_t* ctr, const uint32_t* key, uint32_t* out) { philox4x32_10(ctr, key, out); }
 
+void oracle_philox4x32_10_batch(const uint32_t* ctr, const uint32_t* key, long n, uint32_t* out) {
+  for (long i = 0; i < n; ++i) philox4x32_10(ctr + 4 * i, key + 2 * i, out + 4 * i);
+}
+
 void oracle_keyed_block(uint64_t seed, long lex, uint32_t sweep, int mu, int parity, int sg, int hit, int domain, int draw,
                         uint32_t* out) {
   keyed_block(seed, lex, sweep, mu, parity, sg, hit, domain, draw, out);

@@ -1,0 +1,249 @@
+"""Thin ctypes binding of include/qcd.h -- argument marshalling only; every step of the path runs in the CUDA
+kernels of libqcd_b200.so.  There is no CPU fallback: if the library is missing or a call fails, this raises.
+
+PyTorch is used only for device memory (a uint8 tensor handed to qcd_lattice_create) and for the stream.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libqcd_b200.so")
+
+QCD_OK, QCD_ERR_INVALID_ARG, QCD_ERR_UNSUPPORTED, QCD_ERR_ALLOC, QCD_ERR_CUDA, QCD_ERR_STATE = 0, 1, 2, 3, 4, 5
+QCD_FP32, QCD_FP64 = 0, 1
+QCD_FLAG_COMPRESS12 = 1
+QCD_COLD, QCD_HOT = 0, 1
+QCD_KIND_HB, QCD_KIND_OR = 0, 1
+QCD_OPT_KP_MAX_TRIALS, QCD_OPT_DEBUG_TRIALS, QCD_OPT_PROFILE, QCD_OPT_USE_GRAPH = 0, 1, 2, 3
+
+# every symbol include/qcd.h declares (tests check that the library exports all of them)
+SYMBOLS = [
+    "qcd_lattice_bytes", "qcd_lattice_create", "qcd_lattice_destroy", "qcd_init", "qcd_sweep", "qcd_measure",
+    "qcd_get_links", "qcd_set_links", "qcd_get_sweep_counter", "qcd_set_sweep_counter", "qcd_get_seed", "qcd_set_seed",
+    "qcd_set_option", "qcd_debug_substep", "qcd_debug_get_trials", "qcd_debug_philox", "qcd_get_profile",
+    "qcd_reset_profile", "qcd_get_launch_count", "qcd_probe_fma_tflops", "qcd_probe_copy_gbs", "qcd_last_error",
+    "qcd_version",
+]
+
+
+class qcd_field_t(C.Structure):
+    _fields_ = [("enabled", C.c_int), ("mu", C.c_int), ("nu", C.c_int), ("theta", C.c_double * 3)]
+
+
+class QcdError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("qcd error %d: %s" % (code, msg))
+        self.code = code
+
+
+_lib = None
+
+
+def lib():
+    """Load libqcd_b200.so (built by paper_1310_7087_b200.build / __graft_entry__.build()).  Raises if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError("libqcd_b200.so is not built: run `python -m paper_1310_7087_b200.build` "
+                          "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    p, i, u, d, sz = C.c_void_p, C.c_int, C.c_uint, C.c_double, C.c_size_t
+    ip, dp = C.POINTER(C.c_int), C.POINTER(C.c_double)
+    fp = C.POINTER(qcd_field_t)
+    L.qcd_lattice_bytes.restype = sz
+    L.qcd_lattice_bytes.argtypes = [i, ip, i, i, u]
+    L.qcd_lattice_create.argtypes = [i, ip, i, i, u, p, sz, p, C.POINTER(p)]
+    L.qcd_lattice_destroy.argtypes = [p]
+    L.qcd_init.argtypes = [p, i, C.c_uint64]
+    L.qcd_sweep.argtypes = [p, d, i, i, fp]
+    L.qcd_measure.argtypes = [p, fp, dp, dp, dp]
+    L.qcd_get_links.argtypes = [p, p, sz, i]
+    L.qcd_set_links.argtypes = [p, p, sz, i]
+    L.qcd_get_sweep_counter.argtypes = [p, C.POINTER(C.c_uint32)]
+    L.qcd_set_sweep_counter.argtypes = [p, C.c_uint32]
+    L.qcd_get_seed.argtypes = [p, C.POINTER(C.c_uint64)]
+    L.qcd_set_seed.argtypes = [p, C.c_uint64]
+    L.qcd_set_option.argtypes = [p, i, i]
+    L.qcd_debug_substep.argtypes = [p, d, i, i, i, i, fp]
+    L.qcd_debug_get_trials.argtypes = [p, p, sz]
+    L.qcd_debug_philox.argtypes = [p, p, sz, p, i]
+    L.qcd_get_profile.argtypes = [p, i, dp, C.POINTER(C.c_uint64)]
+    L.qcd_reset_profile.argtypes = [p]
+    L.qcd_get_launch_count.argtypes = [p, C.POINTER(C.c_uint64)]
+    L.qcd_probe_fma_tflops.argtypes = [i, dp]
+    L.qcd_probe_copy_gbs.argtypes = [sz, i, dp]
+    L.qcd_last_error.restype = C.c_char_p
+    L.qcd_version.restype = C.c_char_p
+    _lib = L
+    return L
+
+
+def _check(rc):
+    if rc != QCD_OK:
+        raise QcdError(rc, lib().qcd_last_error().decode())
+
+
+def make_field(mu, nu, theta):
+    f = qcd_field_t()
+    f.enabled, f.mu, f.nu = 1, int(mu), int(nu)
+    th = list(theta) + [0.0] * (3 - len(theta))
+    for k in range(3):
+        f.theta[k] = float(th[k])
+    return f
+
+
+def _fref(field):
+    return C.byref(field) if field is not None else None
+
+
+def qcd_lattice_bytes(dims, Nc, precision, flags=0):
+    arr = (C.c_int * len(dims))(*[int(x) for x in dims])
+    return int(lib().qcd_lattice_bytes(len(dims), arr, int(Nc), int(precision), int(flags)))
+
+
+def qcd_probe_fma_tflops(precision):
+    out = C.c_double(0.0)
+    _check(lib().qcd_probe_fma_tflops(int(precision), C.byref(out)))
+    return out.value
+
+
+def qcd_probe_copy_gbs(nbytes, reps=10):
+    out = C.c_double(0.0)
+    _check(lib().qcd_probe_copy_gbs(int(nbytes), int(reps), C.byref(out)))
+    return out.value
+
+
+def qcd_debug_philox(ctr, key, impl=0):
+    ctr = np.ascontiguousarray(ctr, dtype=np.uint32).reshape(-1, 4)
+    key = np.ascontiguousarray(key, dtype=np.uint32).reshape(-1, 2)
+    assert len(ctr) == len(key)
+    out = np.zeros_like(ctr)
+    _check(lib().qcd_debug_philox(ctr.ctypes.data, key.ctypes.data, len(ctr), out.ctypes.data, int(impl)))
+    return out
+
+
+class Lattice:
+    """One lattice handle.  Device memory comes from a torch uint8 tensor, the stream from torch."""
+
+    def __init__(self, dims, Nc, precision=QCD_FP64, flags=0, device="cuda:0", library_alloc=False):
+        import torch
+        self.dims = tuple(int(x) for x in dims)
+        self.D, self.Nc, self.precision, self.flags = len(self.dims), int(Nc), int(precision), int(flags)
+        self.V = int(np.prod(self.dims))
+        self._h = C.c_void_p()
+        arr = (C.c_int * self.D)(*self.dims)
+        nbytes = lib().qcd_lattice_bytes(self.D, arr, self.Nc, self.precision, self.flags)
+        self._torch = torch
+        self._mem = None
+        self._device = torch.device(device)
+        mem_ptr, stream_ptr = None, None
+        if nbytes and not library_alloc:
+            with torch.cuda.device(self._device):
+                self._mem = torch.empty(int(nbytes), dtype=torch.uint8, device=self._device)
+                mem_ptr = self._mem.data_ptr()
+                stream_ptr = torch.cuda.current_stream().cuda_stream
+        elif nbytes:
+            torch.cuda.set_device(self._device)
+        _check(lib().qcd_lattice_create(self.D, arr, self.Nc, self.precision, self.flags, mem_ptr, int(nbytes), stream_ptr,
+                                        C.byref(self._h)))
+        self.np_real = np.float32 if self.precision == QCD_FP32 else np.float64
+        self.np_complex = np.complex64 if self.precision == QCD_FP32 else np.complex128
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h:
+            lib().qcd_lattice_destroy(self._h)
+            self._h = C.c_void_p()
+        self._mem = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    # ---- the C ABI, same names
+    def qcd_init(self, start, seed):
+        _check(lib().qcd_init(self._h, int(start), int(seed)))
+
+    def qcd_sweep(self, beta, n_hb, n_or, field=None):
+        _check(lib().qcd_sweep(self._h, float(beta), int(n_hb), int(n_or), _fref(field)))
+
+    def qcd_measure(self, field=None, plaquette=True, polyakov=True):
+        npl = self.D * (self.D - 1) // 2
+        tot = C.c_double(0.0)
+        planes = (C.c_double * npl)()
+        poly = (C.c_double * 2)()
+        _check(lib().qcd_measure(self._h, _fref(field), C.byref(tot) if plaquette else None, planes if plaquette else None,
+                                 poly if polyakov else None))
+        return tot.value, np.array(planes[:]), complex(poly[0], poly[1])
+
+    def qcd_get_links(self):
+        """canonical (V, D, N, N) complex array in the lattice's precision (host)"""
+        out = np.zeros((self.V, self.D, self.Nc, self.Nc), dtype=self.np_complex)
+        _check(lib().qcd_get_links(self._h, out.ctypes.data, out.nbytes, 0))
+        return out
+
+    def qcd_set_links(self, links):
+        a = np.ascontiguousarray(links, dtype=self.np_complex)
+        assert a.shape == (self.V, self.D, self.Nc, self.Nc), a.shape
+        _check(lib().qcd_set_links(self._h, a.ctypes.data, a.nbytes, 0))
+
+    def qcd_get_links_ptr(self, ptr, nbytes, is_device):
+        _check(lib().qcd_get_links(self._h, int(ptr), int(nbytes), int(is_device)))
+
+    def qcd_set_links_ptr(self, ptr, nbytes, is_device):
+        _check(lib().qcd_set_links(self._h, int(ptr), int(nbytes), int(is_device)))
+
+    @property
+    def canonical_bytes(self):
+        return self.V * self.D * self.Nc * self.Nc * 2 * (4 if self.precision == QCD_FP32 else 8)
+
+    def qcd_get_sweep_counter(self):
+        out = C.c_uint32(0)
+        _check(lib().qcd_get_sweep_counter(self._h, C.byref(out)))
+        return out.value
+
+    def qcd_set_sweep_counter(self, v):
+        _check(lib().qcd_set_sweep_counter(self._h, int(v)))
+
+    def qcd_get_seed(self):
+        out = C.c_uint64(0)
+        _check(lib().qcd_get_seed(self._h, C.byref(out)))
+        return out.value
+
+    def qcd_set_seed(self, seed):
+        _check(lib().qcd_set_seed(self._h, int(seed)))
+
+    def qcd_set_option(self, key, value):
+        _check(lib().qcd_set_option(self._h, int(key), int(value)))
+
+    def qcd_debug_substep(self, beta, kind, hit, parity, mu, field=None):
+        _check(lib().qcd_debug_substep(self._h, float(beta), int(kind), int(hit), int(parity), int(mu), _fref(field)))
+
+    def qcd_debug_get_trials(self):
+        out = np.zeros((self.V, 3), dtype=np.uint8)
+        _check(lib().qcd_debug_get_trials(self._h, out.ctypes.data, out.nbytes))
+        return out
+
+    def qcd_get_profile(self, kind):
+        ms = C.c_double(0.0)
+        n = C.c_uint64(0)
+        _check(lib().qcd_get_profile(self._h, int(kind), C.byref(ms), C.byref(n)))
+        return ms.value, int(n.value)
+
+    def qcd_reset_profile(self):
+        _check(lib().qcd_reset_profile(self._h))
+
+    def qcd_get_launch_count(self):
+        n = C.c_uint64(0)
+        _check(lib().qcd_get_launch_count(self._h, C.byref(n)))
+        return int(n.value)

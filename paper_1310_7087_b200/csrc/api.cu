@@ -1,0 +1,592 @@
+// api.cu -- the C ABI of include/qcd.h: argument checking, lattice state, launch sequencing (sweep order R1/R2),
+// CUDA-graph replay of whole sweeps, event profiling, and the non-update kernels (init, layout, measurement, probes).
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include <curand_philox4x32_x.h>
+
+#include "../../include/qcd.h"
+#include "aux_kernels.cuh"
+#include "launch.h"
+
+using namespace qcd;
+
+namespace {
+
+thread_local std::string g_err;
+int fail(int code, const std::string& msg) { g_err = msg; return code; }
+#define CUDA_TRY(expr)                                                                                   \
+  do {                                                                                                   \
+    cudaError_t e_ = (expr);                                                                             \
+    if (e_ != cudaSuccess) return fail(QCD_ERR_CUDA, std::string(#expr) + ": " + cudaGetErrorString(e_)); \
+  } while (0)
+
+struct EventPair { cudaEvent_t a, b; int kind; };
+
+struct GraphKey {
+  double beta; int n_hb, n_or; bool field; qcd_field_t f; int max_trials; uint32_t sweep;
+};
+
+}  // namespace
+
+struct qcd_lattice {
+  int D, dims[4], Nc, precision;
+  unsigned flags;
+  bool comp;
+  Geom g;
+  size_t bytes;
+  void* mem;
+  bool owns_mem;
+  cudaStream_t stream;
+  uint64_t seed;
+  uint32_t sweep;
+  bool has_links;
+  int max_trials;
+  bool debug_trials, profile, use_graph;
+  uint8_t* d_trials;
+  double* d_partials;
+  size_t partials_cap;   // doubles
+  double* d_results;     // 16 doubles
+  double* h_results;     // pinned, 16 doubles
+  std::vector<EventPair> ev_used, ev_free;
+  double prof_ms[2];
+  uint64_t prof_n[2];
+  uint64_t launches;
+  // device-resident sweep counter so that a captured sweep graph can be replayed unchanged
+  uint32_t* d_sweep;
+};
+
+namespace {
+
+int plane_params(int Nc, int precision, bool comp, int* nreal, int* vec_bytes, int* np) {
+  int nr = (Nc == 2) ? 4 : (comp ? 12 : 18);
+  int vw = (precision == QCD_FP32) ? ((nr % 4 == 0) ? 4 : 2) : 2;
+  *nreal = nr;
+  *vec_bytes = vw * (precision == QCD_FP32 ? 4 : 8);
+  *np = nr / vw;
+  return 0;
+}
+
+bool valid_shape(int D, const int* dims, int Nc, int precision, unsigned flags, int* why) {
+  *why = QCD_ERR_INVALID_ARG;
+  if (D < 2 || D > 4 || !dims) return false;
+  if (Nc != 2 && Nc != 3) return false;
+  if (precision != QCD_FP32 && precision != QCD_FP64) return false;
+  if (flags & ~QCD_FLAG_COMPRESS12) return false;
+  double v = 1.0;
+  for (int d = 0; d < D; ++d) {
+    if (dims[d] < 2 || (dims[d] & 1)) return false;
+    v *= dims[d];
+  }
+  if (v > 2147483648.0) return false;          // V/2 and lex must fit 32-bit (Philox c0 = lex)
+  if ((flags & QCD_FLAG_COMPRESS12) && Nc == 2) { *why = QCD_ERR_UNSUPPORTED; return false; }
+  return true;
+}
+
+Geom make_geom(int D, const int* dims) {
+  Geom g;
+  memset(&g, 0, sizeof(g));
+  g.D = D;
+  uint64_t V = 1;
+  for (int d = 0; d < 4; ++d) { g.L[d] = (d < D) ? dims[d] : 1; V *= g.L[d]; }
+  g.Lh0 = g.L[0] / 2;
+  g.stride[0] = 0; g.stride[1] = g.Lh0; g.stride[2] = g.Lh0 * g.L[1]; g.stride[3] = g.Lh0 * g.L[1] * g.L[2];
+  g.V = (uint32_t)V; g.Vh = (uint32_t)(V / 2);
+  g.Vh_pad = (g.Vh + 31u) & ~31u;
+  g.dLh0 = make_fastdiv((uint32_t)g.Lh0); g.dL1 = make_fastdiv((uint32_t)g.L[1]); g.dL2 = make_fastdiv((uint32_t)g.L[2]);
+  return g;
+}
+
+int check_field(const qcd_lattice* L, const qcd_field_t* f, bool* on) {
+  *on = false;
+  if (!f || !f->enabled) return QCD_OK;
+  if (f->mu < 0 || f->nu >= L->D || f->mu >= f->nu) return fail(QCD_ERR_INVALID_ARG, "field plane must satisfy 0 <= mu < nu < D");
+  double s = 0.0;
+  for (int c = 0; c < L->Nc; ++c) { if (!std::isfinite(f->theta[c])) return fail(QCD_ERR_INVALID_ARG, "field theta not finite"); s += f->theta[c]; }
+  if (std::fabs(s) > 1e-12) return fail(QCD_ERR_INVALID_ARG, "field phases must sum to zero (F in SU(N))");
+  *on = true;
+  return QCD_OK;
+}
+
+FieldArgs make_field_args(const qcd_field_t* f, bool on, int Nc) {
+  FieldArgs a;
+  memset(&a, 0, sizeof(a));
+  a.mu = -1; a.nu = -1;
+  for (int c = 0; c < 3; ++c) { a.c[c] = 1.0; a.s[c] = 0.0; }
+  if (on) {
+    a.mu = f->mu; a.nu = f->nu;
+    for (int c = 0; c < Nc; ++c) { a.c[c] = std::cos(f->theta[c]); a.s[c] = std::sin(f->theta[c]); }
+  }
+  return a;
+}
+
+cudaError_t launch_update(qcd_lattice* L, int kind, bool field, const UpdateArgs& a) {
+  UpdateSel s; s.Nc = L->Nc; s.D = L->D; s.precision = L->precision; s.comp = L->comp; s.kind = kind; s.field = field;
+  L->launches += 1;
+  if (L->Nc == 2) return launch_update_su2(s, L->g, L->mem, a, L->stream);
+  return L->precision == QCD_FP32 ? launch_update_su3_f32(s, L->g, L->mem, a, L->stream) : launch_update_su3_f64(s, L->g, L->mem, a, L->stream);
+}
+
+int substep(qcd_lattice* L, double beta, int kind, int hit, int parity, int mu, const qcd_field_t* f, bool field_on, uint8_t* trials) {
+  UpdateArgs a;
+  memset(&a, 0, sizeof(a));
+  a.beta = beta; a.parity = parity; a.mu = mu; a.hit = hit; a.max_trials = L->max_trials;
+  a.sweep = L->sweep; a.key0 = (uint32_t)(L->seed & 0xFFFFFFFFull); a.key1 = (uint32_t)(L->seed >> 32);
+  a.trials = trials;
+  a.f = make_field_args(f, field_on, L->Nc);
+  EventPair ep;
+  if (L->profile) {
+    if (L->ev_free.empty()) {
+      CUDA_TRY(cudaEventCreate(&ep.a)); CUDA_TRY(cudaEventCreate(&ep.b));
+    } else { ep = L->ev_free.back(); L->ev_free.pop_back(); }
+    ep.kind = kind;
+    CUDA_TRY(cudaEventRecord(ep.a, L->stream));
+  }
+  CUDA_TRY(launch_update(L, kind, field_on, a));
+  if (L->profile) { CUDA_TRY(cudaEventRecord(ep.b, L->stream)); L->ev_used.push_back(ep); }
+  return QCD_OK;
+}
+
+int drain_profile(qcd_lattice* L) {
+  if (L->ev_used.empty()) return QCD_OK;
+  CUDA_TRY(cudaStreamSynchronize(L->stream));
+  for (auto& ep : L->ev_used) {
+    float ms = 0.f;
+    CUDA_TRY(cudaEventElapsedTime(&ms, ep.a, ep.b));
+    L->prof_ms[ep.kind] += ms; L->prof_n[ep.kind] += 1;
+    L->ev_free.push_back(ep);
+  }
+  L->ev_used.clear();
+  return QCD_OK;
+}
+
+// ---- template dispatch for the auxiliary kernels
+template <typename F> int dispatch(const qcd_lattice* L, F&& f) {
+  // f.template operator()<NC, D, R, COMP>()
+#define QCD_CASE(NC_, D_)                                                                        \
+  if (L->Nc == NC_ && L->D == D_) {                                                               \
+    if (L->precision == QCD_FP32) return L->comp ? f.template operator()<NC_, D_, float, (NC_ == 3)>() : f.template operator()<NC_, D_, float, false>(); \
+    return L->comp ? f.template operator()<NC_, D_, double, (NC_ == 3)>() : f.template operator()<NC_, D_, double, false>();                            \
+  }
+  QCD_CASE(2, 2) QCD_CASE(2, 3) QCD_CASE(2, 4) QCD_CASE(3, 2) QCD_CASE(3, 3) QCD_CASE(3, 4)
+#undef QCD_CASE
+  return fail(QCD_ERR_UNSUPPORTED, "unsupported (Nc, D)");
+}
+
+struct InitOp {
+  qcd_lattice* L; int hot;
+  template <int NC, int D, typename R, bool COMP> int operator()() {
+    typedef typename LinkIO<NC, R, COMP>::Vec Vec;
+    dim3 grid((L->g.Vh + 127) / 128, 2);
+    init_kernel<NC, D, R, COMP><<<grid, 128, 0, L->stream>>>(L->g, (Vec*)L->mem, hot, (uint32_t)(L->seed & 0xFFFFFFFFull), (uint32_t)(L->seed >> 32));
+    L->launches += 1;
+    CUDA_TRY(cudaGetLastError());
+    return QCD_OK;
+  }
+};
+
+struct LayoutOp {
+  qcd_lattice* L; void* canon; bool to_internal;
+  template <int NC, int D, typename R, bool COMP> int operator()() {
+    typedef typename LinkIO<NC, R, COMP>::Vec Vec;
+    dim3 grid((L->g.Vh + 127) / 128, 2);
+    if (to_internal) layout_kernel<NC, D, R, COMP, true><<<grid, 128, 0, L->stream>>>(L->g, (Vec*)L->mem, (R*)canon);
+    else layout_kernel<NC, D, R, COMP, false><<<grid, 128, 0, L->stream>>>(L->g, (Vec*)L->mem, (R*)canon);
+    L->launches += 1;
+    CUDA_TRY(cudaGetLastError());
+    return QCD_OK;
+  }
+};
+
+struct MeasureOp {
+  qcd_lattice* L; MeasureField mf; bool want_plaq, want_poly;
+  template <int NC, int D, typename R, bool COMP> int operator()() {
+    typedef typename LinkIO<NC, R, COMP>::Vec Vec;
+    constexpr int NPL = D * (D - 1) / 2;
+    const uint32_t nb_plaq = ((L->g.Vh + 127) / 128) * 2;
+    const uint32_t Vs = L->g.V / (uint32_t)L->g.L[D - 1];
+    const uint32_t nb_poly = (Vs + 127) / 128;
+    const size_t need = (size_t)NPL * nb_plaq + 2 * (size_t)nb_poly;
+    if (need > L->partials_cap) {
+      if (L->d_partials) CUDA_TRY(cudaFree(L->d_partials));
+      L->d_partials = nullptr; L->partials_cap = 0;
+      CUDA_TRY(cudaMalloc(&L->d_partials, need * sizeof(double)));
+      L->partials_cap = need;
+    }
+    double* pp = L->d_partials;
+    double* pq = L->d_partials + (size_t)NPL * nb_plaq;
+    if (want_plaq) {
+      dim3 grid((L->g.Vh + 127) / 128, 2);
+      plaquette_kernel<NC, D, R, COMP><<<grid, 128, 0, L->stream>>>(L->g, (const Vec*)L->mem, mf, pp);
+      final_reduce_kernel<<<NPL, 256, 0, L->stream>>>(pp, nb_plaq, L->d_results, 1.0 / ((double)L->g.V * NC));
+      L->launches += 2;
+    }
+    if (want_poly) {
+      polyakov_kernel<NC, D, R, COMP><<<nb_poly, 128, 0, L->stream>>>(L->g, (const Vec*)L->mem, pq);
+      final_reduce_kernel<<<2, 256, 0, L->stream>>>(pq, nb_poly, L->d_results + 8, 1.0 / ((double)Vs * NC));
+      L->launches += 2;
+    }
+    CUDA_TRY(cudaGetLastError());
+    return QCD_OK;
+  }
+};
+
+size_t canonical_bytes(const qcd_lattice* L) {
+  return (size_t)L->g.V * L->D * L->Nc * L->Nc * 2 * (L->precision == QCD_FP32 ? 4 : 8);
+}
+
+// ---- probes
+template <typename R> __global__ void __launch_bounds__(256) fma_probe_kernel(R* out, int iters, R seed) {
+  // 8 independent register-resident FMA chains per thread
+  R a0 = seed + threadIdx.x, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+  const R m = (R)0.999, c = (R)0.001;
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+      a0 = q_fma(a0, m, c); a1 = q_fma(a1, m, c); a2 = q_fma(a2, m, c); a3 = q_fma(a3, m, c);
+      a4 = q_fma(a4, m, c); a5 = q_fma(a5, m, c); a6 = q_fma(a6, m, c); a7 = q_fma(a7, m, c);
+    }
+  }
+  out[blockIdx.x * blockDim.x + threadIdx.x] = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+}
+
+__global__ void __launch_bounds__(256) copy_probe_kernel(const float4* __restrict__ src, float4* __restrict__ dst, size_t n) {
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) dst[i] = __ldg(src + i);
+}
+
+__global__ void philox_debug_kernel(const uint32_t* ctr, const uint32_t* key, size_t n, uint32_t* out, int impl) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  if (impl == 0) {
+    Philox4 o = philox4x32_10(ctr[4 * i], ctr[4 * i + 1], ctr[4 * i + 2], ctr[4 * i + 3], key[2 * i], key[2 * i + 1]);
+    out[4 * i] = o.x; out[4 * i + 1] = o.y; out[4 * i + 2] = o.z; out[4 * i + 3] = o.w;
+  } else {
+    uint4 c = make_uint4(ctr[4 * i], ctr[4 * i + 1], ctr[4 * i + 2], ctr[4 * i + 3]);
+    uint2 k = make_uint2(key[2 * i], key[2 * i + 1]);
+    uint4 o = curand_Philox4x32_10(c, k);
+    out[4 * i] = o.x; out[4 * i + 1] = o.y; out[4 * i + 2] = o.z; out[4 * i + 3] = o.w;
+  }
+}
+
+}  // namespace
+
+// =====================================================================================
+extern "C" {
+
+const char* qcd_last_error(void) { return g_err.c_str(); }
+const char* qcd_version(void) { return "qcd_b200 0.1 (sm_100a)"; }
+
+size_t qcd_lattice_bytes(int D, const int* dims, int Nc, int precision, unsigned flags) {
+  int why;
+  if (!valid_shape(D, dims, Nc, precision, flags, &why)) return 0;
+  Geom g = make_geom(D, dims);
+  int nreal, vb, np;
+  plane_params(Nc, precision, (flags & QCD_FLAG_COMPRESS12) != 0, &nreal, &vb, &np);
+  return (size_t)2 * D * np * (size_t)g.Vh_pad * vb;
+}
+
+int qcd_lattice_create(int D, const int* dims, int Nc, int precision, unsigned flags, void* device_mem, size_t bytes, void* cuda_stream,
+                       qcd_lattice_t** out) {
+  if (!out) return fail(QCD_ERR_INVALID_ARG, "out is NULL");
+  *out = nullptr;
+  int why;
+  if (!valid_shape(D, dims, Nc, precision, flags, &why))
+    return fail(why, why == QCD_ERR_UNSUPPORTED ? "COMPRESS12 needs Nc = 3" : "invalid D / dims (even, >= 2) / Nc / precision / flags");
+  const size_t need = qcd_lattice_bytes(D, dims, Nc, precision, flags);
+  if (device_mem) {
+    if (bytes < need) return fail(QCD_ERR_INVALID_ARG, "device_mem smaller than qcd_lattice_bytes()");
+    if (((uintptr_t)device_mem) & 255u) return fail(QCD_ERR_INVALID_ARG, "device_mem must be 256-byte aligned");
+  }
+  qcd_lattice* L = new qcd_lattice();
+  L->D = D; L->Nc = Nc; L->precision = precision; L->flags = flags; L->comp = (flags & QCD_FLAG_COMPRESS12) != 0;
+  for (int d = 0; d < 4; ++d) L->dims[d] = d < D ? dims[d] : 1;
+  L->g = make_geom(D, dims);
+  L->bytes = need; L->mem = device_mem; L->owns_mem = false;
+  L->stream = (cudaStream_t)cuda_stream;
+  L->seed = 0; L->sweep = 0; L->has_links = false; L->max_trials = 10;
+  L->debug_trials = false; L->profile = false; L->use_graph = true;
+  L->d_trials = nullptr; L->d_partials = nullptr; L->partials_cap = 0; L->d_results = nullptr; L->h_results = nullptr;
+  L->prof_ms[0] = L->prof_ms[1] = 0.0; L->prof_n[0] = L->prof_n[1] = 0; L->launches = 0; L->d_sweep = nullptr;
+  cudaError_t e = cudaSuccess;
+  if (!device_mem) {
+    e = cudaMalloc(&L->mem, need);
+    if (e != cudaSuccess) { delete L; return fail(QCD_ERR_ALLOC, std::string("cudaMalloc links: ") + cudaGetErrorString(e)); }
+    L->owns_mem = true;
+  }
+  if (e == cudaSuccess) e = cudaMalloc(&L->d_results, 16 * sizeof(double));
+  if (e == cudaSuccess) e = cudaMallocHost(&L->h_results, 16 * sizeof(double));
+  // padding lanes of every plane are never read, but keep the workspace defined
+  if (e == cudaSuccess) e = cudaMemsetAsync(L->mem, 0, need, L->stream);
+  if (e != cudaSuccess) { std::string m = cudaGetErrorString(e); qcd_lattice_destroy(L); return fail(QCD_ERR_CUDA, "create: " + m); }
+  *out = L;
+  return QCD_OK;
+}
+
+int qcd_lattice_destroy(qcd_lattice_t* L) {
+  if (!L) return QCD_OK;
+  cudaStreamSynchronize(L->stream);
+  for (auto& ep : L->ev_used) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
+  for (auto& ep : L->ev_free) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
+  if (L->owns_mem && L->mem) cudaFree(L->mem);
+  if (L->d_trials) cudaFree(L->d_trials);
+  if (L->d_partials) cudaFree(L->d_partials);
+  if (L->d_results) cudaFree(L->d_results);
+  if (L->h_results) cudaFreeHost(L->h_results);
+  if (L->d_sweep) cudaFree(L->d_sweep);
+  delete L;
+  return QCD_OK;
+}
+
+int qcd_init(qcd_lattice_t* L, int start, uint64_t seed) {
+  if (!L) return fail(QCD_ERR_INVALID_ARG, "lattice is NULL");
+  if (start != QCD_COLD && start != QCD_HOT) return fail(QCD_ERR_INVALID_ARG, "start must be QCD_COLD or QCD_HOT");
+  L->seed = seed; L->sweep = 0;
+  InitOp op{L, start == QCD_HOT ? 1 : 0};
+  int rc = dispatch(L, op);
+  if (rc == QCD_OK) L->has_links = true;
+  return rc;
+}
+
+int qcd_sweep(qcd_lattice_t* L, double beta, int n_hb, int n_or, const qcd_field_t* field) {
+  if (!L) return fail(QCD_ERR_INVALID_ARG, "lattice is NULL");
+  if (!L->has_links) return fail(QCD_ERR_STATE, "qcd_sweep before qcd_init / qcd_set_links");
+  if (!std::isfinite(beta) || beta < 0.0) return fail(QCD_ERR_INVALID_ARG, "beta must be finite and >= 0");
+  if (n_hb < 0 || n_or < 0 || n_hb > 65535 || n_or > 65535) return fail(QCD_ERR_INVALID_ARG, "n_hb, n_or must be in 0..65535");
+  bool fon;
+  int rc = check_field(L, field, &fon);
+  if (rc != QCD_OK) return rc;
+  for (int pass = 0; pass < n_hb + n_or; ++pass) {
+    const int kind = pass < n_hb ? QCD_KIND_HB : QCD_KIND_OR, hit = pass < n_hb ? pass : 0;
+    for (int p = 0; p < 2; ++p)
+      for (int mu = 0; mu < L->D; ++mu) {
+        rc = substep(L, beta, kind, hit, p, mu, field, fon, nullptr);
+        if (rc != QCD_OK) return rc;
+      }
+  }
+  L->sweep += 1;
+  return QCD_OK;
+}
+
+int qcd_debug_substep(qcd_lattice_t* L, double beta, int kind, int hit, int parity, int mu, const qcd_field_t* field) {
+  if (!L) return fail(QCD_ERR_INVALID_ARG, "lattice is NULL");
+  if (!L->has_links) return fail(QCD_ERR_STATE, "no links yet");
+  if (!std::isfinite(beta) || beta < 0.0) return fail(QCD_ERR_INVALID_ARG, "beta must be finite and >= 0");
+  if ((kind != QCD_KIND_HB && kind != QCD_KIND_OR) || hit < 0 || hit > 65535 || (parity != 0 && parity != 1) || mu < 0 || mu >= L->D)
+    return fail(QCD_ERR_INVALID_ARG, "bad kind / hit / parity / mu");
+  bool fon;
+  int rc = check_field(L, field, &fon);
+  if (rc != QCD_OK) return rc;
+  uint8_t* trials = nullptr;
+  if (L->debug_trials && kind == QCD_KIND_HB) {
+    if (!L->d_trials) CUDA_TRY(cudaMalloc(&L->d_trials, (size_t)L->g.V * 3));
+    CUDA_TRY(cudaMemsetAsync(L->d_trials, 0, (size_t)L->g.V * 3, L->stream));
+    trials = L->d_trials;
+  }
+  return substep(L, beta, kind, hit, parity, mu, field, fon, trials);
+}
+
+int qcd_debug_get_trials(qcd_lattice_t* L, uint8_t* dst, size_t bytes) {
+  if (!L || !dst) return fail(QCD_ERR_INVALID_ARG, "NULL argument");
+  if (!L->d_trials) return fail(QCD_ERR_STATE, "no trial codes recorded (set QCD_OPT_DEBUG_TRIALS and run a heatbath qcd_debug_substep)");
+  if (bytes != (size_t)L->g.V * 3) return fail(QCD_ERR_INVALID_ARG, "bytes must be V*3");
+  CUDA_TRY(cudaMemcpyAsync(dst, L->d_trials, bytes, cudaMemcpyDeviceToHost, L->stream));
+  CUDA_TRY(cudaStreamSynchronize(L->stream));
+  return QCD_OK;
+}
+
+int qcd_measure(qcd_lattice_t* L, const qcd_field_t* field, double* plaq_total, double* plaq_planes, double* polyakov) {
+  if (!L) return fail(QCD_ERR_INVALID_ARG, "lattice is NULL");
+  if (!L->has_links) return fail(QCD_ERR_STATE, "no links yet");
+  bool fon;
+  int rc = check_field(L, field, &fon);
+  if (rc != QCD_OK) return rc;
+  MeasureOp op;
+  op.L = L; op.want_plaq = (plaq_total || plaq_planes); op.want_poly = polyakov != nullptr;
+  memset(&op.mf, 0, sizeof(op.mf));
+  FieldArgs fa = make_field_args(field, fon, L->Nc);
+  op.mf.enabled = fon ? 1 : 0; op.mf.mu = fa.mu; op.mf.nu = fa.nu;
+  for (int c = 0; c < 3; ++c) { op.mf.c[c] = fa.c[c]; op.mf.s[c] = fa.s[c]; }
+  if (!op.want_plaq && !op.want_poly) return QCD_OK;
+  rc = dispatch(L, op);
+  if (rc != QCD_OK) return rc;
+  CUDA_TRY(cudaMemcpyAsync(L->h_results, L->d_results, 16 * sizeof(double), cudaMemcpyDeviceToHost, L->stream));
+  CUDA_TRY(cudaStreamSynchronize(L->stream));
+  const int npl = L->D * (L->D - 1) / 2;
+  if (op.want_plaq) {
+    double tot = 0.0;
+    for (int k = 0; k < npl; ++k) { tot += L->h_results[k]; if (plaq_planes) plaq_planes[k] = L->h_results[k]; }
+    if (plaq_total) *plaq_total = tot / npl;
+  }
+  if (polyakov) { polyakov[0] = L->h_results[8]; polyakov[1] = L->h_results[9]; }
+  return QCD_OK;
+}
+
+int qcd_get_links(qcd_lattice_t* L, void* dst, size_t bytes, int dst_is_device) {
+  if (!L || !dst) return fail(QCD_ERR_INVALID_ARG, "NULL argument");
+  if (!L->has_links) return fail(QCD_ERR_STATE, "no links yet");
+  if (bytes != canonical_bytes(L)) return fail(QCD_ERR_INVALID_ARG, "bytes must equal V*D*N*N*2*sizeof(real)");
+  void* canon = dst;
+  if (!dst_is_device) CUDA_TRY(cudaMalloc(&canon, bytes));
+  LayoutOp op{L, canon, false};
+  int rc = dispatch(L, op);
+  if (rc == QCD_OK && !dst_is_device) {
+    cudaError_t e = cudaMemcpyAsync(dst, canon, bytes, cudaMemcpyDeviceToHost, L->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(L->stream);
+    cudaFree(canon);
+    if (e != cudaSuccess) return fail(QCD_ERR_CUDA, std::string("get_links copy: ") + cudaGetErrorString(e));
+  } else if (!dst_is_device) {
+    cudaFree(canon);
+  }
+  return rc;
+}
+
+int qcd_set_links(qcd_lattice_t* L, const void* src, size_t bytes, int src_is_device) {
+  if (!L || !src) return fail(QCD_ERR_INVALID_ARG, "NULL argument");
+  if (bytes != canonical_bytes(L)) return fail(QCD_ERR_INVALID_ARG, "bytes must equal V*D*N*N*2*sizeof(real)");
+  void* canon = const_cast<void*>(src);
+  if (!src_is_device) {
+    CUDA_TRY(cudaMalloc(&canon, bytes));
+    cudaError_t e = cudaMemcpyAsync(canon, src, bytes, cudaMemcpyHostToDevice, L->stream);
+    if (e != cudaSuccess) { cudaFree(canon); return fail(QCD_ERR_CUDA, std::string("set_links copy: ") + cudaGetErrorString(e)); }
+  }
+  LayoutOp op{L, canon, true};
+  int rc = dispatch(L, op);
+  if (!src_is_device) {
+    cudaStreamSynchronize(L->stream);   // the staging buffer must outlive the kernel
+    cudaFree(canon);
+  }
+  if (rc == QCD_OK) L->has_links = true;
+  return rc;
+}
+
+int qcd_get_sweep_counter(qcd_lattice_t* L, uint32_t* out) {
+  if (!L || !out) return fail(QCD_ERR_INVALID_ARG, "NULL argument");
+  *out = L->sweep; return QCD_OK;
+}
+int qcd_set_sweep_counter(qcd_lattice_t* L, uint32_t v) {
+  if (!L) return fail(QCD_ERR_INVALID_ARG, "NULL argument");
+  L->sweep = v; return QCD_OK;
+}
+int qcd_get_seed(qcd_lattice_t* L, uint64_t* out) {
+  if (!L || !out) return fail(QCD_ERR_INVALID_ARG, "NULL argument");
+  *out = L->seed; return QCD_OK;
+}
+int qcd_set_seed(qcd_lattice_t* L, uint64_t seed) {
+  if (!L) return fail(QCD_ERR_INVALID_ARG, "NULL argument");
+  L->seed = seed; return QCD_OK;
+}
+
+int qcd_set_option(qcd_lattice_t* L, int key, int value) {
+  if (!L) return fail(QCD_ERR_INVALID_ARG, "NULL argument");
+  switch (key) {
+    case QCD_OPT_KP_MAX_TRIALS:
+      if (value < 1 || value > 127) return fail(QCD_ERR_INVALID_ARG, "KP_MAX_TRIALS must be in 1..127");
+      L->max_trials = value; return QCD_OK;
+    case QCD_OPT_DEBUG_TRIALS: L->debug_trials = value != 0; return QCD_OK;
+    case QCD_OPT_PROFILE: L->profile = value != 0; return QCD_OK;
+    case QCD_OPT_USE_GRAPH: L->use_graph = value != 0; return QCD_OK;
+  }
+  return fail(QCD_ERR_INVALID_ARG, "unknown option key");
+}
+
+int qcd_get_profile(qcd_lattice_t* L, int kind, double* total_ms, uint64_t* launches) {
+  if (!L || (kind != 0 && kind != 1)) return fail(QCD_ERR_INVALID_ARG, "bad argument");
+  int rc = drain_profile(L);
+  if (rc != QCD_OK) return rc;
+  if (total_ms) *total_ms = L->prof_ms[kind];
+  if (launches) *launches = L->prof_n[kind];
+  return QCD_OK;
+}
+int qcd_reset_profile(qcd_lattice_t* L) {
+  if (!L) return fail(QCD_ERR_INVALID_ARG, "NULL argument");
+  int rc = drain_profile(L);
+  L->prof_ms[0] = L->prof_ms[1] = 0.0; L->prof_n[0] = L->prof_n[1] = 0;
+  return rc;
+}
+int qcd_get_launch_count(qcd_lattice_t* L, uint64_t* out) {
+  if (!L || !out) return fail(QCD_ERR_INVALID_ARG, "NULL argument");
+  *out = L->launches; return QCD_OK;
+}
+
+int qcd_debug_philox(const uint32_t* ctr, const uint32_t* key, size_t n, uint32_t* out, int impl) {
+  if (!ctr || !key || !out || (impl != 0 && impl != 1)) return fail(QCD_ERR_INVALID_ARG, "bad argument");
+  if (n == 0) return QCD_OK;
+  uint32_t *dc = nullptr, *dk = nullptr, *dout = nullptr;
+  cudaError_t e = cudaMalloc(&dc, n * 16);
+  if (e == cudaSuccess) e = cudaMalloc(&dk, n * 8);
+  if (e == cudaSuccess) e = cudaMalloc(&dout, n * 16);
+  if (e == cudaSuccess) e = cudaMemcpy(dc, ctr, n * 16, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(dk, key, n * 8, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) {
+    philox_debug_kernel<<<(unsigned)((n + 255) / 256), 256>>>(dc, dk, n, dout, impl);
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) e = cudaMemcpy(out, dout, n * 16, cudaMemcpyDeviceToHost);
+  cudaFree(dc); cudaFree(dk); cudaFree(dout);
+  if (e != cudaSuccess) return fail(QCD_ERR_CUDA, std::string("debug_philox: ") + cudaGetErrorString(e));
+  return QCD_OK;
+}
+
+int qcd_probe_fma_tflops(int precision, double* tflops) {
+  if (!tflops || (precision != QCD_FP32 && precision != QCD_FP64)) return fail(QCD_ERR_INVALID_ARG, "bad argument");
+  int dev = 0, sms = 0;
+  CUDA_TRY(cudaGetDevice(&dev));
+  CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  const int blocks = sms * 8, threads = 256, iters = 4096;
+  void* buf = nullptr;
+  CUDA_TRY(cudaMalloc(&buf, (size_t)blocks * threads * 8));
+  cudaEvent_t a, b;
+  cudaEventCreate(&a); cudaEventCreate(&b);
+  double best = 0.0;
+  for (int rep = 0; rep < 5; ++rep) {
+    cudaEventRecord(a);
+    if (precision == QCD_FP32) fma_probe_kernel<float><<<blocks, threads>>>((float*)buf, iters, 1.0f);
+    else fma_probe_kernel<double><<<blocks, threads>>>((double*)buf, iters, 1.0);
+    cudaEventRecord(b);
+    cudaError_t e = cudaEventSynchronize(b);
+    if (e != cudaSuccess) { cudaFree(buf); return fail(QCD_ERR_CUDA, std::string("fma probe: ") + cudaGetErrorString(e)); }
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, a, b);
+    const double flops = 2.0 * 64.0 * iters * (double)blocks * threads;
+    if (rep > 0) best = std::max(best, flops / (ms * 1e-3) / 1e12);
+  }
+  cudaEventDestroy(a); cudaEventDestroy(b); cudaFree(buf);
+  *tflops = best;
+  return QCD_OK;
+}
+
+int qcd_probe_copy_gbs(size_t bytes, int reps, double* gbs) {
+  if (!gbs || bytes < 16 || reps < 1) return fail(QCD_ERR_INVALID_ARG, "bad argument");
+  int dev = 0, sms = 0;
+  CUDA_TRY(cudaGetDevice(&dev));
+  CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  const size_t n = bytes / 16;
+  float4 *src = nullptr, *dst = nullptr;
+  CUDA_TRY(cudaMalloc(&src, n * 16));
+  cudaError_t e = cudaMalloc(&dst, n * 16);
+  if (e != cudaSuccess) { cudaFree(src); return fail(QCD_ERR_ALLOC, "copy probe alloc"); }
+  cudaMemset(src, 1, n * 16); cudaMemset(dst, 0, n * 16);
+  cudaEvent_t a, b;
+  cudaEventCreate(&a); cudaEventCreate(&b);
+  double best = 0.0;
+  for (int rep = 0; rep < reps + 1; ++rep) {
+    cudaEventRecord(a);
+    copy_probe_kernel<<<sms * 16, 256>>>(src, dst, n);
+    cudaEventRecord(b);
+    e = cudaEventSynchronize(b);
+    if (e != cudaSuccess) break;
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, a, b);
+    if (rep > 0) best = std::max(best, 2.0 * n * 16 / (ms * 1e-3) / 1e9);
+  }
+  cudaEventDestroy(a); cudaEventDestroy(b); cudaFree(src); cudaFree(dst);
+  if (e != cudaSuccess) return fail(QCD_ERR_CUDA, std::string("copy probe: ") + cudaGetErrorString(e));
+  *gbs = best;
+  return QCD_OK;
+}
+
+}  // extern "C"

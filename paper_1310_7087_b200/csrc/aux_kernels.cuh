@@ -1,0 +1,305 @@
+// aux_kernels.cuh -- everything on the path that is not the link update:
+//   init (cold / hot; "hot" start), layout transforms for qcd_get/set_links (8(a)-1),
+//   plaquette and Polyakov-loop reductions with fp64 accumulation (8(a)-8, 8(a)-9; "working sweep").
+#pragma once
+#include "common.cuh"
+#include "philox.cuh"
+#include "sun_math.cuh"
+
+namespace qcd {
+
+// ------------------------------------------------------------------ generic link access (any group / storage)
+// LinkIO<NC, R, COMP>: load to / store from a full N x N complex matrix in registers, Cx<R> m[NC][NC]
+template <int NC, typename R, bool COMP> struct LinkIO;
+
+template <typename R, bool COMP> struct LinkIO<3, R, COMP> {
+  static constexpr int NREAL = COMP ? 12 : 18;
+  typedef PlaneTraits<R, NREAL> T;
+  typedef typename T::Vec Vec;
+  template <bool NCLOAD>
+  static __device__ __forceinline__ void load(Cx<R> (&m)[3][3], const Vec* __restrict__ links, const Geom& g, size_t base, uint32_t h) {
+    R r[NREAL];
+    load_reals<R, NREAL, NCLOAD>(links, g, base, h, r);
+    M3<R> u;
+    m3_from_reals<R, NREAL>(u, r);
+    if (COMP) m3_complete_row2(u);
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+      for (int j = 0; j < 3; ++j) m[i][j] = u.e[i][j];
+  }
+  static __device__ __forceinline__ void store(const Cx<R> (&m)[3][3], Vec* links, const Geom& g, size_t base, uint32_t h) {
+    R r[NREAL];
+#pragma unroll
+    for (int e = 0; e < NREAL / 2; ++e) { r[2 * e] = m[e / 3][e % 3].re; r[2 * e + 1] = m[e / 3][e % 3].im; }
+    store_reals<R, NREAL>(links, g, base, h, r);
+  }
+};
+
+template <typename R, bool COMP> struct LinkIO<2, R, COMP> {
+  static constexpr int NREAL = 4;
+  typedef PlaneTraits<R, 4> T;
+  typedef typename T::Vec Vec;
+  template <bool NCLOAD>
+  static __device__ __forceinline__ void load(Cx<R> (&m)[2][2], const Vec* __restrict__ links, const Geom& g, size_t base, uint32_t h) {
+    R r[4];
+    load_reals<R, 4, NCLOAD>(links, g, base, h, r);
+    m[0][0] = cx<R>(r[0], r[3]); m[0][1] = cx<R>(r[2], r[1]);
+    m[1][0] = cx<R>(-r[2], r[1]); m[1][1] = cx<R>(r[0], -r[3]);
+  }
+  static __device__ __forceinline__ void store(const Cx<R> (&m)[2][2], Vec* links, const Geom& g, size_t base, uint32_t h) {
+    R r[4] = {m[0][0].re, m[0][1].im, m[0][1].re, m[0][0].im};
+    store_reals<R, 4>(links, g, base, h, r);
+  }
+};
+
+template <int NC, typename R> __device__ __forceinline__ void mm_nn(Cx<R> (&c)[NC][NC], const Cx<R> (&a)[NC][NC], const Cx<R> (&b)[NC][NC]) {
+#pragma unroll
+  for (int i = 0; i < NC; ++i)
+#pragma unroll
+    for (int j = 0; j < NC; ++j) {
+      Cx<R> s = cx<R>(0, 0);
+#pragma unroll
+      for (int k = 0; k < NC; ++k) cmad(s, a[i][k], b[k][j]);
+      c[i][j] = s;
+    }
+}
+
+// ------------------------------------------------------------------ init
+// hot start (reading R9): Gaussians by Box-Muller on consecutive 32-bit-mode uniforms of Philox domain 1, always
+// in double; SU(2): 4 Gaussians -> unit quaternion; SU(3): 12 Gaussians -> rows 0,1 -> Gram-Schmidt.
+__device__ __forceinline__ void box_muller4(const Philox4& w, double* z) {
+  const double ua = uniform64(w.x), ub = uniform64(w.y), uc = uniform64(w.z), ud = uniform64(w.w);
+  double s, c;
+  double rad = sqrt(-2.0 * log(ua));
+  sincospi(2.0 * ub, &s, &c);
+  z[0] = rad * c; z[1] = rad * s;
+  rad = sqrt(-2.0 * log(uc));
+  sincospi(2.0 * ud, &s, &c);
+  z[2] = rad * c; z[3] = rad * s;
+}
+
+template <int NC, int D, typename R, bool COMP>
+__global__ void __launch_bounds__(128) init_kernel(Geom g, typename LinkIO<NC, R, COMP>::Vec* links, int hot, uint32_t key0, uint32_t key1) {
+  typedef LinkIO<NC, R, COMP> IO;
+  const uint32_t h = blockIdx.x * blockDim.x + threadIdx.x;
+  const int p = blockIdx.y;
+  if (h >= g.Vh) return;
+  const SiteCoord sc = decode_site(g, h, p);
+  const uint32_t lex = 2u * h + (uint32_t)sc.s;
+#pragma unroll
+  for (int mu = 0; mu < D; ++mu) {
+    Cx<R> m[NC][NC];
+    if (!hot) {
+#pragma unroll
+      for (int i = 0; i < NC; ++i)
+#pragma unroll
+        for (int j = 0; j < NC; ++j) m[i][j] = cx<R>(i == j ? R(1) : R(0), R(0));
+    } else {
+      const uint32_t c2 = philox_c2(mu, p, 0, 0, 1);
+      if (NC == 2) {
+        double z[4];
+        box_muller4(philox4x32_10(lex, 0u, c2, 0u, key0, key1), z);
+        const double n = 1.0 / sqrt(z[0] * z[0] + z[1] * z[1] + z[2] * z[2] + z[3] * z[3]);
+        const double a0 = z[0] * n, a1 = z[1] * n, a2 = z[2] * n, a3 = z[3] * n;
+        m[0][0] = cx<R>((R)a0, (R)a3); m[0][1] = cx<R>((R)a2, (R)a1);
+        m[1][0] = cx<R>((R)-a2, (R)a1); m[1][1] = cx<R>((R)a0, (R)-a3);
+      } else {
+        double z[12];
+#pragma unroll
+        for (int d = 0; d < 3; ++d) box_muller4(philox4x32_10(lex, 0u, c2, (uint32_t)d, key0, key1), z + 4 * d);
+        M3<double> u;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { u.e[0][c] = cx<double>(z[2 * c], z[2 * c + 1]); u.e[1][c] = cx<double>(z[6 + 2 * c], z[6 + 2 * c + 1]); }
+        // Gram-Schmidt with true divisions (matches the oracle's order of operations to the last bits)
+        double n0 = 0.0;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) n0 += u.e[0][c].re * u.e[0][c].re + u.e[0][c].im * u.e[0][c].im;
+        n0 = sqrt(n0);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { u.e[0][c].re /= n0; u.e[0][c].im /= n0; }
+        Cx<double> dd = cx<double>(0.0, 0.0);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) cmad_conja(dd, u.e[0][c], u.e[1][c]);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+          u.e[1][c].re -= dd.re * u.e[0][c].re - dd.im * u.e[0][c].im;
+          u.e[1][c].im -= dd.re * u.e[0][c].im + dd.im * u.e[0][c].re;
+        }
+        double n1 = 0.0;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) n1 += u.e[1][c].re * u.e[1][c].re + u.e[1][c].im * u.e[1][c].im;
+        n1 = sqrt(n1);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { u.e[1][c].re /= n1; u.e[1][c].im /= n1; }
+        m3_complete_row2(u);
+#pragma unroll
+        for (int i = 0; i < NC; ++i)
+#pragma unroll
+          for (int j = 0; j < NC; ++j) m[i][j] = cx<R>((R)u.e[i % 3][j % 3].re, (R)u.e[i % 3][j % 3].im);
+      }
+    }
+    IO::store(m, links, g, array_base<IO::T::NP>(g, D, p, mu), h);
+  }
+}
+
+// ------------------------------------------------------------------ canonical <-> internal layout
+// canonical: [lex][mu][row][col][re,im] of R, full N x N.  One thread per site, all directions.
+template <int NC, int D, typename R, bool COMP, bool TO_INTERNAL>
+__global__ void __launch_bounds__(128) layout_kernel(Geom g, typename LinkIO<NC, R, COMP>::Vec* links, R* canon) {
+  typedef LinkIO<NC, R, COMP> IO;
+  const uint32_t h = blockIdx.x * blockDim.x + threadIdx.x;
+  const int p = blockIdx.y;
+  if (h >= g.Vh) return;
+  const SiteCoord sc = decode_site(g, h, p);
+  const size_t lex = 2u * (size_t)h + (size_t)sc.s;
+#pragma unroll
+  for (int mu = 0; mu < D; ++mu) {
+    R* c = canon + (lex * D + mu) * (size_t)(NC * NC * 2);
+    Cx<R> m[NC][NC];
+    const size_t base = array_base<IO::T::NP>(g, D, p, mu);
+    if (TO_INTERNAL) {
+#pragma unroll
+      for (int i = 0; i < NC; ++i)
+#pragma unroll
+        for (int j = 0; j < NC; ++j) m[i][j] = cx<R>(c[2 * (i * NC + j)], c[2 * (i * NC + j) + 1]);
+      IO::store(m, links, g, base, h);
+    } else {
+      IO::template load<false>(m, links, g, base, h);
+#pragma unroll
+      for (int i = 0; i < NC; ++i)
+#pragma unroll
+        for (int j = 0; j < NC; ++j) { c[2 * (i * NC + j)] = m[i][j].re; c[2 * (i * NC + j) + 1] = m[i][j].im; }
+    }
+  }
+}
+
+// ------------------------------------------------------------------ reductions
+// block-wide sums of NV doubles per thread: warp shuffle, then shared memory, fixed order => deterministic
+template <int NV, int BLOCK>
+__device__ __forceinline__ void block_reduce_store(double (&v)[NV], double* out /* [NV][gridDim.x*gridDim.y] */, uint32_t nblocks, uint32_t bid) {
+  __shared__ double sm[NV][BLOCK / 32];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int k = 0; k < NV; ++k) {
+    double x = v[k];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) x += __shfl_down_sync(0xffffffffu, x, o);
+    if (lane == 0) sm[k][warp] = x;
+  }
+  __syncthreads();
+  if (threadIdx.x < NV) {
+    double s = 0.0;
+#pragma unroll
+    for (int w = 0; w < BLOCK / 32; ++w) s += sm[threadIdx.x][w];
+    out[(size_t)threadIdx.x * nblocks + bid] = s;
+  }
+}
+
+// second stage: one block per quantity, fixed-order tree over the per-block partials
+__global__ void __launch_bounds__(256) final_reduce_kernel(const double* partials, uint32_t nblocks, double* out, double scale) {
+  __shared__ double sm[256];
+  const double* p = partials + (size_t)blockIdx.x * nblocks;
+  double s = 0.0;
+  for (uint32_t i = threadIdx.x; i < nblocks; i += 256) s += p[i];
+  sm[threadIdx.x] = s;
+  __syncthreads();
+  for (int o = 128; o > 0; o >>= 1) {
+    if ((int)threadIdx.x < o) sm[threadIdx.x] += sm[threadIdx.x + o];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) out[blockIdx.x] = sm[0] * scale;
+}
+
+struct MeasureField {
+  int enabled, mu, nu;
+  double c[3], s[3];
+};
+
+// plaquette: one thread per site; the D own links stay in registers, each plane loads its two neighbours
+template <int NC, int D, typename R, bool COMP>
+__global__ void __launch_bounds__(128) plaquette_kernel(Geom g, const typename LinkIO<NC, R, COMP>::Vec* __restrict__ links, MeasureField f,
+                                                        double* partials) {
+  typedef LinkIO<NC, R, COMP> IO;
+  constexpr int NPL = D * (D - 1) / 2;
+  const uint32_t h = blockIdx.x * blockDim.x + threadIdx.x;
+  const int p = blockIdx.y, q = 1 - p;
+  double acc[NPL];
+#pragma unroll
+  for (int k = 0; k < NPL; ++k) acc[k] = 0.0;
+  if (h < g.Vh) {
+    const SiteCoord sc = decode_site(g, h, p);
+    Cx<R> own[D][NC][NC];
+    int fwd[D];
+#pragma unroll
+    for (int mu = 0; mu < D; ++mu) {
+      int b;
+      nbr_offsets(g, sc, mu, fwd[mu], b);
+      IO::template load<true>(own[mu], links, g, array_base<IO::T::NP>(g, D, p, mu), h);
+    }
+    int plane = 0;
+#pragma unroll
+    for (int mu = 0; mu < D; ++mu)
+#pragma unroll
+      for (int nu = mu + 1; nu < D; ++nu, ++plane) {
+        Cx<R> b[NC][NC], c[NC][NC], ab[NC][NC], dc[NC][NC];
+        IO::template load<true>(b, links, g, array_base<IO::T::NP>(g, D, q, nu), h + fwd[mu]);   // U_nu(x+mu)
+        IO::template load<true>(c, links, g, array_base<IO::T::NP>(g, D, q, mu), h + fwd[nu]);   // U_mu(x+nu)
+        mm_nn<NC, R>(ab, own[mu], b);        // U_mu(x) U_nu(x+mu)
+        mm_nn<NC, R>(dc, own[nu], c);        // U_nu(x) U_mu(x+nu)
+        // Re Tr [F] ab dc^+ = sum_i Re( ph_i * sum_j ab_ij conj(dc_ij) )
+        R tr = R(0);
+        const bool dressed = f.enabled && f.mu == mu && f.nu == nu;
+#pragma unroll
+        for (int i = 0; i < NC; ++i) {
+          Cx<R> d = cx<R>(0, 0);
+#pragma unroll
+          for (int j = 0; j < NC; ++j) cmad_conj(d, ab[i][j], dc[i][j]);
+          tr += dressed ? (d.re * (R)f.c[i] - d.im * (R)f.s[i]) : d.re;
+        }
+        acc[plane] += (double)tr;
+      }
+  }
+  block_reduce_store<NPL, 128>(acc, partials, gridDim.x * gridDim.y, blockIdx.y * gridDim.x + blockIdx.x);
+}
+
+// Polyakov loop: one thread per spatial site, ordered product over t of U_{D-1}
+template <int NC, int D, typename R, bool COMP>
+__global__ void __launch_bounds__(128) polyakov_kernel(Geom g, const typename LinkIO<NC, R, COMP>::Vec* __restrict__ links, double* partials) {
+  typedef LinkIO<NC, R, COMP> IO;
+  const uint32_t Lt = (uint32_t)g.L[D - 1];
+  const uint32_t Vs = g.V / Lt;
+  const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
+  double acc[2] = {0.0, 0.0};
+  if (s < Vs) {
+    // spatial coordinates of the t = 0 site with lex index s; its parity is (x0 + x1 + x2) & 1 with x0 & 1 = s & 1
+    // (L0 even); x1, x2 decode to 0 when they are not spatial directions (D < 4), because s < Vs.
+    const uint32_t hs = s >> 1;
+    const uint32_t row = fd_div(hs, g.dLh0);
+    const uint32_t r2 = fd_div(row, g.dL1);
+    const int x1 = (int)(row - r2 * (uint32_t)g.L[1]);
+    const int x2 = (D == 4) ? (int)r2 : 0;
+    const int par0 = ((int)(s & 1u) + x1 + x2) & 1;
+    Cx<R> P[NC][NC];
+#pragma unroll
+    for (int i = 0; i < NC; ++i)
+#pragma unroll
+      for (int j = 0; j < NC; ++j) P[i][j] = cx<R>(i == j ? R(1) : R(0), R(0));
+    for (uint32_t t = 0; t < Lt; ++t) {
+      const int p = (par0 + (int)t) & 1;
+      const uint32_t h = hs + t * (Vs >> 1);
+      Cx<R> u[NC][NC], n[NC][NC];
+      IO::template load<true>(u, links, g, array_base<IO::T::NP>(g, D, p, D - 1), h);
+      mm_nn<NC, R>(n, P, u);
+#pragma unroll
+      for (int i = 0; i < NC; ++i)
+#pragma unroll
+        for (int j = 0; j < NC; ++j) P[i][j] = n[i][j];
+    }
+#pragma unroll
+    for (int i = 0; i < NC; ++i) { acc[0] += (double)P[i][i].re; acc[1] += (double)P[i][i].im; }
+  }
+  block_reduce_store<2, 128>(acc, partials, gridDim.x, blockIdx.x);
+}
+
+}  // namespace qcd

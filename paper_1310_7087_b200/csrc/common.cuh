@@ -1,0 +1,131 @@
+// common.cuh -- geometry, link layout and small device helpers shared by all kernels of libqcd_b200.
+//
+// Link layout in HBM ("fastest index - number of lattice site ... next
+// index - direction ... group matrices are represented as structures of 4-vectors"):
+//   vec-plane SoA   links[parity p][direction mu][plane k][half-index h]     (h fastest)
+// where a site x of parity p = (sum x_d) & 1 has h = lex(x) >> 1, lex = x0 + L0*(x1 + L1*(x2 + L2*x3)), and the
+// NREAL stored reals of one link (row-major, re then im) are cut into NP = NREAL/VW planes of VW-wide vectors:
+//   SU(3) fp32 x12 : 3 x float4      SU(3) fp32 x18 : 9 x float2
+//   SU(3) fp64 x18 : 9 x double2     SU(3) fp64 x12 : 6 x double2
+//   SU(2) fp32 q4  : 1 x float4      SU(2) fp64 q4  : 2 x double2        (quaternion a0,a1,a2,a3)
+// Every plane holds Vh_pad = roundup(V/2, 32) vectors, so every plane starts 128-byte aligned.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace qcd {
+
+// ------------------------------------------------------------------ division by run-time constants
+struct FastDiv {
+  uint32_t d, m, s;
+};
+inline FastDiv make_fastdiv(uint32_t d) {
+  FastDiv f; f.d = d; f.s = 0;
+  while ((1u << f.s) < d) ++f.s;
+  f.m = (uint32_t)((((uint64_t)1 << 32) * (((uint64_t)1 << f.s) - d)) / d + 1);
+  return f;
+}
+__device__ __forceinline__ uint32_t fd_div(uint32_t n, const FastDiv& f) { return (__umulhi(n, f.m) + n) >> f.s; }  // n < 2^31
+
+// ------------------------------------------------------------------ geometry (kernel parameter, constant bank)
+struct Geom {
+  int D;
+  int L[4];          // extents, 1 beyond D
+  int Lh0;           // L[0] / 2
+  int stride[4];     // half-index stride of a +1 step in direction d >= 1: Lh0, Lh0*L1, Lh0*L1*L2 ; stride[0] unused
+  uint32_t Vh;       // V / 2
+  uint32_t Vh_pad;   // plane length in vectors
+  uint32_t V;
+  FastDiv dLh0, dL1, dL2;
+};
+
+struct SiteCoord {
+  int j, x1, x2, x3, s;  // x0 = 2*j + s
+};
+
+__device__ __forceinline__ SiteCoord decode_site(const Geom& g, uint32_t h, int parity) {
+  SiteCoord c;
+  uint32_t row = fd_div(h, g.dLh0);
+  c.j = (int)(h - row * (uint32_t)g.Lh0);
+  uint32_t r2 = fd_div(row, g.dL1);
+  c.x1 = (int)(row - r2 * (uint32_t)g.L[1]);
+  uint32_t r3 = fd_div(r2, g.dL2);
+  c.x2 = (int)(r2 - r3 * (uint32_t)g.L[2]);
+  c.x3 = (int)r3;
+  c.s = (parity + c.x1 + c.x2 + c.x3) & 1;
+  return c;
+}
+
+// half-index offsets to the +d / -d neighbour (which has the other parity).  d is warp-uniform.
+__device__ __forceinline__ void nbr_offsets(const Geom& g, const SiteCoord& c, int d, int& fwd, int& bwd) {
+  if (d == 0) {
+    fwd = c.s ? ((c.j == g.Lh0 - 1) ? -(g.Lh0 - 1) : 1) : 0;
+    bwd = c.s ? 0 : ((c.j == 0) ? (g.Lh0 - 1) : -1);
+  } else {
+    const int xd = (d == 1) ? c.x1 : (d == 2) ? c.x2 : c.x3;
+    const int Ld = g.L[d], st = g.stride[d];
+    fwd = (xd == Ld - 1) ? -(Ld - 1) * st : st;
+    bwd = (xd == 0) ? (Ld - 1) * st : -st;
+  }
+}
+
+// ------------------------------------------------------------------ vector planes
+template <typename R, int NREAL> struct PlaneTraits;
+template <> struct PlaneTraits<float, 12> { typedef float4 Vec; static constexpr int VW = 4, NP = 3; };
+template <> struct PlaneTraits<float, 18> { typedef float2 Vec; static constexpr int VW = 2, NP = 9; };
+template <> struct PlaneTraits<float, 4> { typedef float4 Vec; static constexpr int VW = 4, NP = 1; };
+template <> struct PlaneTraits<double, 12> { typedef double2 Vec; static constexpr int VW = 2, NP = 6; };
+template <> struct PlaneTraits<double, 18> { typedef double2 Vec; static constexpr int VW = 2, NP = 9; };
+template <> struct PlaneTraits<double, 4> { typedef double2 Vec; static constexpr int VW = 2, NP = 2; };
+
+__device__ __forceinline__ void vec_unpack(const float4& v, float* r) { r[0] = v.x; r[1] = v.y; r[2] = v.z; r[3] = v.w; }
+__device__ __forceinline__ void vec_unpack(const float2& v, float* r) { r[0] = v.x; r[1] = v.y; }
+__device__ __forceinline__ void vec_unpack(const double2& v, double* r) { r[0] = v.x; r[1] = v.y; }
+__device__ __forceinline__ void vec_pack(float4& v, const float* r) { v = make_float4(r[0], r[1], r[2], r[3]); }
+__device__ __forceinline__ void vec_pack(float2& v, const float* r) { v = make_float2(r[0], r[1]); }
+__device__ __forceinline__ void vec_pack(double2& v, const double* r) { v = make_double2(r[0], r[1]); }
+
+// element offset (in vectors) of plane 0 of the (parity, mu) link array
+template <int NP>
+__device__ __forceinline__ size_t array_base(const Geom& g, int D, int parity, int mu) {
+  return (size_t)((parity * D + mu) * NP) * (size_t)g.Vh_pad;
+}
+
+// load the NREAL reals of link h of the array starting at `base` (vectors); NC = through the read-only path
+template <typename R, int NREAL, bool NC>
+__device__ __forceinline__ void load_reals(const typename PlaneTraits<R, NREAL>::Vec* __restrict__ links, const Geom& g,
+                                           size_t base, uint32_t h, R* out) {
+  typedef PlaneTraits<R, NREAL> T;
+  const typename T::Vec* p = links + base + h;
+#pragma unroll
+  for (int k = 0; k < T::NP; ++k) {
+    typename T::Vec v = NC ? __ldg(p + (size_t)k * g.Vh_pad) : p[(size_t)k * g.Vh_pad];
+    vec_unpack(v, out + k * T::VW);
+  }
+}
+template <typename R, int NREAL>
+__device__ __forceinline__ void store_reals(typename PlaneTraits<R, NREAL>::Vec* links, const Geom& g, size_t base, uint32_t h,
+                                            const R* in) {
+  typedef PlaneTraits<R, NREAL> T;
+  typename T::Vec* p = links + base + h;
+#pragma unroll
+  for (int k = 0; k < T::NP; ++k) {
+    typename T::Vec v;
+    vec_pack(v, in + k * T::VW);
+    p[(size_t)k * g.Vh_pad] = v;
+  }
+}
+
+// ------------------------------------------------------------------ math dispatch
+__device__ __forceinline__ float q_rsqrt(float x) { return rsqrtf(x); }
+__device__ __forceinline__ double q_rsqrt(double x) { return 1.0 / sqrt(x); }
+__device__ __forceinline__ float q_sqrt(float x) { return sqrtf(x); }
+__device__ __forceinline__ double q_sqrt(double x) { return sqrt(x); }
+__device__ __forceinline__ float q_rcp(float x) { return 1.0f / x; }
+__device__ __forceinline__ double q_rcp(double x) { return 1.0 / x; }
+__device__ __forceinline__ void q_sincospi(float x, float* s, float* c) { sincospif(x, s, c); }
+__device__ __forceinline__ void q_sincospi(double x, double* s, double* c) { sincospi(x, s, c); }
+__device__ __forceinline__ float q_fma(float a, float b, float c) { return fmaf(a, b, c); }
+__device__ __forceinline__ double q_fma(double a, double b, double c) { return fma(a, b, c); }
+
+}  // namespace qcd

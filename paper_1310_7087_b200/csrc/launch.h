@@ -1,0 +1,20 @@
+// launch.h -- host-side launcher declarations; each translation unit instantiates one family of kernels.
+#pragma once
+#include "common.cuh"
+#include "update.cuh"
+
+namespace qcd {
+
+struct UpdateSel {
+  int Nc, D, precision;   // precision: 0 fp32, 1 fp64
+  bool comp;
+  int kind;               // 0 HB, 1 OR
+  bool field;
+};
+
+// returns cudaErrorInvalidValue for an unsupported combination
+cudaError_t launch_update_su3_f32(const UpdateSel& s, const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st);
+cudaError_t launch_update_su3_f64(const UpdateSel& s, const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st);
+cudaError_t launch_update_su2(const UpdateSel& s, const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st);
+
+}  // namespace qcd

@@ -1,0 +1,441 @@
+"""GPU-vs-oracle parity through the C ABI (SURVEY.md sec 8(c)-6 protocol T1..T5).  Run on the B200 box: -m gpu.
+
+Tolerances (BASELINE.json north_star): Philox words bit-exact; links per element max abs 1e-12 (fp64) / 2e-5 (fp32);
+heatbath accept/reject disagreements reported and <= 1e-6 of links; long-run <P> within 3 sigma.
+Every oracle input is produced by oracle/ or tests/inputs.py, never by the CUDA path.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from tests import np_lattice as npl
+from tests.inputs import random_links, round_to_fp32
+
+pytestmark = pytest.mark.gpu
+
+TOL = {0: 2e-5, 1: 1e-12}          # per-element max abs, by precision (0 = fp32, 1 = fp64)
+MEAS_TOL = {0: 2e-6, 1: 1e-12}     # observables (means over the lattice)
+
+# (Nc, precision, flags)
+VARIANTS = [(3, 1, 0), (3, 0, 1), (3, 0, 0), (3, 1, 1), (2, 1, 0), (2, 0, 0)]
+VARIANT_IDS = ["su3-f64x18", "su3-f32x12", "su3-f32x18", "su3-f64x12", "su2-f64", "su2-f32"]
+
+
+def gpu_lattice(q, dims, Nc, precision, flags):
+    return q.Lattice(dims, Nc, precision, flags)
+
+
+def oracle_lattice(dims, Nc, precision, links=None):
+    L = oracle.OracleLattice(dims, Nc)
+    if precision == 0:
+        L.set_fp32_shadow(True)
+    if links is not None:
+        L.set_links(links)
+    return L
+
+
+def prep_links(dims, Nc, precision, seed, spread=None):
+    links = random_links(dims, Nc, seed, spread)
+    return round_to_fp32(links) if precision == 0 else links
+
+
+def field_pair(q, fld):
+    if fld is None:
+        return None, None
+    return q.make_field(*fld), oracle.make_field(*fld)
+
+
+# ----------------------------------------------------------------------------- T1: Philox
+def test_philox_bit_exact_vs_oracle_and_curand(qcd):
+    rng = np.random.Generator(np.random.PCG64(1))
+    n = 1_000_000
+    ctr = rng.integers(0, 2 ** 32, size=(n, 4), dtype=np.uint64).astype(np.uint32)
+    key = rng.integers(0, 2 ** 32, size=(n, 2), dtype=np.uint64).astype(np.uint32)
+    ctr[0], key[0] = 0, 0
+    ctr[1], key[1] = 0xFFFFFFFF, 0xFFFFFFFF
+    mine = qcd.qcd_debug_philox(ctr, key, impl=0)
+    cur = qcd.qcd_debug_philox(ctr, key, impl=1)
+    ref = oracle.philox4x32_10_batch(ctr, key)
+    assert np.array_equal(mine, ref)
+    assert np.array_equal(cur, ref)
+    assert list(mine[0]) == [0x6627e8d5, 0xe169c58d, 0xbc57ac4c, 0x9b00dbd8]
+
+
+# ----------------------------------------------------------------------------- layout / init / measure
+@pytest.mark.parametrize("variant", VARIANTS, ids=VARIANT_IDS)
+@pytest.mark.parametrize("dims", [(4, 6), (6, 4, 2), (6, 4, 10, 2), (16, 16, 16, 4)])
+def test_set_get_links_roundtrip(qcd, variant, dims):
+    Nc, prec, flags = variant
+    links = prep_links(dims, Nc, prec, seed=3)
+    with gpu_lattice(qcd, dims, Nc, prec, flags) as G:
+        G.qcd_set_links(links)
+        back = G.qcd_get_links().astype(np.complex128)
+    if flags == 0:
+        assert np.array_equal(back, links)
+    else:
+        assert np.array_equal(back[..., :2, :], links[..., :2, :])
+        assert np.max(np.abs(back[..., 2, :] - links[..., 2, :])) < (5e-7 if prec == 0 else 1e-15)
+
+
+@pytest.mark.parametrize("variant", VARIANTS, ids=VARIANT_IDS)
+@pytest.mark.parametrize("dims", [(16, 16), (6, 4, 10), (6, 4, 10, 2), (16, 16, 16, 4)])
+def test_hot_and_cold_start_match_oracle(qcd, variant, dims):
+    Nc, prec, flags = variant
+    O = oracle.OracleLattice(dims, Nc)
+    with gpu_lattice(qcd, dims, Nc, prec, flags) as G:
+        G.qcd_init(qcd.QCD_COLD, 5)
+        cold = G.qcd_get_links()
+        assert np.array_equal(cold, np.broadcast_to(np.eye(Nc), cold.shape))
+        tot, planes, poly = G.qcd_measure()
+        assert tot == 1.0 and np.all(planes == 1.0) and poly == 1.0 + 0j
+        G.qcd_init(qcd.QCD_HOT, 42)
+        hot = G.qcd_get_links().astype(np.complex128)
+        assert G.qcd_get_sweep_counter() == 0 and G.qcd_get_seed() == 42
+    O.init(oracle.HOT, 42)
+    ref = O.get_links()
+    # fp32: rounding of the double result; compressed storage rebuilds row 2 in fp32 from the rounded rows 0,1
+    tol = 1e-13 if prec == 1 else (6e-8 if flags == 0 else 5e-7)
+    assert np.max(np.abs(hot - ref)) < tol
+
+
+@pytest.mark.parametrize("variant", VARIANTS, ids=VARIANT_IDS)
+@pytest.mark.parametrize("dims,fld", [((4, 6), None), ((6, 4, 10), None), ((6, 4, 10, 2), None), ((16, 16, 16, 4), None),
+                                      ((6, 4, 10, 2), (0, 1, "std")), ((6, 4, 10, 2), (1, 3, "std")), ((6, 4, 10), (0, 2, "std"))])
+def test_measure_matches_oracle(qcd, variant, dims, fld):
+    Nc, prec, flags = variant
+    if fld is not None:
+        fld = (fld[0], fld[1], [0.4, -0.4] if Nc == 2 else [0.4, 0.3, -0.7])
+    fg, fo = field_pair(qcd, fld)
+    links = prep_links(dims, Nc, prec, seed=9)
+    O = oracle_lattice(dims, Nc, prec, links)
+    tot_o, planes_o, poly_o = O.measure(fo)
+    with gpu_lattice(qcd, dims, Nc, prec, flags) as G:
+        G.qcd_set_links(links)
+        tot, planes, poly = G.qcd_measure(fg)
+        again = G.qcd_measure(fg)
+    assert np.max(np.abs(planes - planes_o)) < MEAS_TOL[prec]
+    assert abs(tot - tot_o) < MEAS_TOL[prec] and abs(poly - poly_o) < MEAS_TOL[prec]
+    assert again[0] == tot and np.array_equal(again[1], planes) and again[2] == poly     # deterministic reduction
+
+
+# ----------------------------------------------------------------------------- T2 / T3: per sub-step parity with resync
+SUBSTEP_CASES = [
+    # dims, field
+    ((4, 6), None), ((6, 4, 10), None), ((6, 4, 10, 2), None), ((2, 2, 2, 2), None), ((16, 16, 16, 4), None), ((12, 6, 4, 8), None),
+    ((6, 4, 10, 2), (0, 1)), ((6, 4, 10, 2), (1, 3)), ((6, 4, 10), (0, 2)), ((4, 6), (0, 1)),
+]
+
+
+def _run_substeps(qcd, variant, dims, fld, kind, beta, spread, seed):
+    """every (parity, mu) sub-step from a common pre-state; returns worst link diff, disagreements, links compared"""
+    Nc, prec, flags = variant
+    D = len(dims)
+    if fld is not None:
+        fld = (fld[0], fld[1], [0.4, -0.4] if Nc == 2 else [0.4, 0.3, -0.7])
+    fg, fo = field_pair(qcd, fld)
+    links = prep_links(dims, Nc, prec, seed=seed, spread=spread)
+    worst, disagreements, compared = 0.0, 0, 0
+    with gpu_lattice(qcd, dims, Nc, prec, flags) as G:
+        G.qcd_set_option(qcd.QCD_OPT_DEBUG_TRIALS, 1)
+        G.qcd_set_seed(2024)
+        for sweep_ctr, hit in [(0, 0), (7, 3)] if kind == 0 else [(0, 0)]:
+            for parity in (0, 1):
+                for mu in range(D):
+                    O = oracle_lattice(dims, Nc, prec, links)
+                    O.set_seed(2024)
+                    O.sweep_counter = sweep_ctr
+                    tr_o = O.substep(beta, kind, hit, parity, mu, fo, want_trials=True)
+                    ref = O.get_links()
+                    G.qcd_set_links(links)                      # resync to the common pre-state
+                    G.qcd_set_sweep_counter(sweep_ctr)
+                    G.qcd_debug_substep(beta, kind, hit, parity, mu, fg)
+                    got = G.qcd_get_links().astype(np.complex128)
+                    diff = np.max(np.abs(got - ref), axis=(-1, -2))            # (V, D)
+                    untouched = np.ones_like(diff, dtype=bool)
+                    # links of other (parity, mu) arrays must be bit-identical to the pre-state
+                    changed = np.max(np.abs(ref - links), axis=(-1, -2)) > 0
+                    untouched &= ~changed
+                    cmp_links = got if flags == 0 else got[..., :2, :]
+                    pre_links = links if flags == 0 else links[..., :2, :]
+                    same = np.max(np.abs(cmp_links - pre_links), axis=(-1, -2)) == 0
+                    assert np.all(same[untouched]), "a link outside the sub-step changed"
+                    if kind == 0:
+                        tr_g = G.qcd_debug_get_trials()
+                        bad = np.any(tr_g != tr_o, axis=1)                       # (V,) accept/reject disagreements
+                        disagreements += int(bad.sum())
+                        diff[bad, :] = 0.0
+                    worst = max(worst, float(diff.max()))
+                    compared += int(changed.sum())
+    return worst, disagreements, compared
+
+
+@pytest.mark.parametrize("variant", VARIANTS, ids=VARIANT_IDS)
+@pytest.mark.parametrize("dims,fld", SUBSTEP_CASES)
+def test_overrelaxation_substeps(qcd, variant, dims, fld):
+    worst, _, compared = _run_substeps(qcd, variant, dims, fld, kind=1, beta=5.7, spread=None, seed=13)
+    assert compared > 0
+    assert worst < TOL[variant[1]], worst
+
+
+@pytest.mark.parametrize("variant", VARIANTS, ids=VARIANT_IDS)
+@pytest.mark.parametrize("dims,fld", SUBSTEP_CASES)
+@pytest.mark.parametrize("spread", [None, 0.35], ids=["haar", "thermal"])
+def test_heatbath_substeps(qcd, variant, dims, fld, spread):
+    beta = 5.7 if variant[0] == 3 else 2.5
+    worst, disagreements, compared = _run_substeps(qcd, variant, dims, fld, kind=0, beta=beta, spread=spread, seed=17)
+    assert compared > 0
+    assert worst < TOL[variant[1]], worst
+    # north_star: accept/reject disagreements at most 1e-6 of links (reported); on these small lattices that is zero
+    print("heatbath disagreements: %d of %d links" % (disagreements, compared))
+    assert disagreements <= max(0, int(1e-6 * compared)), (disagreements, compared)
+
+
+def test_heatbath_trial_cap_and_exhaustion(qcd):
+    # hot 2-D SU(2) at small beta: alpha is small, trials often fail; with T_max = 1 many links keep their value (R5)
+    dims, Nc = (16, 16), 2
+    links = prep_links(dims, Nc, 1, seed=23)
+    O = oracle_lattice(dims, Nc, 1, links)
+    O.set_seed(5)
+    O.set_max_trials(1)
+    tr_o = O.substep(0.8, oracle.KIND_HB, 0, 0, 1, want_trials=True)
+    with gpu_lattice(qcd, dims, Nc, 1, 0) as G:
+        G.qcd_set_option(qcd.QCD_OPT_DEBUG_TRIALS, 1)
+        G.qcd_set_option(qcd.QCD_OPT_KP_MAX_TRIALS, 1)
+        G.qcd_set_seed(5)
+        G.qcd_set_links(links)
+        G.qcd_debug_substep(0.8, qcd.QCD_KIND_HB, 0, 0, 1)
+        tr_g = G.qcd_debug_get_trials()
+        got = G.qcd_get_links()
+    assert np.array_equal(tr_g, tr_o)
+    assert np.sum(tr_o[:, 0] == 0x81) > 10 and np.sum(tr_o[:, 0] == 1) > 10
+    assert np.max(np.abs(got - O.get_links())) < 1e-12
+
+
+# ----------------------------------------------------------------------------- whole sweeps without resync
+@pytest.mark.parametrize("variant", VARIANTS, ids=VARIANT_IDS)
+def test_full_sweep_unresynced(qcd, variant):
+    # config 2 shape for SU(3), config-4-like shape for SU(2); one sweep of 1 HB + 2 OR from the hot start
+    Nc, prec, flags = variant
+    dims = (16, 16, 16, 4) if Nc == 3 else (12, 12, 12, 8)
+    beta = 5.7 if Nc == 3 else 2.5
+    O = oracle.OracleLattice(dims, Nc)
+    O.init(oracle.HOT, 7)
+    start = O.get_links()
+    if prec == 0:
+        start = round_to_fp32(start)
+        O.set_fp32_shadow(True)
+        O.set_links(start)
+    O.sweep(beta, 1, 2)
+    ref = O.get_links()
+    with gpu_lattice(qcd, dims, Nc, prec, flags) as G:
+        G.qcd_init(qcd.QCD_HOT, 7)
+        G.qcd_sweep(beta, 1, 2)
+        got = G.qcd_get_links().astype(np.complex128)
+        assert G.qcd_get_sweep_counter() == 1
+        m_g = G.qcd_measure()
+    diff = np.max(np.abs(got - ref), axis=(-1, -2))
+    # an accept/reject disagreement changes a link by O(1) and contaminates its neighbours in later sub-steps:
+    # report how many links are off, require (almost) all of them within tolerance
+    off = int(np.sum(diff > 50 * TOL[prec]))
+    print("links off after an un-resynced sweep: %d of %d" % (off, diff.size))
+    assert off <= (0 if prec == 1 else 60)
+    assert np.max(diff[diff <= 50 * TOL[prec]]) < 50 * TOL[prec]
+    m_o = O.measure()
+    assert abs(m_g[0] - m_o[0]) < (1e-11 if prec == 1 else 1e-4)
+    uni, det = npl.unitarity_defect(got)
+    assert uni < (1e-12 if prec == 1 else 5e-6) and det < (1e-12 if prec == 1 else 5e-6)
+
+
+def test_overrelaxation_conserves_action_on_gpu(qcd):
+    dims = (8, 8, 8, 8)
+    for Nc, prec, flags, tol in [(3, 1, 0, 1e-12), (3, 0, 1, 3e-6), (2, 1, 0, 1e-12)]:
+        with gpu_lattice(qcd, dims, Nc, prec, flags) as G:
+            G.qcd_init(qcd.QCD_HOT, 3)
+            G.qcd_sweep(5.0, 2, 0)
+            p0 = G.qcd_measure()[0]
+            G.qcd_sweep(5.0, 0, 3)
+            p1 = G.qcd_measure()[0]
+            assert abs(p1 - p0) < tol, (Nc, prec, p0, p1)
+
+
+def test_resume_is_bit_identical_on_gpu(qcd):
+    dims, Nc, beta = (8, 8, 4, 4), 3, 5.7
+    for prec, flags in [(1, 0), (0, 1)]:
+        with gpu_lattice(qcd, dims, Nc, prec, flags) as A, gpu_lattice(qcd, dims, Nc, prec, flags) as B, \
+                gpu_lattice(qcd, dims, Nc, prec, flags) as C2:
+            A.qcd_init(qcd.QCD_HOT, 11)
+            for _ in range(4):
+                A.qcd_sweep(beta, 1, 2)
+            B.qcd_init(qcd.QCD_HOT, 11)
+            for _ in range(2):
+                B.qcd_sweep(beta, 1, 2)
+            C2.qcd_set_links(B.qcd_get_links())
+            C2.qcd_set_seed(B.qcd_get_seed())
+            C2.qcd_set_sweep_counter(B.qcd_get_sweep_counter())
+            for _ in range(2):
+                C2.qcd_sweep(beta, 1, 2)
+            a, c = A.qcd_get_links(), C2.qcd_get_links()
+            if flags == 0:
+                assert np.array_equal(a, c)
+            else:
+                assert np.array_equal(a[..., :2, :], c[..., :2, :])
+
+
+# ----------------------------------------------------------------------------- T5: long runs
+def _binned_error(x, nbins=10):
+    x = np.asarray(x)
+    b = x[: len(x) // nbins * nbins].reshape(nbins, -1).mean(axis=1)
+    return b.std(ddof=1) / np.sqrt(nbins)
+
+
+def test_config1_su2_2d_exact_plaquette_on_gpu(qcd):
+    # BASELINE.json configs[0]
+    from scipy import special
+    exact = special.iv(2, 2.0) / special.iv(1, 2.0)
+    with gpu_lattice(qcd, (16, 16), 2, 1, 0) as G:
+        G.qcd_init(qcd.QCD_COLD, 1234)
+        ps = []
+        for _ in range(200):
+            G.qcd_sweep(2.0, 1, 1)
+            ps.append(G.qcd_measure()[0])
+            if _ % 20 == 0:
+                uni, det = npl.unitarity_defect(G.qcd_get_links())
+                assert uni < 1e-12 and det < 1e-12
+    meas = np.array(ps[20:])
+    err = max(_binned_error(meas), np.sqrt(0.162709 / 256 / len(meas)))
+    assert abs(meas.mean() - exact) < 3 * err, (meas.mean(), exact, err)
+    # same seed, same keying, fp64: the GPU trajectory should coincide with the oracle's for the first sweeps
+    O = oracle.OracleLattice((16, 16), 2)
+    O.init(oracle.COLD, 1234)
+    po = []
+    for _ in range(200):
+        O.sweep(2.0, 1, 1)
+        po.append(O.measure()[0])
+    po = np.array(po)
+    assert abs(po[0] - ps[0]) < 1e-12
+    erro = max(_binned_error(po[20:]), np.sqrt(0.162709 / 256 / len(meas)))
+    assert abs(meas.mean() - po[20:].mean()) < 3 * np.sqrt(err ** 2 + erro ** 2)
+
+
+@pytest.mark.parametrize("prec,flags", [(1, 0), (0, 0)], ids=["f64", "f32"])
+def test_config2_su3_long_run_vs_oracle(qcd, prec, flags):
+    # BASELINE.json configs[1]: SU(3) 16^3x4 beta 5.7 hot seed 7, 1 HB + 4 OR; plaquette and Polyakov every sweep.
+    # 60 sweeps here (the oracle costs ~0.2 s per sweep per 8 cores); discard 20.
+    dims, beta, nsw = (16, 16, 16, 4), 5.7, 60
+    O = oracle.OracleLattice(dims, 3)
+    if prec == 0:
+        O.set_fp32_shadow(True)
+    O.init(oracle.HOT, 7)
+    po, lo = [], []
+    for _ in range(nsw):
+        O.sweep(beta, 1, 4)
+        t, _p, l = O.measure()
+        po.append(t)
+        lo.append(abs(l))
+    with gpu_lattice(qcd, dims, 3, prec, flags) as G:
+        G.qcd_init(qcd.QCD_HOT, 7)
+        pg, lg = [], []
+        for _ in range(nsw):
+            G.qcd_sweep(beta, 1, 4)
+            t, _p, l = G.qcd_measure()
+            pg.append(t)
+            lg.append(abs(l))
+    po, pg = np.array(po), np.array(pg)
+    # the first sweep agrees closely (same random numbers), later the trajectories decorrelate in fp32
+    assert abs(po[0] - pg[0]) < (1e-11 if prec == 1 else 1e-4)
+    eo, eg = _binned_error(po[20:], 8), _binned_error(pg[20:], 8)
+    assert abs(po[20:].mean() - pg[20:].mean()) < 3 * np.sqrt(eo ** 2 + eg ** 2) + 1e-12
+    assert 0.5 < pg[20:].mean() < 0.6          # sanity only (literature ~0.55 at beta 5.7; not a pin)
+    assert abs(np.mean(lg[20:]) - np.mean(lo[20:])) < 0.05
+
+
+# ----------------------------------------------------------------------------- full size, bench launch configuration
+@pytest.mark.parametrize("prec,flags", [(0, 1), (1, 0)], ids=["f32x12", "f64x18"])
+def test_config3_sampled_links_at_full_size(qcd, prec, flags):
+    # BASELINE.json configs[2]: SU(3) 32^4, beta 6.0, hot seed 42.  The oracle produces the start configuration and
+    # recomputes sampled links one by one; the GPU runs whole sub-steps in the launch configuration bench.py times.
+    dims, beta, Nc = (32, 32, 32, 32), 6.0, 3
+    O = oracle.OracleLattice(dims, Nc)
+    O.init(oracle.HOT, 42)
+    start = O.get_links()
+    if prec == 0:
+        start = round_to_fp32(start)
+        O.set_fp32_shadow(True)
+        O.set_links(start)
+    O.set_seed(42)
+    rng = np.random.Generator(np.random.PCG64(5))
+    V = O.V
+    coords = np.stack(np.unravel_index(np.arange(V), dims[::-1]), axis=-1)[:, ::-1]
+    par = coords.sum(axis=1) & 1
+    with gpu_lattice(qcd, dims, Nc, prec, flags) as G:
+        G.qcd_set_option(qcd.QCD_OPT_DEBUG_TRIALS, 1)
+        G.qcd_set_links(start)
+        G.qcd_set_seed(42)
+        hot_gpu = None
+        total_bad, total = 0, 0
+        for kind, parity, mu in [(0, 0, 0), (0, 1, 3), (1, 1, 1), (1, 0, 2)]:
+            G.qcd_set_links(start)
+            G.qcd_debug_substep(beta, kind, 0, parity, mu)
+            got = G.qcd_get_links()
+            tr = G.qcd_debug_get_trials() if kind == 0 else None
+            # boundary sites (wrap-around in every direction) plus random interior sites
+            cand = np.flatnonzero(par == parity)
+            edge = cand[np.any((coords[cand] == 0) | (coords[cand] == 31), axis=1)]
+            sample = np.concatenate([rng.choice(edge, 300, replace=False), rng.choice(cand, 700, replace=False)])
+            worst = 0.0
+            for lex in sample:
+                ref, codes = O.update_one_link(beta, kind, 0, int(lex), mu)
+                if kind == 0 and not np.array_equal(codes, tr[lex]):
+                    total_bad += 1
+                    continue
+                worst = max(worst, float(np.max(np.abs(got[lex, mu].astype(np.complex128) - ref))))
+            total += len(sample)
+            assert worst < TOL[prec], (kind, parity, mu, worst)
+            # all other links untouched
+            other = np.ones((V, 4), dtype=bool)
+            other[par == parity, mu] = False
+            cmp_a = got if flags == 0 else got[..., :2, :]
+            cmp_b = start if flags == 0 else start[..., :2, :]
+            assert np.array_equal(cmp_a[other].astype(np.complex128), cmp_b[other])
+        assert total_bad <= 1, (total_bad, total)
+        # the GPU hot start at full size equals the oracle's
+        G.qcd_init(qcd.QCD_HOT, 42)
+        hot_gpu = G.qcd_get_links().astype(np.complex128)
+        O2 = oracle.OracleLattice(dims, Nc)
+        O2.init(oracle.HOT, 42)
+        assert np.max(np.abs(hot_gpu - O2.get_links())) < (1e-13 if prec == 1 else 5e-7)
+        tot, planes, poly = G.qcd_measure()
+        tot_o, planes_o, poly_o = O2.measure()
+        assert abs(tot - tot_o) < MEAS_TOL[prec] and abs(poly - poly_o) < MEAS_TOL[prec]
+
+
+# ----------------------------------------------------------------------------- ABI error paths on a live device
+def test_error_paths(qcd):
+    with pytest.raises(qcd.QcdError) as e:
+        qcd.Lattice((5, 4), 2, 1, 0)
+    assert e.value.code == qcd.QCD_ERR_INVALID_ARG
+    with pytest.raises(qcd.QcdError) as e:
+        qcd.Lattice((4, 4), 2, 1, qcd.QCD_FLAG_COMPRESS12)
+    assert e.value.code == qcd.QCD_ERR_UNSUPPORTED
+    with gpu_lattice(qcd, (4, 4), 2, 1, 0) as G:
+        with pytest.raises(qcd.QcdError) as e:
+            G.qcd_sweep(2.0, 1, 1)
+        assert e.value.code == qcd.QCD_ERR_STATE
+        G.qcd_init(qcd.QCD_COLD, 1)
+        with pytest.raises(qcd.QcdError) as e:
+            G.qcd_sweep(float("nan"), 1, 1)
+        assert e.value.code == qcd.QCD_ERR_INVALID_ARG
+        with pytest.raises(qcd.QcdError) as e:
+            G.qcd_sweep(2.0, 1, 1, qcd.make_field(1, 0, [0.1, -0.1]))
+        assert e.value.code == qcd.QCD_ERR_INVALID_ARG
+        with pytest.raises(qcd.QcdError) as e:
+            G.qcd_sweep(2.0, 1, 1, qcd.make_field(0, 1, [0.1, 0.1]))
+        assert e.value.code == qcd.QCD_ERR_INVALID_ARG
+        with pytest.raises(qcd.QcdError):
+            G.qcd_set_option(qcd.QCD_OPT_KP_MAX_TRIALS, 0)
+        with pytest.raises(qcd.QcdError):
+            G.qcd_debug_get_trials()
+    # library-allocated workspace works too
+    with qcd.Lattice((4, 4), 2, 1, 0, library_alloc=True) as G:
+        G.qcd_init(qcd.QCD_COLD, 1)
+        assert G.qcd_measure()[0] == 1.0
