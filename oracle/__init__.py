@@ -50,9 +50,11 @@ def lib():
         L.oracle_get_links.argtypes = [C.c_void_p, C.c_void_p]
         L.oracle_set_links.argtypes = [C.c_void_p, C.c_void_p]
         L.oracle_substep.argtypes = [C.c_void_p, C.c_double, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
+        L.oracle_substep_diag.argtypes = [C.c_void_p, C.c_double, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p,
+                                          C.c_void_p]
         L.oracle_sweep.argtypes = [C.c_void_p, C.c_double, C.c_int, C.c_int, C.c_void_p]
         L.oracle_update_one_link.argtypes = [C.c_void_p, C.c_double, C.c_int, C.c_int, C.c_long, C.c_int, C.c_void_p,
-                                             C.c_void_p, C.c_void_p]
+                                             C.c_void_p, C.c_void_p, C.c_void_p]
         L.oracle_staple.argtypes = [C.c_void_p, C.c_long, C.c_int, C.c_void_p, C.c_void_p]
         L.oracle_measure.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.oracle_kp_samples.argtypes = [C.c_double, C.c_uint64, C.c_long, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
@@ -161,14 +163,25 @@ class OracleLattice:
                              trials.ctypes.data if want_trials else None)
         return trials
 
+    def substep_diag(self, beta, kind, hit, parity, mu, field=None):
+        """substep that also returns (trial codes (V,3), kmin (V,)): kmin = smallest subgroup projection norm k of each
+        updated link (inf elsewhere) -- the conditioning of that update, used by the fp32 tolerance rule."""
+        trials = np.zeros((self.V, 3), dtype=np.uint8)
+        kmin = np.full(self.V, np.inf, dtype=np.float64)
+        lib().oracle_substep_diag(self._h, float(beta), int(kind), int(hit), int(parity), int(mu), _fptr(field),
+                                  trials.ctypes.data, kmin.ctypes.data)
+        return trials, kmin
+
     def sweep(self, beta, n_hb, n_or, field=None):
         lib().oracle_sweep(self._h, float(beta), int(n_hb), int(n_or), _fptr(field))
 
     def update_one_link(self, beta, kind, hit, lex, mu, field=None):
         out = np.zeros((self.N, self.N), dtype=np.complex128)
         codes = np.zeros(3, dtype=np.uint8)
+        kmin = C.c_double(0.0)
         lib().oracle_update_one_link(self._h, float(beta), int(kind), int(hit), int(lex), int(mu), _fptr(field),
-                                     out.ctypes.data, codes.ctypes.data)
+                                     out.ctypes.data, codes.ctypes.data, C.byref(kmin))
+        self.last_kmin = kmin.value
         return out, codes
 
     def staple(self, lex, mu, field=None):

@@ -264,8 +264,9 @@ bool kennedy_pendleton(double alpha, uint64_t seed, long lex, uint32_t sweep, in
 
 // ------------------------------------------------------------------ Cabibbo-Marinari update of one link
 // kind 0: heatbath hit `hit`; kind 1: overrelaxation.  trial_codes[sg] receives the KP code (0 if skipped / OR).
+// *kmin (optional) receives the smallest subgroup projection norm k met (conditioning of the update, test diagnostics).
 Mat cm_update(const Lattice& L, const Mat& U_in, const Mat& A, double beta, int kind, int hit, long lex, int mu, int parity,
-              int trial_codes[3]) {
+              int trial_codes[3], double* kmin = nullptr) {
   const int N = L.N;
   static const int sub_i[3] = {0, 0, 1}, sub_j[3] = {1, 2, 2};       // reading R3
   const int n_sub = (N == 2) ? 1 : 3;
@@ -281,6 +282,7 @@ Mat cm_update(const Lattice& L, const Mat& U_in, const Mat& A, double beta, int 
     v.q[2] = 0.5 * (M01 - M10).real();
     v.q[3] = 0.5 * (M00 - M11).imag();
     double k2 = v.q[0] * v.q[0] + v.q[1] * v.q[1] + v.q[2] * v.q[2] + v.q[3] * v.q[3];
+    if (kmin && (sg == 0 || std::sqrt(k2) < *kmin)) *kmin = std::sqrt(k2);
     if (k2 < 1e-30) continue;                                        // reading R4
     double k = std::sqrt(k2);
     Quat vt = {{v.q[0] / k, v.q[1] / k, v.q[2] / k, v.q[3] / k}};
@@ -307,20 +309,22 @@ Mat cm_update(const Lattice& L, const Mat& U_in, const Mat& A, double beta, int 
   return reunitarise(U, N);                                          // once per link-hit, before the store
 }
 
-void update_one_link(Lattice& L, long lex, int mu, double beta, int kind, int hit, const Field* field, Mat* out, int codes[3]) {
+void update_one_link(Lattice& L, long lex, int mu, double beta, int kind, int hit, const Field* field, Mat* out, int codes[3],
+                     double* kmin = nullptr) {
   int x[4]; lex_to_coord(L, lex, x);
   Mat A = staple_sum(L, lex, mu, field);
-  *out = cm_update(L, get_link(L, lex, mu), A, beta, kind, hit, lex, mu, site_parity(L, x), codes);
+  *out = cm_update(L, get_link(L, lex, mu), A, beta, kind, hit, lex, mu, site_parity(L, x), codes, kmin);
 }
 
 // one (parity, mu) sub-step over all sites of that parity (any order: sites are independent)
-void substep(Lattice& L, double beta, int kind, int hit, int parity, int mu, const Field* field, uint8_t* trials) {
+void substep(Lattice& L, double beta, int kind, int hit, int parity, int mu, const Field* field, uint8_t* trials,
+             double* kmin = nullptr) {
 #pragma omp parallel for schedule(static)
   for (long lex = 0; lex < L.V; ++lex) {
     int x[4]; lex_to_coord(L, lex, x);
     if (site_parity(L, x) != parity) continue;
     Mat Unew; int codes[3];
-    update_one_link(L, lex, mu, beta, kind, hit, field, &Unew, codes);
+    update_one_link(L, lex, mu, beta, kind, hit, field, &Unew, codes, kmin ? &kmin[lex] : nullptr);
     put_link(L, lex, mu, Unew);        // writes U_mu on parity p only; nobody else reads it in this sub-step
     if (trials) for (int sg = 0; sg < 3; ++sg) trials[(size_t)lex * 3 + sg] = (uint8_t)codes[sg];
   }
@@ -428,6 +432,11 @@ void oracle_set_links(void* h, const double* src) {
 void oracle_substep(void* h, double beta, int kind, int hit, int parity, int mu, const Field* field, uint8_t* trials) {
   substep(*(Lattice*)h, beta, kind, hit, parity, mu, field, trials);
 }
+// same, and kmin[lex] (V doubles, only sites of `parity` written) = smallest subgroup projection norm of that link update
+void oracle_substep_diag(void* h, double beta, int kind, int hit, int parity, int mu, const Field* field, uint8_t* trials,
+                         double* kmin) {
+  substep(*(Lattice*)h, beta, kind, hit, parity, mu, field, trials, kmin);
+}
 
 // One qcd_sweep: passes outermost (R1), then parity, then direction (R2); counter += 1 at the end.
 void oracle_sweep(void* h, double beta, int n_hb, int n_or, const Field* field) {
@@ -442,10 +451,10 @@ void oracle_sweep(void* h, double beta, int n_hb, int n_or, const Field* field) 
 
 // new value of the single link (lex, mu) from the CURRENT configuration (does not store it).
 void oracle_update_one_link(void* h, double beta, int kind, int hit, long lex, int mu, const Field* field, double* out_link,
-                            uint8_t* codes_out) {
+                            uint8_t* codes_out, double* kmin_out) {
   Lattice* L = (Lattice*)h;
   Mat u; int codes[3];
-  update_one_link(*L, lex, mu, beta, kind, hit, field, &u, codes);
+  update_one_link(*L, lex, mu, beta, kind, hit, field, &u, codes, kmin_out);
   for (int i = 0; i < L->N; ++i) for (int j = 0; j < L->N; ++j) {
     out_link[2 * (i * L->N + j)] = u.m[i][j].real(); out_link[2 * (i * L->N + j) + 1] = u.m[i][j].imag();
   }

@@ -31,6 +31,10 @@ def random_links(dims, N, seed, spread=None):
         h = h - (np.trace(h, axis1=1, axis2=2) / N)[:, None, None] * np.eye(N)
         w, v = np.linalg.eigh(h)
         u = (v * np.exp(1j * spread * w)[:, None, :]) @ np.conj(np.swapaxes(v, 1, 2))
+    if N == 2:
+        # exact quaternion form [[a, b], [-conj(b), conj(a)]] so that the 4-real SU(2) storage round-trips bit for bit
+        u[:, 1, 0] = -np.conj(u[:, 0, 1])
+        u[:, 1, 1] = np.conj(u[:, 0, 0])
     return np.ascontiguousarray(u.reshape(V, D, N, N))
 
 
