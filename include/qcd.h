@@ -44,7 +44,8 @@ enum { QCD_KIND_HB = 0, QCD_KIND_OR = 1 };
 enum {
   QCD_OPT_KP_MAX_TRIALS = 0, /* Kennedy-Pendleton trial cap, 1..127, default 10 ("NHIT=10", R5) */
   QCD_OPT_DEBUG_TRIALS = 1,  /* 1: qcd_debug_substep records per-(link,subgroup) trial codes (allocates V*3 bytes) */
-  QCD_OPT_PROFILE = 2,       /* 1: bracket every update-kernel launch with CUDA events (see qcd_get_profile) */
+  QCD_OPT_PROFILE = 2,       /* 1: CUDA events around the update kernels: one pair per run of same-kind launches in qcd_sweep,
+                                one pair per launch in qcd_debug_substep (see qcd_get_profile) */
   QCD_OPT_USE_GRAPH = 3      /* 1: qcd_sweep replays a captured CUDA graph when its arguments repeat (default 1) */
 };
 

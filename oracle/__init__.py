@@ -68,6 +68,11 @@ def lib():
     return _LIB
 
 
+def num_threads():
+    """OpenMP threads the oracle's site loops run on"""
+    return int(lib().oracle_num_threads())
+
+
 def _fptr(field):
     return C.byref(field) if field is not None else None
 

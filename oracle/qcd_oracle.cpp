@@ -31,6 +31,9 @@
 // "parity unpinned": absolute 4-D plaquette values at production beta (5.7, 6.0, 6.2, 2.5)
 // have no closed form; only relative GPU-vs-oracle parity is checked there.
 // =====================================================================================
+#ifdef _OPENMP
+#include <omp.h>
+#endif
 #include <algorithm>
 #include <cmath>
 #include <complex>
@@ -514,6 +517,15 @@ void oracle_kp_samples(double alpha, uint64_t seed, long n, int max_trials, int 
     kennedy_pendleton(alpha, seed, i, 0, 0, 0, 0, 0, max_trials, uniform_mode, &g0, &code);
     g0_out[i] = g0; codes_out[i] = (uint8_t)code;
   }
+}
+
+// threads the OpenMP loops of substep / measure use (reported by bench.py's cpu_baseline as "cores")
+int oracle_num_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
 }
 
 }  // extern "C"

@@ -24,7 +24,7 @@ int fail(int code, const std::string& msg) { g_err = msg; return code; }
     if (e_ != cudaSuccess) return fail(QCD_ERR_CUDA, std::string(#expr) + ": " + cudaGetErrorString(e_)); \
   } while (0)
 
-struct EventPair { cudaEvent_t a, b; int kind; };
+struct EventPair { cudaEvent_t a, b; int kind; int n; };   // n = update-kernel launches between a and b
 
 struct GraphKey {
   double beta; int n_hb, n_or; bool field; qcd_field_t f; int max_trials; uint32_t sweep;
@@ -57,6 +57,8 @@ struct qcd_lattice {
   uint64_t launches;
   // device-resident sweep counter so that a captured sweep graph can be replayed unchanged
   uint32_t* d_sweep;
+  // persistent staging buffer for qcd_get/set_links with HOST pointers (canonical layout, allocated on first use)
+  void* d_canon;
 };
 
 namespace {
@@ -130,7 +132,24 @@ cudaError_t launch_update(qcd_lattice* L, int kind, bool field, const UpdateArgs
   return L->precision == QCD_FP32 ? launch_update_su3_f32(s, L->g, L->mem, a, L->stream) : launch_update_su3_f64(s, L->g, L->mem, a, L->stream);
 }
 
-int substep(qcd_lattice* L, double beta, int kind, int hit, int parity, int mu, const qcd_field_t* f, bool field_on, uint8_t* trials) {
+int prof_begin(qcd_lattice* L, int kind, EventPair* ep) {
+  if (L->ev_free.empty()) {
+    CUDA_TRY(cudaEventCreate(&ep->a)); CUDA_TRY(cudaEventCreate(&ep->b));
+  } else { *ep = L->ev_free.back(); L->ev_free.pop_back(); }
+  ep->kind = kind; ep->n = 0;
+  CUDA_TRY(cudaEventRecord(ep->a, L->stream));
+  return QCD_OK;
+}
+int prof_end(qcd_lattice* L, EventPair* ep, int n) {
+  ep->n = n;
+  CUDA_TRY(cudaEventRecord(ep->b, L->stream));
+  L->ev_used.push_back(*ep);
+  return QCD_OK;
+}
+
+// bracket: time this single launch with its own event pair (qcd_debug_substep); qcd_sweep brackets whole passes instead
+int substep(qcd_lattice* L, double beta, int kind, int hit, int parity, int mu, const qcd_field_t* f, bool field_on, uint8_t* trials,
+            bool bracket) {
   UpdateArgs a;
   memset(&a, 0, sizeof(a));
   a.beta = beta; a.parity = parity; a.mu = mu; a.hit = hit; a.max_trials = L->max_trials;
@@ -138,15 +157,10 @@ int substep(qcd_lattice* L, double beta, int kind, int hit, int parity, int mu, 
   a.trials = trials;
   a.f = make_field_args(f, field_on, L->Nc);
   EventPair ep;
-  if (L->profile) {
-    if (L->ev_free.empty()) {
-      CUDA_TRY(cudaEventCreate(&ep.a)); CUDA_TRY(cudaEventCreate(&ep.b));
-    } else { ep = L->ev_free.back(); L->ev_free.pop_back(); }
-    ep.kind = kind;
-    CUDA_TRY(cudaEventRecord(ep.a, L->stream));
-  }
+  const bool prof = L->profile && bracket;
+  if (prof) { int rc = prof_begin(L, kind, &ep); if (rc != QCD_OK) return rc; }
   CUDA_TRY(launch_update(L, kind, field_on, a));
-  if (L->profile) { CUDA_TRY(cudaEventRecord(ep.b, L->stream)); L->ev_used.push_back(ep); }
+  if (prof) return prof_end(L, &ep, 1);
   return QCD_OK;
 }
 
@@ -156,7 +170,7 @@ int drain_profile(qcd_lattice* L) {
   for (auto& ep : L->ev_used) {
     float ms = 0.f;
     CUDA_TRY(cudaEventElapsedTime(&ms, ep.a, ep.b));
-    L->prof_ms[ep.kind] += ms; L->prof_n[ep.kind] += 1;
+    L->prof_ms[ep.kind] += ms; L->prof_n[ep.kind] += (uint64_t)ep.n;
     L->ev_free.push_back(ep);
   }
   L->ev_used.clear();
@@ -310,7 +324,7 @@ int qcd_lattice_create(int D, const int* dims, int Nc, int precision, unsigned f
   L->seed = 0; L->sweep = 0; L->has_links = false; L->max_trials = 10;
   L->debug_trials = false; L->profile = false; L->use_graph = true;
   L->d_trials = nullptr; L->d_partials = nullptr; L->partials_cap = 0; L->d_results = nullptr; L->h_results = nullptr;
-  L->prof_ms[0] = L->prof_ms[1] = 0.0; L->prof_n[0] = L->prof_n[1] = 0; L->launches = 0; L->d_sweep = nullptr;
+  L->prof_ms[0] = L->prof_ms[1] = 0.0; L->prof_n[0] = L->prof_n[1] = 0; L->launches = 0; L->d_sweep = nullptr; L->d_canon = nullptr;
   cudaError_t e = cudaSuccess;
   if (!device_mem) {
     e = cudaMalloc(&L->mem, need);
@@ -337,6 +351,7 @@ int qcd_lattice_destroy(qcd_lattice_t* L) {
   if (L->d_results) cudaFree(L->d_results);
   if (L->h_results) cudaFreeHost(L->h_results);
   if (L->d_sweep) cudaFree(L->d_sweep);
+  if (L->d_canon) cudaFree(L->d_canon);
   delete L;
   return QCD_OK;
 }
@@ -359,13 +374,21 @@ int qcd_sweep(qcd_lattice_t* L, double beta, int n_hb, int n_or, const qcd_field
   bool fon;
   int rc = check_field(L, field, &fon);
   if (rc != QCD_OK) return rc;
+  // profiling brackets the run of heatbath launches and the run of overrelaxation launches with one event pair each
+  // (3 events per sweep), so the timed stream is not perturbed between kernels
+  EventPair ep;
   for (int pass = 0; pass < n_hb + n_or; ++pass) {
     const int kind = pass < n_hb ? QCD_KIND_HB : QCD_KIND_OR, hit = pass < n_hb ? pass : 0;
+    if (L->profile && (pass == 0 || pass == n_hb)) { rc = prof_begin(L, kind, &ep); if (rc != QCD_OK) return rc; }
     for (int p = 0; p < 2; ++p)
       for (int mu = 0; mu < L->D; ++mu) {
-        rc = substep(L, beta, kind, hit, p, mu, field, fon, nullptr);
+        rc = substep(L, beta, kind, hit, p, mu, field, fon, nullptr, false);
         if (rc != QCD_OK) return rc;
       }
+    if (L->profile && (pass == n_hb - 1 || pass == n_hb + n_or - 1)) {
+      rc = prof_end(L, &ep, 2 * L->D * (kind == QCD_KIND_HB ? n_hb : n_or));
+      if (rc != QCD_OK) return rc;
+    }
   }
   L->sweep += 1;
   return QCD_OK;
@@ -386,7 +409,7 @@ int qcd_debug_substep(qcd_lattice_t* L, double beta, int kind, int hit, int pari
     CUDA_TRY(cudaMemsetAsync(L->d_trials, 0, (size_t)L->g.V * 3, L->stream));
     trials = L->d_trials;
   }
-  return substep(L, beta, kind, hit, parity, mu, field, fon, trials);
+  return substep(L, beta, kind, hit, parity, mu, field, fon, trials, true);
 }
 
 int qcd_debug_get_trials(qcd_lattice_t* L, uint8_t* dst, size_t bytes) {
@@ -430,16 +453,15 @@ int qcd_get_links(qcd_lattice_t* L, void* dst, size_t bytes, int dst_is_device) 
   if (!L->has_links) return fail(QCD_ERR_STATE, "no links yet");
   if (bytes != canonical_bytes(L)) return fail(QCD_ERR_INVALID_ARG, "bytes must equal V*D*N*N*2*sizeof(real)");
   void* canon = dst;
-  if (!dst_is_device) CUDA_TRY(cudaMalloc(&canon, bytes));
+  if (!dst_is_device) {
+    if (!L->d_canon && cudaMalloc(&L->d_canon, bytes) != cudaSuccess) { L->d_canon = nullptr; cudaGetLastError(); return fail(QCD_ERR_ALLOC, "staging buffer"); }
+    canon = L->d_canon;
+  }
   LayoutOp op{L, canon, false};
   int rc = dispatch(L, op);
   if (rc == QCD_OK && !dst_is_device) {
-    cudaError_t e = cudaMemcpyAsync(dst, canon, bytes, cudaMemcpyDeviceToHost, L->stream);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(L->stream);
-    cudaFree(canon);
-    if (e != cudaSuccess) return fail(QCD_ERR_CUDA, std::string("get_links copy: ") + cudaGetErrorString(e));
-  } else if (!dst_is_device) {
-    cudaFree(canon);
+    CUDA_TRY(cudaMemcpyAsync(dst, canon, bytes, cudaMemcpyDeviceToHost, L->stream));
+    CUDA_TRY(cudaStreamSynchronize(L->stream));
   }
   return rc;
 }
@@ -449,16 +471,14 @@ int qcd_set_links(qcd_lattice_t* L, const void* src, size_t bytes, int src_is_de
   if (bytes != canonical_bytes(L)) return fail(QCD_ERR_INVALID_ARG, "bytes must equal V*D*N*N*2*sizeof(real)");
   void* canon = const_cast<void*>(src);
   if (!src_is_device) {
-    CUDA_TRY(cudaMalloc(&canon, bytes));
-    cudaError_t e = cudaMemcpyAsync(canon, src, bytes, cudaMemcpyHostToDevice, L->stream);
-    if (e != cudaSuccess) { cudaFree(canon); return fail(QCD_ERR_CUDA, std::string("set_links copy: ") + cudaGetErrorString(e)); }
+    if (!L->d_canon && cudaMalloc(&L->d_canon, bytes) != cudaSuccess) { L->d_canon = nullptr; cudaGetLastError(); return fail(QCD_ERR_ALLOC, "staging buffer"); }
+    canon = L->d_canon;
+    // stream-ordered: a later call reuses the staging buffer only after this kernel, on the same stream; the host
+    // buffer may be pageable, in which case cudaMemcpyAsync returns after it has been staged by the driver
+    CUDA_TRY(cudaMemcpyAsync(canon, src, bytes, cudaMemcpyHostToDevice, L->stream));
   }
   LayoutOp op{L, canon, true};
   int rc = dispatch(L, op);
-  if (!src_is_device) {
-    cudaStreamSynchronize(L->stream);   // the staging buffer must outlive the kernel
-    cudaFree(canon);
-  }
   if (rc == QCD_OK) L->has_links = true;
   return rc;
 }
