@@ -9,7 +9,8 @@ import os
 import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(HERE, "libqcd_b200.so")
+# QCD_B200_LIB: load another build of the same library (kernel tuning variants); default is the in-tree build
+LIB_PATH = os.environ.get("QCD_B200_LIB") or os.path.join(HERE, "libqcd_b200.so")
 
 QCD_OK, QCD_ERR_INVALID_ARG, QCD_ERR_UNSUPPORTED, QCD_ERR_ALLOC, QCD_ERR_CUDA, QCD_ERR_STATE = 0, 1, 2, 3, 4, 5
 QCD_FP32, QCD_FP64 = 0, 1

@@ -15,6 +15,8 @@ struct UpdateSel {
 // returns cudaErrorInvalidValue for an unsupported combination
 cudaError_t launch_update_su3_f32(const UpdateSel& s, const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st);
 cudaError_t launch_update_su3_f64(const UpdateSel& s, const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st);
+cudaError_t launch_update_su3_f32_d4(const UpdateSel& s, const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st);
+cudaError_t launch_update_su3_f64_d4(const UpdateSel& s, const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st);
 cudaError_t launch_update_su2(const UpdateSel& s, const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st);
 
 }  // namespace qcd

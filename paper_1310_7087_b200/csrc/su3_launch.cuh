@@ -1,0 +1,100 @@
+// su3_launch.cuh -- host-side selection of the SU(3) update kernel instantiation and its ring geometry.
+#pragma once
+#include "launch.h"
+
+namespace qcd {
+
+// Ring geometry per storage format: B threads per CTA, K link slots per thread (K-1 links in flight).
+// Shared memory per CTA = K * (bytes per link) * B; chosen so that several CTAs fit in the 227 KB of an SM.
+// K = 0 selects direct global loads; MINB is the second __launch_bounds__ argument (register cap).
+#ifndef QCD_F32X12_B
+#define QCD_F32X12_B 128
+#endif
+#ifndef QCD_F32X12_K
+#define QCD_F32X12_K 6
+#endif
+#ifndef QCD_F32X12_MINB
+#define QCD_F32X12_MINB 1
+#endif
+#ifndef QCD_F32X18_B
+#define QCD_F32X18_B 128
+#endif
+#ifndef QCD_F32X18_K
+#define QCD_F32X18_K 0
+#endif
+#ifndef QCD_F32X18_MINB
+#define QCD_F32X18_MINB 1
+#endif
+#ifndef QCD_F64X12_B
+#define QCD_F64X12_B 64
+#endif
+#ifndef QCD_F64X12_K
+#define QCD_F64X12_K 6
+#endif
+#ifndef QCD_F64X12_MINB
+#define QCD_F64X12_MINB 1
+#endif
+#ifndef QCD_F64X18_B
+#define QCD_F64X18_B 64
+#endif
+#ifndef QCD_F64X18_K
+#define QCD_F64X18_K 6
+#endif
+#ifndef QCD_F64X18_MINB
+#define QCD_F64X18_MINB 1
+#endif
+template <int B_, int K_, int MINB_> struct RingShape { static constexpr int B = B_, K = K_, MINB = MINB_; };
+template <typename R, bool COMP> struct RingCfg;
+template <> struct RingCfg<float, true> : RingShape<QCD_F32X12_B, QCD_F32X12_K, QCD_F32X12_MINB> {};
+template <> struct RingCfg<float, false> : RingShape<QCD_F32X18_B, QCD_F32X18_K, QCD_F32X18_MINB> {};
+template <> struct RingCfg<double, true> : RingShape<QCD_F64X12_B, QCD_F64X12_K, QCD_F64X12_MINB> {};
+template <> struct RingCfg<double, false> : RingShape<QCD_F64X18_B, QCD_F64X18_K, QCD_F64X18_MINB> {};
+
+template <typename R, int D, int MU, bool COMP, int KIND, bool FIELD>
+static cudaError_t su3_go(const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st) {
+  typedef PlaneTraits<R, (COMP ? 12 : 18)> T;
+  typedef typename T::Vec Vec;
+  constexpr int B = RingCfg<R, COMP>::B, K = RingCfg<R, COMP>::K, MINB = RingCfg<R, COMP>::MINB;
+  constexpr size_t smem = (size_t)K * T::NP * B * sizeof(Vec);
+  auto kern = su3_update_kernel<R, D, MU, COMP, KIND, FIELD, B, K, MINB>;
+  static int attr_dev = -1;                  // opt in to > 48 KB of dynamic shared memory once per device
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (smem > 0 && attr_dev != dev) {
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    attr_dev = dev;
+  }
+  const unsigned grid = (g.Vh + B - 1) / B;
+  kern<<<grid, B, smem, st>>>(g, (Vec*)links, a);
+  return cudaGetLastError();
+}
+template <typename R, int D, int MU, bool COMP>
+static cudaError_t su3_sel_kind(const UpdateSel& s, const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st) {
+#ifdef QCD_TUNE_MINIMAL   // tuning builds: only what bench.py launches (D = 4, no field, x12 in float, x18 in double)
+  if (D != 4 || s.field || COMP != std::is_same<R, float>::value) return cudaErrorInvalidValue;
+  if constexpr (D == 4 && COMP == std::is_same<R, float>::value)
+    return s.kind == 0 ? su3_go<R, D, MU, COMP, 0, false>(g, links, a, st) : su3_go<R, D, MU, COMP, 1, false>(g, links, a, st);
+  return cudaErrorInvalidValue;
+#else
+  if (s.kind == 0) return s.field ? su3_go<R, D, MU, COMP, 0, true>(g, links, a, st) : su3_go<R, D, MU, COMP, 0, false>(g, links, a, st);
+  return s.field ? su3_go<R, D, MU, COMP, 1, true>(g, links, a, st) : su3_go<R, D, MU, COMP, 1, false>(g, links, a, st);
+#endif
+}
+template <typename R, int D, int MU>
+static cudaError_t su3_sel_comp(const UpdateSel& s, const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st) {
+  return s.comp ? su3_sel_kind<R, D, MU, true>(s, g, links, a, st) : su3_sel_kind<R, D, MU, false>(s, g, links, a, st);
+}
+template <typename R, int D>
+static cudaError_t su3_sel_mu(const UpdateSel& s, const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st) {
+  switch (a.mu) {
+    case 0: return su3_sel_comp<R, D, 0>(s, g, links, a, st);
+    case 1: return su3_sel_comp<R, D, 1>(s, g, links, a, st);
+    case 2: if constexpr (D > 2) return su3_sel_comp<R, D, 2>(s, g, links, a, st); break;
+    case 3: if constexpr (D > 3) return su3_sel_comp<R, D, 3>(s, g, links, a, st); break;
+  }
+  return cudaErrorInvalidValue;
+}
+
+}  // namespace qcd

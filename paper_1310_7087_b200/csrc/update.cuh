@@ -4,7 +4,16 @@
 //   PAPER.md:108, :134) or overrelaxation (BASELINE.json north_star)                       -> 8(a)-5, 8(a)-6
 //   reunitarise + store ("reunitarization")                                   -> 8(a)-7
 // A sub-step writes only U_mu on parity p and reads it only at the thread's own site, so it is race-free.
+//
+// Data movement: the 6(D-1) neighbour links and the own link of a thread are consumed in a
+// fixed order; they are fetched by cp.async (LDGSTS, 16 B per plane) into a per-thread ring of K link slots in shared
+// memory, K-1 links ahead of the arithmetic, so the loads of the next staples are in flight while the current 3x3 products
+// run and no registers are held by data that is not being multiplied yet.  Every thread reads back only the slots it
+// filled itself, so the ring needs no block barrier.  mu is a template parameter: every array base, neighbour direction
+// and field role is resolved at compile time.
 #pragma once
+#include <type_traits>
+
 #include "common.cuh"
 #include "philox.cuh"
 #include "sun_math.cuh"
@@ -24,19 +33,79 @@ struct UpdateArgs {
   FieldArgs f;
 };
 
+// ------------------------------------------------------------------ compile-time loops and cp.async
+template <int I, int N, typename F> __device__ __forceinline__ void static_for(F&& f) {
+  if constexpr (I < N) {
+    f(std::integral_constant<int, I>{});
+    static_for<I + 1, N>(f);
+  }
+}
+
+// .cg: the copy bypasses L1 (measured: with .ca the L1, shrunk by the ring's shared memory, thrashes and costs an extra
+// pass through the L1 data path -- 202 us instead of 133 us for the fp64 overrelaxation kernel at 32^4)
+template <int BYTES> __device__ __forceinline__ void cp_async_vec(void* smem_dst, const void* gmem_src) {
+  static_assert(BYTES == 8 || BYTES == 16, "plane vectors are 8 or 16 bytes");
+  const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
+#ifndef QCD_CP_ASYNC_CA
+  if constexpr (BYTES == 16) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem_src) : "memory");
+    return;
+  }
+#endif
+  asm volatile("cp.async.ca.shared.global [%0], [%1], %2;\n" ::"r"(s), "l"(gmem_src), "n"(BYTES) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
+
 // ------------------------------------------------------------------ Kennedy-Pendleton draw of g0 (reading R5)
-// The accept decision is taken in double in both precisions so that it agrees with the fp64 oracle whenever
-// alpha agrees; the uniforms are exactly representable in the storage precision (R8).
+// The accept decision is the fp64 one in both precisions, so that it agrees with the fp64 oracle whenever alpha agrees;
+// the uniforms are exactly representable in the storage precision (R8).
+__device__ __forceinline__ bool kp_trial_f64(double alpha, double r1, double r2, double r3, double r4, double* g0) {
+  const double c = cospi(2.0 * r2);
+  const double delta = -(log(r1) + c * c * log(r3)) / alpha;
+  *g0 = 1.0 - delta;
+  return r4 * r4 <= 1.0 - 0.5 * delta;
+}
+// out-of-line copy for the rare guard-band path of the fp32 kernels (keeps the fp64 libm code out of their hot loop)
+static __device__ __noinline__ bool kp_trial_f64_cold(double alpha, double r1, double r2, double r3, double r4, double* g0) {
+  return kp_trial_f64(alpha, r1, r2, r3, r4, g0);
+}
+template <typename R> __device__ __forceinline__ R kp_alpha(double beta, R k, int nc);
+template <> __device__ __forceinline__ double kp_alpha<double>(double beta, double k, int nc) { return 2.0 * beta * k / (double)nc; }
+template <> __device__ __forceinline__ float kp_alpha<float>(double beta, float k, int nc) { return (float)(2.0 * beta / (double)nc) * k; }
+
+template <typename R> struct KpTrial;
+template <> struct KpTrial<double> {
+  static __device__ __forceinline__ bool run(double alpha, const Philox4& w, double& g0) {
+    return kp_trial_f64(alpha, uniform64(w.x), uniform64(w.y), uniform64(w.z), uniform64(w.w), &g0);
+  }
+};
+// fp32: evaluate the test in float; delta has no cancellation (both terms have the same sign), so its relative error is a
+// few ulp (< 1e-6) and the two sides of the test are known to |err| < 4e-6*delta + 1e-6.  Inside that guard band
+// (probability ~1e-5 per trial) the trial is re-evaluated in double: the decision is always the fp64 one.
+template <> struct KpTrial<float> {
+  static __device__ __forceinline__ bool run(float alpha, const Philox4& w, float& g0) {
+    const float r1 = uniform23f(w.x), r2 = uniform23f(w.y), r3 = uniform23f(w.z), r4 = uniform23f(w.w);
+    const float c = cospif(2.0f * r2);
+    const float delta = -(logf(r1) + c * c * logf(r3)) / alpha;
+    const float margin = (1.0f - 0.5f * delta) - r4 * r4;
+    g0 = 1.0f - delta;
+    if (fabsf(margin) < 4e-6f * delta + 1e-6f) {
+      double g0d;
+      const bool acc = kp_trial_f64_cold((double)alpha, uniform23(w.x), uniform23(w.y), uniform23(w.z), uniform23(w.w), &g0d);
+      g0 = (float)g0d;
+      return acc;
+    }
+    return margin >= 0.0f;
+  }
+};
+
 template <typename R>
-__device__ __forceinline__ bool kp_draw(double alpha, uint32_t lex, const UpdateArgs& a, int sg, double& g0, int& code) {
-  const uint32_t c2 = philox_c2(a.mu, a.parity, sg, a.hit, 0);
-  const double inv_alpha = 1.0 / alpha;
+__device__ __forceinline__ bool kp_draw(R alpha, uint32_t lex, const UpdateArgs& a, int mu, int sg, R& g0, int& code) {
+  const uint32_t c2 = philox_c2(mu, a.parity, sg, a.hit, 0);
   for (int t = 0; t < a.max_trials; ++t) {
     const Philox4 w = philox4x32_10(lex, a.sweep, c2, 1u + (uint32_t)t, a.key0, a.key1);
-    const double r1 = uniform_for<R>(w.x), r2 = uniform_for<R>(w.y), r3 = uniform_for<R>(w.z), r4 = uniform_for<R>(w.w);
-    const double c = cospi(2.0 * r2);
-    const double delta = -(log(r1) + c * c * log(r3)) * inv_alpha;
-    if (r4 * r4 <= 1.0 - 0.5 * delta) { g0 = 1.0 - delta; code = t + 1; return true; }
+    if (KpTrial<R>::run(alpha, w, g0)) { code = t + 1; return true; }
   }
   code = 0x80 | a.max_trials;
   return false;
@@ -44,7 +113,8 @@ __device__ __forceinline__ bool kp_draw(double alpha, uint32_t lex, const Update
 
 // quaternion a of the subgroup update from the projected v = proj(W) (not normalised), k2 = |v|^2
 template <typename R, int KIND, int NC>
-__device__ __forceinline__ bool subgroup_quaternion(const Q4<R>& v, R k2, uint32_t lex, const UpdateArgs& a, int sg, Q4<R>& out, int& code) {
+__device__ __forceinline__ bool subgroup_quaternion(const Q4<R>& v, R k2, uint32_t lex, const UpdateArgs& a, int mu, int sg, Q4<R>& out,
+                                                    int& code) {
   if (KIND == 1) {
     // overrelaxation: a = (vt^dagger)^2 = (v0^2 - |vec v|^2, -2 v0 vec v) / k^2
     const R inv = q_rcp(k2);
@@ -55,12 +125,11 @@ __device__ __forceinline__ bool subgroup_quaternion(const Q4<R>& v, R k2, uint32
   } else {
     const R rk = q_rsqrt(k2);
     const R k = k2 * rk;
-    const double alpha = 2.0 * a.beta * (double)k / (double)NC;
-    double g0d;
-    if (!kp_draw<R>(alpha, lex, a, sg, g0d, code)) return false;
-    const Philox4 w = philox4x32_10(lex, a.sweep, philox_c2(a.mu, a.parity, sg, a.hit, 0), 0u, a.key0, a.key1);
-    const R u1 = (R)uniform_for<R>(w.x), u2 = (R)uniform_for<R>(w.y);
-    const R g0 = (R)g0d;
+    const R alpha = kp_alpha<R>(a.beta, k, NC);
+    R g0;
+    if (!kp_draw<R>(alpha, lex, a, mu, sg, g0, code)) return false;
+    const Philox4 w = philox4x32_10(lex, a.sweep, philox_c2(mu, a.parity, sg, a.hit, 0), 0u, a.key0, a.key1);
+    const R u1 = uniform_real<R>(w.x), u2 = uniform_real<R>(w.y);
     const R ct = R(1) - R(2) * u1;
     const R st = q_sqrt(R(1) - ct * ct);
     R sphi, cphi;
@@ -80,22 +149,9 @@ template <> struct Tiny<double> { static __device__ __forceinline__ double k2() 
 // =====================================================================================
 // SU(3)
 // =====================================================================================
-template <typename R, bool COMP> struct Su3Store { static constexpr int NREAL = COMP ? 12 : 18; };
-
-// load a link; ROW2: make sure row 2 is valid (reconstructed when compressed)
-template <typename R, bool COMP, bool NC, bool ROW2>
-__device__ __forceinline__ void su3_load(M3<R>& u, const typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* __restrict__ links,
-                                         const Geom& g, size_t base, uint32_t h) {
-  constexpr int NREAL = COMP ? 12 : 18;
-  R r[NREAL];
-  load_reals<R, NREAL, NC>(links, g, base, h, r);
-  m3_from_reals<R, NREAL>(u, r);
-  if (COMP && ROW2) m3_complete_row2(u);
-}
-
 // one Cabibbo-Marinari subgroup hit on rows (I,J) of U given the staple sum A
 template <typename R, int KIND, int I, int J>
-__device__ __forceinline__ void su3_subgroup_hit(M3<R>& U, const M3<R>& A, uint32_t lex, const UpdateArgs& a, int sg, int& code) {
+__device__ __forceinline__ void su3_subgroup_hit(M3<R>& U, const M3<R>& A, uint32_t lex, const UpdateArgs& a, int mu, int sg, int& code) {
   Cx<R> wii = cx<R>(0, 0), wij = cx<R>(0, 0), wji = cx<R>(0, 0), wjj = cx<R>(0, 0);
 #pragma unroll
   for (int k = 0; k < 3; ++k) {
@@ -111,7 +167,7 @@ __device__ __forceinline__ void su3_subgroup_hit(M3<R>& U, const M3<R>& A, uint3
   code = 0;
   if (k2 < Tiny<R>::k2()) return;                    // reading R4
   Q4<R> q;
-  if (!subgroup_quaternion<R, KIND, 3>(v, k2, lex, a, sg, q, code)) return;
+  if (!subgroup_quaternion<R, KIND, 3>(v, k2, lex, a, mu, sg, q, code)) return;
   const Cx<R> aii = cx<R>(q.a0, q.a3), aij = cx<R>(q.a2, q.a1), aji = cx<R>(-q.a2, q.a1), ajj = cx<R>(q.a0, -q.a3);
 #pragma unroll
   for (int c = 0; c < 3; ++c) {
@@ -139,107 +195,203 @@ template <typename R> __device__ __forceinline__ void su3_scale_rows(M3<R>& m, c
     for (int j = 0; j < 3; ++j) m.e[r][j] = cmul(m.e[r][j], ph);
   }
 }
+template <typename R> __device__ __forceinline__ void m3_add(M3<R>& a, const M3<R>& s) {
+#pragma unroll
+  for (int r = 0; r < 3; ++r)
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { a.e[r][c].re += s.e[r][c].re; a.e[r][c].im += s.e[r][c].im; }
+}
 
-template <typename R, int D, bool COMP, int KIND, bool FIELD>
-__global__ void __launch_bounds__(128)
+// swap rows r1 <-> r2 of U and columns r1 <-> r2 of A: afterwards the subgroup acting on rows/columns (0,1) of the
+// permuted pair is the subgroup (frame[0], frame[1]) of the original one (W' = P W P^T)
+template <typename R, int R1, int R2> __device__ __forceinline__ void su3_swap_frame(M3<R>& U, M3<R>& A) {
+#pragma unroll
+  for (int c = 0; c < 3; ++c) { const Cx<R> t = U.e[R1][c]; U.e[R1][c] = U.e[R2][c]; U.e[R2][c] = t; }
+#pragma unroll
+  for (int r = 0; r < 3; ++r) { const Cx<R> t = A.e[r][R1]; A.e[r][R1] = A.e[r][R2]; A.e[r][R2] = t; }
+}
+
+// The links a thread consumes, in order.  For the i-th direction nu != MU, slot j = 0..5:
+//   j=0  U2  = U_mu(x+nu)        j=1  U3  = U_nu(x)        j=2  U1  = U_nu(x+mu)          upper staple U1 (U3 U2)^+
+//   j=3  U1' = U_nu(x+mu-nu)     j=4  U2' = U_mu(x-nu)     j=5  U3' = U_nu(x-nu)          lower staple (U2' U1')^+ U3'
+// and last the thread's own link U_mu(x).
+//
+// Template parameters: K = ring slots per thread (3 or 6, so that the slot of link (i, j) is j % K whatever i is; K = 0:
+// no ring, every link is loaded from global memory when it is consumed); B threads per CTA; MINB = CTAs per SM the
+// register allocation must allow.  The loop over nu and the loop over the SU(2) subgroups of the heatbath are NOT unrolled:
+// the straight-line code of a fully unrolled link update (39 KB overrelaxation, 64 KB heatbath) does not fit the 32 KB
+// instruction cache level and the warps of an SM, which sit at different places of it, stall on instruction fetch.
+template <typename R, int D, int MU, bool COMP, int KIND, bool FIELD, int B, int K, int MINB>
+__global__ void __launch_bounds__(B, MINB)
 su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links, UpdateArgs a) {
   typedef PlaneTraits<R, (COMP ? 12 : 18)> T;
-  constexpr int NREAL = COMP ? 12 : 18;
-  const uint32_t h = blockIdx.x * blockDim.x + threadIdx.x;
-  if (h >= g.Vh) return;
-  const int p = a.parity, mu = a.mu, q = 1 - p;
-  const SiteCoord sc = decode_site(g, h, p);
-  int fmu, bmu;
-  nbr_offsets(g, sc, mu, fmu, bmu);
+  typedef typename T::Vec Vec;
+  constexpr int NREAL = COMP ? 12 : 18, NP = T::NP, NR = COMP ? 2 : 3;
+  static_assert(K == 0 || K == 3 || K == 6, "ring slots must divide the 6 links of one direction");
+  constexpr int KR = K > 0 ? K : 1;
+  extern __shared__ __align__(16) unsigned char ring_raw[];
+  Vec* ring = reinterpret_cast<Vec*>(ring_raw) + threadIdx.x;      // [slot][plane][B], this thread's column
 
-  M3<R> A;
-  m3_zero(A);
-  const typename T::Vec* __restrict__ ro = links;   // neighbour arrays are never written in this sub-step
+  const uint32_t h = blockIdx.x * B + threadIdx.x;
+  if (h >= g.Vh) return;                                           // no block barrier anywhere below
+  const int p = a.parity;
+  const SiteCoord sc = decode_site(g, h, p);
+  int fo[D], bo[D];
 #pragma unroll
-  for (int i = 0; i < D - 1; ++i) {
-    const int nu = i + (i >= mu ? 1 : 0);
-    int fnu, bnu;
-    nbr_offsets(g, sc, nu, fnu, bnu);
-    int fsign = 0;   // +1: field role "first direction" (F on upper, F^+ in lower); -1: "second direction"
-    if (FIELD) fsign = (mu == a.f.mu && nu == a.f.nu) ? 1 : (mu == a.f.nu && nu == a.f.mu) ? -1 : 0;
-    {
-      // upper staple  U_nu(x+mu) U_mu(x+nu)^+ U_nu(x)^+ = U1 (U3 U2)^+
-      M3<R> U1, U2, U3, X, S;
-      su3_load<R, COMP, true, !COMP>(U1, ro, g, array_base<T::NP>(g, D, q, nu), h + fmu);
-      su3_load<R, COMP, true, true>(U2, ro, g, array_base<T::NP>(g, D, q, mu), h + fnu);
-      su3_load<R, COMP, true, !COMP>(U3, ro, g, array_base<T::NP>(g, D, p, nu), h);
-      m3_zero(X);
-      if (COMP) {
-        m3_mad_nn<R, 2>(X, U3, U2); m3_complete_row2(X);
-        if (FIELD && fsign != 0) {
-          m3_zero(S); m3_mad_nd<R, 2>(S, U1, X); m3_complete_row2(S);
-          su3_scale_cols(S, a.f, fsign < 0);
+  for (int d = 0; d < D; ++d) nbr_offsets(g, sc, d, fo[d], bo[d]);
+  const uint32_t arr = (uint32_t)NP * g.Vh_pad;                    // vectors per (parity, direction) array
+  const uint32_t own_idx = (uint32_t)(p * D + MU) * arr + h;
+  const uint32_t qmu_idx = (uint32_t)((1 - p) * D + MU) * arr + h;
+
+  struct Dir { uint32_t p_idx, q_idx; int f, b, nu; };             // per-direction addressing, run-time nu
+  auto make_dir = [&](int i) {
+    Dir d;
+    d.nu = i + (i >= MU ? 1 : 0);
+    d.f = fo[0]; d.b = bo[0];
 #pragma unroll
-          for (int r = 0; r < 3; ++r)
+    for (int k = 1; k < D; ++k) if (d.nu == k) { d.f = fo[k]; d.b = bo[k]; }
+    d.p_idx = (uint32_t)(p * D + d.nu) * arr + h;
+    d.q_idx = (uint32_t)((1 - p) * D + d.nu) * arr + h;
+    return d;
+  };
+  // vector index of plane 0 of link j of direction d (j = 6: the own link)
+  auto link_idx = [&](auto jc, const Dir& d) -> uint32_t {
+    constexpr int J = decltype(jc)::value;
+    if constexpr (J == 0) return qmu_idx + (uint32_t)d.f;
+    else if constexpr (J == 1) return d.p_idx;
+    else if constexpr (J == 2) return d.q_idx + (uint32_t)fo[MU];
+    else if constexpr (J == 3) return d.p_idx + (uint32_t)(fo[MU] + d.b);
+    else if constexpr (J == 4) return qmu_idx + (uint32_t)d.b;
+    else if constexpr (J == 5) return d.q_idx + (uint32_t)d.b;
+    else return own_idx;
+  };
+  auto issue = [&](auto jc, const Dir& d) {                         // cp.async link j into ring slot j % K
+    constexpr int J = decltype(jc)::value;
+    const Vec* src = links + link_idx(jc, d);
+    Vec* dst = ring + (J % KR) * NP * B;
 #pragma unroll
-            for (int c = 0; c < 3; ++c) { A.e[r][c].re += S.e[r][c].re; A.e[r][c].im += S.e[r][c].im; }
-        } else {
-          m3_zero(S); m3_mad_nd<R, 2>(S, U1, X); m3_complete_row2(S);
+    for (int k = 0; k < NP; ++k) cp_async_vec<(int)sizeof(Vec)>(dst + k * B, src + (size_t)k * g.Vh_pad);
+  };
+  auto fetch = [&](auto jc, const Dir& d, M3<R>& u, bool row2) {
+    constexpr int J = decltype(jc)::value;
+    R r[NREAL];
+    if constexpr (K > 0) {
+      const Vec* src = ring + (J % KR) * NP * B;
 #pragma unroll
-          for (int r = 0; r < 3; ++r)
+      for (int k = 0; k < NP; ++k) vec_unpack(src[k * B], r + k * T::VW);
+    } else {
+      const Vec* src = links + link_idx(jc, d);
+      // the own-link array is written by this kernel (each thread its own element): plain load; the rest is read-only
 #pragma unroll
-            for (int c = 0; c < 3; ++c) { A.e[r][c].re += S.e[r][c].re; A.e[r][c].im += S.e[r][c].im; }
-        }
-      } else {
-        m3_mad_nn<R, 3>(X, U3, U2);
-        if (FIELD && fsign != 0) {
-          m3_zero(S); m3_mad_nd<R, 3>(S, U1, X);
-          su3_scale_cols(S, a.f, fsign < 0);
-#pragma unroll
-          for (int r = 0; r < 3; ++r)
-#pragma unroll
-            for (int c = 0; c < 3; ++c) { A.e[r][c].re += S.e[r][c].re; A.e[r][c].im += S.e[r][c].im; }
-        } else {
-          m3_mad_nd<R, 3>(A, U1, X);
-        }
-      }
+      for (int k = 0; k < NP; ++k) vec_unpack(J == 6 ? src[(size_t)k * g.Vh_pad] : __ldg(src + (size_t)k * g.Vh_pad), r + k * T::VW);
     }
-    {
-      // lower staple  U_nu(x+mu-nu)^+ U_mu(x-nu)^+ [F^+|F] U_nu(x-nu) = (U2 U1)^+ [F^+|F] U3
-      M3<R> U1, U2, U3, Y;
-      su3_load<R, COMP, true, true>(U1, ro, g, array_base<T::NP>(g, D, p, nu), h + fmu + bnu);
-      su3_load<R, COMP, true, !COMP>(U2, ro, g, array_base<T::NP>(g, D, q, mu), h + bnu);
-      su3_load<R, COMP, true, true>(U3, ro, g, array_base<T::NP>(g, D, q, nu), h + bnu);
-      if (FIELD && fsign != 0) su3_scale_rows(U3, a.f, fsign > 0);   // first direction: F^+ U3 ; second: F U3
-      m3_zero(Y);
-      if (COMP) {
-        M3<R> S;
-        m3_mad_nn<R, 2>(Y, U2, U1); m3_complete_row2(Y);
-        m3_zero(S); m3_mad_dn<R, 2>(S, Y, U3); m3_complete_row2(S);
-#pragma unroll
-        for (int r = 0; r < 3; ++r)
-#pragma unroll
-          for (int c = 0; c < 3; ++c) { A.e[r][c].re += S.e[r][c].re; A.e[r][c].im += S.e[r][c].im; }
-      } else {
-        m3_mad_nn<R, 3>(Y, U2, U1);
-        m3_mad_dn<R, 3>(A, Y, U3);
-      }
-    }
+    m3_from_reals<R, NREAL>(u, r);
+    if (COMP && row2) m3_complete_row2(u);
+  };
+
+  Dir cur = make_dir(0);
+  if constexpr (K > 0) {                                           // prologue: links 0 .. K-2 of the first direction
+    static_for<0, KR - 1>([&](auto jc) { issue(jc, cur); cp_async_commit(); });
   }
 
-  // own link (plain load: this array is written by this kernel, each thread only its own element)
+  M3<R> A, P, Q;      // A: staple sum; P: the link kept for the next product (U2 / U1'); Q: X = U3 U2 or Y = U2' U1'
+  m3_zero(A);
+#pragma unroll 1
+  for (int i = 0; i < D - 1; ++i) {
+    const bool last = (i == D - 2);
+    const Dir nxt = make_dir(last ? i : i + 1);
+    const int fsign = !FIELD ? 0 : (MU == a.f.mu && cur.nu == a.f.nu) ? 1 : (MU == a.f.nu && cur.nu == a.f.mu) ? -1 : 0;
+    static_for<0, 6>([&](auto jc) {
+      constexpr int J = decltype(jc)::value;
+      if constexpr (K > 0) {
+        // keep K-1 links in flight: the link K-1 ahead goes to the slot whose previous content has been consumed
+        constexpr int JA = J + KR - 1;
+        if constexpr (JA < 6) {
+          issue(std::integral_constant<int, JA>{}, cur);
+        } else {
+          if (!last) issue(std::integral_constant<int, JA - 6>{}, nxt);
+          else if (JA == 6) issue(std::integral_constant<int, 6>{}, cur);     // the own link, once, after the last direction
+        }
+        cp_async_commit();                                         // one group per step, possibly empty
+        cp_async_wait<KR - 1>();                                   // link (i, J) has landed
+      }
+      if constexpr (J == 0) {
+        fetch(jc, cur, P, true);                                   // U2, all rows
+      } else if constexpr (J == 1) {
+        M3<R> U3;
+        fetch(jc, cur, U3, false);
+        m3_zero(Q);
+        m3_mad_nn<R, NR>(Q, U3, P);                                // X = U3 U2
+        if (COMP) m3_complete_row2(Q);
+      } else if constexpr (J == 2) {
+        M3<R> U1;
+        fetch(jc, cur, U1, false);
+        if (COMP || FIELD) {
+          M3<R> Sm;
+          m3_zero(Sm);
+          m3_mad_nd<R, NR>(Sm, U1, Q);                             // U1 X^+
+          if (COMP) m3_complete_row2(Sm);
+          if (FIELD && fsign != 0) su3_scale_cols(Sm, a.f, fsign < 0);   // first direction: . F ; second: . F^+
+          m3_add(A, Sm);
+        } else {
+          m3_mad_nd<R, 3>(A, U1, Q);
+        }
+      } else if constexpr (J == 3) {
+        fetch(jc, cur, P, true);                                   // U1', all rows
+      } else if constexpr (J == 4) {
+        M3<R> U2;
+        fetch(jc, cur, U2, false);
+        m3_zero(Q);
+        m3_mad_nn<R, NR>(Q, U2, P);                                // Y = U2' U1'
+        if (COMP) m3_complete_row2(Q);
+      } else {
+        M3<R> U3;
+        fetch(jc, cur, U3, true);
+        if (FIELD && fsign != 0) su3_scale_rows(U3, a.f, fsign > 0);   // first direction: F^+ U3' ; second: F U3'
+        if (COMP) {
+          M3<R> Sm;
+          m3_zero(Sm);
+          m3_mad_dn<R, 2>(Sm, Q, U3);                              // Y^+ U3'
+          m3_complete_row2(Sm);
+          m3_add(A, Sm);
+        } else {
+          m3_mad_dn<R, 3>(A, Q, U3);
+        }
+      }
+    });
+    cur = nxt;
+  }
+
+  // own link: the last one through the ring
+  if constexpr (K > 0) cp_async_wait<0>();
   M3<R> U;
-  const size_t own = array_base<T::NP>(g, D, p, mu);
-  su3_load<R, COMP, false, true>(U, links, g, own, h);
+  fetch(std::integral_constant<int, 6>{}, cur, U, true);
 
   const uint32_t lex = 2u * h + (uint32_t)sc.s;
-  int c0, c1, c2;
-  su3_subgroup_hit<R, KIND, 0, 1>(U, A, lex, a, 0, c0);
-  su3_subgroup_hit<R, KIND, 0, 2>(U, A, lex, a, 1, c1);
-  su3_subgroup_hit<R, KIND, 1, 2>(U, A, lex, a, 2, c2);
+  if constexpr (KIND == 1) {
+    int c;
+    su3_subgroup_hit<R, KIND, 0, 1>(U, A, lex, a, MU, 0, c);
+    su3_subgroup_hit<R, KIND, 0, 2>(U, A, lex, a, MU, 1, c);
+    su3_subgroup_hit<R, KIND, 1, 2>(U, A, lex, a, MU, 2, c);
+  } else {
+    // one copy of the heatbath hit, on rows (0,1) of a permuted frame: (0,1,2) -> (0,2,1) -> (1,2,0)   (reading R3)
+#pragma unroll 1
+    for (int sg = 0; sg < 3; ++sg) {
+      int c;
+      su3_subgroup_hit<R, KIND, 0, 1>(U, A, lex, a, MU, sg, c);
+      if (a.trials) a.trials[(size_t)lex * 3 + sg] = (uint8_t)c;
+      if (sg == 0) su3_swap_frame<R, 1, 2>(U, A);
+      else if (sg == 1) su3_swap_frame<R, 0, 2>(U, A);
+    }
+    // frame (1,2,0) back to (0,1,2): row 0 <- cur 2, row 1 <- cur 0, row 2 <- cur 1
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { const Cx<R> t = U.e[2][c]; U.e[2][c] = U.e[1][c]; U.e[1][c] = U.e[0][c]; U.e[0][c] = t; }
+  }
   m3_reunitarise(U);
 
   R r[NREAL];
   m3_to_reals<R, NREAL>(U, r);
-  store_reals<R, NREAL>(links, g, own, h, r);
-  if (KIND == 0 && a.trials) {
-    a.trials[(size_t)lex * 3 + 0] = (uint8_t)c0; a.trials[(size_t)lex * 3 + 1] = (uint8_t)c1; a.trials[(size_t)lex * 3 + 2] = (uint8_t)c2;
-  }
+  store_reals<R, NREAL>(links, g, (size_t)(p * D + MU) * arr, h, r);
 }
 
 // =====================================================================================
@@ -298,7 +450,7 @@ su2_update_kernel(Geom g, typename PlaneTraits<R, 4>::Vec* links, UpdateArgs a) 
   int code = 0;
   if (!(k2 < Tiny<R>::k2())) {
     Q4<R> qa;
-    if (subgroup_quaternion<R, KIND, 2>(v, k2, lex, a, 0, qa, code)) U = q4_mul(qa, U);
+    if (subgroup_quaternion<R, KIND, 2>(v, k2, lex, a, mu, 0, qa, code)) U = q4_mul(qa, U);
   }
   const R n = q_rsqrt(U.a0 * U.a0 + U.a1 * U.a1 + U.a2 * U.a2 + U.a3 * U.a3);
   R r[4] = {U.a0 * n, U.a1 * n, U.a2 * n, U.a3 * n};
