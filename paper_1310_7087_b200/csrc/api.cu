@@ -152,7 +152,7 @@ int substep(qcd_lattice* L, double beta, int kind, int hit, int parity, int mu, 
             bool bracket) {
   UpdateArgs a;
   memset(&a, 0, sizeof(a));
-  a.beta = beta; a.parity = parity; a.mu = mu; a.hit = hit; a.max_trials = L->max_trials;
+  a.beta = beta; a.inv_c = (double)L->Nc / (2.0 * beta); a.parity = parity; a.mu = mu; a.hit = hit; a.max_trials = L->max_trials;
   a.sweep = L->sweep; a.key0 = (uint32_t)(L->seed & 0xFFFFFFFFull); a.key1 = (uint32_t)(L->seed >> 32);
   a.trials = trials;
   a.f = make_field_args(f, field_on, L->Nc);

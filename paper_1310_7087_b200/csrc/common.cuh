@@ -118,7 +118,7 @@ __device__ __forceinline__ void store_reals(typename PlaneTraits<R, NREAL>::Vec*
 
 // ------------------------------------------------------------------ math dispatch
 __device__ __forceinline__ float q_rsqrt(float x) { return rsqrtf(x); }
-__device__ __forceinline__ double q_rsqrt(double x) { return 1.0 / sqrt(x); }
+__device__ __forceinline__ double q_rsqrt(double x) { return rsqrt(x); }
 __device__ __forceinline__ float q_sqrt(float x) { return sqrtf(x); }
 __device__ __forceinline__ double q_sqrt(double x) { return sqrt(x); }
 __device__ __forceinline__ float q_rcp(float x) { return 1.0f / x; }

@@ -43,6 +43,26 @@ namespace qcd {
 #ifndef QCD_F64X18_MINB
 #define QCD_F64X18_MINB 1
 #endif
+// Loop shape per precision and kind (measured at 32^4, see profiles/): ROLL = keep the direction / subgroup loops rolled,
+// PRE = heatbath random part of trial 0 precomputed into shared memory.
+#ifndef QCD_F32_ROLL
+#define QCD_F32_ROLL true
+#endif
+#ifndef QCD_F32_PRE
+#define QCD_F32_PRE true
+#endif
+#ifndef QCD_F64_ROLL_OR
+#define QCD_F64_ROLL_OR false
+#endif
+#ifndef QCD_F64_ROLL_HB
+#define QCD_F64_ROLL_HB true
+#endif
+#ifndef QCD_F64_PRE
+#define QCD_F64_PRE false
+#endif
+template <typename R, int KIND> struct LoopCfg;
+template <int KIND> struct LoopCfg<float, KIND> { static constexpr bool ROLL = QCD_F32_ROLL, PRE = QCD_F32_PRE; };
+template <int KIND> struct LoopCfg<double, KIND> { static constexpr bool ROLL = (KIND == 0) ? QCD_F64_ROLL_HB : QCD_F64_ROLL_OR, PRE = QCD_F64_PRE; };
 template <int B_, int K_, int MINB_> struct RingShape { static constexpr int B = B_, K = K_, MINB = MINB_; };
 template <typename R, bool COMP> struct RingCfg;
 template <> struct RingCfg<float, true> : RingShape<QCD_F32X12_B, QCD_F32X12_K, QCD_F32X12_MINB> {};
@@ -55,13 +75,14 @@ static cudaError_t su3_go(const Geom& g, void* links, const UpdateArgs& a, cudaS
   typedef PlaneTraits<R, (COMP ? 12 : 18)> T;
   typedef typename T::Vec Vec;
   constexpr int B = RingCfg<R, COMP>::B, K = RingCfg<R, COMP>::K, MINB = RingCfg<R, COMP>::MINB;
-  constexpr size_t smem = (size_t)K * T::NP * B * sizeof(Vec);
-  auto kern = su3_update_kernel<R, D, MU, COMP, KIND, FIELD, B, K, MINB>;
+  constexpr bool ROLL = LoopCfg<R, KIND>::ROLL, PRE = LoopCfg<R, KIND>::PRE;
+  constexpr size_t smem = (size_t)K * T::NP * B * sizeof(Vec) + ((KIND == 0 && PRE) ? (size_t)15 * B * sizeof(R) : 0);
+  auto kern = su3_update_kernel<R, D, MU, COMP, KIND, FIELD, B, K, MINB, ROLL, PRE>;
   static int attr_dev = -1;                  // opt in to > 48 KB of dynamic shared memory once per device
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return e;
-  if (smem > 0 && attr_dev != dev) {
+  if (smem > 48 * 1024 && attr_dev != dev) {
     e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     attr_dev = dev;

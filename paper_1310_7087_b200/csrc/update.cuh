@@ -27,6 +27,7 @@ struct FieldArgs {   // F = diag(exp(i theta_c)) on plane (mu,nu), mu<nu; cos/si
 
 struct UpdateArgs {
   double beta;
+  double inv_c;      // N / (2 beta): delta = E / alpha = E * inv_c / k   (host-computed; inf when beta = 0 -> every trial fails)
   int parity, mu, hit, max_trials;
   uint32_t sweep, key0, key1;
   uint8_t* trials;   // NULL or [lex][3] debug trial codes
@@ -57,64 +58,87 @@ template <int BYTES> __device__ __forceinline__ void cp_async_vec(void* smem_dst
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
 
-// ------------------------------------------------------------------ Kennedy-Pendleton draw of g0 (reading R5)
+// ------------------------------------------------------------------ Kennedy-Pendleton heatbath (reading R5)
+// One trial:  delta = -(ln r1 + cos^2(2 pi r2) ln r3) / alpha,  accept iff r4^2 <= 1 - delta/2,  g0 = 1 - delta.
+// Everything but the division by alpha depends on the random numbers only, so it is split off:
+//   E = -(ln r1 + cos^2(2 pi r2) ln r3),  w = r4^2            (KpRand, from Philox draw 1+t)
+//   n = unit vector (st cos phi, st sin phi, ct)              (hb_direction, from Philox draw 0)
+// and evaluated for trial 0 of all subgroups at the start of the kernel, while the first links are in flight.
 // The accept decision is the fp64 one in both precisions, so that it agrees with the fp64 oracle whenever alpha agrees;
 // the uniforms are exactly representable in the storage precision (R8).
-__device__ __forceinline__ bool kp_trial_f64(double alpha, double r1, double r2, double r3, double r4, double* g0) {
+template <typename R> struct HbDraw { R E, w, n1, n2, n3; };
+
+template <typename R> struct KpRand;
+template <> struct KpRand<double> {
+  static __device__ __forceinline__ void run(const Philox4& x, double& E, double& w) {
+    const double r1 = uniform64(x.x), r2 = uniform64(x.y), r3 = uniform64(x.z), r4 = uniform64(x.w);
+    const double c = cospi(2.0 * r2);
+    E = -(log(r1) + c * c * log(r3));
+    w = r4 * r4;
+  }
+};
+// fp32: __logf is 3 ulp (2^-21.4 absolute near 1), cospif 2 ulp: E is known to ~1e-6 E.  The accept test of the fp32
+// kernels is taken in float and re-evaluated in double inside a guard band (kp_accept below).
+template <> struct KpRand<float> {
+  static __device__ __forceinline__ void run(const Philox4& x, float& E, float& w) {
+    const float r1 = uniform23f(x.x), r2 = uniform23f(x.y), r3 = uniform23f(x.z), r4 = uniform23f(x.w);
+    const float c = cospif(2.0f * r2);
+    E = -(__logf(r1) + c * c * __logf(r3));
+    w = r4 * r4;
+  }
+};
+template <typename R> __device__ __forceinline__ void hb_direction(const Philox4& x, R& n1, R& n2, R& n3) {
+  const R u1 = uniform_real<R>(x.x), u2 = uniform_real<R>(x.y);
+  const R ct = R(1) - R(2) * u1;
+  const R st = q_sqrt(R(1) - ct * ct);
+  R sphi, cphi;
+  q_sincospi(R(2) * u2, &sphi, &cphi);
+  n1 = st * cphi; n2 = st * sphi; n3 = ct;
+}
+// trial 0 and direction of subgroup sg of this link
+template <typename R>
+__device__ __forceinline__ HbDraw<R> hb_first_draw(uint32_t lex, const UpdateArgs& a, int mu, int sg) {
+  const uint32_t c2 = philox_c2(mu, a.parity, sg, a.hit, 0);
+  HbDraw<R> d;
+  KpRand<R>::run(philox4x32_10(lex, a.sweep, c2, 1u, a.key0, a.key1), d.E, d.w);
+  hb_direction<R>(philox4x32_10(lex, a.sweep, c2, 0u, a.key0, a.key1), d.n1, d.n2, d.n3);
+  return d;
+}
+
+// the whole trial in double from the Philox block (guard-band path of the fp32 kernels; out of line, rarely taken)
+static __device__ __noinline__ bool kp_trial_f64_cold(double alpha, uint32_t x, uint32_t y, uint32_t z, uint32_t w, double* g0) {
+  const double r1 = uniform23(x), r2 = uniform23(y), r3 = uniform23(z), r4 = uniform23(w);
   const double c = cospi(2.0 * r2);
   const double delta = -(log(r1) + c * c * log(r3)) / alpha;
   *g0 = 1.0 - delta;
   return r4 * r4 <= 1.0 - 0.5 * delta;
 }
-// out-of-line copy for the rare guard-band path of the fp32 kernels (keeps the fp64 libm code out of their hot loop)
-static __device__ __noinline__ bool kp_trial_f64_cold(double alpha, double r1, double r2, double r3, double r4, double* g0) {
-  return kp_trial_f64(alpha, r1, r2, r3, r4, g0);
+// accept test of one trial given its random part (E, w); blk = the Philox block the pair came from
+__device__ __forceinline__ bool kp_accept(double inv_alpha, double E, double w, const Philox4&, double& g0) {
+  const double delta = E * inv_alpha;
+  g0 = 1.0 - delta;
+  return w <= 1.0 - 0.5 * delta;
 }
-template <typename R> __device__ __forceinline__ R kp_alpha(double beta, R k, int nc);
-template <> __device__ __forceinline__ double kp_alpha<double>(double beta, double k, int nc) { return 2.0 * beta * k / (double)nc; }
-template <> __device__ __forceinline__ float kp_alpha<float>(double beta, float k, int nc) { return (float)(2.0 * beta / (double)nc) * k; }
-
-template <typename R> struct KpTrial;
-template <> struct KpTrial<double> {
-  static __device__ __forceinline__ bool run(double alpha, const Philox4& w, double& g0) {
-    return kp_trial_f64(alpha, uniform64(w.x), uniform64(w.y), uniform64(w.z), uniform64(w.w), &g0);
+// fp32: |error of delta| < (2e-6 E + 1e-6) / alpha, so outside the guard band below the float decision is the fp64 one;
+// inside it (probability ~1e-5 per trial) the trial is recomputed in double.
+__device__ __forceinline__ bool kp_accept(float inv, float E, float w, const Philox4& blk, float& g0) {
+  const float delta = E * inv;
+  const float margin = (1.0f - 0.5f * delta) - w;
+  g0 = 1.0f - delta;
+  if (fabsf(margin) < (4e-6f * E + 2e-6f) * inv + 5e-7f) {
+    double g0d;
+    const bool acc = kp_trial_f64_cold(1.0 / (double)inv, blk.x, blk.y, blk.z, blk.w, &g0d);
+    g0 = (float)g0d;
+    return acc;
   }
-};
-// fp32: evaluate the test in float; delta has no cancellation (both terms have the same sign), so its relative error is a
-// few ulp (< 1e-6) and the two sides of the test are known to |err| < 4e-6*delta + 1e-6.  Inside that guard band
-// (probability ~1e-5 per trial) the trial is re-evaluated in double: the decision is always the fp64 one.
-template <> struct KpTrial<float> {
-  static __device__ __forceinline__ bool run(float alpha, const Philox4& w, float& g0) {
-    const float r1 = uniform23f(w.x), r2 = uniform23f(w.y), r3 = uniform23f(w.z), r4 = uniform23f(w.w);
-    const float c = cospif(2.0f * r2);
-    const float delta = -(logf(r1) + c * c * logf(r3)) / alpha;
-    const float margin = (1.0f - 0.5f * delta) - r4 * r4;
-    g0 = 1.0f - delta;
-    if (fabsf(margin) < 4e-6f * delta + 1e-6f) {
-      double g0d;
-      const bool acc = kp_trial_f64_cold((double)alpha, uniform23(w.x), uniform23(w.y), uniform23(w.z), uniform23(w.w), &g0d);
-      g0 = (float)g0d;
-      return acc;
-    }
-    return margin >= 0.0f;
-  }
-};
-
-template <typename R>
-__device__ __forceinline__ bool kp_draw(R alpha, uint32_t lex, const UpdateArgs& a, int mu, int sg, R& g0, int& code) {
-  const uint32_t c2 = philox_c2(mu, a.parity, sg, a.hit, 0);
-  for (int t = 0; t < a.max_trials; ++t) {
-    const Philox4 w = philox4x32_10(lex, a.sweep, c2, 1u + (uint32_t)t, a.key0, a.key1);
-    if (KpTrial<R>::run(alpha, w, g0)) { code = t + 1; return true; }
-  }
-  code = 0x80 | a.max_trials;
-  return false;
+  return margin >= 0.0f;
 }
 
-// quaternion a of the subgroup update from the projected v = proj(W) (not normalised), k2 = |v|^2
+// quaternion a of the subgroup update from the projected v = proj(W) (not normalised), k2 = |v|^2;
+// d0 = trial 0 and direction (heatbath only)
 template <typename R, int KIND, int NC>
-__device__ __forceinline__ bool subgroup_quaternion(const Q4<R>& v, R k2, uint32_t lex, const UpdateArgs& a, int mu, int sg, Q4<R>& out,
-                                                    int& code) {
+__device__ __forceinline__ bool subgroup_quaternion(const Q4<R>& v, R k2, uint32_t lex, const UpdateArgs& a, int mu, int sg,
+                                                    const HbDraw<R>& d0, Q4<R>& out, int& code) {
   if (KIND == 1) {
     // overrelaxation: a = (vt^dagger)^2 = (v0^2 - |vec v|^2, -2 v0 vec v) / k^2
     const R inv = q_rcp(k2);
@@ -124,18 +148,32 @@ __device__ __forceinline__ bool subgroup_quaternion(const Q4<R>& v, R k2, uint32
     return true;
   } else {
     const R rk = q_rsqrt(k2);
-    const R k = k2 * rk;
-    const R alpha = kp_alpha<R>(a.beta, k, NC);
+    const R inv_alpha = (R)a.inv_c * rk;                 // 1 / alpha, alpha = 2 beta k / N
+    const uint32_t c2 = philox_c2(mu, a.parity, sg, a.hit, 0);
     R g0;
-    if (!kp_draw<R>(alpha, lex, a, mu, sg, g0, code)) return false;
-    const Philox4 w = philox4x32_10(lex, a.sweep, philox_c2(mu, a.parity, sg, a.hit, 0), 0u, a.key0, a.key1);
-    const R u1 = uniform_real<R>(w.x), u2 = uniform_real<R>(w.y);
-    const R ct = R(1) - R(2) * u1;
-    const R st = q_sqrt(R(1) - ct * ct);
-    R sphi, cphi;
-    q_sincospi(R(2) * u2, &sphi, &cphi);
+    // trial 0 from the precomputed random part; its Philox block is regenerated only inside the fp32 guard band
+    Philox4 blk; blk.x = blk.y = blk.z = blk.w = 0u;
+    bool acc;
+    if (sizeof(R) == 4) {
+      // cheap pre-test, so that the common case does not pay for the Philox block
+      const float inv = (float)inv_alpha;
+      const float margin = (1.0f - 0.5f * (float)d0.E * inv) - (float)d0.w;
+      if (fabsf(margin) < (4e-6f * (float)d0.E + 2e-6f) * inv + 5e-7f) blk = philox4x32_10(lex, a.sweep, c2, 1u, a.key0, a.key1);
+    }
+    acc = kp_accept(inv_alpha, d0.E, d0.w, blk, g0);
+    code = 1;
+    if (!acc) {
+      code = 0x80 | a.max_trials;
+      for (int t = 1; t < a.max_trials; ++t) {
+        const Philox4 x = philox4x32_10(lex, a.sweep, c2, 1u + (uint32_t)t, a.key0, a.key1);
+        R E, w;
+        KpRand<R>::run(x, E, w);
+        if (kp_accept(inv_alpha, E, w, x, g0)) { acc = true; code = t + 1; break; }
+      }
+      if (!acc) return false;
+    }
     const R rr = q_sqrt(fmax(R(0), R(1) - g0 * g0));
-    const Q4<R> g = q4<R>(g0, rr * st * cphi, rr * st * sphi, rr * ct);
+    const Q4<R> g = q4<R>(g0, rr * d0.n1, rr * d0.n2, rr * d0.n3);
     const Q4<R> vtc = q4<R>(v.a0 * rk, -v.a1 * rk, -v.a2 * rk, -v.a3 * rk);   // vt^dagger
     out = q4_mul(g, vtc);
     return true;
@@ -151,7 +189,8 @@ template <> struct Tiny<double> { static __device__ __forceinline__ double k2() 
 // =====================================================================================
 // one Cabibbo-Marinari subgroup hit on rows (I,J) of U given the staple sum A
 template <typename R, int KIND, int I, int J>
-__device__ __forceinline__ void su3_subgroup_hit(M3<R>& U, const M3<R>& A, uint32_t lex, const UpdateArgs& a, int mu, int sg, int& code) {
+__device__ __forceinline__ void su3_subgroup_hit(M3<R>& U, const M3<R>& A, uint32_t lex, const UpdateArgs& a, int mu, int sg,
+                                                 const HbDraw<R>& d0, int& code) {
   Cx<R> wii = cx<R>(0, 0), wij = cx<R>(0, 0), wji = cx<R>(0, 0), wjj = cx<R>(0, 0);
 #pragma unroll
   for (int k = 0; k < 3; ++k) {
@@ -167,7 +206,7 @@ __device__ __forceinline__ void su3_subgroup_hit(M3<R>& U, const M3<R>& A, uint3
   code = 0;
   if (k2 < Tiny<R>::k2()) return;                    // reading R4
   Q4<R> q;
-  if (!subgroup_quaternion<R, KIND, 3>(v, k2, lex, a, mu, sg, q, code)) return;
+  if (!subgroup_quaternion<R, KIND, 3>(v, k2, lex, a, mu, sg, d0, q, code)) return;
   const Cx<R> aii = cx<R>(q.a0, q.a3), aij = cx<R>(q.a2, q.a1), aji = cx<R>(-q.a2, q.a1), ajj = cx<R>(q.a0, -q.a3);
 #pragma unroll
   for (int c = 0; c < 3; ++c) {
@@ -218,10 +257,12 @@ template <typename R, int R1, int R2> __device__ __forceinline__ void su3_swap_f
 //
 // Template parameters: K = ring slots per thread (3 or 6, so that the slot of link (i, j) is j % K whatever i is; K = 0:
 // no ring, every link is loaded from global memory when it is consumed); B threads per CTA; MINB = CTAs per SM the
-// register allocation must allow.  The loop over nu and the loop over the SU(2) subgroups of the heatbath are NOT unrolled:
-// the straight-line code of a fully unrolled link update (39 KB overrelaxation, 64 KB heatbath) does not fit the 32 KB
-// instruction cache level and the warps of an SM, which sit at different places of it, stall on instruction fetch.
-template <typename R, int D, int MU, bool COMP, int KIND, bool FIELD, int B, int K, int MINB>
+// register allocation must allow.  ROLL: the loop over nu and the loop over the SU(2) subgroups of the heatbath are not
+// unrolled (the straight-line code of a fully unrolled link update, 39 KB overrelaxation / 64 KB heatbath, does not fit the
+// 32 KB instruction cache level; the fp32 kernels, which are issue-bound, take it; the fp64 kernels, which run few warps
+// and live on instruction-level parallelism, are faster unrolled).  PRE: heatbath only, park the random-number-only part
+// of trial 0 of every subgroup in shared memory at the start of the kernel instead of computing it inside the hit.
+template <typename R, int D, int MU, bool COMP, int KIND, bool FIELD, int B, int K, int MINB, bool ROLL, bool PRE>
 __global__ void __launch_bounds__(B, MINB)
 su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links, UpdateArgs a) {
   typedef PlaneTraits<R, (COMP ? 12 : 18)> T;
@@ -294,10 +335,22 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
     static_for<0, KR - 1>([&](auto jc) { issue(jc, cur); cp_async_commit(); });
   }
 
+  const uint32_t lex = 2u * h + (uint32_t)sc.s;
+  // heatbath: the random-number-only part of trial 0 and the direction of each subgroup, computed while the first links
+  // are in flight and parked in shared memory behind the ring ([subgroup][5][B] reals, this thread's column)
+  R* draws = reinterpret_cast<R*>(ring_raw + (size_t)K * NP * B * sizeof(Vec)) + threadIdx.x;
+  if constexpr (KIND == 0 && PRE) {
+#pragma unroll 1
+    for (int sg = 0; sg < 3; ++sg) {
+      const HbDraw<R> d = hb_first_draw<R>(lex, a, MU, sg);
+      R* o = draws + sg * 5 * B;
+      o[0] = d.E; o[B] = d.w; o[2 * B] = d.n1; o[3 * B] = d.n2; o[4 * B] = d.n3;
+    }
+  }
+
   M3<R> A, P, Q;      // A: staple sum; P: the link kept for the next product (U2 / U1'); Q: X = U3 U2 or Y = U2' U1'
   m3_zero(A);
-#pragma unroll 1
-  for (int i = 0; i < D - 1; ++i) {
+  auto direction_step = [&](int i) {
     const bool last = (i == D - 2);
     const Dir nxt = make_dir(last ? i : i + 1);
     const int fsign = !FIELD ? 0 : (MU == a.f.mu && cur.nu == a.f.nu) ? 1 : (MU == a.f.nu && cur.nu == a.f.mu) ? -1 : 0;
@@ -360,6 +413,13 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
       }
     });
     cur = nxt;
+  };
+  if constexpr (ROLL) {
+#pragma unroll 1
+    for (int i = 0; i < D - 1; ++i) direction_step(i);
+  } else {
+#pragma unroll
+    for (int i = 0; i < D - 1; ++i) direction_step(i);
   }
 
   // own link: the last one through the ring
@@ -367,25 +427,46 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
   M3<R> U;
   fetch(std::integral_constant<int, 6>{}, cur, U, true);
 
-  const uint32_t lex = 2u * h + (uint32_t)sc.s;
   if constexpr (KIND == 1) {
     int c;
-    su3_subgroup_hit<R, KIND, 0, 1>(U, A, lex, a, MU, 0, c);
-    su3_subgroup_hit<R, KIND, 0, 2>(U, A, lex, a, MU, 1, c);
-    su3_subgroup_hit<R, KIND, 1, 2>(U, A, lex, a, MU, 2, c);
+    HbDraw<R> none;
+    none.E = none.w = none.n1 = none.n2 = none.n3 = R(0);
+    su3_subgroup_hit<R, KIND, 0, 1>(U, A, lex, a, MU, 0, none, c);
+    su3_subgroup_hit<R, KIND, 0, 2>(U, A, lex, a, MU, 1, none, c);
+    su3_subgroup_hit<R, KIND, 1, 2>(U, A, lex, a, MU, 2, none, c);
   } else {
-    // one copy of the heatbath hit, on rows (0,1) of a permuted frame: (0,1,2) -> (0,2,1) -> (1,2,0)   (reading R3)
+    auto first_draw = [&](int sg) {
+      HbDraw<R> d;
+      if constexpr (PRE) {
+        const R* o = draws + sg * 5 * B;
+        d.E = o[0]; d.w = o[B]; d.n1 = o[2 * B]; d.n2 = o[3 * B]; d.n3 = o[4 * B];
+      } else {
+        d = hb_first_draw<R>(lex, a, MU, sg);
+      }
+      return d;
+    };
+    if constexpr (ROLL) {
+      // one copy of the heatbath hit, on rows (0,1) of a permuted frame: (0,1,2) -> (0,2,1) -> (1,2,0)   (reading R3)
 #pragma unroll 1
-    for (int sg = 0; sg < 3; ++sg) {
-      int c;
-      su3_subgroup_hit<R, KIND, 0, 1>(U, A, lex, a, MU, sg, c);
-      if (a.trials) a.trials[(size_t)lex * 3 + sg] = (uint8_t)c;
-      if (sg == 0) su3_swap_frame<R, 1, 2>(U, A);
-      else if (sg == 1) su3_swap_frame<R, 0, 2>(U, A);
-    }
-    // frame (1,2,0) back to (0,1,2): row 0 <- cur 2, row 1 <- cur 0, row 2 <- cur 1
+      for (int sg = 0; sg < 3; ++sg) {
+        int c;
+        su3_subgroup_hit<R, KIND, 0, 1>(U, A, lex, a, MU, sg, first_draw(sg), c);
+        if (a.trials) a.trials[(size_t)lex * 3 + sg] = (uint8_t)c;
+        if (sg == 0) su3_swap_frame<R, 1, 2>(U, A);
+        else if (sg == 1) su3_swap_frame<R, 0, 2>(U, A);
+      }
+      // frame (1,2,0) back to (0,1,2): row 0 <- cur 2, row 1 <- cur 0, row 2 <- cur 1
 #pragma unroll
-    for (int c = 0; c < 3; ++c) { const Cx<R> t = U.e[2][c]; U.e[2][c] = U.e[1][c]; U.e[1][c] = U.e[0][c]; U.e[0][c] = t; }
+      for (int c = 0; c < 3; ++c) { const Cx<R> t = U.e[2][c]; U.e[2][c] = U.e[1][c]; U.e[1][c] = U.e[0][c]; U.e[0][c] = t; }
+    } else {
+      int c0, c1, c2;
+      su3_subgroup_hit<R, KIND, 0, 1>(U, A, lex, a, MU, 0, first_draw(0), c0);
+      su3_subgroup_hit<R, KIND, 0, 2>(U, A, lex, a, MU, 1, first_draw(1), c1);
+      su3_subgroup_hit<R, KIND, 1, 2>(U, A, lex, a, MU, 2, first_draw(2), c2);
+      if (a.trials) {
+        a.trials[(size_t)lex * 3 + 0] = (uint8_t)c0; a.trials[(size_t)lex * 3 + 1] = (uint8_t)c1; a.trials[(size_t)lex * 3 + 2] = (uint8_t)c2;
+      }
+    }
   }
   m3_reunitarise(U);
 
@@ -450,7 +531,10 @@ su2_update_kernel(Geom g, typename PlaneTraits<R, 4>::Vec* links, UpdateArgs a) 
   int code = 0;
   if (!(k2 < Tiny<R>::k2())) {
     Q4<R> qa;
-    if (subgroup_quaternion<R, KIND, 2>(v, k2, lex, a, mu, 0, qa, code)) U = q4_mul(qa, U);
+    HbDraw<R> d0;
+    if (KIND == 0) d0 = hb_first_draw<R>(lex, a, mu, 0);
+    else d0.E = d0.w = d0.n1 = d0.n2 = d0.n3 = R(0);
+    if (subgroup_quaternion<R, KIND, 2>(v, k2, lex, a, mu, 0, d0, qa, code)) U = q4_mul(qa, U);
   }
   const R n = q_rsqrt(U.a0 * U.a0 + U.a1 * U.a1 + U.a2 * U.a2 + U.a3 * U.a3);
   R r[4] = {U.a0 * n, U.a1 * n, U.a2 * n, U.a3 * n};
