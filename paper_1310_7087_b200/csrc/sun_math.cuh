@@ -28,6 +28,57 @@ template <typename R> __device__ __forceinline__ Cx<R> cmul(const Cx<R>& a, cons
   return cx<R>(a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re);
 }
 
+// ---- complex dot products, the unit every 3x3 product here is made of
+//   cdot3<MODE>(acc, a0,a1,a2, b0,b1,b2):  acc += sum_k op(a_k, b_k),   NN: a*b   ND: a*conj(b)   DN: conj(a)*b
+//   cdot2<MODE>: the same over two terms, result returned (not accumulated)
+enum { CD_NN = 0, CD_ND = 1, CD_DN = 2 };
+template <int MODE, typename R>
+__device__ __forceinline__ void cdot3(Cx<R>& acc, const Cx<R>& a0, const Cx<R>& a1, const Cx<R>& a2, const Cx<R>& b0, const Cx<R>& b1,
+                                      const Cx<R>& b2) {
+  if (MODE == CD_NN) { cmad(acc, a0, b0); cmad(acc, a1, b1); cmad(acc, a2, b2); }
+  else if (MODE == CD_ND) { cmad_conj(acc, a0, b0); cmad_conj(acc, a1, b1); cmad_conj(acc, a2, b2); }
+  else { cmad_conja(acc, a0, b0); cmad_conja(acc, a1, b1); cmad_conja(acc, a2, b2); }
+}
+template <typename R> __device__ __forceinline__ Cx<R> cdot2_nn(const Cx<R>& a0, const Cx<R>& a1, const Cx<R>& b0, const Cx<R>& b1) {
+  Cx<R> r = cmul(a0, b0);
+  cmad(r, a1, b1);
+  return r;
+}
+
+// fp32: the packed FP32x2 pipe of sm_100 (FFMA2 / FMUL2 work on an aligned register pair; ptxas folds the scalar broadcast
+// (a.re, a.re) and the swap (b.im, b.re) into operand modifiers, but not a sign on one half).  So the real-part and
+// imaginary-part coefficients are summed in two packed accumulators
+//     T1 = sum_k a_k.re * (b_k.re, b_k.im)        T2 = sum_k a_k.im * (b_k.im, b_k.re)
+// and the signs are applied once per dot product:  NN (T1.x - T2.x, T1.y + T2.y)   ND (T1.x + T2.x, T2.y - T1.y)
+// DN (T1.x + T2.x, T1.y - T2.y):  8 issue slots per 3-term dot product instead of 12.
+#ifndef QCD_NO_FFMA2
+__device__ __forceinline__ float2 f2_bcast(float x) { return make_float2(x, x); }
+__device__ __forceinline__ float2 f2_of(const Cx<float>& c) { return make_float2(c.re, c.im); }
+__device__ __forceinline__ float2 f2_swap(const Cx<float>& c) { return make_float2(c.im, c.re); }
+template <int MODE>
+__device__ __forceinline__ void cdot3(Cx<float>& acc, const Cx<float>& a0, const Cx<float>& a1, const Cx<float>& a2, const Cx<float>& b0,
+                                      const Cx<float>& b1, const Cx<float>& b2) {
+  float2 t1 = make_float2(acc.re, MODE == CD_ND ? -acc.im : acc.im);
+  t1 = __ffma2_rn(f2_bcast(a0.re), f2_of(b0), t1);
+  t1 = __ffma2_rn(f2_bcast(a1.re), f2_of(b1), t1);
+  t1 = __ffma2_rn(f2_bcast(a2.re), f2_of(b2), t1);
+  float2 t2 = __fmul2_rn(f2_bcast(a0.im), f2_swap(b0));
+  t2 = __ffma2_rn(f2_bcast(a1.im), f2_swap(b1), t2);
+  t2 = __ffma2_rn(f2_bcast(a2.im), f2_swap(b2), t2);
+  if (MODE == CD_NN) { acc.re = t1.x - t2.x; acc.im = t1.y + t2.y; }
+  else if (MODE == CD_ND) { acc.re = t1.x + t2.x; acc.im = t2.y - t1.y; }
+  else { acc.re = t1.x + t2.x; acc.im = t1.y - t2.y; }
+}
+__device__ __forceinline__ Cx<float> cdot2_nn(const Cx<float>& a0, const Cx<float>& a1, const Cx<float>& b0, const Cx<float>& b1) {
+  float2 t1 = __fmul2_rn(f2_bcast(a0.re), f2_of(b0));
+  t1 = __ffma2_rn(f2_bcast(a1.re), f2_of(b1), t1);
+  float2 t2 = __fmul2_rn(f2_bcast(a0.im), f2_swap(b0));
+  t2 = __ffma2_rn(f2_bcast(a1.im), f2_swap(b1), t2);
+  Cx<float> r; r.re = t1.x - t2.x; r.im = t1.y + t2.y;
+  return r;
+}
+#endif
+
 template <typename R> struct M3 { Cx<R> e[3][3]; };
 
 // row 2 = conj(row0 x row1)   (valid for SU(3): third-row reconstruction of the 12-real compression)
@@ -42,14 +93,30 @@ template <typename R> __device__ __forceinline__ void m3_complete_row2(M3<R>& a)
   }
 }
 
+#ifndef QCD_NO_FFMA2
+// fp32: each component conj(p*q - r*s) as two packed accumulators, 6 issue slots instead of 8
+__device__ __forceinline__ void m3_complete_row2(M3<float>& a) {
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    const int c1 = (c + 1) % 3, c2 = (c + 2) % 3;
+    const Cx<float>&p = a.e[0][c1], &q = a.e[1][c2], &r = a.e[0][c2], &s = a.e[1][c1];
+    float2 t1 = __fmul2_rn(f2_bcast(p.re), f2_of(q));
+    t1 = __ffma2_rn(f2_bcast(-r.re), f2_of(s), t1);
+    float2 t2 = __fmul2_rn(f2_bcast(p.im), f2_swap(q));
+    t2 = __ffma2_rn(f2_bcast(-r.im), f2_swap(s), t2);
+    a.e[2][c].re = t1.x - t2.x;
+    a.e[2][c].im = -(t1.y + t2.y);
+  }
+}
+#endif
+
 // rows [0,NR) of  acc += a*b
 template <typename R, int NR> __device__ __forceinline__ void m3_mad_nn(M3<R>& acc, const M3<R>& a, const M3<R>& b) {
 #pragma unroll
   for (int i = 0; i < NR; ++i)
 #pragma unroll
     for (int j = 0; j < 3; ++j)
-#pragma unroll
-      for (int k = 0; k < 3; ++k) cmad(acc.e[i][j], a.e[i][k], b.e[k][j]);
+      cdot3<CD_NN>(acc.e[i][j], a.e[i][0], a.e[i][1], a.e[i][2], b.e[0][j], b.e[1][j], b.e[2][j]);
 }
 // rows [0,NR) of acc += a * b^dagger      (needs rows [0,NR) of a and ALL rows of b)
 template <typename R, int NR> __device__ __forceinline__ void m3_mad_nd(M3<R>& acc, const M3<R>& a, const M3<R>& b) {
@@ -57,8 +124,7 @@ template <typename R, int NR> __device__ __forceinline__ void m3_mad_nd(M3<R>& a
   for (int i = 0; i < NR; ++i)
 #pragma unroll
     for (int j = 0; j < 3; ++j)
-#pragma unroll
-      for (int k = 0; k < 3; ++k) cmad_conj(acc.e[i][j], a.e[i][k], b.e[j][k]);
+      cdot3<CD_ND>(acc.e[i][j], a.e[i][0], a.e[i][1], a.e[i][2], b.e[j][0], b.e[j][1], b.e[j][2]);
 }
 // rows [0,NR) of acc += a^dagger * b      (needs ALL rows of a and b)
 template <typename R, int NR> __device__ __forceinline__ void m3_mad_dn(M3<R>& acc, const M3<R>& a, const M3<R>& b) {
@@ -66,8 +132,7 @@ template <typename R, int NR> __device__ __forceinline__ void m3_mad_dn(M3<R>& a
   for (int i = 0; i < NR; ++i)
 #pragma unroll
     for (int j = 0; j < 3; ++j)
-#pragma unroll
-      for (int k = 0; k < 3; ++k) cmad_conja(acc.e[i][j], a.e[k][i], b.e[k][j]);
+      cdot3<CD_DN>(acc.e[i][j], a.e[0][i], a.e[1][i], a.e[2][i], b.e[0][j], b.e[1][j], b.e[2][j]);
 }
 template <typename R> __device__ __forceinline__ void m3_zero(M3<R>& a) {
 #pragma unroll

@@ -192,11 +192,10 @@ template <typename R, int KIND, int I, int J>
 __device__ __forceinline__ void su3_subgroup_hit(M3<R>& U, const M3<R>& A, uint32_t lex, const UpdateArgs& a, int mu, int sg,
                                                  const HbDraw<R>& d0, int& code) {
   Cx<R> wii = cx<R>(0, 0), wij = cx<R>(0, 0), wji = cx<R>(0, 0), wjj = cx<R>(0, 0);
-#pragma unroll
-  for (int k = 0; k < 3; ++k) {
-    cmad(wii, U.e[I][k], A.e[k][I]); cmad(wij, U.e[I][k], A.e[k][J]);
-    cmad(wji, U.e[J][k], A.e[k][I]); cmad(wjj, U.e[J][k], A.e[k][J]);
-  }
+  cdot3<CD_NN>(wii, U.e[I][0], U.e[I][1], U.e[I][2], A.e[0][I], A.e[1][I], A.e[2][I]);
+  cdot3<CD_NN>(wij, U.e[I][0], U.e[I][1], U.e[I][2], A.e[0][J], A.e[1][J], A.e[2][J]);
+  cdot3<CD_NN>(wji, U.e[J][0], U.e[J][1], U.e[J][2], A.e[0][I], A.e[1][I], A.e[2][I]);
+  cdot3<CD_NN>(wjj, U.e[J][0], U.e[J][1], U.e[J][2], A.e[0][J], A.e[1][J], A.e[2][J]);
   Q4<R> v;
   v.a0 = R(0.5) * (wii.re + wjj.re);
   v.a1 = R(0.5) * (wij.im + wji.im);
@@ -211,9 +210,8 @@ __device__ __forceinline__ void su3_subgroup_hit(M3<R>& U, const M3<R>& A, uint3
 #pragma unroll
   for (int c = 0; c < 3; ++c) {
     const Cx<R> ui = U.e[I][c], uj = U.e[J][c];
-    Cx<R> ni = cmul(aii, ui); cmad(ni, aij, uj);
-    Cx<R> nj = cmul(aji, ui); cmad(nj, ajj, uj);
-    U.e[I][c] = ni; U.e[J][c] = nj;
+    U.e[I][c] = cdot2_nn(aii, aij, ui, uj);
+    U.e[J][c] = cdot2_nn(aji, ajj, ui, uj);
   }
 }
 
@@ -234,6 +232,17 @@ template <typename R> __device__ __forceinline__ void su3_scale_rows(M3<R>& m, c
     for (int j = 0; j < 3; ++j) m.e[r][j] = cmul(m.e[r][j], ph);
   }
 }
+#ifndef QCD_NO_FFMA2
+__device__ __forceinline__ void m3_add(M3<float>& a, const M3<float>& s) {
+#pragma unroll
+  for (int r = 0; r < 3; ++r)
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const float2 v = __fadd2_rn(f2_of(a.e[r][c]), f2_of(s.e[r][c]));
+      a.e[r][c].re = v.x; a.e[r][c].im = v.y;
+    }
+}
+#endif
 template <typename R> __device__ __forceinline__ void m3_add(M3<R>& a, const M3<R>& s) {
 #pragma unroll
   for (int r = 0; r < 3; ++r)
