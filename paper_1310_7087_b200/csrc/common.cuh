@@ -56,6 +56,35 @@ __device__ __forceinline__ SiteCoord decode_site(const Geom& g, uint32_t h, int 
   return c;
 }
 
+// ------------------------------------------------------------------ CTA tile mapping
+// A CTA's threads can cover a 4-D box of sites (power-of-two extents e_d = 1 << s_d, e_0 counted in half-indices) instead of
+// B consecutive half-indices, so that the links one thread reads as a neighbour are the links another thread of the CTA
+// reads too (they then hit in L1 / are fetched once) -- DESIGN.md "Tile mapping".
+struct TileMap {
+  int on;              // 0: linear mapping h = blockIdx.x * B + threadIdx.x
+  int s0, s1, s2;      // log2 of the tile extents in directions 0 (half-indices), 1, 2; direction 3 takes the rest of B
+  FastDiv n0, n1, n2;  // tiles per direction 0, 1, 2
+};
+__device__ __forceinline__ SiteCoord decode_site_tiled(const Geom& g, const TileMap& tm, int parity, uint32_t& h) {
+  uint32_t t = threadIdx.x;
+  const uint32_t jl = t & ((1u << tm.s0) - 1u); t >>= tm.s0;
+  const uint32_t y1 = t & ((1u << tm.s1) - 1u); t >>= tm.s1;
+  const uint32_t y2 = t & ((1u << tm.s2) - 1u); t >>= tm.s2;
+  uint32_t b = blockIdx.x;
+  uint32_t q = fd_div(b, tm.n0); const uint32_t b0 = b - q * tm.n0.d; b = q;
+  q = fd_div(b, tm.n1); const uint32_t b1 = b - q * tm.n1.d; b = q;
+  q = fd_div(b, tm.n2); const uint32_t b2 = b - q * tm.n2.d; const uint32_t b3 = q;
+  SiteCoord c;
+  c.j = (int)((b0 << tm.s0) + jl);
+  c.x1 = (int)((b1 << tm.s1) + y1);
+  c.x2 = (int)((b2 << tm.s2) + y2);
+  const int s3 = 31 - __clz((int)blockDim.x) - tm.s0 - tm.s1 - tm.s2;
+  c.x3 = (int)((b3 << s3) + t);
+  c.s = (parity + c.x1 + c.x2 + c.x3) & 1;
+  h = (uint32_t)(((c.x3 * g.L[2] + c.x2) * g.L[1] + c.x1) * g.Lh0 + c.j);
+  return c;
+}
+
 // half-index offsets to the +d / -d neighbour (which has the other parity).  d is warp-uniform.
 __device__ __forceinline__ void nbr_offsets(const Geom& g, const SiteCoord& c, int d, int& fwd, int& bwd) {
   if (d == 0) {

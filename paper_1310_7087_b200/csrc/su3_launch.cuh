@@ -1,5 +1,9 @@
 // su3_launch.cuh -- host-side selection of the SU(3) update kernel instantiation and its ring geometry.
 #pragma once
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+
 #include "launch.h"
 
 namespace qcd {
@@ -70,6 +74,40 @@ template <> struct RingCfg<float, false> : RingShape<QCD_F32X18_B, QCD_F32X18_K,
 template <> struct RingCfg<double, true> : RingShape<QCD_F64X12_B, QCD_F64X12_K, QCD_F64X12_MINB> {};
 template <> struct RingCfg<double, false> : RingShape<QCD_F64X18_B, QCD_F64X18_K, QCD_F64X18_MINB> {};
 
+// Tile of B threads: e0 half-indices along x0, then powers of two along x1, x2, (x3); every extent must divide the lattice.
+// QCD_TILE="s0,s1,s2" (log2 extents) overrides the default choice; QCD_TILE=off selects the linear mapping.
+static inline TileMap choose_tile(const Geom& g, int B) {
+  TileMap tm;
+  memset(&tm, 0, sizeof(tm));
+  if (g.D != 4 || (B & (B - 1))) return tm;
+  int lb = 0;
+  while ((1 << lb) < B) ++lb;
+  auto pow2_part = [](int x) { int s = 0; while (!(x & 1)) { x >>= 1; ++s; } return s; };
+  const int m[4] = {pow2_part(g.Lh0), pow2_part(g.L[1]), pow2_part(g.L[2]), pow2_part(g.L[3])};
+  int s[4] = {0, 0, 0, 0};
+  const char* env = getenv("QCD_TILE");
+  if (env && !strcmp(env, "off")) return tm;
+  if (env && sscanf(env, "%d,%d,%d", &s[0], &s[1], &s[2]) == 3) {
+    s[3] = lb - s[0] - s[1] - s[2];
+  } else {
+    // default: 8 half-indices along x0 (one 128-byte line of 16-byte vectors), the rest spread over x1, x2, x3
+    s[0] = m[0] < 3 ? m[0] : 3;
+    int left = lb - s[0];
+    for (int d = 1; left > 0; d = d % 3 + 1) {
+      bool any = false;
+      for (int k = 1; k < 4; ++k) any = any || s[k] < m[k];
+      if (!any) break;
+      if (s[d] < m[d]) { ++s[d]; --left; }
+    }
+    if (left > 0) { s[0] += left; }
+  }
+  for (int d = 0; d < 4; ++d) if (s[d] < 0 || s[d] > m[d]) return tm;      // does not tile this lattice: linear mapping
+  if (s[0] + s[1] + s[2] + s[3] != lb) return tm;
+  tm.on = 1; tm.s0 = s[0]; tm.s1 = s[1]; tm.s2 = s[2];
+  tm.n0 = make_fastdiv((uint32_t)(g.Lh0 >> s[0])); tm.n1 = make_fastdiv((uint32_t)(g.L[1] >> s[1])); tm.n2 = make_fastdiv((uint32_t)(g.L[2] >> s[2]));
+  return tm;
+}
+
 template <typename R, int D, int MU, bool COMP, int KIND, bool FIELD>
 static cudaError_t su3_go(const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st) {
   typedef PlaneTraits<R, (COMP ? 12 : 18)> T;
@@ -88,7 +126,9 @@ static cudaError_t su3_go(const Geom& g, void* links, const UpdateArgs& a, cudaS
     attr_dev = dev;
   }
   const unsigned grid = (g.Vh + B - 1) / B;
-  kern<<<grid, B, smem, st>>>(g, (Vec*)links, a);
+  UpdateArgs a2 = a;
+  a2.tm = choose_tile(g, B);
+  kern<<<grid, B, smem, st>>>(g, (Vec*)links, a2);
   return cudaGetLastError();
 }
 template <typename R, int D, int MU, bool COMP>

@@ -110,30 +110,72 @@ __device__ __forceinline__ void m3_complete_row2(M3<float>& a) {
 }
 #endif
 
-// rows [0,NR) of  acc += a*b
-template <typename R, int NR> __device__ __forceinline__ void m3_mad_nn(M3<R>& acc, const M3<R>& a, const M3<R>& b) {
+// The three product shapes, rows [0,NR) of acc += op(a) op(b), written as outer-product accumulation over k: the six
+// consecutive multiply-adds that follow share the scalar a.re (then a.im) in the same operand slot, which lets the
+// register-operand reuse cache serve it (the FP32 pipe is bounded by register-file reads).
+//   SA, SB select the element of a / b:  nn: a[i][k] b[k][j]   nd: a[i][k] conj(b[j][k])   dn: conj(a[k][i]) b[k][j]
+template <int NR, int MODE, typename R> __device__ __forceinline__ void m3_mad(M3<R>& acc, const M3<R>& a, const M3<R>& b) {
+#pragma unroll
+  for (int k = 0; k < 3; ++k)
+#pragma unroll
+    for (int i = 0; i < NR; ++i) {
+      const Cx<R> x = (MODE == CD_DN) ? a.e[k][i] : a.e[i][k];
+      const R are = x.re, aim = (MODE == CD_DN) ? -x.im : x.im;
+#pragma unroll
+      for (int j = 0; j < 3; ++j) {
+        const Cx<R> y = (MODE == CD_ND) ? b.e[j][k] : b.e[k][j];
+        const R bim = (MODE == CD_ND) ? -y.im : y.im;
+        acc.e[i][j].re = q_fma(are, y.re, acc.e[i][j].re);
+        acc.e[i][j].im = q_fma(are, bim, acc.e[i][j].im);
+      }
+#pragma unroll
+      for (int j = 0; j < 3; ++j) {
+        const Cx<R> y = (MODE == CD_ND) ? b.e[j][k] : b.e[k][j];
+        const R bim = (MODE == CD_ND) ? -y.im : y.im;
+        acc.e[i][j].re = q_fma(-aim, bim, acc.e[i][j].re);
+        acc.e[i][j].im = q_fma(aim, y.re, acc.e[i][j].im);
+      }
+    }
+}
+#if !defined(QCD_NO_FFMA2) && !defined(QCD_OUTER_SCALAR)
+// fp32 packed: per (i,j) two accumulators T1 += a.re * (b.re, b.im), T2 += a.im * (b.im, b.re), same k-outer order
+template <int NR, int MODE> __device__ __forceinline__ void m3_mad(M3<float>& acc, const M3<float>& a, const M3<float>& b) {
+  float2 t1[NR][3], t2[NR][3];
 #pragma unroll
   for (int i = 0; i < NR; ++i)
 #pragma unroll
-    for (int j = 0; j < 3; ++j)
-      cdot3<CD_NN>(acc.e[i][j], a.e[i][0], a.e[i][1], a.e[i][2], b.e[0][j], b.e[1][j], b.e[2][j]);
+    for (int j = 0; j < 3; ++j) t1[i][j] = make_float2(acc.e[i][j].re, MODE == CD_ND ? -acc.e[i][j].im : acc.e[i][j].im);
+#pragma unroll
+  for (int k = 0; k < 3; ++k)
+#pragma unroll
+    for (int i = 0; i < NR; ++i) {
+      const Cx<float> x = (MODE == CD_DN) ? a.e[k][i] : a.e[i][k];
+#pragma unroll
+      for (int j = 0; j < 3; ++j) {
+        const Cx<float> y = (MODE == CD_ND) ? b.e[j][k] : b.e[k][j];
+        t1[i][j] = __ffma2_rn(f2_bcast(x.re), f2_of(y), t1[i][j]);
+      }
+#pragma unroll
+      for (int j = 0; j < 3; ++j) {
+        const Cx<float> y = (MODE == CD_ND) ? b.e[j][k] : b.e[k][j];
+        t2[i][j] = (k == 0) ? __fmul2_rn(f2_bcast(x.im), f2_swap(y)) : __ffma2_rn(f2_bcast(x.im), f2_swap(y), t2[i][j]);
+      }
+    }
+#pragma unroll
+  for (int i = 0; i < NR; ++i)
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+      if (MODE == CD_NN) { acc.e[i][j].re = t1[i][j].x - t2[i][j].x; acc.e[i][j].im = t1[i][j].y + t2[i][j].y; }
+      else if (MODE == CD_ND) { acc.e[i][j].re = t1[i][j].x + t2[i][j].x; acc.e[i][j].im = t2[i][j].y - t1[i][j].y; }
+      else { acc.e[i][j].re = t1[i][j].x + t2[i][j].x; acc.e[i][j].im = t1[i][j].y - t2[i][j].y; }
+    }
 }
+#endif
+template <typename R, int NR> __device__ __forceinline__ void m3_mad_nn(M3<R>& acc, const M3<R>& a, const M3<R>& b) { m3_mad<NR, CD_NN>(acc, a, b); }
 // rows [0,NR) of acc += a * b^dagger      (needs rows [0,NR) of a and ALL rows of b)
-template <typename R, int NR> __device__ __forceinline__ void m3_mad_nd(M3<R>& acc, const M3<R>& a, const M3<R>& b) {
-#pragma unroll
-  for (int i = 0; i < NR; ++i)
-#pragma unroll
-    for (int j = 0; j < 3; ++j)
-      cdot3<CD_ND>(acc.e[i][j], a.e[i][0], a.e[i][1], a.e[i][2], b.e[j][0], b.e[j][1], b.e[j][2]);
-}
+template <typename R, int NR> __device__ __forceinline__ void m3_mad_nd(M3<R>& acc, const M3<R>& a, const M3<R>& b) { m3_mad<NR, CD_ND>(acc, a, b); }
 // rows [0,NR) of acc += a^dagger * b      (needs ALL rows of a and b)
-template <typename R, int NR> __device__ __forceinline__ void m3_mad_dn(M3<R>& acc, const M3<R>& a, const M3<R>& b) {
-#pragma unroll
-  for (int i = 0; i < NR; ++i)
-#pragma unroll
-    for (int j = 0; j < 3; ++j)
-      cdot3<CD_DN>(acc.e[i][j], a.e[0][i], a.e[1][i], a.e[2][i], b.e[0][j], b.e[1][j], b.e[2][j]);
-}
+template <typename R, int NR> __device__ __forceinline__ void m3_mad_dn(M3<R>& acc, const M3<R>& a, const M3<R>& b) { m3_mad<NR, CD_DN>(acc, a, b); }
 template <typename R> __device__ __forceinline__ void m3_zero(M3<R>& a) {
 #pragma unroll
   for (int i = 0; i < 3; ++i)

@@ -31,6 +31,7 @@ struct UpdateArgs {
   int parity, mu, hit, max_trials;
   uint32_t sweep, key0, key1;
   uint8_t* trials;   // NULL or [lex][3] debug trial codes
+  TileMap tm;        // thread -> site mapping of the SU(3) kernels (set by the launcher)
   FieldArgs f;
 };
 
@@ -282,10 +283,16 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
   extern __shared__ __align__(16) unsigned char ring_raw[];
   Vec* ring = reinterpret_cast<Vec*>(ring_raw) + threadIdx.x;      // [slot][plane][B], this thread's column
 
-  const uint32_t h = blockIdx.x * B + threadIdx.x;
-  if (h >= g.Vh) return;                                           // no block barrier anywhere below
   const int p = a.parity;
-  const SiteCoord sc = decode_site(g, h, p);
+  uint32_t h;
+  SiteCoord sc;
+  if (a.tm.on) {
+    sc = decode_site_tiled(g, a.tm, p, h);                         // the tiles cover the lattice exactly
+  } else {
+    h = blockIdx.x * B + threadIdx.x;
+    if (h >= g.Vh) return;                                         // no block barrier anywhere below
+    sc = decode_site(g, h, p);
+  }
   int fo[D], bo[D];
 #pragma unroll
   for (int d = 0; d < D; ++d) nbr_offsets(g, sc, d, fo[d], bo[d]);
@@ -317,6 +324,9 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
   };
   auto issue = [&](auto jc, const Dir& d) {                         // cp.async link j into ring slot j % K
     constexpr int J = decltype(jc)::value;
+#ifdef QCD_EXP_NOLOAD
+    return;
+#endif
     const Vec* src = links + link_idx(jc, d);
     Vec* dst = ring + (J % KR) * NP * B;
 #pragma unroll
@@ -325,6 +335,12 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
   auto fetch = [&](auto jc, const Dir& d, M3<R>& u, bool row2) {
     constexpr int J = decltype(jc)::value;
     R r[NREAL];
+#ifdef QCD_EXP_NOLOAD
+    if (true) {
+#pragma unroll
+      for (int k = 0; k < NREAL; ++k) r[k] = (R)((h + J) & 7u) * R(0.01) + R(0.1) * (R)k + (R)d.f * R(1e-9);
+    } else
+#endif
     if constexpr (K > 0) {
       const Vec* src = ring + (J % KR) * NP * B;
 #pragma unroll
@@ -377,6 +393,15 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
         cp_async_commit();                                         // one group per step, possibly empty
         cp_async_wait<KR - 1>();                                   // link (i, J) has landed
       }
+#ifdef QCD_EXP_NOCOMPUTE
+      if (true) {
+        M3<R> Ux;
+        m3_zero(Ux);
+        fetch(jc, cur, Ux, false);
+        m3_add(A, Ux);
+        return;
+      }
+#endif
       if constexpr (J == 0) {
         fetch(jc, cur, P, true);                                   // U2, all rows
       } else if constexpr (J == 1) {
@@ -436,6 +461,14 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
   M3<R> U;
   fetch(std::integral_constant<int, 6>{}, cur, U, true);
 
+#if defined(QCD_EXP_NOCOMPUTE) || defined(QCD_EXP_NOHIT)
+  if (true) {
+#pragma unroll
+    for (int r = 0; r < 3; ++r)
+#pragma unroll
+      for (int c = 0; c < 3; ++c) { U.e[r][c].re += R(1e-30) * A.e[r][c].re; U.e[r][c].im += R(1e-30) * A.e[r][c].im; }
+  } else
+#endif
   if constexpr (KIND == 1) {
     int c;
     HbDraw<R> none;
@@ -477,7 +510,9 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
       }
     }
   }
+#ifndef QCD_EXP_NOHIT
   m3_reunitarise(U);
+#endif
 
   R r[NREAL];
   m3_to_reals<R, NREAL>(U, r);
