@@ -145,6 +145,35 @@ __device__ __forceinline__ void store_reals(typename PlaneTraits<R, NREAL>::Vec*
   }
 }
 
+// ------------------------------------------------------------------ programmatic dependent launch
+// The sub-steps of a sweep are a chain of dependent kernels on one stream.  Each update kernel is launched with the
+// programmatic-stream-serialization attribute: its CTAs may become resident while the previous kernel drains, run the part
+// that does not touch the links (site decoding, neighbour offsets, the heatbath's random numbers) and then block in
+// pdl_wait() until the previous grid has completed and its stores are visible.  pdl_trigger() at the top of a kernel lets
+// the next one do the same.  Without the attribute both are no-ops.
+#ifndef QCD_NO_PDL
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+#else
+__device__ __forceinline__ void pdl_trigger() {}
+__device__ __forceinline__ void pdl_wait() {}
+#endif
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+  cudaLaunchConfig_t cfg;
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+#ifndef QCD_NO_PDL
+  cfg.numAttrs = 1;
+#else
+  cfg.numAttrs = 0;
+#endif
+  return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+
 // ------------------------------------------------------------------ math dispatch
 __device__ __forceinline__ float q_rsqrt(float x) { return rsqrtf(x); }
 __device__ __forceinline__ double q_rsqrt(double x) { return rsqrt(x); }

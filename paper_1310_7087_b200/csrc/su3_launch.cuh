@@ -39,18 +39,21 @@ namespace qcd {
 #define QCD_F64X12_MINB 1
 #endif
 #ifndef QCD_F64X18_B
-#define QCD_F64X18_B 64
+#define QCD_F64X18_B 128
 #endif
 #ifndef QCD_F64X18_K
-#define QCD_F64X18_K 6
+#define QCD_F64X18_K 3
 #endif
 #ifndef QCD_F64X18_MINB
-#define QCD_F64X18_MINB 1
+#define QCD_F64X18_MINB 3
 #endif
 // Loop shape per precision and kind (measured at 32^4, see profiles/): ROLL = keep the direction / subgroup loops rolled,
 // PRE = heatbath random part of trial 0 precomputed into shared memory.
-#ifndef QCD_F32_ROLL
-#define QCD_F32_ROLL true
+#ifndef QCD_F32_ROLL_HB
+#define QCD_F32_ROLL_HB true
+#endif
+#ifndef QCD_F32_ROLL_OR
+#define QCD_F32_ROLL_OR false
 #endif
 #ifndef QCD_F32_PRE
 #define QCD_F32_PRE true
@@ -65,7 +68,7 @@ namespace qcd {
 #define QCD_F64_PRE false
 #endif
 template <typename R, int KIND> struct LoopCfg;
-template <int KIND> struct LoopCfg<float, KIND> { static constexpr bool ROLL = QCD_F32_ROLL, PRE = QCD_F32_PRE; };
+template <int KIND> struct LoopCfg<float, KIND> { static constexpr bool ROLL = (KIND == 0) ? QCD_F32_ROLL_HB : QCD_F32_ROLL_OR, PRE = QCD_F32_PRE; };
 template <int KIND> struct LoopCfg<double, KIND> { static constexpr bool ROLL = (KIND == 0) ? QCD_F64_ROLL_HB : QCD_F64_ROLL_OR, PRE = QCD_F64_PRE; };
 template <int B_, int K_, int MINB_> struct RingShape { static constexpr int B = B_, K = K_, MINB = MINB_; };
 template <typename R, bool COMP> struct RingCfg;
@@ -128,8 +131,7 @@ static cudaError_t su3_go(const Geom& g, void* links, const UpdateArgs& a, cudaS
   const unsigned grid = (g.Vh + B - 1) / B;
   UpdateArgs a2 = a;
   a2.tm = choose_tile(g, B);
-  kern<<<grid, B, smem, st>>>(g, (Vec*)links, a2);
-  return cudaGetLastError();
+  return launch_pdl(kern, dim3(grid), dim3(B), smem, st, g, (Vec*)links, a2);
 }
 template <typename R, int D, int MU, bool COMP>
 static cudaError_t su3_sel_kind(const UpdateSel& s, const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st) {

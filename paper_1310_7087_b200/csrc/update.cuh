@@ -282,6 +282,7 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
   constexpr int KR = K > 0 ? K : 1;
   extern __shared__ __align__(16) unsigned char ring_raw[];
   Vec* ring = reinterpret_cast<Vec*>(ring_raw) + threadIdx.x;      // [slot][plane][B], this thread's column
+  pdl_trigger();
 
   const int p = a.parity;
   uint32_t h;
@@ -355,14 +356,10 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
     if (COMP && row2) m3_complete_row2(u);
   };
 
-  Dir cur = make_dir(0);
-  if constexpr (K > 0) {                                           // prologue: links 0 .. K-2 of the first direction
-    static_for<0, KR - 1>([&](auto jc) { issue(jc, cur); cp_async_commit(); });
-  }
-
   const uint32_t lex = 2u * h + (uint32_t)sc.s;
-  // heatbath: the random-number-only part of trial 0 and the direction of each subgroup, computed while the first links
-  // are in flight and parked in shared memory behind the ring ([subgroup][5][B] reals, this thread's column)
+  // heatbath: the random-number-only part of trial 0 and the direction of each subgroup, parked in shared memory behind
+  // the ring ([subgroup][5][B] reals, this thread's column).  It does not touch the links, so it runs before pdl_wait():
+  // in the tail of the previous sub-step's kernel when this CTA became resident early.
   R* draws = reinterpret_cast<R*>(ring_raw + (size_t)K * NP * B * sizeof(Vec)) + threadIdx.x;
   if constexpr (KIND == 0 && PRE) {
 #pragma unroll 1
@@ -371,6 +368,12 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
       R* o = draws + sg * 5 * B;
       o[0] = d.E; o[B] = d.w; o[2 * B] = d.n1; o[3 * B] = d.n2; o[4 * B] = d.n3;
     }
+  }
+
+  pdl_wait();                                                      // the previous sub-step's links are complete and visible
+  Dir cur = make_dir(0);
+  if constexpr (K > 0) {                                           // prologue: links 0 .. K-2 of the first direction
+    static_for<0, KR - 1>([&](auto jc) { issue(jc, cur); cp_async_commit(); });
   }
 
   M3<R> A, P, Q;      // A: staple sum; P: the link kept for the next product (U2 / U1'); Q: X = U3 U2 or Y = U2' U1'
@@ -534,12 +537,14 @@ template <typename R, int D, int KIND, bool FIELD>
 __global__ void __launch_bounds__(256)
 su2_update_kernel(Geom g, typename PlaneTraits<R, 4>::Vec* links, UpdateArgs a) {
   typedef PlaneTraits<R, 4> T;
+  pdl_trigger();
   const uint32_t h = blockIdx.x * blockDim.x + threadIdx.x;
   if (h >= g.Vh) return;
   const int p = a.parity, mu = a.mu, q = 1 - p;
   const SiteCoord sc = decode_site(g, h, p);
   int fmu, bmu;
   nbr_offsets(g, sc, mu, fmu, bmu);
+  pdl_wait();
   const typename T::Vec* __restrict__ ro = links;
   Q4<R> A = q4<R>(0, 0, 0, 0);
 #pragma unroll

@@ -7,8 +7,7 @@ template <typename R, int D, int KIND, bool FIELD>
 static cudaError_t go(const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st) {
   typedef typename PlaneTraits<R, 4>::Vec Vec;
   const unsigned block = 256, grid = (g.Vh + block - 1) / block;
-  su2_update_kernel<R, D, KIND, FIELD><<<grid, block, 0, st>>>(g, (Vec*)links, a);
-  return cudaGetLastError();
+  return launch_pdl(su2_update_kernel<R, D, KIND, FIELD>, dim3(grid), dim3(block), 0, st, g, (Vec*)links, a);
 }
 template <typename R, int D>
 static cudaError_t sel2(const UpdateSel& s, const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st) {
