@@ -5,8 +5,42 @@
 #include <cstring>
 
 #include "launch.h"
+#include "update_tiled.cuh"
 
 namespace qcd {
+
+// Tiled kernel (update_tiled.cuh), D = 4 only: box of sites per CTA for direction mu (extent 0 in half-indices; default: 128
+// sites, extent 1 in direction mu where the box has no faces; one hex digit per extent), ring slots per thread, CTAs per SM the register allocation
+// must allow.  QCD_TILED=0 in the environment, or a lattice the box does not divide, selects the ring kernel of update.cuh.
+#ifndef QCD_TILE_MU0
+#define QCD_TILE_MU0 0x8441
+#endif
+#ifndef QCD_TILE_MU1
+#define QCD_TILE_MU1 0x8144
+#endif
+#ifndef QCD_TILE_MU2
+#define QCD_TILE_MU2 0x8414
+#endif
+#ifndef QCD_TILE_MU3
+#define QCD_TILE_MU3 0x8441
+#endif
+#ifndef QCD_TILE_F32X12_K
+#define QCD_TILE_F32X12_K 4
+#endif
+#ifndef QCD_TILE_F32X12_MINB
+#define QCD_TILE_F32X12_MINB 5
+#endif
+template <int X> struct TileHex { typedef TileDims<((X >> 12) & 15), ((X >> 8) & 15), ((X >> 4) & 15), (X & 15)> TD; };
+template <int MU> struct TileFor;
+template <> struct TileFor<0> { typedef TileHex<QCD_TILE_MU0>::TD TD; };
+template <> struct TileFor<1> { typedef TileHex<QCD_TILE_MU1>::TD TD; };
+template <> struct TileFor<2> { typedef TileHex<QCD_TILE_MU2>::TD TD; };
+template <> struct TileFor<3> { typedef TileHex<QCD_TILE_MU3>::TD TD; };
+// Measured at 32^4 (profiles/r1_c_tiling.md): the resident region pays only for fp32 x12 overrelaxation (sustained 52.0
+// vs 53.2 us); the fp64 kernels lose more from the occupancy the region costs (2 instead of 3 CTAs per SM) than they gain
+// from the lighter L2 traffic, and the heatbath kernels are bound by their random numbers.  Those keep the ring kernel.
+template <typename R, bool COMP, int KIND> struct TiledCfg { static constexpr bool ON = false; static constexpr int K = 2, MINB = 1; };
+template <> struct TiledCfg<float, true, 1> { static constexpr bool ON = true; static constexpr int K = QCD_TILE_F32X12_K, MINB = QCD_TILE_F32X12_MINB; };
 
 // Ring geometry per storage format: B threads per CTA, K link slots per thread (K-1 links in flight).
 // Shared memory per CTA = K * (bytes per link) * B; chosen so that several CTAs fit in the 227 KB of an SM.
@@ -111,10 +145,47 @@ static inline TileMap choose_tile(const Geom& g, int B) {
   return tm;
 }
 
+static inline bool tiled_enabled() {
+  static int on = -1;
+  if (on < 0) { const char* e = getenv("QCD_TILED"); on = (e && e[0] == '0') ? 0 : 1; }
+  return on != 0;
+}
+
+template <typename R, int MU, bool COMP, int KIND, bool FIELD>
+static cudaError_t su3_go_tiled(const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st) {
+  typedef PlaneTraits<R, (COMP ? 12 : 18)> T;
+  typedef typename T::Vec Vec;
+  typedef typename TileFor<MU>::TD TD;
+  constexpr int K = TiledCfg<R, COMP, KIND>::K, MINB = TiledCfg<R, COMP, KIND>::MINB;
+  constexpr bool ROLL = LoopCfg<R, KIND>::ROLL && (4 % K == 0);
+  constexpr size_t smem = (size_t)(TD::res_slots(MU) + K * TD::B) * T::NP * sizeof(Vec);
+  auto kern = su3_update_tiled_kernel<R, MU, COMP, KIND, FIELD, TD, K, MINB, ROLL>;
+  static int attr_dev = -1;
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (smem > 48 * 1024 && attr_dev != dev) {
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    attr_dev = dev;
+  }
+  UpdateArgs a2 = a;
+  memset(&a2.tm, 0, sizeof(a2.tm));
+  a2.tm.on = 1;
+  a2.tm.n0 = make_fastdiv((uint32_t)(g.Lh0 / TD::T0)); a2.tm.n1 = make_fastdiv((uint32_t)(g.L[1] / TD::T1));
+  a2.tm.n2 = make_fastdiv((uint32_t)(g.L[2] / TD::T2));
+  return launch_pdl(kern, dim3(g.Vh / TD::B), dim3(TD::B), smem, st, g, (Vec*)links, a2);
+}
+
 template <typename R, int D, int MU, bool COMP, int KIND, bool FIELD>
 static cudaError_t su3_go(const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st) {
   typedef PlaneTraits<R, (COMP ? 12 : 18)> T;
   typedef typename T::Vec Vec;
+  if constexpr (D == 4 && TiledCfg<R, COMP, KIND>::ON) {
+    typedef typename TileFor<MU>::TD TD;
+    if (tiled_enabled() && g.Lh0 % TD::T0 == 0 && g.L[1] % TD::T1 == 0 && g.L[2] % TD::T2 == 0 && g.L[3] % TD::T3 == 0)
+      return su3_go_tiled<R, MU, COMP, KIND, FIELD>(g, links, a, st);
+  }
   constexpr int B = RingCfg<R, COMP>::B, K = RingCfg<R, COMP>::K, MINB = RingCfg<R, COMP>::MINB;
   constexpr bool ROLL = LoopCfg<R, KIND>::ROLL, PRE = LoopCfg<R, KIND>::PRE;
   constexpr size_t smem = (size_t)K * T::NP * B * sizeof(Vec) + ((KIND == 0 && PRE) ? (size_t)15 * B * sizeof(R) : 0);

@@ -1,0 +1,290 @@
+// update_tiled.cuh -- the D = 4 SU(3) sub-step with the U_mu neighbourhood of a CTA resident in shared memory.
+//
+// Why (profiles/r1_c_*): with a private copy of its 19 links per thread (the cp.async ring of update.cuh) a launch pulls
+// 19 link-sizes per link-hit through the L2 -> SM crossbar although only 9 are compulsory from DRAM; at 32^4 that is
+// 478 MB (fp32 x12) / 1434 MB (fp64 x18) per launch, and the L2 slices deliver ~11-12 TB/s: the fp64 kernel sits on that
+// limit (load path alone 116 us) and the fp32 kernel's load path (44-51 us alone) is as long as its arithmetic.
+// The most re-used operand is U_mu on the other parity q = 1-p:  U_mu(y) is read by the six threads y -+ nu (nu != mu).
+// A CTA covers a box of T0 x T1 x T2 x T3 sites of parity p in (half-index j, x1, x2, x3) coordinates and stages the
+// box of U_mu^q plus its one-deep faces in the directions nu != mu ONCE (one __syncthreads per kernel); the staple
+// operands U_mu(x+nu), U_mu(x-nu) of all three directions are then read from there.  The other 12 neighbour links and
+// the own link keep going through the per-thread cp.async ring (latency-tolerant, no further barrier).
+// L2 -> SM traffic per link-hit: 13 + (1 + sum_{nu>=1} 2/T_nu + [mu != 0]/T0)  ~ 15.3 link-sizes instead of 19.
+// A step of +-1 in direction 0 moves the half-index j by s or s-1 (s = x0 & 1 of the site), so a row of the box needs
+// only ONE of its two j-faces; periodic wrap enters only the global address, slots are addressed box-relative.
+//
+// The arithmetic (products, Cabibbo-Marinari hits, reunitarisation) is the one of update.cuh and the links are consumed
+// in the same order; the two kernels agree to rounding (the compiler's FMA contraction may differ between them).
+#pragma once
+#include "update.cuh"
+
+namespace qcd {
+
+// Slots of the resident region (one plane): the box itself, then per direction d != mu the faces:
+//   d >= 1: low face (box coordinate -1) and high face (T_d), B / T_d slots each;  d = 0: one face, B / T0 slots.
+template <int T0_, int T1_, int T2_, int T3_> struct TileDims {
+  static constexpr int T0 = T0_, T1 = T1_, T2 = T2_, T3 = T3_, B = T0_ * T1_ * T2_ * T3_;
+  __host__ __device__ static constexpr int T(int d) { return d == 0 ? T0 : d == 1 ? T1 : d == 2 ? T2 : T3; }
+  __host__ __device__ static constexpr int face_slots(int d) { return d == 0 ? B / T0 : 2 * (B / T(d)); }
+  // first slot of the face(s) of direction d in a kernel of direction mu
+  __host__ __device__ static constexpr int face_base(int mu, int d) {
+    int o = B;
+    for (int k = 0; k < d; ++k) if (k != mu) o += face_slots(k);
+    return o;
+  }
+  __host__ __device__ static constexpr int res_slots(int mu) { return face_base(mu, 4); }
+};
+
+// K ring slots per thread (K-1 links in flight); the ring carries, per direction nu, the four links
+//   r=0  U3  = U_nu(x)      r=1  U1  = U_nu(x+mu)      r=2  U1' = U_nu(x+mu-nu)      r=3  U3' = U_nu(x-nu)
+// and last the own link; link n = 4 i + r goes to slot n % K (ROLL, the rolled loop over nu, needs K | 4).
+template <typename R, int MU, bool COMP, int KIND, bool FIELD, typename TD, int K, int MINB, bool ROLL>
+__global__ void __launch_bounds__(TD::B, MINB)
+su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links, UpdateArgs a) {
+  typedef PlaneTraits<R, (COMP ? 12 : 18)> T;
+  typedef typename T::Vec Vec;
+  constexpr int D = 4, NREAL = COMP ? 12 : 18, NP = T::NP, NR = COMP ? 2 : 3, B = TD::B, RES = TD::res_slots(MU);
+  static_assert(K >= 2 && K <= 5 && (!ROLL || 4 % K == 0), "ring slots");
+  extern __shared__ __align__(16) unsigned char tile_raw[];
+  Vec* const res = reinterpret_cast<Vec*>(tile_raw);                        // [plane][RES]
+  Vec* const ring = res + NP * RES + threadIdx.x;                            // [slot][plane][B], this thread's column
+  pdl_trigger();
+
+  // thread -> box-relative coordinates (c0 fastest), CTA -> box origin
+  const int p = a.parity;
+  int c[4];
+  {
+    uint32_t t = threadIdx.x;
+    c[0] = (int)(t % TD::T0); t /= TD::T0;
+    c[1] = (int)(t % TD::T1); t /= TD::T1;
+    c[2] = (int)(t % TD::T2); t /= TD::T2;
+    c[3] = (int)t;
+  }
+  SiteCoord sc;
+  uint32_t h;
+  {
+    uint32_t b = blockIdx.x;
+    uint32_t q = fd_div(b, a.tm.n0); const uint32_t b0 = b - q * a.tm.n0.d; b = q;
+    q = fd_div(b, a.tm.n1); const uint32_t b1 = b - q * a.tm.n1.d; b = q;
+    q = fd_div(b, a.tm.n2); const uint32_t b2 = b - q * a.tm.n2.d; const uint32_t b3 = q;
+    sc.j = (int)b0 * TD::T0 + c[0];
+    sc.x1 = (int)b1 * TD::T1 + c[1];
+    sc.x2 = (int)b2 * TD::T2 + c[2];
+    sc.x3 = (int)b3 * TD::T3 + c[3];
+    sc.s = (p + sc.x1 + sc.x2 + sc.x3) & 1;
+    h = (uint32_t)(((sc.x3 * g.L[2] + sc.x2) * g.L[1] + sc.x1) * g.Lh0 + sc.j);
+  }
+  const int s = sc.s;
+  int fo[D], bo[D];
+#pragma unroll
+  for (int d = 0; d < D; ++d) nbr_offsets(g, sc, d, fo[d], bo[d]);
+  const uint32_t arr = (uint32_t)NP * g.Vh_pad;
+  const uint32_t own_idx = (uint32_t)(p * D + MU) * arr + h;
+  const uint32_t qmu_idx = (uint32_t)((1 - p) * D + MU) * arr + h;
+  const uint32_t lex = 2u * h + (uint32_t)s;
+  const int lin = (int)threadIdx.x;                                          // slot of box element c
+  // index of c inside the face of direction d (the d-th coordinate dropped)
+  auto lin3 = [&](int d) -> int {
+    return d == 0 ? c[1] + TD::T1 * (c[2] + TD::T2 * c[3])
+         : d == 1 ? c[0] + TD::T0 * (c[2] + TD::T2 * c[3])
+         : d == 2 ? c[0] + TD::T0 * (c[1] + TD::T1 * c[3])
+                  : c[0] + TD::T0 * (c[1] + TD::T1 * c[2]);
+  };
+
+  pdl_wait();                                                  // the previous sub-step's links are complete and visible
+  // ---- resident region: U_mu^q on the box and its faces, every element fetched by exactly one thread
+  {
+    auto stage = [&](int slot, uint32_t src_idx) {
+      const Vec* src = links + src_idx;
+#pragma unroll
+      for (int k = 0; k < NP; ++k) cp_async_vec<(int)sizeof(Vec)>(res + k * RES + slot, src + (size_t)k * g.Vh_pad);
+    };
+    stage(lin, qmu_idx);
+#pragma unroll
+    for (int d = 0; d < D; ++d) {
+      if (d == MU) continue;
+      const int fb = TD::face_base(MU, d), l3 = lin3(d);
+      if (d == 0) {
+        // a row with s = 0 needs j-1 of its first site, a row with s = 1 needs j+1 of its last site
+        if (c[0] == 0 && s == 0) stage(fb + l3, qmu_idx + (uint32_t)bo[0]);
+        if (c[0] == TD::T0 - 1 && s == 1) stage(fb + l3, qmu_idx + (uint32_t)fo[0]);
+      } else {
+        if (c[d] == 0) stage(fb + l3, qmu_idx + (uint32_t)bo[d]);
+        if (c[d] == TD::T(d) - 1) stage(fb + B / TD::T(d) + l3, qmu_idx + (uint32_t)fo[d]);
+      }
+    }
+    cp_async_commit();
+  }
+
+  // ---- ring
+  struct Dir { uint32_t p_idx, q_idx; int b, nu; };
+  auto make_dir = [&](int i) {
+    Dir d;
+    d.nu = i + (i >= MU ? 1 : 0);
+    d.b = bo[0];
+#pragma unroll
+    for (int k = 1; k < D; ++k) if (d.nu == k) d.b = bo[k];
+    d.p_idx = (uint32_t)(p * D + d.nu) * arr + h;
+    d.q_idx = (uint32_t)((1 - p) * D + d.nu) * arr + h;
+    return d;
+  };
+  auto ring_idx = [&](auto rc, const Dir& d) -> uint32_t {
+    constexpr int RR = decltype(rc)::value;
+    if constexpr (RR == 0) return d.p_idx;
+    else if constexpr (RR == 1) return d.q_idx + (uint32_t)fo[MU];
+    else if constexpr (RR == 2) return d.p_idx + (uint32_t)(fo[MU] + d.b);
+    else if constexpr (RR == 3) return d.q_idx + (uint32_t)d.b;
+    else return own_idx;
+  };
+  auto issue = [&](int n, uint32_t src_idx) {                   // link n of the sequence -> slot n % K
+    const Vec* src = links + src_idx;
+    Vec* dst = ring + (n % K) * NP * B;
+#pragma unroll
+    for (int k = 0; k < NP; ++k) cp_async_vec<(int)sizeof(Vec)>(dst + k * B, src + (size_t)k * g.Vh_pad);
+  };
+  auto from_ring = [&](int n, M3<R>& u, bool row2) {
+    const Vec* src = ring + (n % K) * NP * B;
+    R r[NREAL];
+#pragma unroll
+    for (int k = 0; k < NP; ++k) vec_unpack(src[k * B], r + k * T::VW);
+    m3_from_reals<R, NREAL>(u, r);
+    if (COMP && row2) m3_complete_row2(u);
+  };
+  auto from_res = [&](int slot, M3<R>& u, bool row2) {
+    R r[NREAL];
+#pragma unroll
+    for (int k = 0; k < NP; ++k) vec_unpack(res[k * RES + slot], r + k * T::VW);
+    m3_from_reals<R, NREAL>(u, r);
+    if (COMP && row2) m3_complete_row2(u);
+  };
+
+  Dir cur = make_dir(0);
+  static_for<0, K - 1>([&](auto rc) { issue(decltype(rc)::value, ring_idx(rc, cur)); cp_async_commit(); });
+
+  M3<R> A, P, Q;
+  m3_zero(A);
+  auto phase = [&](int i) {
+    const bool last = (i == D - 2);
+    const Dir nxt = make_dir(last ? i : i + 1);
+    const int nu = cur.nu;
+    // keep K-1 links in flight, then wait for link 4 i + r
+    auto ring_step = [&](auto rc) {
+      constexpr int RR = decltype(rc)::value, RA = RR + K - 1;
+      if constexpr (RA < 4) {
+        issue(4 * i + RA, ring_idx(std::integral_constant<int, RA>{}, cur));
+      } else {
+        if (!last) issue(4 * i + RA, ring_idx(std::integral_constant<int, RA - 4>{}, nxt));
+        else if (RA == 4) issue(4 * i + RA, own_idx);          // the own link, once, after the last direction
+      }
+      cp_async_commit();                                       // one group per step, possibly empty
+      cp_async_wait<K - 1>();
+    };
+    // slots of U_mu(x+nu), U_mu(x-nu) in the resident region
+    int cnu = c[0], Tnu = TD::T0, stnu = 1, fb = TD::face_base(MU, 0), l3 = lin3(0), hi_off = 0;
+#pragma unroll
+    for (int k = 1; k < D; ++k)
+      if (nu == k) {
+        cnu = c[k]; Tnu = TD::T(k); fb = TD::face_base(MU, k); l3 = lin3(k); hi_off = B / TD::T(k);
+        stnu = (k == 1) ? TD::T0 : (k == 2) ? TD::T0 * TD::T1 : TD::T0 * TD::T1 * TD::T2;
+      }
+    const int up = (nu == 0) ? s : 1, dn = (nu == 0) ? s - 1 : -1;
+    const int slot_up = (cnu + up < Tnu) ? lin + up * stnu : fb + hi_off + l3;
+    const int slot_dn = (cnu + dn >= 0) ? lin + dn * stnu : fb + l3;
+    const int fsign = !FIELD ? 0 : (MU == a.f.mu && nu == a.f.nu) ? 1 : (MU == a.f.nu && nu == a.f.mu) ? -1 : 0;
+
+    ring_step(std::integral_constant<int, 0>{});
+    if (i == 0) __syncthreads();                               // the resident region is complete (every thread waited for its part)
+    {                                                          // upper staple  U1 (U3 U2)^+
+      from_res(slot_up, P, true);                              // U2 = U_mu(x+nu), all rows
+      M3<R> U3;
+      from_ring(4 * i + 0, U3, false);
+      m3_zero(Q);
+      m3_mad_nn<R, NR>(Q, U3, P);                              // X = U3 U2
+      if (COMP) m3_complete_row2(Q);
+      ring_step(std::integral_constant<int, 1>{});
+      M3<R> U1;
+      from_ring(4 * i + 1, U1, false);
+      if (COMP || FIELD) {
+        M3<R> Sm;
+        m3_zero(Sm);
+        m3_mad_nd<R, NR>(Sm, U1, Q);                           // U1 X^+
+        if (COMP) m3_complete_row2(Sm);
+        if (FIELD && fsign != 0) su3_scale_cols(Sm, a.f, fsign < 0);
+        m3_add(A, Sm);
+      } else {
+        m3_mad_nd<R, 3>(A, U1, Q);
+      }
+    }
+    {                                                          // lower staple  (U2' U1')^+ U3'
+      ring_step(std::integral_constant<int, 2>{});
+      from_ring(4 * i + 2, P, true);                           // U1' = U_nu(x+mu-nu), all rows
+      M3<R> U2;
+      from_res(slot_dn, U2, false);                            // U2' = U_mu(x-nu)
+      m3_zero(Q);
+      m3_mad_nn<R, NR>(Q, U2, P);                              // Y = U2' U1'
+      if (COMP) m3_complete_row2(Q);
+      ring_step(std::integral_constant<int, 3>{});
+      M3<R> U3;
+      from_ring(4 * i + 3, U3, true);
+      if (FIELD && fsign != 0) su3_scale_rows(U3, a.f, fsign > 0);
+      if (COMP) {
+        M3<R> Sm;
+        m3_zero(Sm);
+        m3_mad_dn<R, 2>(Sm, Q, U3);                            // Y^+ U3'
+        m3_complete_row2(Sm);
+        m3_add(A, Sm);
+      } else {
+        m3_mad_dn<R, 3>(A, Q, U3);
+      }
+    }
+    cur = nxt;
+  };
+  if constexpr (ROLL) {
+#pragma unroll 1
+    for (int i = 0; i < D - 1; ++i) phase(i);
+  } else {
+#pragma unroll
+    for (int i = 0; i < D - 1; ++i) phase(i);
+  }
+
+  // own link: the last one through the ring
+  cp_async_wait<0>();
+  M3<R> U;
+  from_ring(4 * (D - 1), U, true);
+
+  if constexpr (KIND == 1) {
+    int cd;
+    HbDraw<R> none;
+    none.E = none.w = none.n1 = none.n2 = none.n3 = R(0);
+    su3_subgroup_hit<R, KIND, 0, 1>(U, A, lex, a, MU, 0, none, cd);
+    su3_subgroup_hit<R, KIND, 0, 2>(U, A, lex, a, MU, 1, none, cd);
+    su3_subgroup_hit<R, KIND, 1, 2>(U, A, lex, a, MU, 2, none, cd);
+  } else if constexpr (ROLL) {
+    // one copy of the heatbath hit, on rows (0,1) of a permuted frame: (0,1,2) -> (0,2,1) -> (1,2,0)   (reading R3)
+#pragma unroll 1
+    for (int sg = 0; sg < 3; ++sg) {
+      int cd;
+      su3_subgroup_hit<R, KIND, 0, 1>(U, A, lex, a, MU, sg, hb_first_draw<R>(lex, a, MU, sg), cd);
+      if (a.trials) a.trials[(size_t)lex * 3 + sg] = (uint8_t)cd;
+      if (sg == 0) su3_swap_frame<R, 1, 2>(U, A);
+      else if (sg == 1) su3_swap_frame<R, 0, 2>(U, A);
+    }
+#pragma unroll
+    for (int k = 0; k < 3; ++k) { const Cx<R> t = U.e[2][k]; U.e[2][k] = U.e[1][k]; U.e[1][k] = U.e[0][k]; U.e[0][k] = t; }
+  } else {
+    int c0, c1, c2;
+    su3_subgroup_hit<R, KIND, 0, 1>(U, A, lex, a, MU, 0, hb_first_draw<R>(lex, a, MU, 0), c0);
+    su3_subgroup_hit<R, KIND, 0, 2>(U, A, lex, a, MU, 1, hb_first_draw<R>(lex, a, MU, 1), c1);
+    su3_subgroup_hit<R, KIND, 1, 2>(U, A, lex, a, MU, 2, hb_first_draw<R>(lex, a, MU, 2), c2);
+    if (a.trials) {
+      a.trials[(size_t)lex * 3 + 0] = (uint8_t)c0; a.trials[(size_t)lex * 3 + 1] = (uint8_t)c1; a.trials[(size_t)lex * 3 + 2] = (uint8_t)c2;
+    }
+  }
+  m3_reunitarise(U);
+
+  R r[NREAL];
+  m3_to_reals<R, NREAL>(U, r);
+  store_reals<R, NREAL>(links, g, (size_t)(p * D + MU) * arr, h, r);
+}
+
+}  // namespace qcd
