@@ -41,6 +41,13 @@ LINK_SIZES_PER_HIT = 2 * len(DIMS) + 1
 FLOPS_PER_HIT = {"f32": {"hb": 4270.0, "or": 4030.0}, "f64": {"hb": 3900.0, "or": 3270.0}}
 
 
+# the dominant kernel of each arm (overrelaxation: 32 of the 40 update launches of a step) and its DRAM traffic per launch,
+# dram__bytes_read.sum + dram__bytes_write.sum of one `ncu --set full` capture of this workload (bytes)
+OR_KERNEL = {"f32": "su3_update_tiled_kernel<float, x12, OR>", "f64": "su3_update_kernel<double, x18, OR>"}
+NCU_TRAFFIC = {"f32": {"or": 222265088, "hb": 221323264}, "f64": {"or": 721993728, "hb": 720757248},
+               "source": "profiles/r1_c_ncu_full.md"}
+
+
 def load_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -174,26 +181,38 @@ def time_arm(q, torch, prec_name, steps, warmup, therm, seed, dist, sampler, do_
     return out
 
 
-def max_over_ranks(torch, dist, x):
+def max_over_ranks(torch, dist, x, device="cuda"):
+    """replicas only: the one cross-rank operation of the bench is this MAX of the timed region"""
     if dist is None:
         return x
-    t = torch.tensor([x], dtype=torch.float64, device="cuda")
+    t = torch.tensor([x], dtype=torch.float64, device=device)
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
     return float(t.item())
+
+
+def replica_seed(rank):
+    """every rank runs an independent lattice of the same workload: same recipe, its own Philox seed"""
+    return SEED + rank
+
+
+def aggregate_value(n_gpus, links_per_replica, steps, ms_total_max):
+    """whole-job composite link updates/s: all replicas' links over the slowest rank's time"""
+    return n_gpus * links_per_replica * steps / (ms_total_max * 1e-3)
 
 
 def summarise(arm, prec_name, steps, n_gpus, hbm_peak, fma_peak_tflops):
     """per-arm JSON fragments: value, roofline of the dominant (overrelaxation) kernel, sweep breakdown"""
     links = arm["links"]
     ms_step = arm["ms_total"] / steps
-    value = n_gpus * links * steps / (arm["ms_total"] * 1e-3)
+    value = aggregate_value(n_gpus, links, steps, arm["ms_total"])
     hits = links // (2 * len(DIMS))                                  # links updated by one launch = V/2
     bytes_launch = LINK_SIZES_PER_HIT * LINK_BYTES[prec_name] * hits
     or_us = arm["or_ms"] / max(arm["or_n"], 1) * 1e3
     hb_us = arm["hb_ms"] / max(arm["hb_n"], 1) * 1e3
     achieved = bytes_launch / (or_us * 1e-6) / 1e9
-    roof = {"bound": "hbm", "kernel": "su3_update_kernel<%s, OR>" % prec_name, "achieved": round(achieved, 1), "peak": hbm_peak,
-            "unit": "GB/s", "frac": round(achieved / hbm_peak, 4), "traffic": None,
+    roof = {"bound": "hbm", "kernel": OR_KERNEL[prec_name], "achieved": round(achieved, 1), "peak": hbm_peak,
+            "unit": "GB/s", "frac": round(achieved / hbm_peak, 4), "traffic": NCU_TRAFFIC[prec_name]["or"],
+            "traffic_source": NCU_TRAFFIC["source"],
             "bytes_per_launch": bytes_launch, "us_per_launch": round(or_us, 2), "launches_timed": arm["or_n"],
             "hb_us_per_launch": round(hb_us, 2),
             "hb_frac": round(bytes_launch / (hb_us * 1e-6) / 1e9 / hbm_peak, 4) if hb_us > 0 else None}
@@ -230,7 +249,7 @@ def run_ours(args):
     other = "f64" if primary == "f32" else "f32"
     arms = {}
     for name in (primary, other):
-        arms[name] = time_arm(q, torch, name, args.steps, args.warmup, args.therm, SEED + rank, dist, sampler)
+        arms[name] = time_arm(q, torch, name, args.steps, args.warmup, args.therm, replica_seed(rank), dist, sampler)
         arms[name]["ms_total"] = max_over_ranks(torch, dist, arms[name]["ms_total"])
         arms[name]["e2e_ms_total"] = max_over_ranks(torch, dist, arms[name]["e2e_ms_total"])
     clocks = sampler.stop()
@@ -240,7 +259,7 @@ def run_ours(args):
         for name in (primary, other):
             value, ms_step, roof = summarise(arms[name], name, args.steps, world, hbm_peak, fma[name])
             a = arms[name]
-            e2e_val = world * a["links"] * args.steps / (a["e2e_ms_total"] * 1e-3)
+            e2e_val = aggregate_value(world, a["links"], args.steps, a["e2e_ms_total"])
             frag[name] = {"value": value, "ms_per_step": ms_step, "roofline": roof,
                           "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": a["h2d"], "d2h_bytes_per_step": a["d2h"],
                                   "ms_per_step": a["e2e_ms_total"] / args.steps},
