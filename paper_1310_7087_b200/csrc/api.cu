@@ -55,6 +55,9 @@ struct qcd_lattice {
   double prof_ms[2];
   uint64_t prof_n[2];
   uint64_t launches;
+  // (parity, mu) of the update kernel launched last on the stream, -1 if the last kernel was not an update kernel: the
+  // next update kernel may fetch, before its griddepcontrol.wait, only arrays that kernel does not write (update.cuh)
+  int last_parity, last_mu;
   // device-resident sweep counter so that a captured sweep graph can be replayed unchanged
   uint32_t* d_sweep;
   // persistent staging buffer for qcd_get/set_links with HOST pointers (canonical layout, allocated on first use)
@@ -125,9 +128,12 @@ FieldArgs make_field_args(const qcd_field_t* f, bool on, int Nc) {
   return a;
 }
 
-cudaError_t launch_update(qcd_lattice* L, int kind, bool field, const UpdateArgs& a) {
+cudaError_t launch_update(qcd_lattice* L, int kind, bool field, const UpdateArgs& a0) {
   UpdateSel s; s.Nc = L->Nc; s.D = L->D; s.precision = L->precision; s.comp = L->comp; s.kind = kind; s.field = field;
   L->launches += 1;
+  UpdateArgs a = a0;
+  a.prev_parity = L->last_parity; a.prev_mu = L->last_mu;
+  L->last_parity = a.parity; L->last_mu = a.mu;
   if (L->Nc == 2) return launch_update_su2(s, L->g, L->mem, a, L->stream);
   return L->precision == QCD_FP32 ? launch_update_su3_f32(s, L->g, L->mem, a, L->stream) : launch_update_su3_f64(s, L->g, L->mem, a, L->stream);
 }
@@ -197,6 +203,7 @@ struct InitOp {
     dim3 grid((L->g.Vh + 127) / 128, 2);
     init_kernel<NC, D, R, COMP><<<grid, 128, 0, L->stream>>>(L->g, (Vec*)L->mem, hot, (uint32_t)(L->seed & 0xFFFFFFFFull), (uint32_t)(L->seed >> 32));
     L->launches += 1;
+    L->last_parity = L->last_mu = -1;
     CUDA_TRY(cudaGetLastError());
     return QCD_OK;
   }
@@ -210,6 +217,7 @@ struct LayoutOp {
     if (to_internal) layout_kernel<NC, D, R, COMP, true><<<grid, 128, 0, L->stream>>>(L->g, (Vec*)L->mem, (R*)canon);
     else layout_kernel<NC, D, R, COMP, false><<<grid, 128, 0, L->stream>>>(L->g, (Vec*)L->mem, (R*)canon);
     L->launches += 1;
+    L->last_parity = L->last_mu = -1;
     CUDA_TRY(cudaGetLastError());
     return QCD_OK;
   }
@@ -237,11 +245,13 @@ struct MeasureOp {
       plaquette_kernel<NC, D, R, COMP><<<grid, 128, 0, L->stream>>>(L->g, (const Vec*)L->mem, mf, pp);
       final_reduce_kernel<<<NPL, 256, 0, L->stream>>>(pp, nb_plaq, L->d_results, 1.0 / ((double)L->g.V * NC));
       L->launches += 2;
+      L->last_parity = L->last_mu = -1;
     }
     if (want_poly) {
       polyakov_kernel<NC, D, R, COMP><<<nb_poly, 128, 0, L->stream>>>(L->g, (const Vec*)L->mem, pq);
       final_reduce_kernel<<<2, 256, 0, L->stream>>>(pq, nb_poly, L->d_results + 8, 1.0 / ((double)Vs * NC));
       L->launches += 2;
+      L->last_parity = L->last_mu = -1;
     }
     CUDA_TRY(cudaGetLastError());
     return QCD_OK;
@@ -324,7 +334,7 @@ int qcd_lattice_create(int D, const int* dims, int Nc, int precision, unsigned f
   L->seed = 0; L->sweep = 0; L->has_links = false; L->max_trials = 10;
   L->debug_trials = false; L->profile = false; L->use_graph = true;
   L->d_trials = nullptr; L->d_partials = nullptr; L->partials_cap = 0; L->d_results = nullptr; L->h_results = nullptr;
-  L->prof_ms[0] = L->prof_ms[1] = 0.0; L->prof_n[0] = L->prof_n[1] = 0; L->launches = 0; L->d_sweep = nullptr; L->d_canon = nullptr;
+  L->prof_ms[0] = L->prof_ms[1] = 0.0; L->prof_n[0] = L->prof_n[1] = 0; L->launches = 0; L->last_parity = L->last_mu = -1; L->d_sweep = nullptr; L->d_canon = nullptr;
   cudaError_t e = cudaSuccess;
   if (!device_mem) {
     e = cudaMalloc(&L->mem, need);

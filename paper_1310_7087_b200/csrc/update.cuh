@@ -29,6 +29,8 @@ struct UpdateArgs {
   double beta;
   double inv_c;      // N / (2 beta): delta = E / alpha = E * inv_c / k   (host-computed; inf when beta = 0 -> every trial fails)
   int parity, mu, hit, max_trials;
+  int prev_parity, prev_mu;   // the update kernel launched just before this one on the stream (-1: none): its output array
+                              // (prev_parity, prev_mu) is the only one that may not be read before griddepcontrol.wait
   uint32_t sweep, key0, key1;
   uint8_t* trials;   // NULL or [lex][3] debug trial codes
   TileMap tm;        // thread -> site mapping of the SU(3) kernels (set by the launcher)
@@ -282,7 +284,6 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
   constexpr int KR = K > 0 ? K : 1;
   extern __shared__ __align__(16) unsigned char ring_raw[];
   Vec* ring = reinterpret_cast<Vec*>(ring_raw) + threadIdx.x;      // [slot][plane][B], this thread's column
-  pdl_trigger();
 
   const int p = a.parity;
   uint32_t h;
@@ -370,11 +371,19 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
     }
   }
 
-  pdl_wait();                                                      // the previous sub-step's links are complete and visible
+  // Prologue: links 0 .. K-2 of the first direction nu0.  They come from the arrays (q, mu), (p, nu0), (q, nu0); unless the
+  // update kernel running just before this one writes one of them, they are fetched before griddepcontrol.wait, i.e.
+  // while that kernel drains (in sweep order the previous kernel writes (p, mu-1): only mu = 1 has to wait).  The trigger
+  // for the next kernel comes after this kernel's own wait, so at most one earlier update kernel is ever in flight.
   Dir cur = make_dir(0);
-  if constexpr (K > 0) {                                           // prologue: links 0 .. K-2 of the first direction
-    static_for<0, KR - 1>([&](auto jc) { issue(jc, cur); cp_async_commit(); });
-  }
+  const bool early = !((a.prev_parity == 1 - p && (a.prev_mu == MU || a.prev_mu == cur.nu)) || (a.prev_parity == p && a.prev_mu == cur.nu));
+  auto prologue = [&]() {
+    if constexpr (K > 0) static_for<0, KR - 1>([&](auto jc) { issue(jc, cur); cp_async_commit(); });
+  };
+  if (early) prologue();
+  pdl_wait();                                                      // the previous sub-step's links are complete and visible
+  pdl_trigger();
+  if (!early) prologue();
 
   M3<R> A, P, Q;      // A: staple sum; P: the link kept for the next product (U2 / U1'); Q: X = U3 U2 or Y = U2' U1'
   m3_zero(A);
@@ -537,14 +546,14 @@ template <typename R, int D, int KIND, bool FIELD>
 __global__ void __launch_bounds__(256)
 su2_update_kernel(Geom g, typename PlaneTraits<R, 4>::Vec* links, UpdateArgs a) {
   typedef PlaneTraits<R, 4> T;
-  pdl_trigger();
   const uint32_t h = blockIdx.x * blockDim.x + threadIdx.x;
-  if (h >= g.Vh) return;
+  if (h >= g.Vh) { pdl_wait(); pdl_trigger(); return; }
   const int p = a.parity, mu = a.mu, q = 1 - p;
   const SiteCoord sc = decode_site(g, h, p);
   int fmu, bmu;
   nbr_offsets(g, sc, mu, fmu, bmu);
   pdl_wait();
+  pdl_trigger();
   const typename T::Vec* __restrict__ ro = links;
   Q4<R> A = q4<R>(0, 0, 0, 0);
 #pragma unroll

@@ -48,7 +48,6 @@ su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* 
   extern __shared__ __align__(16) unsigned char tile_raw[];
   Vec* const res = reinterpret_cast<Vec*>(tile_raw);                        // [plane][RES]
   Vec* const ring = res + NP * RES + threadIdx.x;                            // [slot][plane][B], this thread's column
-  pdl_trigger();
 
   // thread -> box-relative coordinates (c0 fastest), CTA -> box origin
   const int p = a.parity;
@@ -91,9 +90,10 @@ su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* 
                   : c[0] + TD::T0 * (c[1] + TD::T1 * c[2]);
   };
 
-  pdl_wait();                                                  // the previous sub-step's links are complete and visible
-  // ---- resident region: U_mu^q on the box and its faces, every element fetched by exactly one thread
-  {
+  // ---- resident region: U_mu^q on the box and its faces, every element fetched by exactly one thread.  Unless the update
+  // kernel running just before this one writes the array (q, mu) -- in sweep order it never does -- the region is fetched
+  // before griddepcontrol.wait, while that kernel drains.
+  auto stage_resident = [&]() {
     auto stage = [&](int slot, uint32_t src_idx) {
       const Vec* src = links + src_idx;
 #pragma unroll
@@ -114,7 +114,7 @@ su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* 
       }
     }
     cp_async_commit();
-  }
+  };
 
   // ---- ring
   struct Dir { uint32_t p_idx, q_idx; int b, nu; };
@@ -158,8 +158,17 @@ su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* 
     if (COMP && row2) m3_complete_row2(u);
   };
 
+  // The first K-1 ring links come from the arrays (p, nu0), (q, nu0) of the first direction: same rule.
   Dir cur = make_dir(0);
-  static_for<0, K - 1>([&](auto rc) { issue(decltype(rc)::value, ring_idx(rc, cur)); cp_async_commit(); });
+  auto prologue = [&]() { static_for<0, K - 1>([&](auto rc) { issue(decltype(rc)::value, ring_idx(rc, cur)); cp_async_commit(); }); };
+  const bool early_res = !(a.prev_parity == 1 - p && a.prev_mu == MU);
+  const bool early_ring = early_res && a.prev_mu != cur.nu;
+  if (early_res) stage_resident();
+  if (early_ring) prologue();
+  pdl_wait();                                                  // the previous sub-step's links are complete and visible
+  pdl_trigger();                                               // after the wait: at most one earlier update kernel is in flight
+  if (!early_res) stage_resident();
+  if (!early_ring) prologue();
 
   M3<R> A, P, Q;
   m3_zero(A);
