@@ -46,7 +46,7 @@ enum {
   QCD_OPT_DEBUG_TRIALS = 1,  /* 1: qcd_debug_substep records per-(link,subgroup) trial codes (allocates V*3 bytes) */
   QCD_OPT_PROFILE = 2,       /* 1: CUDA events around the update kernels: one pair per run of same-kind launches in qcd_sweep,
                                 one pair per launch in qcd_debug_substep (see qcd_get_profile) */
-  QCD_OPT_USE_GRAPH = 3      /* 1: qcd_sweep replays a captured CUDA graph when its arguments repeat (default 1) */
+  QCD_OPT_USE_GRAPH = 3      /* accepted and ignored: qcd_sweep chains its launches by programmatic dependent launch */
 };
 
 /* Constant abelian background: every plaquette of plane (mu,nu), mu < nu, is multiplied on the left, at its

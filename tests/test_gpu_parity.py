@@ -434,41 +434,42 @@ def test_long_run_plaquette_3sigma(qcd, Nc, prec, flags, dims, beta):
 
 
 # ----------------------------------------------------------------------------- full size, bench launch configuration
-@pytest.mark.parametrize("prec,flags", [(0, 1), (1, 0)], ids=["f32x12", "f64x18"])
-def test_config3_sampled_links_at_full_size(qcd, prec, flags):
-    # BASELINE.json configs[2]: SU(3) 32^4, beta 6.0, hot seed 42.  The oracle produces the start configuration and
-    # recomputes sampled links one by one; the GPU runs whole sub-steps in the launch configuration bench.py times.
-    dims, beta, Nc = (32, 32, 32, 32), 6.0, 3
+def _sampled_links_at_full_size(qcd, dims, Nc, prec, flags, beta, seed, fld, substeps, n_edge=300, n_any=700):
+    """The oracle produces the hot start and recomputes sampled links one by one (update_one_link); the GPU runs whole
+    sub-steps in the launch configuration bench.py times.  Sampled links must agree within the per-link tolerance, all
+    links outside the sub-step must be bit-unchanged, heatbath accept/reject disagreements are counted (<= 1 allowed),
+    and the hot start and the observables of the full lattice must equal the oracle's."""
+    fg, fo = field_pair(qcd, fld)
     O = oracle.OracleLattice(dims, Nc)
-    O.init(oracle.HOT, 42)
+    O.init(oracle.HOT, seed)
     start = O.get_links()
     if prec == 0:
         start = round_to_fp32(start)
         O.set_fp32_shadow(True)
         O.set_links(start)
-    O.set_seed(42)
+    O.set_seed(seed)
     rng = np.random.Generator(np.random.PCG64(5))
-    V = O.V
+    V, D = O.V, len(dims)
     coords = np.stack(np.unravel_index(np.arange(V), dims[::-1]), axis=-1)[:, ::-1]
     par = coords.sum(axis=1) & 1
+    on_edge = np.any((coords == 0) | (coords == np.array(dims) - 1), axis=1)
     with gpu_lattice(qcd, dims, Nc, prec, flags) as G:
         G.qcd_set_option(qcd.QCD_OPT_DEBUG_TRIALS, 1)
         G.qcd_set_links(start)
-        G.qcd_set_seed(42)
-        hot_gpu = None
+        G.qcd_set_seed(seed)
         total_bad, total = 0, 0
-        for kind, parity, mu in [(0, 0, 0), (0, 1, 3), (1, 1, 1), (1, 0, 2)]:
+        for kind, parity, mu in substeps:
             G.qcd_set_links(start)
-            G.qcd_debug_substep(beta, kind, 0, parity, mu)
+            G.qcd_debug_substep(beta, kind, 0, parity, mu, fg)
             got = G.qcd_get_links()
             tr = G.qcd_debug_get_trials() if kind == 0 else None
-            # boundary sites (wrap-around in every direction) plus random interior sites
+            # boundary sites (a wrap-around neighbour in some direction) plus random sites
             cand = np.flatnonzero(par == parity)
-            edge = cand[np.any((coords[cand] == 0) | (coords[cand] == 31), axis=1)]
-            sample = np.concatenate([rng.choice(edge, 300, replace=False), rng.choice(cand, 700, replace=False)])
+            edge = cand[on_edge[cand]]
+            sample = np.concatenate([rng.choice(edge, n_edge, replace=False), rng.choice(cand, n_any, replace=False)])
             worst = 0.0
             for lex in sample:
-                ref, codes = O.update_one_link(beta, kind, 0, int(lex), mu)
+                ref, codes = O.update_one_link(beta, kind, 0, int(lex), mu, fo)
                 if kind == 0 and not np.array_equal(codes, tr[lex]):
                     total_bad += 1
                     continue
@@ -477,21 +478,113 @@ def test_config3_sampled_links_at_full_size(qcd, prec, flags):
             total += len(sample)
             assert worst < 1.0, (kind, parity, mu, worst)
             # all other links untouched
-            other = np.ones((V, 4), dtype=bool)
+            other = np.ones((V, D), dtype=bool)
             other[par == parity, mu] = False
-            cmp_a = got if flags == 0 else got[..., :2, :]
-            cmp_b = start if flags == 0 else start[..., :2, :]
-            assert np.array_equal(cmp_a[other].astype(np.complex128), cmp_b[other])
+            cmp_a = got if (flags == 0 or Nc == 2) else got[..., :2, :]
+            cmp_b = start if (flags == 0 or Nc == 2) else start[..., :2, :]
+            assert np.array_equal(cmp_a[other], cmp_b[other].astype(cmp_a.dtype))
+            del got
         assert total_bad <= 1, (total_bad, total)
-        # the GPU hot start at full size equals the oracle's
-        G.qcd_init(qcd.QCD_HOT, 42)
-        hot_gpu = G.qcd_get_links().astype(np.complex128)
+        # the GPU hot start at full size equals the oracle's, and so do the observables measured on it
+        G.qcd_init(qcd.QCD_HOT, seed)
+        hot_gpu = G.qcd_get_links()
         O2 = oracle.OracleLattice(dims, Nc)
-        O2.init(oracle.HOT, 42)
+        O2.init(oracle.HOT, seed)
         assert np.max(np.abs(hot_gpu - O2.get_links())) < (1e-13 if prec == 1 else 5e-7)
-        tot, planes, poly = G.qcd_measure()
-        tot_o, planes_o, poly_o = O2.measure()
+        tot, planes, poly = G.qcd_measure(fg)
+        tot_o, planes_o, poly_o = O2.measure(fo)
         assert abs(tot - tot_o) < MEAS_TOL[prec] and abs(poly - poly_o) < MEAS_TOL[prec]
+        assert np.max(np.abs(planes - planes_o)) < MEAS_TOL[prec]
+
+
+@pytest.mark.parametrize("prec,flags", [(0, 1), (1, 0)], ids=["f32x12", "f64x18"])
+def test_config3_sampled_links_at_full_size(qcd, prec, flags):
+    # BASELINE.json configs[2]: SU(3) 32^4, beta 6.0, hot seed 42 -- the workload bench.py times
+    _sampled_links_at_full_size(qcd, (32, 32, 32, 32), 3, prec, flags, 6.0, 42, None,
+                                [(0, 0, 0), (0, 1, 3), (1, 1, 1), (1, 0, 2)])
+
+
+def test_config4_su2_background_field_at_full_size(qcd):
+    # BASELINE.json configs[3]: SU(2) 48^3 x 8, beta 2.5, fp32, constant abelian field along sigma_3 on the x-y plane,
+    # every x-y plaquette times exp(i phi sigma_3 / 2), phi = 2 pi n_f / (Lx Ly), n_f = 4; hot seed 99
+    phi = 2.0 * np.pi * 4 / (48 * 48)
+    _sampled_links_at_full_size(qcd, (48, 48, 48, 8), 2, 0, 0, 2.5, 99, (0, 1, [0.5 * phi, -0.5 * phi]),
+                                [(0, 0, 0), (0, 1, 1), (1, 1, 0), (1, 0, 1), (0, 1, 3), (1, 0, 2)])
+
+
+def test_config5_su3_large_volume_fp32_sampled_links(qcd):
+    # BASELINE.json configs[4], fp32 arm: SU(3) 64^3 x 16, beta 6.2, 12-real links, hot seed 2024 (805 MB of links)
+    _sampled_links_at_full_size(qcd, (64, 64, 64, 16), 3, 0, 1, 6.2, 2024, None, [(0, 1, 0), (1, 0, 3), (1, 1, 2)],
+                                n_edge=200, n_any=300)
+
+
+def test_config5_su3_64to4_fp64_properties_at_full_size(qcd):
+    """BASELINE.json configs[4], fp64 arm: SU(3) 64^4, 18 reals, 9.66 GB of links -- too large for the oracle to hold next
+    to the test, so this checks what holds at any size and ties it to oracle-verified results:
+      * the hot start depends on (seed, lex, mu) only, so its first V' links equal the oracle's hot start of 64^3 x 2;
+      * an overrelaxation sub-step is deterministic and local: on a 64^4 configuration that repeats a 32^4 one with period 32
+        in every direction it must reproduce, bit for bit and on all 67 M links, the periodic repetition of the same sub-step
+        on the 32^4 lattice (whose sub-steps test_config3 checks against the oracle);
+      * after a full sweep (1 HB + 4 OR, beta 6.2) every link is unitary with det 1 to 1e-12, the plaquette moved off the
+        hot start, and an overrelaxation-only sweep conserves it to 1e-12."""
+    import torch
+    big, small, Nc, seed, beta = (64, 64, 64, 64), (32, 32, 32, 32), 3, 2024, 6.2
+    dev = torch.device("cuda:0")
+    Vb, Vs = 64 ** 4, 32 ** 4
+
+    def links_to_device(G, V):
+        t = torch.empty((V, 4, 3, 3), dtype=torch.complex128, device=dev)
+        G.qcd_get_links_ptr(t.data_ptr(), t.numel() * 16, 1)
+        return t
+
+    with gpu_lattice(qcd, small, Nc, 1, 0) as S:
+        S.qcd_init(qcd.QCD_HOT, seed)
+        S.qcd_sweep(beta, 1, 1)
+        base = links_to_device(S, Vs)
+        ext = base.view(32, 32, 32, 32, 4, 3, 3).repeat(2, 2, 2, 2, 1, 1, 1).contiguous()      # [x3][x2][x1][x0]: lex order
+        results = {}
+        for parity, mu in [(0, 0), (1, 3), (1, 1)]:
+            S.qcd_set_links_ptr(base.data_ptr(), base.numel() * 16, 1)
+            S.qcd_debug_substep(beta, qcd.QCD_KIND_OR, 0, parity, mu)
+            results[(parity, mu)] = links_to_device(S, Vs)
+    with gpu_lattice(qcd, big, Nc, 1, 0) as G:
+        for (parity, mu), res in results.items():
+            G.qcd_set_links_ptr(ext.data_ptr(), ext.numel() * 16, 1)
+            G.qcd_debug_substep(beta, qcd.QCD_KIND_OR, 0, parity, mu)
+            got = links_to_device(G, Vb).view(64, 64, 64, 64, 4, 3, 3)
+            for o3 in (0, 32):
+                for o2 in (0, 32):
+                    for o1 in (0, 32):
+                        for o0 in (0, 32):
+                            blk = got[o3:o3 + 32, o2:o2 + 32, o1:o1 + 32, o0:o0 + 32]
+                            assert torch.equal(blk.reshape(Vs, 4, 3, 3), res), (parity, mu, o3, o2, o1, o0)
+            del got
+        del ext, results
+        # hot start: first V' links against the oracle's 64^3 x 2 lattice
+        G.qcd_init(qcd.QCD_HOT, seed)
+        O = oracle.OracleLattice((64, 64, 64, 2), Nc)
+        O.init(oracle.HOT, seed)
+        ref = torch.from_numpy(O.get_links()).to(dev)
+        hot = links_to_device(G, Vb)
+        assert float((hot[:O.V] - ref).abs().max()) < 1e-13
+        del ref, O
+        p_hot = G.qcd_measure()[0]
+        assert abs(p_hot) < 5e-4                                   # Haar-random links: <P> = 0, sigma ~ 1e-5 at this volume
+        del hot
+        G.qcd_sweep(beta, 1, 4)
+        p1, planes, poly = G.qcd_measure()
+        assert 0.2 < p1 < 0.7 and np.all(np.abs(planes - p1) < 0.01) and abs(poly) < 0.01
+        U = links_to_device(G, Vb).view(-1, 3, 3)
+        eye = torch.eye(3, dtype=torch.complex128, device=dev)
+        worst_u, worst_d = 0.0, 0.0
+        for c in torch.split(U, 1 << 23):
+            worst_u = max(worst_u, float((c @ c.conj().transpose(1, 2) - eye).abs().max()))
+            worst_d = max(worst_d, float((torch.linalg.det(c) - 1.0).abs().max()))
+        assert worst_u < 1e-12 and worst_d < 1e-12, (worst_u, worst_d)
+        del U
+        G.qcd_sweep(beta, 0, 2)
+        p2 = G.qcd_measure()[0]
+        assert abs(p2 - p1) < 1e-12, (p1, p2)
 
 
 # ----------------------------------------------------------------------------- ABI error paths on a live device
