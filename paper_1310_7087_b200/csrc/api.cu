@@ -58,6 +58,9 @@ struct qcd_lattice {
   // (parity, mu) of the update kernel launched last on the stream, -1 if the last kernel was not an update kernel: the
   // next update kernel may fetch, before its griddepcontrol.wait, only arrays that kernel does not write (update.cuh)
   int last_parity, last_mu;
+  // side stream + events: the latency-bound Polyakov kernel runs beside the plaquette kernel (qcd_measure)
+  cudaStream_t side;
+  cudaEvent_t ev_fork, ev_join;
   // device-resident sweep counter so that a captured sweep graph can be replayed unchanged
   uint32_t* d_sweep;
   // persistent staging buffer for qcd_get/set_links with HOST pointers (canonical layout, allocated on first use)
@@ -240,6 +243,28 @@ struct MeasureOp {
     }
     double* pp = L->d_partials;
     double* pq = L->d_partials + (size_t)NPL * nb_plaq;
+    if (want_plaq && want_poly) {
+      // fork: the Polyakov kernel (one thread per spatial site, bound by the latency of its L_t dependent loads) goes first
+      // on a side stream and runs beside the plaquette kernel; join before the D2H copy of the results
+      if (!L->side) {
+        CUDA_TRY(cudaStreamCreateWithFlags(&L->side, cudaStreamNonBlocking));
+        CUDA_TRY(cudaEventCreateWithFlags(&L->ev_fork, cudaEventDisableTiming));
+        CUDA_TRY(cudaEventCreateWithFlags(&L->ev_join, cudaEventDisableTiming));
+      }
+      CUDA_TRY(cudaEventRecord(L->ev_fork, L->stream));
+      CUDA_TRY(cudaStreamWaitEvent(L->side, L->ev_fork, 0));
+      polyakov_kernel<NC, D, R, COMP><<<nb_poly, 128, 0, L->side>>>(L->g, (const Vec*)L->mem, pq);
+      final_reduce_kernel<<<2, 256, 0, L->side>>>(pq, nb_poly, L->d_results + 8, 1.0 / ((double)Vs * NC));
+      CUDA_TRY(cudaEventRecord(L->ev_join, L->side));
+      dim3 grid((L->g.Vh + 127) / 128, 2);
+      plaquette_kernel<NC, D, R, COMP><<<grid, 128, 0, L->stream>>>(L->g, (const Vec*)L->mem, mf, pp);
+      final_reduce_kernel<<<NPL, 256, 0, L->stream>>>(pp, nb_plaq, L->d_results, 1.0 / ((double)L->g.V * NC));
+      CUDA_TRY(cudaStreamWaitEvent(L->stream, L->ev_join, 0));
+      L->launches += 4;
+      L->last_parity = L->last_mu = -1;
+      CUDA_TRY(cudaGetLastError());
+      return QCD_OK;
+    }
     if (want_plaq) {
       dim3 grid((L->g.Vh + 127) / 128, 2);
       plaquette_kernel<NC, D, R, COMP><<<grid, 128, 0, L->stream>>>(L->g, (const Vec*)L->mem, mf, pp);
@@ -335,6 +360,7 @@ int qcd_lattice_create(int D, const int* dims, int Nc, int precision, unsigned f
   L->debug_trials = false; L->profile = false; L->use_graph = true;
   L->d_trials = nullptr; L->d_partials = nullptr; L->partials_cap = 0; L->d_results = nullptr; L->h_results = nullptr;
   L->prof_ms[0] = L->prof_ms[1] = 0.0; L->prof_n[0] = L->prof_n[1] = 0; L->launches = 0; L->last_parity = L->last_mu = -1; L->d_sweep = nullptr; L->d_canon = nullptr;
+  L->side = nullptr; L->ev_fork = nullptr; L->ev_join = nullptr;
   cudaError_t e = cudaSuccess;
   if (!device_mem) {
     e = cudaMalloc(&L->mem, need);
@@ -361,6 +387,9 @@ int qcd_lattice_destroy(qcd_lattice_t* L) {
   if (L->d_results) cudaFree(L->d_results);
   if (L->h_results) cudaFreeHost(L->h_results);
   if (L->d_sweep) cudaFree(L->d_sweep);
+  if (L->ev_fork) cudaEventDestroy(L->ev_fork);
+  if (L->ev_join) cudaEventDestroy(L->ev_join);
+  if (L->side) cudaStreamDestroy(L->side);
   if (L->d_canon) cudaFree(L->d_canon);
   delete L;
   return QCD_OK;

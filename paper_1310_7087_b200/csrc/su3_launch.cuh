@@ -25,10 +25,10 @@ namespace qcd {
 #define QCD_TILE_MU3 0x8441
 #endif
 #ifndef QCD_TILE_F32X12_K
-#define QCD_TILE_F32X12_K 4
+#define QCD_TILE_F32X12_K 5
 #endif
 #ifndef QCD_TILE_F32X12_MINB
-#define QCD_TILE_F32X12_MINB 5
+#define QCD_TILE_F32X12_MINB 4
 #endif
 template <int X> struct TileHex { typedef TileDims<((X >> 12) & 15), ((X >> 8) & 15), ((X >> 4) & 15), (X & 15)> TD; };
 template <int MU> struct TileFor;
