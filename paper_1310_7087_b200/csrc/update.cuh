@@ -80,12 +80,13 @@ template <> struct KpRand<double> {
     w = r4 * r4;
   }
 };
-// fp32: __logf is 3 ulp (2^-21.4 absolute near 1), cospif 2 ulp: E is known to ~1e-6 E.  The accept test of the fp32
+// fp32: __logf is 3 ulp (2^-21.4 absolute near 1) and cos(2 pi r2) comes from the SFU (__cosf on (-pi, pi): absolute error
+// 2^-21.4, so c^2 ln r3 is off by at most 7.2e-7 |c| |ln r3| <= max(4e-6 E, 2.2e-6)).  The accept test of the fp32
 // kernels is taken in float and re-evaluated in double inside a guard band (kp_accept below).
 template <> struct KpRand<float> {
   static __device__ __forceinline__ void run(const Philox4& x, float& E, float& w) {
     const float r1 = uniform23f(x.x), r2 = uniform23f(x.y), r3 = uniform23f(x.z), r4 = uniform23f(x.w);
-    const float c = cospif(2.0f * r2);
+    const float c = __cosf(6.283185307f * (r2 - 0.5f));          // = -cos(2 pi r2); only c^2 is used
     E = -(__logf(r1) + c * c * __logf(r3));
     w = r4 * r4;
   }
@@ -97,6 +98,15 @@ template <typename R> __device__ __forceinline__ void hb_direction(const Philox4
   R sphi, cphi;
   q_sincospi(R(2) * u2, &sphi, &cphi);
   n1 = st * cphi; n2 = st * sphi; n3 = ct;
+}
+// fp32: the azimuth from the SFU, argument folded into (-pi, pi) where __sinf / __cosf are good to 2^-21.4 absolute
+// (the link tolerance is 2e-5): sin(2 pi u) = -sin(2 pi (u - 1/2)), cos likewise
+template <> __device__ __forceinline__ void hb_direction<float>(const Philox4& x, float& n1, float& n2, float& n3) {
+  const float u1 = uniform23f(x.x), u2 = uniform23f(x.y);
+  const float ct = 1.0f - 2.0f * u1;
+  const float st = sqrtf(1.0f - ct * ct);
+  const float ang = 6.283185307f * (u2 - 0.5f);
+  n1 = -st * __cosf(ang); n2 = -st * __sinf(ang); n3 = ct;
 }
 // trial 0 and direction of subgroup sg of this link
 template <typename R>
@@ -122,13 +132,13 @@ __device__ __forceinline__ bool kp_accept(double inv_alpha, double E, double w, 
   g0 = 1.0 - delta;
   return w <= 1.0 - 0.5 * delta;
 }
-// fp32: |error of delta| < (2e-6 E + 1e-6) / alpha, so outside the guard band below the float decision is the fp64 one;
+// fp32: |error of delta| < (4e-6 E + 2.5e-6) / alpha, so outside the guard band below the float decision is the fp64 one;
 // inside it (probability ~1e-5 per trial) the trial is recomputed in double.
 __device__ __forceinline__ bool kp_accept(float inv, float E, float w, const Philox4& blk, float& g0) {
   const float delta = E * inv;
   const float margin = (1.0f - 0.5f * delta) - w;
   g0 = 1.0f - delta;
-  if (fabsf(margin) < (4e-6f * E + 2e-6f) * inv + 5e-7f) {
+  if (fabsf(margin) < (6e-6f * E + 4e-6f) * inv + 5e-7f) {
     double g0d;
     const bool acc = kp_trial_f64_cold(1.0 / (double)inv, blk.x, blk.y, blk.z, blk.w, &g0d);
     g0 = (float)g0d;
@@ -161,7 +171,7 @@ __device__ __forceinline__ bool subgroup_quaternion(const Q4<R>& v, R k2, uint32
       // cheap pre-test, so that the common case does not pay for the Philox block
       const float inv = (float)inv_alpha;
       const float margin = (1.0f - 0.5f * (float)d0.E * inv) - (float)d0.w;
-      if (fabsf(margin) < (4e-6f * (float)d0.E + 2e-6f) * inv + 5e-7f) blk = philox4x32_10(lex, a.sweep, c2, 1u, a.key0, a.key1);
+      if (fabsf(margin) < (6e-6f * (float)d0.E + 4e-6f) * inv + 5e-7f) blk = philox4x32_10(lex, a.sweep, c2, 1u, a.key0, a.key1);
     }
     acc = kp_accept(inv_alpha, d0.E, d0.w, blk, g0);
     code = 1;
