@@ -183,13 +183,16 @@ __device__ __forceinline__ bool subgroup_quaternion(const Q4<R>& v, R k2, uint32
         KpRand<R>::run(x, E, w);
         if (kp_accept(inv_alpha, E, w, x, g0)) { acc = true; code = t + 1; break; }
       }
-      if (!acc) return false;
     }
+    // fp32: no early return: the lanes that needed further trials re-join the warp here, so what follows is executed
+    // once per warp and not once per divergent path (it was 1.57 times per subgroup at 3 % rejection).  fp64 keeps the
+    // early exit (the straight-line form costs it two spilled registers at its 168-register cap).
+    if constexpr (sizeof(R) == 8) { if (!acc) return false; }
     const R rr = q_sqrt(fmax(R(0), R(1) - g0 * g0));
     const Q4<R> g = q4<R>(g0, rr * d0.n1, rr * d0.n2, rr * d0.n3);
     const Q4<R> vtc = q4<R>(v.a0 * rk, -v.a1 * rk, -v.a2 * rk, -v.a3 * rk);   // vt^dagger
     out = q4_mul(g, vtc);
-    return true;
+    return acc;
   }
 }
 
@@ -215,10 +218,16 @@ __device__ __forceinline__ void su3_subgroup_hit(M3<R>& U, const M3<R>& A, uint3
   v.a2 = R(0.5) * (wij.re - wji.re);
   v.a3 = R(0.5) * (wii.im - wjj.im);
   const R k2 = v.a0 * v.a0 + v.a1 * v.a1 + v.a2 * v.a2 + v.a3 * v.a3;
-  code = 0;
-  if (k2 < Tiny<R>::k2()) return;                    // reading R4
+  // reading R4 (k -> 0) and R5 (all trials rejected): the subgroup factor is the identity.  Applied as a = 1 rather than
+  // by skipping the row update (1 * u + 0 * u' = u exactly), so that the warp does not diverge around it.
+  const bool tiny = k2 < Tiny<R>::k2();
+  if constexpr (sizeof(R) == 8) { if (tiny) { code = 0; return; } }
   Q4<R> q;
-  if (!subgroup_quaternion<R, KIND, 3>(v, k2, lex, a, mu, sg, d0, q, code)) return;
+  int cd = 0;
+  const bool ok = subgroup_quaternion<R, KIND, 3>(v, tiny ? R(1) : k2, lex, a, mu, sg, d0, q, cd) && !tiny;
+  code = tiny ? 0 : cd;
+  if constexpr (sizeof(R) == 8) { if (!ok) return; }
+  if (!ok) q = q4<R>(R(1), R(0), R(0), R(0));
   const Cx<R> aii = cx<R>(q.a0, q.a3), aij = cx<R>(q.a2, q.a1), aji = cx<R>(-q.a2, q.a1), ajj = cx<R>(q.a0, -q.a3);
 #pragma unroll
   for (int c = 0; c < 3; ++c) {
