@@ -227,7 +227,55 @@ __global__ void __launch_bounds__(128) plaquette_kernel(Geom g, const typename L
   double acc[NPL];
 #pragma unroll
   for (int k = 0; k < NPL; ++k) acc[k] = 0.0;
-  if (h < g.Vh) {
+  if constexpr (NC == 3 && COMP) {
+    // 12-real links: rows 0,1 of M = U_mu(x) U_nu(x+mu) and N = U_nu(x) U_mu(x+nu) only.  With G_ab = sum_j M_aj conj(N_bj)
+    // (a, b in {0,1}) the diagonal of M N^+ is (G_00, G_11, conj(G_00 G_11 - G_01 G_10)): the third rows of SU(3)
+    // matrices are conj(row0 x row1), and (a x b).conj(c x d) = (a.conj c)(b.conj d) - (a.conj d)(b.conj c).
+    // The own links need no third row at all; the neighbours do (they are summed over in the products).
+    if (h < g.Vh) {
+      typedef PlaneTraits<R, 12> T12;
+      const SiteCoord sc = decode_site(g, h, p);
+      M3<R> own[D];
+      int fwd[D];
+#pragma unroll
+      for (int mu = 0; mu < D; ++mu) {
+        int b;
+        nbr_offsets(g, sc, mu, fwd[mu], b);
+        R r[12];
+        load_reals<R, 12, true>(links, g, array_base<T12::NP>(g, D, p, mu), h, r);
+        m3_from_reals<R, 12>(own[mu], r);
+      }
+      int plane = 0;
+#pragma unroll
+      for (int mu = 0; mu < D; ++mu)
+#pragma unroll
+        for (int nu = mu + 1; nu < D; ++nu, ++plane) {
+          M3<R> b, c, M, N;
+          R r[12];
+          load_reals<R, 12, true>(links, g, array_base<T12::NP>(g, D, q, nu), h + fwd[mu], r);   // U_nu(x+mu)
+          m3_from_reals<R, 12>(b, r);
+          m3_complete_row2(b);
+          load_reals<R, 12, true>(links, g, array_base<T12::NP>(g, D, q, mu), h + fwd[nu], r);   // U_mu(x+nu)
+          m3_from_reals<R, 12>(c, r);
+          m3_complete_row2(c);
+          m3_zero(M); m3_zero(N);
+          m3_mad_nn<R, 2>(M, own[mu], b);
+          m3_mad_nn<R, 2>(N, own[nu], c);
+          Cx<R> G00 = cx<R>(0, 0), G01 = cx<R>(0, 0), G10 = cx<R>(0, 0), G11 = cx<R>(0, 0);
+          cdot3<CD_ND>(G00, M.e[0][0], M.e[0][1], M.e[0][2], N.e[0][0], N.e[0][1], N.e[0][2]);
+          cdot3<CD_ND>(G01, M.e[0][0], M.e[0][1], M.e[0][2], N.e[1][0], N.e[1][1], N.e[1][2]);
+          cdot3<CD_ND>(G10, M.e[1][0], M.e[1][1], M.e[1][2], N.e[0][0], N.e[0][1], N.e[0][2]);
+          cdot3<CD_ND>(G11, M.e[1][0], M.e[1][1], M.e[1][2], N.e[1][0], N.e[1][1], N.e[1][2]);
+          const Cx<R> dd = cmul(G00, G11), od = cmul(G01, G10);
+          const Cx<R> D2 = cx<R>(dd.re - od.re, -(dd.im - od.im));
+          const bool dressed = f.enabled && f.mu == mu && f.nu == nu;
+          const R tr = dressed ? (G00.re * (R)f.c[0] - G00.im * (R)f.s[0]) + (G11.re * (R)f.c[1] - G11.im * (R)f.s[1]) +
+                                     (D2.re * (R)f.c[2] - D2.im * (R)f.s[2])
+                               : G00.re + G11.re + D2.re;
+          acc[plane] += (double)tr;
+        }
+    }
+  } else if (h < g.Vh) {
     const SiteCoord sc = decode_site(g, h, p);
     Cx<R> own[D][NC][NC];
     int fwd[D];
