@@ -293,6 +293,12 @@ template <typename R, int R1, int R2> __device__ __forceinline__ void su3_swap_f
 // 32 KB instruction cache level; the fp32 kernels, which are issue-bound, take it; the fp64 kernels, which run few warps
 // and live on instruction-level parallelism, are faster unrolled).  PRE: heatbath only, park the random-number-only part
 // of trial 0 of every subgroup in shared memory at the start of the kernel instead of computing it inside the hit.
+// 18-real storage only: the links of which a thread uses rows 0,1 alone (J as in the table above; 6 = the own link, whose
+// third row is rebuilt).  Every product of SU(3) matrices is in SU(3), so the third rows of X = U3 U2, Y = U2' U1' and of
+// the staples are rebuilt as conj(row0 x row1) whatever the storage; what 18-real storage saves is the rebuilding of
+// the third rows of the RIGHT factors U2, U1', U3' (J = 0, 3, 5), which are read in full.
+template <bool COMP> __host__ __device__ constexpr bool rows01_only_t(int J) { return !COMP && (J == 1 || J == 2 || J == 4 || J == 6); }
+
 template <typename R, int D, int MU, bool COMP, int KIND, bool FIELD, int B, int K, int MINB, bool ROLL, bool PRE>
 __global__ void __launch_bounds__(B, MINB)
 su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links, UpdateArgs a) {
@@ -350,8 +356,13 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
 #endif
     const Vec* src = links + link_idx(jc, d);
     Vec* dst = ring + (J % KR) * NP * B;
+    // Links that enter only as the LEFT factor of a product whose third row is rebuilt anyway (U3, U1, U2': J = 1, 2, 4)
+    // and the own link (J = 6) contribute rows 0,1 only: with 18-real storage the planes of their third row are not
+    // fetched (L2 -> SM traffic 19 -> 15.7 link-sizes per link-hit; every neighbour array is still read in full from
+    // DRAM once, by the thread that needs all rows of that link as a right factor).
+    constexpr int NPJ = rows01_only_t<COMP>(J) ? (NP * 2) / 3 : NP;
 #pragma unroll
-    for (int k = 0; k < NP; ++k) cp_async_vec<(int)sizeof(Vec)>(dst + k * B, src + (size_t)k * g.Vh_pad);
+    for (int k = 0; k < NPJ; ++k) cp_async_vec<(int)sizeof(Vec)>(dst + k * B, src + (size_t)k * g.Vh_pad);
   };
   auto fetch = [&](auto jc, const Dir& d, M3<R>& u, bool row2) {
     constexpr int J = decltype(jc)::value;
@@ -372,8 +383,13 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
 #pragma unroll
       for (int k = 0; k < NP; ++k) vec_unpack(J == 6 ? src[(size_t)k * g.Vh_pad] : __ldg(src + (size_t)k * g.Vh_pad), r + k * T::VW);
     }
-    m3_from_reals<R, NREAL>(u, r);
-    if (COMP && row2) m3_complete_row2(u);
+    if constexpr (rows01_only_t<COMP>(J)) {
+      m3_from_reals<R, 12>(u, r);                                  // planes of rows 0,1 (the first 12 reals) only
+      if (row2) m3_complete_row2(u);
+    } else {
+      m3_from_reals<R, NREAL>(u, r);
+      if (COMP && row2) m3_complete_row2(u);
+    }
   };
 
   const uint32_t lex = 2u * h + (uint32_t)sc.s;
@@ -439,29 +455,25 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
         M3<R> U3;
         fetch(jc, cur, U3, false);
         m3_zero(Q);
-        m3_mad_nn<R, NR>(Q, U3, P);                                // X = U3 U2
-        if (COMP) m3_complete_row2(Q);
+        m3_mad_nn<R, 2>(Q, U3, P);                                 // X = U3 U2, rows 0,1; row 2 rebuilt (XY_ROWS)
+        m3_complete_row2(Q);
       } else if constexpr (J == 2) {
         M3<R> U1;
         fetch(jc, cur, U1, false);
-        if (COMP || FIELD) {
-          M3<R> Sm;
-          m3_zero(Sm);
-          m3_mad_nd<R, NR>(Sm, U1, Q);                             // U1 X^+
-          if (COMP) m3_complete_row2(Sm);
-          if (FIELD && fsign != 0) su3_scale_cols(Sm, a.f, fsign < 0);   // first direction: . F ; second: . F^+
-          m3_add(A, Sm);
-        } else {
-          m3_mad_nd<R, 3>(A, U1, Q);
-        }
+        M3<R> Sm;
+        m3_zero(Sm);
+        m3_mad_nd<R, 2>(Sm, U1, Q);                                // U1 X^+, rows 0,1; the staple is in SU(3): row 2 rebuilt
+        m3_complete_row2(Sm);
+        if (FIELD && fsign != 0) su3_scale_cols(Sm, a.f, fsign < 0);     // first direction: . F ; second: . F^+
+        m3_add(A, Sm);
       } else if constexpr (J == 3) {
         fetch(jc, cur, P, true);                                   // U1', all rows
       } else if constexpr (J == 4) {
         M3<R> U2;
         fetch(jc, cur, U2, false);
         m3_zero(Q);
-        m3_mad_nn<R, NR>(Q, U2, P);                                // Y = U2' U1'
-        if (COMP) m3_complete_row2(Q);
+        m3_mad_nn<R, 2>(Q, U2, P);                                 // Y = U2' U1', rows 0,1; row 2 rebuilt
+        m3_complete_row2(Q);
       } else {
         M3<R> U3;
         fetch(jc, cur, U3, true);
