@@ -104,6 +104,13 @@ template <> struct TiledCfg<float, true, 1> { static constexpr bool ON = true; s
 template <typename R, int KIND> struct LoopCfg;
 template <int KIND> struct LoopCfg<float, KIND> { static constexpr bool ROLL = (KIND == 0) ? QCD_F32_ROLL_HB : QCD_F32_ROLL_OR, PRE = QCD_F32_PRE; };
 template <int KIND> struct LoopCfg<double, KIND> { static constexpr bool ROLL = (KIND == 0) ? QCD_F64_ROLL_HB : QCD_F64_ROLL_OR, PRE = QCD_F64_PRE; };
+// Ring slots of the UNROLLED overrelaxation kernels (any K >= 2: the slot of a link is its sequence number mod K); the
+// heatbath kernels, whose direction loop is rolled, need K | 6 and take the K above.
+#ifndef QCD_F64X18_K_OR
+#define QCD_F64X18_K_OR 4
+#endif
+template <typename R, bool COMP> struct RingKOr { static constexpr int K = -1; };          // -1: same as the heatbath kernel
+template <> struct RingKOr<double, false> { static constexpr int K = QCD_F64X18_K_OR; };
 template <int B_, int K_, int MINB_> struct RingShape { static constexpr int B = B_, K = K_, MINB = MINB_; };
 template <typename R, bool COMP> struct RingCfg;
 template <> struct RingCfg<float, true> : RingShape<QCD_F32X12_B, QCD_F32X12_K, QCD_F32X12_MINB> {};
@@ -186,8 +193,9 @@ static cudaError_t su3_go(const Geom& g, void* links, const UpdateArgs& a, cudaS
     if (tiled_enabled() && g.Lh0 % TD::T0 == 0 && g.L[1] % TD::T1 == 0 && g.L[2] % TD::T2 == 0 && g.L[3] % TD::T3 == 0)
       return su3_go_tiled<R, MU, COMP, KIND, FIELD>(g, links, a, st);
   }
-  constexpr int B = RingCfg<R, COMP>::B, K = RingCfg<R, COMP>::K, MINB = RingCfg<R, COMP>::MINB;
   constexpr bool ROLL = LoopCfg<R, KIND>::ROLL, PRE = LoopCfg<R, KIND>::PRE;
+  constexpr int B = RingCfg<R, COMP>::B, MINB = RingCfg<R, COMP>::MINB;
+  constexpr int K = (KIND == 1 && !ROLL && RingKOr<R, COMP>::K >= 0) ? RingKOr<R, COMP>::K : RingCfg<R, COMP>::K;
   constexpr size_t smem = (size_t)K * T::NP * B * sizeof(Vec) + ((KIND == 0 && PRE) ? (size_t)15 * B * sizeof(R) : 0);
   auto kern = su3_update_kernel<R, D, MU, COMP, KIND, FIELD, B, K, MINB, ROLL, PRE>;
   static int attr_dev = -1;                  // opt in to > 48 KB of dynamic shared memory once per device

@@ -305,7 +305,8 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
   typedef PlaneTraits<R, (COMP ? 12 : 18)> T;
   typedef typename T::Vec Vec;
   constexpr int NREAL = COMP ? 12 : 18, NP = T::NP, NR = COMP ? 2 : 3;
-  static_assert(K == 0 || K == 3 || K == 6, "ring slots must divide the 6 links of one direction");
+  // link n = 6 i + J of the sequence goes to slot n % K; with the rolled direction loop the slot must not depend on i
+  static_assert(K == 0 || (K >= 2 && K <= 7 && (!ROLL || 6 % K == 0)), "ring slots: K | 6 when the direction loop is rolled");
   constexpr int KR = K > 0 ? K : 1;
   extern __shared__ __align__(16) unsigned char ring_raw[];
   Vec* ring = reinterpret_cast<Vec*>(ring_raw) + threadIdx.x;      // [slot][plane][B], this thread's column
@@ -349,13 +350,13 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
     else if constexpr (J == 5) return d.q_idx + (uint32_t)d.b;
     else return own_idx;
   };
-  auto issue = [&](auto jc, const Dir& d) {                         // cp.async link j into ring slot j % K
+  auto issue = [&](auto jc, const Dir& d, int n) {                  // cp.async link J (n-th of the sequence) into ring slot n % K
     constexpr int J = decltype(jc)::value;
 #ifdef QCD_EXP_NOLOAD
     return;
 #endif
     const Vec* src = links + link_idx(jc, d);
-    Vec* dst = ring + (J % KR) * NP * B;
+    Vec* dst = ring + (n % KR) * NP * B;
     // Links that enter only as the LEFT factor of a product whose third row is rebuilt anyway (U3, U1, U2': J = 1, 2, 4)
     // and the own link (J = 6) contribute rows 0,1 only: with 18-real storage the planes of their third row are not
     // fetched (L2 -> SM traffic 19 -> 15.7 link-sizes per link-hit; every neighbour array is still read in full from
@@ -364,7 +365,7 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
 #pragma unroll
     for (int k = 0; k < NPJ; ++k) cp_async_vec<(int)sizeof(Vec)>(dst + k * B, src + (size_t)k * g.Vh_pad);
   };
-  auto fetch = [&](auto jc, const Dir& d, M3<R>& u, bool row2) {
+  auto fetch = [&](auto jc, const Dir& d, M3<R>& u, bool row2, int n) {
     constexpr int J = decltype(jc)::value;
     R r[NREAL];
 #ifdef QCD_EXP_NOLOAD
@@ -374,7 +375,7 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
     } else
 #endif
     if constexpr (K > 0) {
-      const Vec* src = ring + (J % KR) * NP * B;
+      const Vec* src = ring + (n % KR) * NP * B;
 #pragma unroll
       for (int k = 0; k < NP; ++k) vec_unpack(src[k * B], r + k * T::VW);
     } else {
@@ -413,7 +414,7 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
   Dir cur = make_dir(0);
   const bool early = !((a.prev_parity == 1 - p && (a.prev_mu == MU || a.prev_mu == cur.nu)) || (a.prev_parity == p && a.prev_mu == cur.nu));
   auto prologue = [&]() {
-    if constexpr (K > 0) static_for<0, KR - 1>([&](auto jc) { issue(jc, cur); cp_async_commit(); });
+    if constexpr (K > 0) static_for<0, KR - 1>([&](auto jc) { issue(jc, cur, decltype(jc)::value); cp_async_commit(); });
   };
   if (early) prologue();
   pdl_wait();                                                      // the previous sub-step's links are complete and visible
@@ -424,6 +425,7 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
   m3_zero(A);
   auto direction_step = [&](int i) {
     const bool last = (i == D - 2);
+    const int n0 = ROLL ? 0 : 6 * i;                               // sequence number of this direction's first link
     const Dir nxt = make_dir(last ? i : i + 1);
     const int fsign = !FIELD ? 0 : (MU == a.f.mu && cur.nu == a.f.nu) ? 1 : (MU == a.f.nu && cur.nu == a.f.mu) ? -1 : 0;
     static_for<0, 6>([&](auto jc) {
@@ -432,10 +434,10 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
         // keep K-1 links in flight: the link K-1 ahead goes to the slot whose previous content has been consumed
         constexpr int JA = J + KR - 1;
         if constexpr (JA < 6) {
-          issue(std::integral_constant<int, JA>{}, cur);
+          issue(std::integral_constant<int, JA>{}, cur, n0 + JA);
         } else {
-          if (!last) issue(std::integral_constant<int, JA - 6>{}, nxt);
-          else if (JA == 6) issue(std::integral_constant<int, 6>{}, cur);     // the own link, once, after the last direction
+          if (!last) issue(std::integral_constant<int, JA - 6>{}, nxt, n0 + JA);
+          else if (JA == 6) issue(std::integral_constant<int, 6>{}, cur, n0 + 6);   // the own link, once, after the last direction
         }
         cp_async_commit();                                         // one group per step, possibly empty
         cp_async_wait<KR - 1>();                                   // link (i, J) has landed
@@ -444,22 +446,22 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
       if (true) {
         M3<R> Ux;
         m3_zero(Ux);
-        fetch(jc, cur, Ux, false);
+        fetch(jc, cur, Ux, false, n0 + decltype(jc)::value);
         m3_add(A, Ux);
         return;
       }
 #endif
       if constexpr (J == 0) {
-        fetch(jc, cur, P, true);                                   // U2, all rows
+        fetch(jc, cur, P, true, n0 + decltype(jc)::value);                                   // U2, all rows
       } else if constexpr (J == 1) {
         M3<R> U3;
-        fetch(jc, cur, U3, false);
+        fetch(jc, cur, U3, false, n0 + decltype(jc)::value);
         m3_zero(Q);
         m3_mad_nn<R, 2>(Q, U3, P);                                 // X = U3 U2, rows 0,1; row 2 rebuilt (XY_ROWS)
         m3_complete_row2(Q);
       } else if constexpr (J == 2) {
         M3<R> U1;
-        fetch(jc, cur, U1, false);
+        fetch(jc, cur, U1, false, n0 + decltype(jc)::value);
         M3<R> Sm;
         m3_zero(Sm);
         m3_mad_nd<R, 2>(Sm, U1, Q);                                // U1 X^+, rows 0,1; the staple is in SU(3): row 2 rebuilt
@@ -467,16 +469,16 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
         if (FIELD && fsign != 0) su3_scale_cols(Sm, a.f, fsign < 0);     // first direction: . F ; second: . F^+
         m3_add(A, Sm);
       } else if constexpr (J == 3) {
-        fetch(jc, cur, P, true);                                   // U1', all rows
+        fetch(jc, cur, P, true, n0 + decltype(jc)::value);                                   // U1', all rows
       } else if constexpr (J == 4) {
         M3<R> U2;
-        fetch(jc, cur, U2, false);
+        fetch(jc, cur, U2, false, n0 + decltype(jc)::value);
         m3_zero(Q);
         m3_mad_nn<R, 2>(Q, U2, P);                                 // Y = U2' U1', rows 0,1; row 2 rebuilt
         m3_complete_row2(Q);
       } else {
         M3<R> U3;
-        fetch(jc, cur, U3, true);
+        fetch(jc, cur, U3, true, n0 + decltype(jc)::value);
         if (FIELD && fsign != 0) su3_scale_rows(U3, a.f, fsign > 0);   // first direction: F^+ U3' ; second: F U3'
         if (COMP) {
           M3<R> Sm;
@@ -502,7 +504,7 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
   // own link: the last one through the ring
   if constexpr (K > 0) cp_async_wait<0>();
   M3<R> U;
-  fetch(std::integral_constant<int, 6>{}, cur, U, true);
+  fetch(std::integral_constant<int, 6>{}, cur, U, true, ROLL ? 6 : 6 * (D - 1));
 
 #if defined(QCD_EXP_NOCOMPUTE) || defined(QCD_EXP_NOHIT)
   if (true) {
