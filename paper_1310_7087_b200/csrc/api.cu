@@ -231,7 +231,12 @@ struct MeasureOp {
   template <int NC, int D, typename R, bool COMP> int operator()() {
     typedef typename LinkIO<NC, R, COMP>::Vec Vec;
     constexpr int NPL = D * (D - 1) / 2;
-    const uint32_t nb_plaq = ((L->g.Vh + 127) / 128) * 2;
+    // boxed thread mapping of the plaquette kernel (aux_kernels.cuh, MeasureField): one grid row of V / 128 CTAs
+    mf.boxed = (D == 4 && L->g.Lh0 % 8 == 0 && !getenv("QCD_PLAQ_LINEAR")) ? 1 : 0;
+    if (mf.boxed) {
+      mf.n0 = make_fastdiv((uint32_t)(L->g.Lh0 / 8)); mf.n1 = make_fastdiv((uint32_t)(L->g.L[1] / 2)); mf.n2 = make_fastdiv((uint32_t)(L->g.L[2] / 2));
+    }
+    const uint32_t nb_plaq = mf.boxed ? L->g.V / 128u : ((L->g.Vh + 127) / 128) * 2;
     const uint32_t Vs = L->g.V / (uint32_t)L->g.L[D - 1];
     const uint32_t nb_poly = (Vs + 127) / 128;
     const size_t need = (size_t)NPL * nb_plaq + 2 * (size_t)nb_poly;
@@ -243,6 +248,7 @@ struct MeasureOp {
     }
     double* pp = L->d_partials;
     double* pq = L->d_partials + (size_t)NPL * nb_plaq;
+    auto plaq_grid = [&]() { return mf.boxed ? dim3(L->g.V / 128, 1) : dim3((L->g.Vh + 127) / 128, 2); };
     if (want_plaq && want_poly) {
       // fork: the Polyakov kernel (one thread per spatial site, bound by the latency of its L_t dependent loads) goes first
       // on a side stream and runs beside the plaquette kernel; join before the D2H copy of the results
@@ -256,8 +262,7 @@ struct MeasureOp {
       polyakov_kernel<NC, D, R, COMP><<<nb_poly, 128, 0, L->side>>>(L->g, (const Vec*)L->mem, pq);
       final_reduce_kernel<<<2, 256, 0, L->side>>>(pq, nb_poly, L->d_results + 8, 1.0 / ((double)Vs * NC));
       CUDA_TRY(cudaEventRecord(L->ev_join, L->side));
-      dim3 grid((L->g.Vh + 127) / 128, 2);
-      plaquette_kernel<NC, D, R, COMP><<<grid, 128, 0, L->stream>>>(L->g, (const Vec*)L->mem, mf, pp);
+      plaquette_kernel<NC, D, R, COMP><<<plaq_grid(), 128, 0, L->stream>>>(L->g, (const Vec*)L->mem, mf, pp);
       final_reduce_kernel<<<NPL, 256, 0, L->stream>>>(pp, nb_plaq, L->d_results, 1.0 / ((double)L->g.V * NC));
       CUDA_TRY(cudaStreamWaitEvent(L->stream, L->ev_join, 0));
       L->launches += 4;
@@ -266,8 +271,7 @@ struct MeasureOp {
       return QCD_OK;
     }
     if (want_plaq) {
-      dim3 grid((L->g.Vh + 127) / 128, 2);
-      plaquette_kernel<NC, D, R, COMP><<<grid, 128, 0, L->stream>>>(L->g, (const Vec*)L->mem, mf, pp);
+      plaquette_kernel<NC, D, R, COMP><<<plaq_grid(), 128, 0, L->stream>>>(L->g, (const Vec*)L->mem, mf, pp);
       final_reduce_kernel<<<NPL, 256, 0, L->stream>>>(pp, nb_plaq, L->d_results, 1.0 / ((double)L->g.V * NC));
       L->launches += 2;
       L->last_parity = L->last_mu = -1;

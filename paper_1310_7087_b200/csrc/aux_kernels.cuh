@@ -214,6 +214,12 @@ __global__ void __launch_bounds__(256) final_reduce_kernel(const double* partial
 struct MeasureField {
   int enabled, mu, nu;
   double c[3], s[3];
+  // plaquette kernel, D = 4 with L0/2 a multiple of 8: a CTA covers a box of 8 half-indices x 2 x 2 x 2 sites on BOTH
+  // parities (128 threads) instead of 128 consecutive half-indices of one parity, so that the link U_nu(y) a site loads as
+  // its own and the three sites y - mu load as a neighbour meet in the same L1 (the kernel uses no shared memory, so the
+  // L1 is ~200 KB).  n0, n1, n2 = boxes per direction 0, 1, 2.
+  int boxed;
+  FastDiv n0, n1, n2;
 };
 
 // plaquette: one thread per site; the D own links stay in registers, each plane loads its two neighbours
@@ -222,82 +228,98 @@ __global__ void __launch_bounds__(128) plaquette_kernel(Geom g, const typename L
                                                         double* partials) {
   typedef LinkIO<NC, R, COMP> IO;
   constexpr int NPL = D * (D - 1) / 2;
-  const uint32_t h = blockIdx.x * blockDim.x + threadIdx.x;
-  const int p = blockIdx.y, q = 1 - p;
+  uint32_t h;
+  int p;
+  SiteCoord sc;
+  bool active;
+  if (D == 4 && f.boxed) {
+    const uint32_t t = threadIdx.x;
+    uint32_t b = blockIdx.x;
+    uint32_t qq = fd_div(b, f.n0); const uint32_t b0 = b - qq * f.n0.d; b = qq;
+    qq = fd_div(b, f.n1); const uint32_t b1 = b - qq * f.n1.d; b = qq;
+    qq = fd_div(b, f.n2); const uint32_t b2 = b - qq * f.n2.d; const uint32_t b3 = qq;
+    p = (int)(t >> 6);
+    sc.j = (int)(b0 * 8u + (t & 7u));
+    sc.x1 = (int)(b1 * 2u + ((t >> 3) & 1u));
+    sc.x2 = (int)(b2 * 2u + ((t >> 4) & 1u));
+    sc.x3 = (int)(b3 * 2u + ((t >> 5) & 1u));
+    sc.s = (p + sc.x1 + sc.x2 + sc.x3) & 1;
+    h = (uint32_t)(((sc.x3 * g.L[2] + sc.x2) * g.L[1] + sc.x1) * g.Lh0 + sc.j);
+    active = true;
+  } else {
+    h = blockIdx.x * blockDim.x + threadIdx.x;
+    p = blockIdx.y;
+    active = h < g.Vh;
+    if (active) sc = decode_site(g, h, p);
+  }
+  const int q = 1 - p;
   double acc[NPL];
 #pragma unroll
   for (int k = 0; k < NPL; ++k) acc[k] = 0.0;
-  if constexpr (NC == 3 && COMP) {
-    // 12-real links: rows 0,1 of M = U_mu(x) U_nu(x+mu) and N = U_nu(x) U_mu(x+nu) only.  With G_ab = sum_j M_aj conj(N_bj)
-    // (a, b in {0,1}) the diagonal of M N^+ is (G_00, G_11, conj(G_00 G_11 - G_01 G_10)): the third rows of SU(3)
-    // matrices are conj(row0 x row1), and (a x b).conj(c x d) = (a.conj c)(b.conj d) - (a.conj d)(b.conj c).
-    // The own links need no third row at all; the neighbours do (they are summed over in the products).
-    if (h < g.Vh) {
-      typedef PlaneTraits<R, 12> T12;
-      const SiteCoord sc = decode_site(g, h, p);
-      M3<R> own[D];
-      int fwd[D];
-#pragma unroll
-      for (int mu = 0; mu < D; ++mu) {
-        int b;
-        nbr_offsets(g, sc, mu, fwd[mu], b);
-        R r[12];
-        load_reals<R, 12, true>(links, g, array_base<T12::NP>(g, D, p, mu), h, r);
-        m3_from_reals<R, 12>(own[mu], r);
-      }
-      int plane = 0;
-#pragma unroll
-      for (int mu = 0; mu < D; ++mu)
-#pragma unroll
-        for (int nu = mu + 1; nu < D; ++nu, ++plane) {
-          M3<R> b, c, M, N;
-          R r[12];
-          load_reals<R, 12, true>(links, g, array_base<T12::NP>(g, D, q, nu), h + fwd[mu], r);   // U_nu(x+mu)
-          m3_from_reals<R, 12>(b, r);
-          m3_complete_row2(b);
-          load_reals<R, 12, true>(links, g, array_base<T12::NP>(g, D, q, mu), h + fwd[nu], r);   // U_mu(x+nu)
-          m3_from_reals<R, 12>(c, r);
-          m3_complete_row2(c);
-          m3_zero(M); m3_zero(N);
-          m3_mad_nn<R, 2>(M, own[mu], b);
-          m3_mad_nn<R, 2>(N, own[nu], c);
-          Cx<R> G00 = cx<R>(0, 0), G01 = cx<R>(0, 0), G10 = cx<R>(0, 0), G11 = cx<R>(0, 0);
-          cdot3<CD_ND>(G00, M.e[0][0], M.e[0][1], M.e[0][2], N.e[0][0], N.e[0][1], N.e[0][2]);
-          cdot3<CD_ND>(G01, M.e[0][0], M.e[0][1], M.e[0][2], N.e[1][0], N.e[1][1], N.e[1][2]);
-          cdot3<CD_ND>(G10, M.e[1][0], M.e[1][1], M.e[1][2], N.e[0][0], N.e[0][1], N.e[0][2]);
-          cdot3<CD_ND>(G11, M.e[1][0], M.e[1][1], M.e[1][2], N.e[1][0], N.e[1][1], N.e[1][2]);
-          const Cx<R> dd = cmul(G00, G11), od = cmul(G01, G10);
-          const Cx<R> D2 = cx<R>(dd.re - od.re, -(dd.im - od.im));
-          const bool dressed = f.enabled && f.mu == mu && f.nu == nu;
-          const R tr = dressed ? (G00.re * (R)f.c[0] - G00.im * (R)f.s[0]) + (G11.re * (R)f.c[1] - G11.im * (R)f.s[1]) +
-                                     (D2.re * (R)f.c[2] - D2.im * (R)f.s[2])
-                               : G00.re + G11.re + D2.re;
-          acc[plane] += (double)tr;
-        }
-    }
-  } else if (h < g.Vh) {
-    const SiteCoord sc = decode_site(g, h, p);
-    Cx<R> own[D][NC][NC];
+  // One plane at a time, loop NOT unrolled: the four links of a plane are loaded when the plane is reached, so a thread
+  // holds one plane's worth of registers (fp64 x18 needed 254 registers with the own links kept across planes: 2 CTAs per
+  // SM, and the kernel is bound by load latency).  The own links are re-read per plane; they hit in L1 (boxed mapping).
+  if (active) {
     int fwd[D];
 #pragma unroll
-    for (int mu = 0; mu < D; ++mu) {
-      int b;
-      nbr_offsets(g, sc, mu, fwd[mu], b);
-      IO::template load<true>(own[mu], links, g, array_base<IO::T::NP>(g, D, p, mu), h);
-    }
-    int plane = 0;
+    for (int d = 0; d < D; ++d) { int bb; nbr_offsets(g, sc, d, fwd[d], bb); }
+#pragma unroll 1
+    for (int pl = 0; pl < NPL; ++pl) {
+      // plane index -> (mu, nu), mu < nu, in the order (0,1),(0,2),..,(D-2,D-1)
+      int mu = 0, nu = 1;
+      {
+        int k = pl;
 #pragma unroll
-    for (int mu = 0; mu < D; ++mu)
+        for (int m = 0; m < D - 1; ++m) { const int cnt = D - 1 - m; if (k >= cnt && mu == m) { k -= cnt; mu = m + 1; } }
+        nu = mu + 1 + k;
+      }
+      int fmu = fwd[0], fnu = fwd[0];
 #pragma unroll
-      for (int nu = mu + 1; nu < D; ++nu, ++plane) {
-        Cx<R> b[NC][NC], c[NC][NC], ab[NC][NC], dc[NC][NC];
-        IO::template load<true>(b, links, g, array_base<IO::T::NP>(g, D, q, nu), h + fwd[mu]);   // U_nu(x+mu)
-        IO::template load<true>(c, links, g, array_base<IO::T::NP>(g, D, q, mu), h + fwd[nu]);   // U_mu(x+nu)
-        mm_nn<NC, R>(ab, own[mu], b);        // U_mu(x) U_nu(x+mu)
-        mm_nn<NC, R>(dc, own[nu], c);        // U_nu(x) U_mu(x+nu)
+      for (int d = 1; d < D; ++d) { if (mu == d) fmu = fwd[d]; if (nu == d) fnu = fwd[d]; }
+      const bool dressed = f.enabled && f.mu == mu && f.nu == nu;
+      R tr;
+      if constexpr (NC == 3 && COMP) {
+        // 12-real links: rows 0,1 of M = U_mu(x) U_nu(x+mu) and N = U_nu(x) U_mu(x+nu) only.  With
+        // G_ab = sum_j M_aj conj(N_bj) (a, b in {0,1}) the diagonal of M N^+ is (G_00, G_11, conj(G_00 G_11 - G_01 G_10)):
+        // third rows of SU(3) matrices are conj(row0 x row1), and (a x b).conj(c x d) = (a.conj c)(b.conj d) - (a.conj d)(b.conj c).
+        // The own links need no third row at all; the neighbours do (they are summed over in the products).
+        typedef PlaneTraits<R, 12> T12;
+        M3<R> u, w, M, N;
+        R r[12];
+        load_reals<R, 12, true>(links, g, array_base<T12::NP>(g, D, q, nu), h + fmu, r);          // U_nu(x+mu)
+        m3_from_reals<R, 12>(w, r);
+        m3_complete_row2(w);
+        load_reals<R, 12, true>(links, g, array_base<T12::NP>(g, D, p, mu), h, r);                // U_mu(x)
+        m3_from_reals<R, 12>(u, r);
+        m3_zero(M);
+        m3_mad_nn<R, 2>(M, u, w);
+        load_reals<R, 12, true>(links, g, array_base<T12::NP>(g, D, q, mu), h + fnu, r);          // U_mu(x+nu)
+        m3_from_reals<R, 12>(w, r);
+        m3_complete_row2(w);
+        load_reals<R, 12, true>(links, g, array_base<T12::NP>(g, D, p, nu), h, r);                // U_nu(x)
+        m3_from_reals<R, 12>(u, r);
+        m3_zero(N);
+        m3_mad_nn<R, 2>(N, u, w);
+        Cx<R> G00 = cx<R>(0, 0), G01 = cx<R>(0, 0), G10 = cx<R>(0, 0), G11 = cx<R>(0, 0);
+        cdot3<CD_ND>(G00, M.e[0][0], M.e[0][1], M.e[0][2], N.e[0][0], N.e[0][1], N.e[0][2]);
+        cdot3<CD_ND>(G01, M.e[0][0], M.e[0][1], M.e[0][2], N.e[1][0], N.e[1][1], N.e[1][2]);
+        cdot3<CD_ND>(G10, M.e[1][0], M.e[1][1], M.e[1][2], N.e[0][0], N.e[0][1], N.e[0][2]);
+        cdot3<CD_ND>(G11, M.e[1][0], M.e[1][1], M.e[1][2], N.e[1][0], N.e[1][1], N.e[1][2]);
+        const Cx<R> dd = cmul(G00, G11), od = cmul(G01, G10);
+        const Cx<R> D2 = cx<R>(dd.re - od.re, -(dd.im - od.im));
+        tr = dressed ? (G00.re * (R)f.c[0] - G00.im * (R)f.s[0]) + (G11.re * (R)f.c[1] - G11.im * (R)f.s[1]) +
+                           (D2.re * (R)f.c[2] - D2.im * (R)f.s[2])
+                     : G00.re + G11.re + D2.re;
+      } else {
+        Cx<R> u[NC][NC], w[NC][NC], ab[NC][NC], dc[NC][NC];
+        IO::template load<true>(u, links, g, array_base<IO::T::NP>(g, D, p, mu), h);             // U_mu(x)
+        IO::template load<true>(w, links, g, array_base<IO::T::NP>(g, D, q, nu), h + fmu);       // U_nu(x+mu)
+        mm_nn<NC, R>(ab, u, w);
+        IO::template load<true>(u, links, g, array_base<IO::T::NP>(g, D, p, nu), h);             // U_nu(x)
+        IO::template load<true>(w, links, g, array_base<IO::T::NP>(g, D, q, mu), h + fnu);       // U_mu(x+nu)
+        mm_nn<NC, R>(dc, u, w);
         // Re Tr [F] ab dc^+ = sum_i Re( ph_i * sum_j ab_ij conj(dc_ij) )
-        R tr = R(0);
-        const bool dressed = f.enabled && f.mu == mu && f.nu == nu;
+        tr = R(0);
 #pragma unroll
         for (int i = 0; i < NC; ++i) {
           Cx<R> d = cx<R>(0, 0);
@@ -305,8 +327,10 @@ __global__ void __launch_bounds__(128) plaquette_kernel(Geom g, const typename L
           for (int j = 0; j < NC; ++j) cmad_conj(d, ab[i][j], dc[i][j]);
           tr += dressed ? (d.re * (R)f.c[i] - d.im * (R)f.s[i]) : d.re;
         }
-        acc[plane] += (double)tr;
       }
+#pragma unroll
+      for (int k = 0; k < NPL; ++k) acc[k] += (k == pl) ? (double)tr : 0.0;
+    }
   }
   block_reduce_store<NPL, 128>(acc, partials, gridDim.x * gridDim.y, blockIdx.y * gridDim.x + blockIdx.x);
 }
