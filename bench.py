@@ -44,8 +44,8 @@ FLOPS_PER_HIT = {"f32": {"hb": 4270.0, "or": 4030.0}, "f64": {"hb": 3900.0, "or"
 # the dominant kernel of each arm (overrelaxation: 32 of the 40 update launches of a step) and its DRAM traffic per launch,
 # dram__bytes_read.sum + dram__bytes_write.sum of one `ncu --set full` capture of this workload (bytes)
 OR_KERNEL = {"f32": "su3_update_tiled_kernel<float, x12, OR>", "f64": "su3_update_kernel<double, x18, OR>"}
-NCU_TRAFFIC = {"f32": {"or": 222280960, "hb": 221551616}, "f64": {"or": 674697984, "hb": 672201984},
-               "source": "profiles/r1_e_launches_and_ncu.md"}
+NCU_TRAFFIC = {"f32": {"or": 222129920, "hb": 221493248}, "f64": {"or": 674832128, "hb": 671554816},
+               "source": "profiles/r1_f_launches_and_ncu.md"}
 
 
 def load_peaks():
