@@ -149,6 +149,19 @@ def time_arm(q, torch, prec_name, steps, warmup, therm, seed, dist, sampler, do_
         G.qcd_set_option(q.QCD_OPT_PROFILE, 0)
         out.update(ms_total=ms, plaquette=plaq, polyakov_abs=abs(poly), hb_ms=hb_ms, hb_n=hb_n, or_ms=or_ms, or_n=or_n)
         out["sweep_counter"] = G.qcd_get_sweep_counter()
+        # the same working sweep with the observables accumulated on the device (qcd_measure_accumulate: no host
+        # synchronisation per step, one qcd_accum_get at the end) -- reported beside the headline, not instead of it
+        G.qcd_accum_reset()
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(steps):
+            G.qcd_sweep(BETA, N_HB, N_OR)
+            G.qcd_measure_accumulate()
+        e1.record()
+        n_acc, s1, _ = G.qcd_accum_get()
+        torch.cuda.synchronize()
+        out["acc_ms_total"] = e0.elapsed_time(e1)
+        out["acc_plaquette_mean"] = float(s1[:6].mean() / max(n_acc, 1))
 
         if do_e2e:
             # end to end through the C ABI with HOST buffers: every step uploads the configuration from pinned host
@@ -263,6 +276,9 @@ def run_ours(args):
             frag[name] = {"value": value, "ms_per_step": ms_step, "roofline": roof,
                           "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": a["h2d"], "d2h_bytes_per_step": a["d2h"],
                                   "ms_per_step": a["e2e_ms_total"] / args.steps},
+                          "accumulate_on_device": {"ms_per_step": a["acc_ms_total"] / args.steps,
+                                                   "value": aggregate_value(world, a["links"], args.steps, a["acc_ms_total"]),
+                                                   "plaquette_mean": a["acc_plaquette_mean"]},
                           "gpu_launches": a["launches"], "plaquette": a["plaquette"], "polyakov_abs": a["polyakov_abs"],
                           "dtype": name, "storage": "12 reals/link" if name == "f32" else "18 reals/link"}
         p = frag[primary]
@@ -275,6 +291,7 @@ def run_ours(args):
                            "storage": p["storage"], "replicas": world, "thermalisation_sweeps_before_warmup": args.therm,
                            "l2": "inputs larger than L2: %d MB of links vs 126 MB" % (arms[primary]["links"] * LINK_BYTES[primary] // 2 ** 20)},
                 "e2e": p["e2e"], "gpu_launches": p["gpu_launches"], "roofline": p["roofline"], "clocks": clocks,
+                "accumulate_on_device": p["accumulate_on_device"],
                 "observables": {"plaquette": p["plaquette"], "polyakov_abs": p["polyakov_abs"]},
                 "other_precision": frag[other]}
         if world == 1 and not args.no_cpu_baseline:

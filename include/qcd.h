@@ -87,6 +87,16 @@ int qcd_sweep(qcd_lattice_t* lat, double beta, int n_hb, int n_or, const qcd_fie
  * Site arithmetic in the lattice's precision, accumulation in fp64, deterministic.  Synchronises the stream. */
 int qcd_measure(qcd_lattice_t* lat, const qcd_field_t* field, double* plaq_total, double* plaq_planes, double* polyakov_re_im);
 
+/* On-device accumulation over configurations (the paper keeps its measurements on the device until
+ * the end of a run).  qcd_measure_accumulate measures like qcd_measure and adds the NQ = D(D-1)/2 + 3
+ * quantities (plane plaquettes in qcd_measure's order, Re L, Im L, |L|) and their squares to accumulators in device
+ * memory; it is asynchronous (no host synchronisation, nothing returned).  qcd_accum_get synchronises and returns the
+ * number of accumulated measurements and the NQ sums and sums of squares (host arrays of `capacity` >= NQ doubles);
+ * qcd_accum_reset zeroes the accumulators (they start at zero).  Fixed summation order: bit-reproducible. */
+int qcd_measure_accumulate(qcd_lattice_t* lat, const qcd_field_t* field);
+int qcd_accum_get(qcd_lattice_t* lat, uint64_t* count, double* sum, double* sumsq, int capacity);
+int qcd_accum_reset(qcd_lattice_t* lat);
+
 /* Copy links out of / into the lattice in the canonical layout.  bytes must equal V*D*N*N*2*sizeof(real).
  * dst_is_device / src_is_device: the pointer is a DEVICE pointer (then the call is asynchronous on the stream).
  * qcd_set_links does not reunitarise; with COMPRESS12 row 2 of the input is dropped; SU(2) input is read from

@@ -24,7 +24,7 @@ SYMBOLS = [
     "qcd_lattice_bytes", "qcd_lattice_create", "qcd_lattice_destroy", "qcd_init", "qcd_sweep", "qcd_measure",
     "qcd_get_links", "qcd_set_links", "qcd_get_sweep_counter", "qcd_set_sweep_counter", "qcd_get_seed", "qcd_set_seed",
     "qcd_set_option", "qcd_debug_substep", "qcd_debug_get_trials", "qcd_debug_philox", "qcd_get_profile",
-    "qcd_reset_profile", "qcd_get_launch_count", "qcd_probe_fma_tflops", "qcd_probe_copy_gbs", "qcd_last_error",
+    "qcd_reset_profile", "qcd_get_launch_count", "qcd_measure_accumulate", "qcd_accum_get", "qcd_accum_reset", "qcd_probe_fma_tflops", "qcd_probe_copy_gbs", "qcd_last_error",
     "qcd_version",
 ]
 
@@ -61,6 +61,9 @@ def lib():
     L.qcd_init.argtypes = [p, i, C.c_uint64]
     L.qcd_sweep.argtypes = [p, d, i, i, fp]
     L.qcd_measure.argtypes = [p, fp, dp, dp, dp]
+    L.qcd_measure_accumulate.argtypes = [p, fp]
+    L.qcd_accum_get.argtypes = [p, C.POINTER(C.c_uint64), dp, dp, i]
+    L.qcd_accum_reset.argtypes = [p]
     L.qcd_get_links.argtypes = [p, p, sz, i]
     L.qcd_set_links.argtypes = [p, p, sz, i]
     L.qcd_get_sweep_counter.argtypes = [p, C.POINTER(C.c_uint32)]
@@ -186,6 +189,20 @@ class Lattice:
         _check(lib().qcd_measure(self._h, _fref(field), C.byref(tot) if plaquette else None, planes if plaquette else None,
                                  poly if polyakov else None))
         return tot.value, np.array(planes[:]), complex(poly[0], poly[1])
+
+    def qcd_measure_accumulate(self, field=None):
+        _check(lib().qcd_measure_accumulate(self._h, _fref(field)))
+
+    def qcd_accum_reset(self):
+        _check(lib().qcd_accum_reset(self._h))
+
+    def qcd_accum_get(self):
+        """(count, sums, sums of squares) of the D(D-1)/2 plane plaquettes, Re L, Im L, |L|"""
+        nq = self.D * (self.D - 1) // 2 + 3
+        n = C.c_uint64(0)
+        s1, s2 = (C.c_double * nq)(), (C.c_double * nq)()
+        _check(lib().qcd_accum_get(self._h, C.byref(n), s1, s2, nq))
+        return int(n.value), np.array(s1[:]), np.array(s2[:])
 
     def qcd_get_links(self):
         """canonical (V, D, N, N) complex array in the lattice's precision (host)"""

@@ -49,8 +49,8 @@ struct qcd_lattice {
   uint8_t* d_trials;
   double* d_partials;
   size_t partials_cap;   // doubles
-  double* d_results;     // 16 doubles
-  double* h_results;     // pinned, 16 doubles
+  double* d_results;     // 48 doubles: last measurement + accumulator (see qcd_lattice_create)
+  double* h_results;     // pinned, 48 doubles
   std::vector<EventPair> ev_used, ev_free;
   double prof_ms[2];
   uint64_t prof_n[2];
@@ -371,8 +371,11 @@ int qcd_lattice_create(int D, const int* dims, int Nc, int precision, unsigned f
     if (e != cudaSuccess) { delete L; return fail(QCD_ERR_ALLOC, std::string("cudaMalloc links: ") + cudaGetErrorString(e)); }
     L->owns_mem = true;
   }
-  if (e == cudaSuccess) e = cudaMalloc(&L->d_results, 16 * sizeof(double));
-  if (e == cudaSuccess) e = cudaMallocHost(&L->h_results, 16 * sizeof(double));
+  // d_results: [0,16) the last measurement (planes at 0.., Polyakov at 8,9); [16,48) the accumulator of
+  // qcd_measure_accumulate: count, then NQ sums, then NQ sums of squares (NQ <= 9)
+  if (e == cudaSuccess) e = cudaMalloc(&L->d_results, 48 * sizeof(double));
+  if (e == cudaSuccess) e = cudaMemsetAsync(L->d_results, 0, 48 * sizeof(double), L->stream);
+  if (e == cudaSuccess) e = cudaMallocHost(&L->h_results, 48 * sizeof(double));
   // padding lanes of every plane are never read, but keep the workspace defined
   if (e == cudaSuccess) e = cudaMemsetAsync(L->mem, 0, need, L->stream);
   if (e != cudaSuccess) { std::string m = cudaGetErrorString(e); qcd_lattice_destroy(L); return fail(QCD_ERR_CUDA, "create: " + m); }
@@ -464,21 +467,64 @@ int qcd_debug_get_trials(qcd_lattice_t* L, uint8_t* dst, size_t bytes) {
   return QCD_OK;
 }
 
-int qcd_measure(qcd_lattice_t* L, const qcd_field_t* field, double* plaq_total, double* plaq_planes, double* polyakov) {
+// enqueue the measurement kernels (results land in d_results); no synchronisation
+static int enqueue_measure(qcd_lattice_t* L, const qcd_field_t* field, bool want_plaq, bool want_poly) {
   if (!L) return fail(QCD_ERR_INVALID_ARG, "lattice is NULL");
   if (!L->has_links) return fail(QCD_ERR_STATE, "no links yet");
   bool fon;
   int rc = check_field(L, field, &fon);
   if (rc != QCD_OK) return rc;
   MeasureOp op;
-  op.L = L; op.want_plaq = (plaq_total || plaq_planes); op.want_poly = polyakov != nullptr;
+  op.L = L; op.want_plaq = want_plaq; op.want_poly = want_poly;
   memset(&op.mf, 0, sizeof(op.mf));
   FieldArgs fa = make_field_args(field, fon, L->Nc);
   op.mf.enabled = fon ? 1 : 0; op.mf.mu = fa.mu; op.mf.nu = fa.nu;
   for (int c = 0; c < 3; ++c) { op.mf.c[c] = fa.c[c]; op.mf.s[c] = fa.s[c]; }
   if (!op.want_plaq && !op.want_poly) return QCD_OK;
-  rc = dispatch(L, op);
+  return dispatch(L, op);
+}
+
+// accumulator update: one thread per quantity (npl plane plaquettes, Re L, Im L, |L|), fixed order => deterministic
+__global__ void accum_kernel(const double* res, double* acc, int npl) {
+  const int k = (int)threadIdx.x, nq = npl + 3;
+  if (k >= nq) return;
+  const double v = k < npl ? res[k] : k == npl ? res[8] : k == npl + 1 ? res[9] : hypot(res[8], res[9]);
+  acc[1 + k] += v;
+  acc[1 + nq + k] += v * v;
+  if (k == 0) acc[0] += 1.0;
+}
+
+int qcd_measure_accumulate(qcd_lattice_t* L, const qcd_field_t* field) {
+  int rc = enqueue_measure(L, field, true, true);
   if (rc != QCD_OK) return rc;
+  accum_kernel<<<1, 32, 0, L->stream>>>(L->d_results, L->d_results + 16, L->D * (L->D - 1) / 2);
+  L->launches += 1;
+  CUDA_TRY(cudaGetLastError());
+  return QCD_OK;
+}
+
+int qcd_accum_reset(qcd_lattice_t* L) {
+  if (!L) return fail(QCD_ERR_INVALID_ARG, "lattice is NULL");
+  CUDA_TRY(cudaMemsetAsync(L->d_results + 16, 0, 32 * sizeof(double), L->stream));
+  return QCD_OK;
+}
+
+int qcd_accum_get(qcd_lattice_t* L, uint64_t* count, double* sum, double* sumsq, int capacity) {
+  if (!L || !count || !sum || !sumsq) return fail(QCD_ERR_INVALID_ARG, "NULL argument");
+  const int nq = L->D * (L->D - 1) / 2 + 3;
+  if (capacity < nq) return fail(QCD_ERR_INVALID_ARG, "capacity must be >= D(D-1)/2 + 3");
+  CUDA_TRY(cudaMemcpyAsync(L->h_results + 16, L->d_results + 16, 32 * sizeof(double), cudaMemcpyDeviceToHost, L->stream));
+  CUDA_TRY(cudaStreamSynchronize(L->stream));
+  *count = (uint64_t)L->h_results[16];
+  for (int k = 0; k < nq; ++k) { sum[k] = L->h_results[17 + k]; sumsq[k] = L->h_results[17 + nq + k]; }
+  return QCD_OK;
+}
+
+int qcd_measure(qcd_lattice_t* L, const qcd_field_t* field, double* plaq_total, double* plaq_planes, double* polyakov) {
+  struct { bool want_plaq, want_poly; } op = {plaq_total || plaq_planes, polyakov != nullptr};
+  int rc = enqueue_measure(L, field, op.want_plaq, op.want_poly);
+  if (rc != QCD_OK) return rc;
+  if (!op.want_plaq && !op.want_poly) return QCD_OK;
   CUDA_TRY(cudaMemcpyAsync(L->h_results, L->d_results, 16 * sizeof(double), cudaMemcpyDeviceToHost, L->stream));
   CUDA_TRY(cudaStreamSynchronize(L->stream));
   const int npl = L->D * (L->D - 1) / 2;

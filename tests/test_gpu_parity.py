@@ -303,6 +303,46 @@ def test_substeps_back_to_back_in_any_order(qcd, variant):
             assert diff < (1e-11 if prec == 1 else 2e-4), (rep, diff)
 
 
+@pytest.mark.parametrize("dims,Nc,fld", [((8, 8, 8, 4), 3, None), ((8, 8, 8, 4), 3, (0, 1)), ((16, 16), 2, None), ((6, 4, 10), 3, (0, 2))])
+def test_measure_accumulate_matches_measure_and_oracle(qcd, dims, Nc, fld):
+    """qcd_measure_accumulate / qcd_accum_get (on-device sums and sums of squares over configurations, no host
+    synchronisation per measurement) against (i) the values qcd_measure returns for the same configurations, summed on the
+    host in the same order, and (ii) the oracle's sweeps and measurements."""
+    beta, n_meas = 5.7 if Nc == 3 else 2.0, 6
+    if fld is not None:
+        fld = (fld[0], fld[1], [0.4, 0.3, -0.7])
+    fg, fo = field_pair(qcd, fld)
+    D = len(dims)
+    npl = D * (D - 1) // 2
+    O = oracle.OracleLattice(dims, Nc)
+    O.init(oracle.HOT, 11)
+    host = np.zeros((2, npl + 3))
+    orac = np.zeros((2, npl + 3))
+    with gpu_lattice(qcd, dims, Nc, 1, 0) as G:
+        G.qcd_init(qcd.QCD_HOT, 11)
+        n0, s0, q0 = G.qcd_accum_get()
+        assert n0 == 0 and not s0.any() and not q0.any()
+        for _ in range(n_meas):
+            O.sweep(beta, 1, 2, fo)
+            G.qcd_set_links(O.get_links())                         # the oracle's configurations (sweeps are tested elsewhere;
+            G.qcd_measure_accumulate(fg)                           # un-resynced trajectories separate chaotically)
+            _, planes, poly = G.qcd_measure(fg)                    # same configuration, deterministic reductions
+            v = np.concatenate([planes, [poly.real, poly.imag, abs(poly)]])
+            host[0] += v
+            host[1] += v * v
+            _, planes_o, poly_o = O.measure(fo)
+            vo = np.concatenate([planes_o, [poly_o.real, poly_o.imag, abs(poly_o)]])
+            orac[0] += vo
+            orac[1] += vo * vo
+        n, s1, s2 = G.qcd_accum_get()
+        assert n == n_meas
+        assert np.max(np.abs(s1 - host[0])) < 1e-14 * n_meas and np.max(np.abs(s2 - host[1])) < 1e-14 * n_meas
+        assert np.max(np.abs(s1 - orac[0])) < 1e-11 and np.max(np.abs(s2 - orac[1])) < 1e-11
+        G.qcd_accum_reset()
+        n, s1, s2 = G.qcd_accum_get()
+        assert n == 0 and not s1.any() and not s2.any()
+
+
 def test_overrelaxation_conserves_action_on_gpu(qcd):
     dims = (8, 8, 8, 8)
     for Nc, prec, flags, tol in [(3, 1, 0, 1e-12), (3, 0, 1, 3e-6), (2, 1, 0, 1e-12)]:
