@@ -401,3 +401,22 @@ def test_single_link_update_matches_substep():
     trials = L.substep(5.7, oracle.KIND_HB, 0, 1, 1, want_trials=True)
     assert np.array_equal(L.get_links()[9, 1], one)
     assert np.array_equal(trials[9], codes) and np.all(codes >= 1)
+
+
+@pytest.mark.parametrize("Nc,beta,lit", [(3, 6.0, 0.5937), (2, 2.5, 0.6520)], ids=["su3-beta6.0", "su2-beta2.5"])
+def test_4d_plaquette_at_production_beta_near_literature_value(Nc, beta, lit):
+    """Loose cross-check of what has no closed form (oracle header: "parity unpinned"): the 4-D Wilson-action plaquette at
+    the production couplings of BASELINE.json configs 3 and 4 against the standard Monte Carlo values of the lattice
+    literature (SU(3) beta = 6.0: 0.5937; SU(2) beta = 2.5: 0.6520; large volume).  On 8^4 the finite-volume shift is
+    +1e-3 and the statistical error of this short run 4e-4, so the bar is 3e-3: enough to catch a dropped staple, a wrong
+    normalisation of beta (beta/N vs beta/2N) or a biased heatbath, each of which moves the plaquette by 1e-2 or more.
+    The value is not the paper's (it prints none); it does not promote the item to "pinned"."""
+    O = make((8, 8, 8, 8), Nc)
+    O.init(oracle.HOT, 5)
+    for _ in range(60):
+        O.sweep(beta, 1, 4)
+    vals = []
+    for _ in range(120):
+        O.sweep(beta, 1, 4)
+        vals.append(O.measure()[0])
+    assert abs(float(np.mean(vals)) - lit) < 3e-3, float(np.mean(vals))
