@@ -58,7 +58,8 @@ typedef struct {
   double theta[3];
 } qcd_field_t;
 
-/* Bytes of device workspace a lattice needs (links in the internal layout).  0 on invalid arguments. */
+/* Bytes of device workspace a lattice needs (links in the internal layout).  0 on invalid arguments and on lattices
+ * beyond the kernels' 32-bit vector indexing (2 D NP V/2 >= 2^32 vectors of 16 bytes: e.g. 128^4 in fp64; UNSUPPORTED). */
 size_t qcd_lattice_bytes(int D, const int* dims, int Nc, int precision, unsigned flags);
 
 /* Create a lattice.  device_mem: DEVICE pointer to >= qcd_lattice_bytes() bytes, 256-byte aligned, owned by the

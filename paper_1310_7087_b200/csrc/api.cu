@@ -91,6 +91,10 @@ bool valid_shape(int D, const int* dims, int Nc, int precision, unsigned flags, 
   }
   if (v > 2147483648.0) return false;          // V/2 and lex must fit 32-bit (Philox c0 = lex)
   if ((flags & QCD_FLAG_COMPRESS12) && Nc == 2) { *why = QCD_ERR_UNSUPPORTED; return false; }
+  // the kernels index the 2 D NP planes of Vh_pad vectors with 32 bits
+  int nreal, vb, np;
+  plane_params(Nc, precision, (flags & QCD_FLAG_COMPRESS12) != 0, &nreal, &vb, &np);
+  if (2.0 * D * np * (v / 2.0 + 32.0) >= 4294967296.0) { *why = QCD_ERR_UNSUPPORTED; return false; }
   return true;
 }
 
