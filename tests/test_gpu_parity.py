@@ -653,6 +653,27 @@ def test_config5_su3_64to4_fp64_properties_at_full_size(qcd):
         assert abs(p2 - p1) < 1e-12, (p1, p2)
 
 
+def test_largest_indexable_lattice_128to4_fp32(qcd):
+    """Edge of the 32-bit vector indexing: SU(3) 128^4 with 12-real fp32 links (51.5 GB, 3.2e9 vectors).  Too large for any
+    host-side comparison; checked by what holds at any size: the cold start measures plaquette = Polyakov loop = 1 exactly,
+    a hot start measures ~0, a heatbath sweep moves the plaquette to its beta = 6 neighbourhood on every plane, and an
+    overrelaxation sweep conserves it (a wrapped or truncated index would break each of these)."""
+    with gpu_lattice(qcd, (128, 128, 128, 128), 3, 0, 1) as G:
+        G.qcd_init(qcd.QCD_COLD, 1)
+        tot, planes, poly = G.qcd_measure()
+        assert tot == 1.0 and np.all(planes == 1.0) and poly == 1.0
+        G.qcd_init(qcd.QCD_HOT, 1)
+        tot, planes, poly = G.qcd_measure()
+        assert abs(tot) < 1e-4 and np.max(np.abs(planes)) < 1e-4 and abs(poly) < 1.5e-3    # 1.4e-5 / 2.3e-4 statistical sigma
+        G.qcd_sweep(6.0, 1, 0)
+        G.qcd_sweep(6.0, 1, 0)
+        p1, planes, _ = G.qcd_measure()
+        assert 0.3 < p1 < 0.62 and np.max(np.abs(planes - p1)) < 2e-2     # two sweeps from hot: planes still order-dependent at 5e-3
+        G.qcd_sweep(6.0, 0, 2)
+        p2, planes2, _ = G.qcd_measure()
+        assert abs(p2 - p1) < 3e-6, (p1, p2)
+
+
 # ----------------------------------------------------------------------------- ABI error paths on a live device
 def test_error_paths(qcd):
     with pytest.raises(qcd.QcdError) as e:
