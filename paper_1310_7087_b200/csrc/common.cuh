@@ -2,7 +2,7 @@
 //
 // Link layout in HBM ("fastest index - number of lattice site ... next
 // index - direction ... group matrices are represented as structures of 4-vectors"):
-//   vec-plane SoA   links[parity p][direction mu][plane k][half-index h]     (h fastest)
+//   vec-plane SoA   links[parity p][direction mu][h / 8][plane k][h % 8]     (blocks of 8 half-indices, see blk_off)
 // where a site x of parity p = (sum x_d) & 1 has h = lex(x) >> 1, lex = x0 + L0*(x1 + L1*(x2 + L2*x3)), and the
 // NREAL stored reals of one link (row-major, re then im) are cut into NP = NREAL/VW planes of VW-wide vectors:
 //   SU(3) fp32 x12 : 3 x float4      SU(3) fp32 x18 : 9 x float2
@@ -120,15 +120,22 @@ __device__ __forceinline__ size_t array_base(const Geom& g, int D, int parity, i
   return (size_t)((parity * D + mu) * NP) * (size_t)g.Vh_pad;
 }
 
+// Inside one (parity, mu) array the vector of (half-index h, plane k) sits at  (h / 8) * (8 NP) + k * 8 + (h % 8):
+// blocks of 8 half-indices (128 bytes of 16-byte vectors) with their NP planes back to back, so the planes of a link are
+// PLANE_STRIDE vectors apart (an immediate offset) and all of a link lies within NP * 128 bytes (page locality on large
+// lattices).  A warp's load of one plane of 8 consecutive half-indices is still one full 128-byte line.
+constexpr int PLANE_STRIDE = 8;
+template <int NP> __device__ __forceinline__ uint32_t blk_off(uint32_t h) { return (h >> 3) * (8u * NP) + (h & 7u); }
+
 // load the NREAL reals of link h of the array starting at `base` (vectors); NC = through the read-only path
 template <typename R, int NREAL, bool NC>
 __device__ __forceinline__ void load_reals(const typename PlaneTraits<R, NREAL>::Vec* __restrict__ links, const Geom& g,
                                            size_t base, uint32_t h, R* out) {
   typedef PlaneTraits<R, NREAL> T;
-  const typename T::Vec* p = links + base + h;
+  const typename T::Vec* p = links + base + blk_off<T::NP>(h);
 #pragma unroll
   for (int k = 0; k < T::NP; ++k) {
-    typename T::Vec v = NC ? __ldg(p + (size_t)k * g.Vh_pad) : p[(size_t)k * g.Vh_pad];
+    typename T::Vec v = NC ? __ldg(p + k * PLANE_STRIDE) : p[k * PLANE_STRIDE];
     vec_unpack(v, out + k * T::VW);
   }
 }
@@ -136,12 +143,12 @@ template <typename R, int NREAL>
 __device__ __forceinline__ void store_reals(typename PlaneTraits<R, NREAL>::Vec* links, const Geom& g, size_t base, uint32_t h,
                                             const R* in) {
   typedef PlaneTraits<R, NREAL> T;
-  typename T::Vec* p = links + base + h;
+  typename T::Vec* p = links + base + blk_off<T::NP>(h);
 #pragma unroll
   for (int k = 0; k < T::NP; ++k) {
     typename T::Vec v;
     vec_pack(v, in + k * T::VW);
-    p[(size_t)k * g.Vh_pad] = v;
+    p[k * PLANE_STRIDE] = v;
   }
 }
 

@@ -325,30 +325,31 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
 #pragma unroll
   for (int d = 0; d < D; ++d) nbr_offsets(g, sc, d, fo[d], bo[d]);
   const uint32_t arr = (uint32_t)NP * g.Vh_pad;                    // vectors per (parity, direction) array
-  const uint32_t own_idx = (uint32_t)(p * D + MU) * arr + h;
-  const uint32_t qmu_idx = (uint32_t)((1 - p) * D + MU) * arr + h;
+  const uint32_t own_base = (uint32_t)(p * D + MU) * arr;         // array bases (vectors); elements at base + blk_off(h')
+  const uint32_t qmu_base = (uint32_t)((1 - p) * D + MU) * arr;
+  auto at = [&](uint32_t base, int off) -> uint32_t { return base + blk_off<NP>(h + (uint32_t)off); };
 
-  struct Dir { uint32_t p_idx, q_idx; int f, b, nu; };             // per-direction addressing, run-time nu
+  struct Dir { uint32_t p_idx, q_idx; int f, b, nu; };             // per-direction addressing (array bases), run-time nu
   auto make_dir = [&](int i) {
     Dir d;
     d.nu = i + (i >= MU ? 1 : 0);
     d.f = fo[0]; d.b = bo[0];
 #pragma unroll
     for (int k = 1; k < D; ++k) if (d.nu == k) { d.f = fo[k]; d.b = bo[k]; }
-    d.p_idx = (uint32_t)(p * D + d.nu) * arr + h;
-    d.q_idx = (uint32_t)((1 - p) * D + d.nu) * arr + h;
+    d.p_idx = (uint32_t)(p * D + d.nu) * arr;
+    d.q_idx = (uint32_t)((1 - p) * D + d.nu) * arr;
     return d;
   };
   // vector index of plane 0 of link j of direction d (j = 6: the own link)
   auto link_idx = [&](auto jc, const Dir& d) -> uint32_t {
     constexpr int J = decltype(jc)::value;
-    if constexpr (J == 0) return qmu_idx + (uint32_t)d.f;
-    else if constexpr (J == 1) return d.p_idx;
-    else if constexpr (J == 2) return d.q_idx + (uint32_t)fo[MU];
-    else if constexpr (J == 3) return d.p_idx + (uint32_t)(fo[MU] + d.b);
-    else if constexpr (J == 4) return qmu_idx + (uint32_t)d.b;
-    else if constexpr (J == 5) return d.q_idx + (uint32_t)d.b;
-    else return own_idx;
+    if constexpr (J == 0) return at(qmu_base, d.f);
+    else if constexpr (J == 1) return at(d.p_idx, 0);
+    else if constexpr (J == 2) return at(d.q_idx, fo[MU]);
+    else if constexpr (J == 3) return at(d.p_idx, fo[MU] + d.b);
+    else if constexpr (J == 4) return at(qmu_base, d.b);
+    else if constexpr (J == 5) return at(d.q_idx, d.b);
+    else return at(own_base, 0);
   };
   auto issue = [&](auto jc, const Dir& d, int n) {                  // cp.async link J (n-th of the sequence) into ring slot n % K
     constexpr int J = decltype(jc)::value;
@@ -363,7 +364,7 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
     // DRAM once, by the thread that needs all rows of that link as a right factor).
     constexpr int NPJ = rows01_only_t<COMP>(J) ? (NP * 2) / 3 : NP;
 #pragma unroll
-    for (int k = 0; k < NPJ; ++k) cp_async_vec<(int)sizeof(Vec)>(dst + k * B, src + (size_t)k * g.Vh_pad);
+    for (int k = 0; k < NPJ; ++k) cp_async_vec<(int)sizeof(Vec)>(dst + k * B, src + k * PLANE_STRIDE);
   };
   auto fetch = [&](auto jc, const Dir& d, M3<R>& u, bool row2, int n) {
     constexpr int J = decltype(jc)::value;
@@ -382,7 +383,7 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
       const Vec* src = links + link_idx(jc, d);
       // the own-link array is written by this kernel (each thread its own element): plain load; the rest is read-only
 #pragma unroll
-      for (int k = 0; k < NP; ++k) vec_unpack(J == 6 ? src[(size_t)k * g.Vh_pad] : __ldg(src + (size_t)k * g.Vh_pad), r + k * T::VW);
+      for (int k = 0; k < NP; ++k) vec_unpack(J == 6 ? src[k * PLANE_STRIDE] : __ldg(src + k * PLANE_STRIDE), r + k * T::VW);
     }
     if constexpr (rows01_only_t<COMP>(J)) {
       m3_from_reals<R, 12>(u, r);                                  // planes of rows 0,1 (the first 12 reals) only

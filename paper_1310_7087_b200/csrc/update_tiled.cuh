@@ -78,8 +78,9 @@ su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* 
 #pragma unroll
   for (int d = 0; d < D; ++d) nbr_offsets(g, sc, d, fo[d], bo[d]);
   const uint32_t arr = (uint32_t)NP * g.Vh_pad;
-  const uint32_t own_idx = (uint32_t)(p * D + MU) * arr + h;
-  const uint32_t qmu_idx = (uint32_t)((1 - p) * D + MU) * arr + h;
+  const uint32_t own_base = (uint32_t)(p * D + MU) * arr;                     // array bases; elements at base + blk_off(h')
+  const uint32_t qmu_base = (uint32_t)((1 - p) * D + MU) * arr;
+  auto at = [&](uint32_t base, int off) -> uint32_t { return base + blk_off<NP>(h + (uint32_t)off); };
   const uint32_t lex = 2u * h + (uint32_t)s;
   const int lin = (int)threadIdx.x;                                          // slot of box element c
   // index of c inside the face of direction d (the d-th coordinate dropped)
@@ -97,20 +98,20 @@ su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* 
     auto stage = [&](int slot, uint32_t src_idx) {
       const Vec* src = links + src_idx;
 #pragma unroll
-      for (int k = 0; k < NP; ++k) cp_async_vec<(int)sizeof(Vec)>(res + k * RES + slot, src + (size_t)k * g.Vh_pad);
+      for (int k = 0; k < NP; ++k) cp_async_vec<(int)sizeof(Vec)>(res + k * RES + slot, src + k * PLANE_STRIDE);
     };
-    stage(lin, qmu_idx);
+    stage(lin, at(qmu_base, 0));
 #pragma unroll
     for (int d = 0; d < D; ++d) {
       if (d == MU) continue;
       const int fb = TD::face_base(MU, d), l3 = lin3(d);
       if (d == 0) {
         // a row with s = 0 needs j-1 of its first site, a row with s = 1 needs j+1 of its last site
-        if (c[0] == 0 && s == 0) stage(fb + l3, qmu_idx + (uint32_t)bo[0]);
-        if (c[0] == TD::T0 - 1 && s == 1) stage(fb + l3, qmu_idx + (uint32_t)fo[0]);
+        if (c[0] == 0 && s == 0) stage(fb + l3, at(qmu_base, bo[0]));
+        if (c[0] == TD::T0 - 1 && s == 1) stage(fb + l3, at(qmu_base, fo[0]));
       } else {
-        if (c[d] == 0) stage(fb + l3, qmu_idx + (uint32_t)bo[d]);
-        if (c[d] == TD::T(d) - 1) stage(fb + B / TD::T(d) + l3, qmu_idx + (uint32_t)fo[d]);
+        if (c[d] == 0) stage(fb + l3, at(qmu_base, bo[d]));
+        if (c[d] == TD::T(d) - 1) stage(fb + B / TD::T(d) + l3, at(qmu_base, fo[d]));
       }
     }
     cp_async_commit();
@@ -124,23 +125,23 @@ su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* 
     d.b = bo[0];
 #pragma unroll
     for (int k = 1; k < D; ++k) if (d.nu == k) d.b = bo[k];
-    d.p_idx = (uint32_t)(p * D + d.nu) * arr + h;
-    d.q_idx = (uint32_t)((1 - p) * D + d.nu) * arr + h;
+    d.p_idx = (uint32_t)(p * D + d.nu) * arr;
+    d.q_idx = (uint32_t)((1 - p) * D + d.nu) * arr;
     return d;
   };
   auto ring_idx = [&](auto rc, const Dir& d) -> uint32_t {
     constexpr int RR = decltype(rc)::value;
-    if constexpr (RR == 0) return d.p_idx;
-    else if constexpr (RR == 1) return d.q_idx + (uint32_t)fo[MU];
-    else if constexpr (RR == 2) return d.p_idx + (uint32_t)(fo[MU] + d.b);
-    else if constexpr (RR == 3) return d.q_idx + (uint32_t)d.b;
-    else return own_idx;
+    if constexpr (RR == 0) return at(d.p_idx, 0);
+    else if constexpr (RR == 1) return at(d.q_idx, fo[MU]);
+    else if constexpr (RR == 2) return at(d.p_idx, fo[MU] + d.b);
+    else if constexpr (RR == 3) return at(d.q_idx, d.b);
+    else return at(own_base, 0);
   };
   auto issue = [&](int n, uint32_t src_idx) {                   // link n of the sequence -> slot n % K
     const Vec* src = links + src_idx;
     Vec* dst = ring + (n % K) * NP * B;
 #pragma unroll
-    for (int k = 0; k < NP; ++k) cp_async_vec<(int)sizeof(Vec)>(dst + k * B, src + (size_t)k * g.Vh_pad);
+    for (int k = 0; k < NP; ++k) cp_async_vec<(int)sizeof(Vec)>(dst + k * B, src + k * PLANE_STRIDE);
   };
   auto from_ring = [&](int n, M3<R>& u, bool row2) {
     const Vec* src = ring + (n % K) * NP * B;
@@ -183,7 +184,7 @@ su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* 
         issue(4 * i + RA, ring_idx(std::integral_constant<int, RA>{}, cur));
       } else {
         if (!last) issue(4 * i + RA, ring_idx(std::integral_constant<int, RA - 4>{}, nxt));
-        else if (RA == 4) issue(4 * i + RA, own_idx);          // the own link, once, after the last direction
+        else if (RA == 4) issue(4 * i + RA, at(own_base, 0));          // the own link, once, after the last direction
       }
       cp_async_commit();                                       // one group per step, possibly empty
       cp_async_wait<K - 1>();
