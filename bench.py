@@ -44,7 +44,7 @@ FLOPS_PER_HIT = {"f32": {"hb": 4270.0, "or": 4030.0}, "f64": {"hb": 3900.0, "or"
 # the dominant kernel of each arm (overrelaxation: 32 of the 40 update launches of a step) and its DRAM traffic per launch,
 # dram__bytes_read.sum + dram__bytes_write.sum of one `ncu --set full` capture of this workload (bytes)
 OR_KERNEL = {"f32": "su3_update_tiled_kernel<float, x12, OR>", "f64": "su3_update_kernel<double, x18, OR>"}
-NCU_TRAFFIC = {"f32": {"or": 222129920, "hb": 221493248}, "f64": {"or": 674832128, "hb": 671554816},
+NCU_TRAFFIC = {"f32": {"or": 221946880, "hb": 220709888}, "f64": {"or": 658459392, "hb": 656831232},
                "source": "profiles/r1_f_launches_and_ncu.md"}
 
 
