@@ -99,7 +99,8 @@ int qcd_accum_get(qcd_lattice_t* lat, uint64_t* count, double* sum, double* sums
 int qcd_accum_reset(qcd_lattice_t* lat);
 
 /* Copy links out of / into the lattice in the canonical layout.  bytes must equal V*D*N*N*2*sizeof(real).
- * dst_is_device / src_is_device: the pointer is a DEVICE pointer (then the call is asynchronous on the stream).
+ * dst_is_device / src_is_device: the pointer is a DEVICE pointer, 16-byte aligned (then the call is asynchronous on the
+ * stream).
  * qcd_set_links does not reunitarise; with COMPRESS12 row 2 of the input is dropped; SU(2) input is read from
  * its first row (a0 = Re U00, a3 = Im U00, a2 = Re U01, a1 = Im U01). */
 int qcd_get_links(qcd_lattice_t* lat, void* dst, size_t bytes, int dst_is_device);

@@ -220,7 +220,7 @@ struct LayoutOp {
   qcd_lattice* L; void* canon; bool to_internal;
   template <int NC, int D, typename R, bool COMP> int operator()() {
     typedef typename LinkIO<NC, R, COMP>::Vec Vec;
-    dim3 grid((L->g.Vh + 127) / 128, 2);
+    dim3 grid((L->g.V + 127) / 128, 1);
     if (to_internal) layout_kernel<NC, D, R, COMP, true><<<grid, 128, 0, L->stream>>>(L->g, (Vec*)L->mem, (R*)canon);
     else layout_kernel<NC, D, R, COMP, false><<<grid, 128, 0, L->stream>>>(L->g, (Vec*)L->mem, (R*)canon);
     L->launches += 1;
@@ -545,6 +545,7 @@ int qcd_get_links(qcd_lattice_t* L, void* dst, size_t bytes, int dst_is_device) 
   if (!L || !dst) return fail(QCD_ERR_INVALID_ARG, "NULL argument");
   if (!L->has_links) return fail(QCD_ERR_STATE, "no links yet");
   if (bytes != canonical_bytes(L)) return fail(QCD_ERR_INVALID_ARG, "bytes must equal V*D*N*N*2*sizeof(real)");
+  if (dst_is_device && ((uintptr_t)dst & 15u)) return fail(QCD_ERR_INVALID_ARG, "device pointer must be 16-byte aligned");
   void* canon = dst;
   if (!dst_is_device) {
     if (!L->d_canon && cudaMalloc(&L->d_canon, bytes) != cudaSuccess) { L->d_canon = nullptr; cudaGetLastError(); return fail(QCD_ERR_ALLOC, "staging buffer"); }
@@ -562,6 +563,7 @@ int qcd_get_links(qcd_lattice_t* L, void* dst, size_t bytes, int dst_is_device) 
 int qcd_set_links(qcd_lattice_t* L, const void* src, size_t bytes, int src_is_device) {
   if (!L || !src) return fail(QCD_ERR_INVALID_ARG, "NULL argument");
   if (bytes != canonical_bytes(L)) return fail(QCD_ERR_INVALID_ARG, "bytes must equal V*D*N*N*2*sizeof(real)");
+  if (src_is_device && ((uintptr_t)src & 15u)) return fail(QCD_ERR_INVALID_ARG, "device pointer must be 16-byte aligned");
   void* canon = const_cast<void*>(src);
   if (!src_is_device) {
     if (!L->d_canon && cudaMalloc(&L->d_canon, bytes) != cudaSuccess) { L->d_canon = nullptr; cudaGetLastError(); return fail(QCD_ERR_ALLOC, "staging buffer"); }
