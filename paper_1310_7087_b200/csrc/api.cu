@@ -220,9 +220,10 @@ struct LayoutOp {
   qcd_lattice* L; void* canon; bool to_internal;
   template <int NC, int D, typename R, bool COMP> int operator()() {
     typedef typename LinkIO<NC, R, COMP>::Vec Vec;
-    dim3 grid((L->g.V + 127) / 128, 1);
-    if (to_internal) layout_kernel<NC, D, R, COMP, true><<<grid, 128, 0, L->stream>>>(L->g, (Vec*)L->mem, (R*)canon);
-    else layout_kernel<NC, D, R, COMP, false><<<grid, 128, 0, L->stream>>>(L->g, (Vec*)L->mem, (R*)canon);
+    constexpr int BL = LayoutShape<R>::BL;
+    dim3 grid((L->g.V + BL - 1) / BL, 1);
+    if (to_internal) layout_kernel<NC, D, R, COMP, true><<<grid, BL, 0, L->stream>>>(L->g, (Vec*)L->mem, (R*)canon);
+    else layout_kernel<NC, D, R, COMP, false><<<grid, BL, 0, L->stream>>>(L->g, (Vec*)L->mem, (R*)canon);
     L->launches += 1;
     L->last_parity = L->last_mu = -1;
     CUDA_TRY(cudaGetLastError());

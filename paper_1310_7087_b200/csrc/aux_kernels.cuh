@@ -147,41 +147,60 @@ __global__ void __launch_bounds__(128) init_kernel(Geom g, typename LinkIO<NC, R
 
 // ------------------------------------------------------------------ canonical <-> internal layout
 // canonical: [lex][mu][row][col][re,im] of R, full N x N.  One thread per site, all directions.
+// sites per CTA of layout_kernel: one CTA's block of the canonical array (BL * D * N*N complex numbers) fits 48 KB
+template <typename R> struct LayoutShape { static constexpr int BL = sizeof(R) == 4 ? 128 : 64; };
+
 template <int NC, int D, typename R, bool COMP, bool TO_INTERNAL>
-__global__ void __launch_bounds__(128) layout_kernel(Geom g, typename LinkIO<NC, R, COMP>::Vec* links, R* canon) {
-  // One thread per site in LEX order (both parities in one CTA): a CTA reads / writes 128 consecutive sites of the
-  // canonical array, i.e. one contiguous block of 128 * D * N*N*2 reals, and each half-warp 16 consecutive half-indices
-  // of one parity of the internal arrays.  (With one parity per CTA every line of the canonical array was touched by two
-  // CTAs far apart in time: 565 us for the 302 MB -> 201 MB conversion of the 32^4 fp32 lattice.)
+__global__ void __launch_bounds__(LayoutShape<R>::BL) layout_kernel(Geom g, typename LinkIO<NC, R, COMP>::Vec* links, R* canon) {
+  // One thread per site in LEX order (both parities in one CTA).  A CTA owns BL consecutive sites, i.e. one contiguous
+  // block of BL * D * N*N complex numbers of the canonical array, and moves it through shared memory: the global side is
+  // a flat, fully coalesced copy (consecutive threads, consecutive complex numbers), the per-site side (a thread's D
+  // links, 36 complex numbers apart from its neighbour's) stays in shared memory (row pitch NCX + 1 against bank
+  // conflicts).  The internal side is one 16-byte vector per thread and plane, 16 consecutive half-indices per parity
+  // and half-warp.
   typedef LinkIO<NC, R, COMP> IO;
-  const uint32_t lex = blockIdx.x * blockDim.x + threadIdx.x;
-  if (lex >= g.V) return;
-  const uint32_t h = lex >> 1;
-  const uint32_t row = fd_div(h, g.dLh0);
-  const uint32_t r2 = fd_div(row, g.dL1);
-  const uint32_t x1 = row - r2 * (uint32_t)g.L[1];
-  const uint32_t r3 = fd_div(r2, g.dL2);
-  const uint32_t x2 = r2 - r3 * (uint32_t)g.L[2], x3 = r3;
-  const int p = (int)(((lex & 1u) + x1 + x2 + x3) & 1u);           // x0 & 1 = lex & 1 (L0 even)
   typedef typename std::conditional<sizeof(R) == 4, float2, double2>::type C2;   // one complex number of the canonical array
+  constexpr int BL = LayoutShape<R>::BL, NCX = D * NC * NC, PITCH = NCX + 1;
+  __shared__ C2 buf[BL * PITCH];
+  const uint32_t lex0 = blockIdx.x * BL, t = threadIdx.x;
+  const uint32_t nsite = (g.V - lex0 < (uint32_t)BL) ? g.V - lex0 : (uint32_t)BL;
+  const uint32_t nel = nsite * NCX;
+  C2* gc = reinterpret_cast<C2*>(canon) + (size_t)lex0 * NCX;
+  if (TO_INTERNAL) {
+    for (uint32_t i = t; i < nel; i += BL) buf[(i / NCX) * PITCH + (i % NCX)] = gc[i];
+    __syncthreads();
+  }
+  if (t < nsite) {
+    const uint32_t lex = lex0 + t, h = lex >> 1;
+    const uint32_t row = fd_div(h, g.dLh0);
+    const uint32_t r2 = fd_div(row, g.dL1);
+    const uint32_t x1 = row - r2 * (uint32_t)g.L[1];
+    const uint32_t r3 = fd_div(r2, g.dL2);
+    const uint32_t x2 = r2 - r3 * (uint32_t)g.L[2], x3 = r3;
+    const int p = (int)(((lex & 1u) + x1 + x2 + x3) & 1u);         // x0 & 1 = lex & 1 (L0 even)
 #pragma unroll
-  for (int mu = 0; mu < D; ++mu) {
-    C2* c = reinterpret_cast<C2*>(canon + ((size_t)lex * D + mu) * (size_t)(NC * NC * 2));
-    Cx<R> m[NC][NC];
-    const size_t base = array_base<IO::T::NP>(g, D, p, mu);
-    if (TO_INTERNAL) {
+    for (int mu = 0; mu < D; ++mu) {
+      C2* c = buf + t * PITCH + mu * NC * NC;
+      Cx<R> m[NC][NC];
+      const size_t base = array_base<IO::T::NP>(g, D, p, mu);
+      if (TO_INTERNAL) {
 #pragma unroll
-      for (int i = 0; i < NC; ++i)
+        for (int i = 0; i < NC; ++i)
 #pragma unroll
-        for (int j = 0; j < NC; ++j) { const C2 v = c[i * NC + j]; m[i][j] = cx<R>(v.x, v.y); }
-      IO::store(m, links, g, base, h);
-    } else {
-      IO::template load<false>(m, links, g, base, h);
+          for (int j = 0; j < NC; ++j) { const C2 v = c[i * NC + j]; m[i][j] = cx<R>(v.x, v.y); }
+        IO::store(m, links, g, base, h);
+      } else {
+        IO::template load<false>(m, links, g, base, h);
 #pragma unroll
-      for (int i = 0; i < NC; ++i)
+        for (int i = 0; i < NC; ++i)
 #pragma unroll
-        for (int j = 0; j < NC; ++j) { C2 v; v.x = m[i][j].re; v.y = m[i][j].im; c[i * NC + j] = v; }
+          for (int j = 0; j < NC; ++j) { C2 v; v.x = m[i][j].re; v.y = m[i][j].im; c[i * NC + j] = v; }
+      }
     }
+  }
+  if (!TO_INTERNAL) {
+    __syncthreads();
+    for (uint32_t i = t; i < nel; i += BL) gc[i] = buf[(i / NCX) * PITCH + (i % NCX)];
   }
 }
 
