@@ -14,6 +14,10 @@ The line's `value` is the --precision arm (default fp32, 12-real compressed link
 measured in the same run and reported under "other_precision".  N > 1: independent replicas, one lattice per GPU, no
 data-path collective (replicas only) -> weak scaling.
 
+Timing: the timed region (exactly --steps steps between barrier + synchronize, CUDA events, MAX over ranks) is REPEATED:
+at least 5 repetitions and until the arm has >= 1 s of device time, so that the power-capped regime of a long run is inside
+the window; `ms_per_step` / `value` are the MEDIAN repetition, min / max ride along ("reps").
+
 --impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
 """
 import argparse
@@ -37,8 +41,11 @@ L2_BYTES = 126 * 1024 * 1024
 # bytes of one stored link, and algorithmic (compulsory) link-sizes moved per link-hit: 2D+1 = 9
 LINK_BYTES = {"f32": 48, "f64": 144}
 LINK_SIZES_PER_HIT = 2 * len(DIMS) + 1
-# algorithmic flops per link-hit (FP instructions of the kernels' SASS, FMA = 2)
-FLOPS_PER_HIT = {"f32": {"hb": 4270.0, "or": 4030.0}, "f64": {"hb": 3900.0, "or": 3270.0}}
+# flops per link-hit EXECUTED by the kernels this file launches: ncu's per-opcode thread-instruction counts
+# (sass__thread_inst_executed_true_per_opcode) of one launch / V/2, weighted FFMA2 4, FMUL2 / FADD2 / FFMA / DFMA 2,
+# FMUL / FADD / DMUL / DADD / MUFU 1  (profiles/r2_flop_count.md; SURVEY 8(d)'s estimates were 4030 / 4270 / 3270 / 3900)
+FLOPS_PER_HIT = {"f32": {"hb": 4031.0, "or": 3722.0}, "f64": {"hb": 3933.0, "or": 3169.0}}
+FLOPS_SOURCE = "profiles/r2_flop_count.md"
 
 
 # the dominant kernel of each arm (overrelaxation: 32 of the 40 update launches of a step) and its DRAM traffic per launch,
@@ -109,89 +116,7 @@ class ClockSampler:
 
 
 # ----------------------------------------------------------------------------- our arm
-def time_arm(q, torch, prec_name, steps, warmup, therm, seed, dist, sampler, do_e2e=True):
-    """device-resident timing + end-to-end timing of one precision arm; returns a dict of raw numbers"""
-    prec = q.QCD_FP32 if prec_name == "f32" else q.QCD_FP64
-    flags = q.QCD_FLAG_COMPRESS12 if prec_name == "f32" else 0
-    V = 1
-    for d in DIMS:
-        V *= d
-    links = len(DIMS) * V
-    out = {}
-    with q.Lattice(DIMS, NC, prec, flags, device=torch.device("cuda", torch.cuda.current_device())) as G:
-        G.qcd_init(q.QCD_HOT, seed)
-        for _ in range(therm):                       # setup: move off the hot start (KP acceptance, staple norms)
-            G.qcd_sweep(BETA, N_HB, N_OR)
-        for _ in range(warmup):
-            G.qcd_sweep(BETA, N_HB, N_OR)
-            G.qcd_measure()
-        G.qcd_set_option(q.QCD_OPT_PROFILE, 1)
-        G.qcd_reset_profile()
-        n0 = G.qcd_get_launch_count()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        if dist is not None:
-            dist.barrier()
-        torch.cuda.synchronize()
-        t0 = time.time()
-        e0.record()
-        for _ in range(steps):
-            G.qcd_sweep(BETA, N_HB, N_OR)
-            plaq, planes, poly = G.qcd_measure()
-        e1.record()
-        torch.cuda.synchronize()
-        sampler.window(t0, time.time())
-        if dist is not None:
-            dist.barrier()
-        ms = e0.elapsed_time(e1)
-        out["launches"] = G.qcd_get_launch_count() - n0
-        hb_ms, hb_n = G.qcd_get_profile(q.QCD_KIND_HB)
-        or_ms, or_n = G.qcd_get_profile(q.QCD_KIND_OR)
-        G.qcd_set_option(q.QCD_OPT_PROFILE, 0)
-        out.update(ms_total=ms, plaquette=plaq, polyakov_abs=abs(poly), hb_ms=hb_ms, hb_n=hb_n, or_ms=or_ms, or_n=or_n)
-        out["sweep_counter"] = G.qcd_get_sweep_counter()
-        # the same working sweep with the observables accumulated on the device (qcd_measure_accumulate: no host
-        # synchronisation per step, one qcd_accum_get at the end) -- reported beside the headline, not instead of it
-        G.qcd_accum_reset()
-        torch.cuda.synchronize()
-        e0.record()
-        for _ in range(steps):
-            G.qcd_sweep(BETA, N_HB, N_OR)
-            G.qcd_measure_accumulate()
-        e1.record()
-        n_acc, s1, _ = G.qcd_accum_get()
-        torch.cuda.synchronize()
-        out["acc_ms_total"] = e0.elapsed_time(e1)
-        out["acc_plaquette_mean"] = float(s1[:6].mean() / max(n_acc, 1))
-
-        if do_e2e:
-            # end to end through the C ABI with HOST buffers: every step uploads the configuration from pinned host
-            # memory (canonical layout), runs the working sweep, reads the observables and downloads the configuration
-            nbytes = G.canonical_bytes
-            host = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
-            G.qcd_get_links_ptr(host.data_ptr(), nbytes, 0)
-            for _ in range(2):
-                G.qcd_set_links_ptr(host.data_ptr(), nbytes, 0)
-                G.qcd_sweep(BETA, N_HB, N_OR)
-                G.qcd_measure()
-                G.qcd_get_links_ptr(host.data_ptr(), nbytes, 0)
-            if dist is not None:
-                dist.barrier()
-            torch.cuda.synchronize()
-            t0 = time.time()
-            e0.record()
-            for _ in range(steps):
-                G.qcd_set_links_ptr(host.data_ptr(), nbytes, 0)
-                G.qcd_sweep(BETA, N_HB, N_OR)
-                G.qcd_measure()
-                G.qcd_get_links_ptr(host.data_ptr(), nbytes, 0)
-            e1.record()
-            torch.cuda.synchronize()
-            sampler.window(t0, time.time())
-            out["e2e_ms_total"] = e0.elapsed_time(e1)
-            out["h2d"] = nbytes
-            out["d2h"] = nbytes + 9 * 8
-    out["links"] = links
-    return out
+MIN_REPS, MAX_REPS, MIN_DEVICE_MS = 5, 80, 1000.0
 
 
 def max_over_ranks(torch, dist, x, device="cuda"):
@@ -201,6 +126,100 @@ def max_over_ranks(torch, dist, x, device="cuda"):
     t = torch.tensor([x], dtype=torch.float64, device=device)
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
     return float(t.item())
+
+
+def timed_reps(torch, dist, sampler, body, steps, min_total_ms=MIN_DEVICE_MS):
+    """Repeat the timed region -- barrier + synchronize, CUDA events around exactly `steps` calls of body(), synchronize +
+    barrier, MAX over ranks -- at least MIN_REPS times and until min_total_ms of device time has been spent.  Returns the list
+    of per-repetition milliseconds (identical on every rank, so every rank leaves the loop together)."""
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    times = []
+    while len(times) < MIN_REPS or (sum(times) < min_total_ms and len(times) < MAX_REPS):
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+        t0 = time.time()
+        e0.record()
+        for _ in range(steps):
+            body()
+        e1.record()
+        torch.cuda.synchronize()
+        sampler.window(t0, time.time())
+        if dist is not None:
+            dist.barrier()
+        times.append(max_over_ranks(torch, dist, e0.elapsed_time(e1)))
+    return times
+
+
+def rep_stats(times, steps):
+    t = sorted(times)
+    med = t[len(t) // 2] if len(t) % 2 else 0.5 * (t[len(t) // 2 - 1] + t[len(t) // 2])
+    return {"median_ms_per_step": med / steps, "min_ms_per_step": t[0] / steps, "max_ms_per_step": t[-1] / steps,
+            "reps": len(t), "device_ms_total": sum(t)}
+
+
+def time_arm(q, torch, prec_name, steps, warmup, therm, seed, dist, sampler):
+    """device-resident timing + end-to-end timing of one precision arm; returns a dict of raw numbers"""
+    prec = q.QCD_FP32 if prec_name == "f32" else q.QCD_FP64
+    flags = q.QCD_FLAG_COMPRESS12 if prec_name == "f32" else 0
+    V = 1
+    for d in DIMS:
+        V *= d
+    out = {"links": len(DIMS) * V}
+    with q.Lattice(DIMS, NC, prec, flags, device=torch.device("cuda", torch.cuda.current_device())) as G:
+        G.qcd_init(q.QCD_HOT, seed)
+        for _ in range(therm):                       # setup: move off the hot start (KP acceptance, staple norms)
+            G.qcd_sweep(BETA, N_HB, N_OR)
+        state = {}
+
+        def working_sweep():
+            G.qcd_sweep(BETA, N_HB, N_OR)
+            state["obs"] = G.qcd_measure()
+
+        for _ in range(warmup):
+            working_sweep()
+        # (1) the headline: working sweep = update + measurement, observables returned to the host every step
+        G.qcd_set_option(q.QCD_OPT_PROFILE, 1)
+        G.qcd_reset_profile()
+        n0 = G.qcd_get_launch_count()
+        out["work"] = timed_reps(torch, dist, sampler, working_sweep, steps)
+        out["launches_per_rep"] = (G.qcd_get_launch_count() - n0) // len(out["work"])
+        hb_ms, hb_n = G.qcd_get_profile(q.QCD_KIND_HB)
+        or_ms, or_n = G.qcd_get_profile(q.QCD_KIND_OR)
+        G.qcd_set_option(q.QCD_OPT_PROFILE, 0)
+        plaq, planes, poly = state["obs"]
+        out.update(plaquette=plaq, polyakov_abs=abs(poly), hb_ms=hb_ms, hb_n=hb_n, or_ms=or_ms, or_n=or_n)
+        # (2) update-only sweep (SURVEY 8(d): measurement excluded), profiling events off
+        out["update"] = timed_reps(torch, dist, sampler, lambda: G.qcd_sweep(BETA, N_HB, N_OR), steps, min_total_ms=500.0)
+        # (3) working sweep with the observables accumulated on the device (no host synchronisation per step)
+        G.qcd_accum_reset()
+
+        def accumulate_sweep():
+            G.qcd_sweep(BETA, N_HB, N_OR)
+            G.qcd_measure_accumulate()
+
+        out["accum"] = timed_reps(torch, dist, sampler, accumulate_sweep, steps, min_total_ms=500.0)
+        n_acc, s1, _ = G.qcd_accum_get()
+        out["acc_plaquette_mean"] = float(s1[:6].mean() / max(n_acc, 1))
+        # (4) end to end through the C ABI with HOST buffers: every step uploads the configuration from pinned host
+        # memory (canonical layout), runs the working sweep, reads the observables and downloads the configuration
+        nbytes = G.canonical_bytes
+        host = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
+        G.qcd_get_links_ptr(host.data_ptr(), nbytes, 0)
+
+        def e2e_step():
+            G.qcd_set_links_ptr(host.data_ptr(), nbytes, 0)
+            G.qcd_sweep(BETA, N_HB, N_OR)
+            state["obs"] = G.qcd_measure()
+            G.qcd_get_links_ptr(host.data_ptr(), nbytes, 0)
+
+        for _ in range(2):
+            e2e_step()
+        out["e2e"] = timed_reps(torch, dist, sampler, e2e_step, steps, min_total_ms=0.0)
+        out["h2d"] = nbytes
+        out["d2h"] = nbytes + 9 * 8
+        out["sweep_counter"] = G.qcd_get_sweep_counter()
+    return out
 
 
 def replica_seed(rank):
@@ -214,30 +233,42 @@ def aggregate_value(n_gpus, links_per_replica, steps, ms_total_max):
 
 
 def summarise(arm, prec_name, steps, n_gpus, hbm_peak, fma_peak_tflops):
-    """per-arm JSON fragments: value, roofline of the dominant (overrelaxation) kernel, sweep breakdown"""
+    """per-arm JSON fragments: value, roofline of the dominant (overrelaxation) kernel, sweep-level fractions"""
     links = arm["links"]
-    ms_step = arm["ms_total"] / steps
-    value = aggregate_value(n_gpus, links, steps, arm["ms_total"])
+    work, upd = rep_stats(arm["work"], steps), rep_stats(arm["update"], steps)
+    ms_step = work["median_ms_per_step"]
+    value = aggregate_value(n_gpus, links, 1, ms_step)
     hits = links // (2 * len(DIMS))                                  # links updated by one launch = V/2
     bytes_launch = LINK_SIZES_PER_HIT * LINK_BYTES[prec_name] * hits
     or_us = arm["or_ms"] / max(arm["or_n"], 1) * 1e3
     hb_us = arm["hb_ms"] / max(arm["hb_n"], 1) * 1e3
     achieved = bytes_launch / (or_us * 1e-6) / 1e9
+    # sweep level (north_star's target is on the sweep): the algorithmic bytes of ALL update launches of a step,
+    # (n_hb + n_or) * 9 link-sizes * D * V = 45 link-sizes per link, over the step time
+    n_launch = 2 * len(DIMS) * (N_HB + N_OR)
+    sweep_bytes = n_launch * bytes_launch
+    sweep_flops = hits * 2 * len(DIMS) * (N_HB * FLOPS_PER_HIT[prec_name]["hb"] + N_OR * FLOPS_PER_HIT[prec_name]["or"])
     roof = {"bound": "hbm", "kernel": OR_KERNEL[prec_name], "achieved": round(achieved, 1), "peak": hbm_peak,
             "unit": "GB/s", "frac": round(achieved / hbm_peak, 4), "traffic": NCU_TRAFFIC[prec_name]["or"],
             "traffic_source": NCU_TRAFFIC["source"],
             "bytes_per_launch": bytes_launch, "us_per_launch": round(or_us, 2), "launches_timed": arm["or_n"],
             "hb_us_per_launch": round(hb_us, 2),
-            "hb_frac": round(bytes_launch / (hb_us * 1e-6) / 1e9 / hbm_peak, 4) if hb_us > 0 else None}
+            "hb_frac": round(bytes_launch / (hb_us * 1e-6) / 1e9 / hbm_peak, 4) if hb_us > 0 else None,
+            # working sweep: update bytes over the whole step (measurement time inside, its bytes not counted)
+            "sweep_frac": round(sweep_bytes / (ms_step * 1e-3) / 1e9 / hbm_peak, 4),
+            # update-only sweep (the SURVEY 8(d) headline form)
+            "update_sweep_frac": round(sweep_bytes / (upd["median_ms_per_step"] * 1e-3) / 1e9 / hbm_peak, 4),
+            "sweep_bytes": sweep_bytes}
     if fma_peak_tflops:
         fl = FLOPS_PER_HIT[prec_name]["or"] * hits
         roof["alu"] = {"achieved_tflops": round(fl / (or_us * 1e-6) / 1e12, 2), "peak_tflops": round(fma_peak_tflops, 2),
                        "frac": round(fl / (or_us * 1e-6) / 1e12 / fma_peak_tflops, 4), "flops_per_link_hit": FLOPS_PER_HIT[prec_name]["or"],
-                       "peak_source": "qcd_probe_fma_tflops, same run"}
+                       "flops_source": FLOPS_SOURCE, "peak_source": "qcd_probe_fma_tflops, same run",
+                       "sweep_frac": round(sweep_flops / (ms_step * 1e-3) / 1e12 / fma_peak_tflops, 4)}
         t_hbm, t_alu = bytes_launch / (hbm_peak * 1e9), fl / (fma_peak_tflops * 1e12)
         roof["binding_limit"] = "hbm" if t_hbm >= t_alu else "alu"
         roof["frac_of_binding_limit"] = round(max(t_hbm, t_alu) / (or_us * 1e-6), 4)
-    return value, ms_step, roof
+    return value, ms_step, roof, work, upd
 
 
 def run_ours(args):
@@ -263,23 +294,24 @@ def run_ours(args):
     arms = {}
     for name in (primary, other):
         arms[name] = time_arm(q, torch, name, args.steps, args.warmup, args.therm, replica_seed(rank), dist, sampler)
-        arms[name]["ms_total"] = max_over_ranks(torch, dist, arms[name]["ms_total"])
-        arms[name]["e2e_ms_total"] = max_over_ranks(torch, dist, arms[name]["e2e_ms_total"])
     clocks = sampler.stop()
     line = None
     if rank == 0:
         frag = {}
         for name in (primary, other):
-            value, ms_step, roof = summarise(arms[name], name, args.steps, world, hbm_peak, fma[name])
+            value, ms_step, roof, work, upd = summarise(arms[name], name, args.steps, world, hbm_peak, fma[name])
             a = arms[name]
-            e2e_val = aggregate_value(world, a["links"], args.steps, a["e2e_ms_total"])
-            frag[name] = {"value": value, "ms_per_step": ms_step, "roofline": roof,
-                          "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": a["h2d"], "d2h_bytes_per_step": a["d2h"],
-                                  "ms_per_step": a["e2e_ms_total"] / args.steps},
-                          "accumulate_on_device": {"ms_per_step": a["acc_ms_total"] / args.steps,
-                                                   "value": aggregate_value(world, a["links"], args.steps, a["acc_ms_total"]),
+            e2e, acc = rep_stats(a["e2e"], args.steps), rep_stats(a["accum"], args.steps)
+            frag[name] = {"value": value, "ms_per_step": ms_step, "reps": work, "roofline": roof,
+                          "update_only_sweep": {"ms_per_step": upd["median_ms_per_step"], "reps": upd,
+                                                "value": aggregate_value(world, a["links"], 1, upd["median_ms_per_step"])},
+                          "e2e": {"value": aggregate_value(world, a["links"], 1, e2e["median_ms_per_step"]), "unit": UNIT,
+                                  "h2d_bytes_per_step": a["h2d"], "d2h_bytes_per_step": a["d2h"],
+                                  "ms_per_step": e2e["median_ms_per_step"], "reps": e2e},
+                          "accumulate_on_device": {"ms_per_step": acc["median_ms_per_step"], "reps": acc,
+                                                   "value": aggregate_value(world, a["links"], 1, acc["median_ms_per_step"]),
                                                    "plaquette_mean": a["acc_plaquette_mean"]},
-                          "gpu_launches": a["launches"], "plaquette": a["plaquette"], "polyakov_abs": a["polyakov_abs"],
+                          "gpu_launches": a["launches_per_rep"], "plaquette": a["plaquette"], "polyakov_abs": a["polyakov_abs"],
                           "dtype": name, "storage": "12 reals/link" if name == "f32" else "18 reals/link"}
         p = frag[primary]
         p["roofline"]["peak_source"] = peak_src
@@ -289,9 +321,11 @@ def run_ours(args):
                 "dtype": primary, "data": "synthetic",
                 "config": {"workload": "BASELINE.json configs[2]: SU(3) D=4 32^4 beta=6.0 hot seed 42, 1 HB + 4 OR + measure per step",
                            "storage": p["storage"], "replicas": world, "thermalisation_sweeps_before_warmup": args.therm,
-                           "l2": "inputs larger than L2: %d MB of links vs 126 MB" % (arms[primary]["links"] * LINK_BYTES[primary] // 2 ** 20)},
-                "e2e": p["e2e"], "gpu_launches": p["gpu_launches"], "roofline": p["roofline"], "clocks": clocks,
-                "accumulate_on_device": p["accumulate_on_device"],
+                           "l2": "inputs larger than L2: %d MB of links vs 126 MB" % (arms[primary]["links"] * LINK_BYTES[primary] // 2 ** 20),
+                           "timing": "median of >= %d repetitions of the %d-step timed region, >= %.0f ms of device time per arm"
+                                     % (MIN_REPS, args.steps, MIN_DEVICE_MS)},
+                "reps": p["reps"], "e2e": p["e2e"], "gpu_launches": p["gpu_launches"], "roofline": p["roofline"], "clocks": clocks,
+                "update_only_sweep": p["update_only_sweep"], "accumulate_on_device": p["accumulate_on_device"],
                 "observables": {"plaquette": p["plaquette"], "polyakov_abs": p["polyakov_abs"]},
                 "other_precision": frag[other]}
         if world == 1 and not args.no_cpu_baseline:
@@ -313,6 +347,12 @@ def _oracle_sample(O, oracle, step):
     return O.V // 2
 
 
+def _set_omp_threads(n):
+    """libgomp's own runtime call: the oracle is timed as it stands, only the thread count of its OpenMP loops changes"""
+    import ctypes
+    ctypes.CDLL("libgomp.so.1").omp_set_num_threads(int(n))
+
+
 def cpu_baseline_sample():
     import oracle
     cores = oracle.num_threads()
@@ -325,9 +365,26 @@ def cpu_baseline_sample():
         done += _oracle_sample(O, oracle, step)
         step += 1
     dt = time.time() - t0
-    return {"value": done / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": "%d x (1 HB + 4 OR on the V/2 links of one (parity, mu)) of the 32^4 lattice from the hot start, "
-                      "= %.2f sweeps (%.1f s)" % (step, step / 8.0, dt)}
+    out = {"value": done / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+           "sample": "%d x (1 HB + 4 OR on the V/2 links of one (parity, mu)) of the 32^4 lattice from the hot start, "
+                     "= %.2f sweeps (%.1f s)" % (step, step / 8.0, dt)}
+    # the same oracle on ONE thread, bounded: 1/4 of one (parity, mu) sample would be enough, the
+    # site loop is not divisible from outside, so one sample it is (~5-8 s)
+    try:
+        _set_omp_threads(1)
+        t0 = time.time()
+        n1 = _oracle_sample(O, oracle, step)
+        dt1 = time.time() - t0
+        out["single_thread"] = {"value": n1 / dt1, "unit": UNIT, "cores": 1,
+                                "sample": "1 x (1 HB + 4 OR on the V/2 links of one (parity, mu)) (%.1f s)" % dt1}
+    except OSError as e:
+        out["single_thread"] = {"unavailable": str(e)}
+    finally:
+        try:
+            _set_omp_threads(cores)
+        except OSError:
+            pass
+    return out
 
 
 def run_reference(args):

@@ -46,7 +46,6 @@ enum {
   QCD_OPT_DEBUG_TRIALS = 1,  /* 1: qcd_debug_substep records per-(link,subgroup) trial codes (allocates V*3 bytes) */
   QCD_OPT_PROFILE = 2,       /* 1: CUDA events around the update kernels: one pair per run of same-kind launches in qcd_sweep,
                                 one pair per launch in qcd_debug_substep (see qcd_get_profile) */
-  QCD_OPT_USE_GRAPH = 3      /* accepted and ignored: qcd_sweep chains its launches by programmatic dependent launch */
 };
 
 /* Constant abelian background: every plaquette of plane (mu,nu), mu < nu, is multiplied on the left, at its
@@ -59,7 +58,8 @@ typedef struct {
 } qcd_field_t;
 
 /* Bytes of device workspace a lattice needs (links in the internal layout).  0 on invalid arguments and on lattices
- * beyond the kernels' 32-bit vector indexing (2 D NP V/2 >= 2^32 vectors of 16 bytes: e.g. 128^4 in fp64; UNSUPPORTED). */
+ * beyond the kernels' indexing: V > 2^31 sites, or one (parity, direction) array of NP planes x V/2 vectors of 16 bytes
+ * reaching 2^32 vectors (UNSUPPORTED; SU(3) 128^4 in fp64 x18, 154.6 GB, is within both). */
 size_t qcd_lattice_bytes(int D, const int* dims, int Nc, int precision, unsigned flags);
 
 /* Create a lattice.  device_mem: DEVICE pointer to >= qcd_lattice_bytes() bytes, 256-byte aligned, owned by the
@@ -100,7 +100,8 @@ int qcd_accum_reset(qcd_lattice_t* lat);
 
 /* Copy links out of / into the lattice in the canonical layout.  bytes must equal V*D*N*N*2*sizeof(real).
  * dst_is_device / src_is_device: the pointer is a DEVICE pointer, 16-byte aligned (then the call is asynchronous on the
- * stream).
+ * stream).  HOST pointers (pageable or pinned): the transfer is staged through a bounded device buffer (64 MiB, allocated
+ * on first use) in chunks of whole sites, and the call returns after the host buffer has been read / filled.
  * qcd_set_links does not reunitarise; with COMPRESS12 row 2 of the input is dropped; SU(2) input is read from
  * its first row (a0 = Re U00, a3 = Im U00, a2 = Re U01, a1 = Im U01). */
 int qcd_get_links(qcd_lattice_t* lat, void* dst, size_t bytes, int dst_is_device);
@@ -130,7 +131,7 @@ int qcd_debug_philox(const uint32_t* ctr, const uint32_t* key, size_t n, uint32_
  * the update kernels of `kind` since the last qcd_reset_profile.  Synchronises the stream. */
 int qcd_get_profile(qcd_lattice_t* lat, int kind, double* total_ms, uint64_t* launches);
 int qcd_reset_profile(qcd_lattice_t* lat);
-/* Number of kernels this library launched for the lattice since creation (graph replays count their nodes). */
+/* Number of kernels this library launched for the lattice since creation . */
 int qcd_get_launch_count(qcd_lattice_t* lat, uint64_t* out);
 
 /* Peaks measured on the current device, for the roofline denominators (north_star: "peaks measured in the same

@@ -9,15 +9,14 @@ import os
 import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-# QCD_B200_LIB: load another build of the same library (kernel tuning variants); default is the in-tree build
-LIB_PATH = os.environ.get("QCD_B200_LIB") or os.path.join(HERE, "libqcd_b200.so")
+LIB_PATH = os.path.join(HERE, "libqcd_b200.so")
 
 QCD_OK, QCD_ERR_INVALID_ARG, QCD_ERR_UNSUPPORTED, QCD_ERR_ALLOC, QCD_ERR_CUDA, QCD_ERR_STATE = 0, 1, 2, 3, 4, 5
 QCD_FP32, QCD_FP64 = 0, 1
 QCD_FLAG_COMPRESS12 = 1
 QCD_COLD, QCD_HOT = 0, 1
 QCD_KIND_HB, QCD_KIND_OR = 0, 1
-QCD_OPT_KP_MAX_TRIALS, QCD_OPT_DEBUG_TRIALS, QCD_OPT_PROFILE, QCD_OPT_USE_GRAPH = 0, 1, 2, 3
+QCD_OPT_KP_MAX_TRIALS, QCD_OPT_DEBUG_TRIALS, QCD_OPT_PROFILE = 0, 1, 2
 
 # every symbol include/qcd.h declares (tests check that the library exports all of them)
 SYMBOLS = [

@@ -36,11 +36,10 @@ def is_stale():
     return any(os.path.getmtime(p) > t for p in _deps())
 
 
-def build_cuda(force=False, verbose=False, defines=(), out=None, objdir=None):
-    """defines / out / objdir: tuning builds (-DNAME=VALUE ...) into another library file; the default build takes none."""
-    lib_out = out or LIB
-    obj_dir = objdir or OBJDIR
-    if not force and not defines and out is None and not is_stale():
+def build_cuda(force=False, verbose=False):
+    lib_out = LIB
+    obj_dir = OBJDIR
+    if not force and not is_stale():
         return LIB
     nvcc = os.environ.get("NVCC", "nvcc")
     os.makedirs(obj_dir, exist_ok=True)
@@ -49,7 +48,7 @@ def build_cuda(force=False, verbose=False, defines=(), out=None, objdir=None):
     for src in _sources():
         obj = os.path.join(obj_dir, os.path.basename(src)[:-3] + ".o")
         objs.append(obj)
-        cmd = [nvcc] + NVCC_FLAGS + ["-D" + d for d in defines] + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj]
+        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj]
         procs.append((src, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
     failed = False
     for src, p in procs:
@@ -70,8 +69,5 @@ if __name__ == "__main__":
     ap = argparse.ArgumentParser()
     ap.add_argument("--force", action="store_true")
     ap.add_argument("-v", action="store_true")
-    ap.add_argument("--define", "-D", action="append", default=[])
-    ap.add_argument("--out", default=None)
-    ap.add_argument("--objdir", default=None)
     a = ap.parse_args()
-    print(build_cuda(force=a.force, verbose=a.v, defines=a.define, out=a.out, objdir=a.objdir))
+    print(build_cuda(force=a.force, verbose=a.v))

@@ -1,5 +1,6 @@
-// api.cu -- the C ABI of include/qcd.h: argument checking, lattice state, launch sequencing (sweep order R1/R2),
-// CUDA-graph replay of whole sweeps, event profiling, and the non-update kernels (init, layout, measurement, probes).
+// api.cu -- the C ABI of include/qcd.h: argument checking, lattice state, launch sequencing (sweep order R1/R2, chained by
+// programmatic dependent launch), event profiling, and the non-update kernels (init, layout, measurement, probes).
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -26,10 +27,6 @@ int fail(int code, const std::string& msg) { g_err = msg; return code; }
 
 struct EventPair { cudaEvent_t a, b; int kind; int n; };   // n = update-kernel launches between a and b
 
-struct GraphKey {
-  double beta; int n_hb, n_or; bool field; qcd_field_t f; int max_trials; uint32_t sweep;
-};
-
 }  // namespace
 
 struct qcd_lattice {
@@ -45,7 +42,7 @@ struct qcd_lattice {
   uint32_t sweep;
   bool has_links;
   int max_trials;
-  bool debug_trials, profile, use_graph;
+  bool debug_trials, profile;
   uint8_t* d_trials;
   double* d_partials;
   size_t partials_cap;   // doubles
@@ -55,15 +52,14 @@ struct qcd_lattice {
   double prof_ms[2];
   uint64_t prof_n[2];
   uint64_t launches;
-  // (parity, mu) of the update kernel launched last on the stream, -1 if the last kernel was not an update kernel: the
-  // next update kernel may fetch, before its griddepcontrol.wait, only arrays that kernel does not write (update.cuh)
+  // What the kernel launched last on the stream wrote: (parity, mu) of an update kernel; -1: no links (measurement,
+  // get_links); -2: all links (init, set_links, the create-time memset).  The next update kernel may fetch, before its
+  // griddepcontrol.wait, only arrays that kernel does not write (update.cuh)
   int last_parity, last_mu;
   // side stream + events: the latency-bound Polyakov kernel runs beside the plaquette kernel (qcd_measure)
   cudaStream_t side;
   cudaEvent_t ev_fork, ev_join;
-  // device-resident sweep counter so that a captured sweep graph can be replayed unchanged
-  uint32_t* d_sweep;
-  // persistent staging buffer for qcd_get/set_links with HOST pointers (canonical layout, allocated on first use)
+  // bounded staging buffer for qcd_get/set_links with HOST pointers (canonical layout, STAGE_BYTES, allocated on first use)
   void* d_canon;
 };
 
@@ -91,10 +87,10 @@ bool valid_shape(int D, const int* dims, int Nc, int precision, unsigned flags, 
   }
   if (v > 2147483648.0) return false;          // V/2 and lex must fit 32-bit (Philox c0 = lex)
   if ((flags & QCD_FLAG_COMPRESS12) && Nc == 2) { *why = QCD_ERR_UNSUPPORTED; return false; }
-  // the kernels index the 2 D NP planes of Vh_pad vectors with 32 bits
+  // the kernels address one (parity, direction) array of NP planes x Vh_pad vectors with 32 bits (array bases are 64-bit)
   int nreal, vb, np;
   plane_params(Nc, precision, (flags & QCD_FLAG_COMPRESS12) != 0, &nreal, &vb, &np);
-  if (2.0 * D * np * (v / 2.0 + 32.0) >= 4294967296.0) { *why = QCD_ERR_UNSUPPORTED; return false; }
+  if ((double)np * (v / 2.0 + 32.0) >= 4294967296.0) { *why = QCD_ERR_UNSUPPORTED; return false; }
   return true;
 }
 
@@ -137,12 +133,13 @@ FieldArgs make_field_args(const qcd_field_t* f, bool on, int Nc) {
 
 cudaError_t launch_update(qcd_lattice* L, int kind, bool field, const UpdateArgs& a0) {
   UpdateSel s; s.Nc = L->Nc; s.D = L->D; s.precision = L->precision; s.comp = L->comp; s.kind = kind; s.field = field;
-  L->launches += 1;
   UpdateArgs a = a0;
   a.prev_parity = L->last_parity; a.prev_mu = L->last_mu;
-  L->last_parity = a.parity; L->last_mu = a.mu;
-  if (L->Nc == 2) return launch_update_su2(s, L->g, L->mem, a, L->stream);
-  return L->precision == QCD_FP32 ? launch_update_su3_f32(s, L->g, L->mem, a, L->stream) : launch_update_su3_f64(s, L->g, L->mem, a, L->stream);
+  const cudaError_t e = (L->Nc == 2)                ? launch_update_su2(s, L->g, L->mem, a, L->stream)
+                        : L->precision == QCD_FP32 ? launch_update_su3_f32(s, L->g, L->mem, a, L->stream)
+                                                   : launch_update_su3_f64(s, L->g, L->mem, a, L->stream);
+  if (e == cudaSuccess) { L->launches += 1; L->last_parity = a.parity; L->last_mu = a.mu; }
+  return e;
 }
 
 int prof_begin(qcd_lattice* L, int kind, EventPair* ep) {
@@ -172,7 +169,11 @@ int substep(qcd_lattice* L, double beta, int kind, int hit, int parity, int mu, 
   EventPair ep;
   const bool prof = L->profile && bracket;
   if (prof) { int rc = prof_begin(L, kind, &ep); if (rc != QCD_OK) return rc; }
-  CUDA_TRY(launch_update(L, kind, field_on, a));
+  const cudaError_t e = launch_update(L, kind, field_on, a);
+  if (e != cudaSuccess) {
+    if (prof) L->ev_free.push_back(ep);                            // the open pair goes back to the pool
+    return fail(QCD_ERR_CUDA, std::string("update kernel launch: ") + cudaGetErrorString(e));
+  }
   if (prof) return prof_end(L, &ep, 1);
   return QCD_OK;
 }
@@ -209,24 +210,26 @@ struct InitOp {
     typedef typename LinkIO<NC, R, COMP>::Vec Vec;
     dim3 grid((L->g.Vh + 127) / 128, 2);
     init_kernel<NC, D, R, COMP><<<grid, 128, 0, L->stream>>>(L->g, (Vec*)L->mem, hot, (uint32_t)(L->seed & 0xFFFFFFFFull), (uint32_t)(L->seed >> 32));
-    L->launches += 1;
-    L->last_parity = L->last_mu = -1;
     CUDA_TRY(cudaGetLastError());
+    L->launches += 1;
+    L->last_parity = L->last_mu = -2;                              // every array was written
     return QCD_OK;
   }
 };
 
 struct LayoutOp {
-  qcd_lattice* L; void* canon; bool to_internal;
+  // sites [lex_begin, lex_end) <-> the canonical block starting at `canon` (= the canonical address of site lex_begin)
+  qcd_lattice* L; void* canon; bool to_internal; uint32_t lex_begin, lex_end;
   template <int NC, int D, typename R, bool COMP> int operator()() {
     typedef typename LinkIO<NC, R, COMP>::Vec Vec;
     constexpr int BL = LayoutShape<R>::BL;
-    dim3 grid((L->g.V + BL - 1) / BL, 1);
-    if (to_internal) layout_kernel<NC, D, R, COMP, true><<<grid, BL, 0, L->stream>>>(L->g, (Vec*)L->mem, (R*)canon);
-    else layout_kernel<NC, D, R, COMP, false><<<grid, BL, 0, L->stream>>>(L->g, (Vec*)L->mem, (R*)canon);
-    L->launches += 1;
-    L->last_parity = L->last_mu = -1;
+    dim3 grid((lex_end - lex_begin + BL - 1) / BL, 1);
+    if (to_internal) layout_kernel<NC, D, R, COMP, true><<<grid, BL, 0, L->stream>>>(L->g, (Vec*)L->mem, (R*)canon, lex_begin, lex_end);
+    else layout_kernel<NC, D, R, COMP, false><<<grid, BL, 0, L->stream>>>(L->g, (Vec*)L->mem, (R*)canon, lex_begin, lex_end);
     CUDA_TRY(cudaGetLastError());
+    L->launches += 1;
+    if (to_internal) L->last_parity = L->last_mu = -2;             // link arrays were written
+    else L->last_parity = L->last_mu = -1;                         // a full (non-PDL) kernel boundary: earlier writes are visible
     return QCD_OK;
   }
 };
@@ -237,7 +240,7 @@ struct MeasureOp {
     typedef typename LinkIO<NC, R, COMP>::Vec Vec;
     constexpr int NPL = D * (D - 1) / 2;
     // boxed thread mapping of the plaquette kernel (aux_kernels.cuh, MeasureField): one grid row of V / 128 CTAs
-    mf.boxed = (D == 4 && L->g.Lh0 % 8 == 0 && !getenv("QCD_PLAQ_LINEAR")) ? 1 : 0;
+    mf.boxed = (D == 4 && L->g.Lh0 % 8 == 0 && L->g.L[1] % 2 == 0) ? 1 : 0;
     if (mf.boxed) {
       mf.n0 = make_fastdiv((uint32_t)(L->g.Lh0 / 8)); mf.n1 = make_fastdiv((uint32_t)(L->g.L[1] / 2)); mf.n2 = make_fastdiv((uint32_t)(L->g.L[2] / 2));
     }
@@ -366,9 +369,9 @@ int qcd_lattice_create(int D, const int* dims, int Nc, int precision, unsigned f
   L->bytes = need; L->mem = device_mem; L->owns_mem = false;
   L->stream = (cudaStream_t)cuda_stream;
   L->seed = 0; L->sweep = 0; L->has_links = false; L->max_trials = 10;
-  L->debug_trials = false; L->profile = false; L->use_graph = true;
+  L->debug_trials = false; L->profile = false;
   L->d_trials = nullptr; L->d_partials = nullptr; L->partials_cap = 0; L->d_results = nullptr; L->h_results = nullptr;
-  L->prof_ms[0] = L->prof_ms[1] = 0.0; L->prof_n[0] = L->prof_n[1] = 0; L->launches = 0; L->last_parity = L->last_mu = -1; L->d_sweep = nullptr; L->d_canon = nullptr;
+  L->prof_ms[0] = L->prof_ms[1] = 0.0; L->prof_n[0] = L->prof_n[1] = 0; L->launches = 0; L->last_parity = L->last_mu = -2; L->d_canon = nullptr;
   L->side = nullptr; L->ev_fork = nullptr; L->ev_join = nullptr;
   cudaError_t e = cudaSuccess;
   if (!device_mem) {
@@ -398,7 +401,6 @@ int qcd_lattice_destroy(qcd_lattice_t* L) {
   if (L->d_partials) cudaFree(L->d_partials);
   if (L->d_results) cudaFree(L->d_results);
   if (L->h_results) cudaFreeHost(L->h_results);
-  if (L->d_sweep) cudaFree(L->d_sweep);
   if (L->ev_fork) cudaEventDestroy(L->ev_fork);
   if (L->ev_join) cudaEventDestroy(L->ev_join);
   if (L->side) cudaStreamDestroy(L->side);
@@ -542,39 +544,50 @@ int qcd_measure(qcd_lattice_t* L, const qcd_field_t* field, double* plaq_total, 
   return QCD_OK;
 }
 
+// Host transfers go through one bounded device staging buffer (STAGE_BYTES, canonical layout) in chunks of whole sites:
+// copy and layout kernel alternate on the lattice's stream, which orders the reuse of the buffer.
+static const size_t STAGE_BYTES = (size_t)64 << 20;
+static int stage_chunks(qcd_lattice_t* L, char* host, bool to_internal) {
+  const size_t site_bytes = canonical_bytes(L) / L->g.V;
+  const size_t per = std::max<size_t>(128, (STAGE_BYTES / site_bytes) / 128 * 128);     // sites per chunk, a multiple of every BL
+  if (!L->d_canon && cudaMalloc(&L->d_canon, per * site_bytes) != cudaSuccess) {
+    L->d_canon = nullptr; cudaGetLastError();
+    return fail(QCD_ERR_ALLOC, "staging buffer");
+  }
+  for (size_t lex0 = 0; lex0 < L->g.V; lex0 += per) {
+    const size_t lex1 = std::min<size_t>(L->g.V, lex0 + per), n = (lex1 - lex0) * site_bytes;
+    if (to_internal) CUDA_TRY(cudaMemcpyAsync(L->d_canon, host + lex0 * site_bytes, n, cudaMemcpyHostToDevice, L->stream));
+    LayoutOp op{L, L->d_canon, to_internal, (uint32_t)lex0, (uint32_t)lex1};
+    const int rc = dispatch(L, op);
+    if (rc != QCD_OK) return rc;
+    if (!to_internal) CUDA_TRY(cudaMemcpyAsync(host + lex0 * site_bytes, L->d_canon, n, cudaMemcpyDeviceToHost, L->stream));
+  }
+  // host memory: the call returns when the host buffer has been read (set) / filled (get), pinned or not
+  CUDA_TRY(cudaStreamSynchronize(L->stream));
+  return QCD_OK;
+}
+
 int qcd_get_links(qcd_lattice_t* L, void* dst, size_t bytes, int dst_is_device) {
   if (!L || !dst) return fail(QCD_ERR_INVALID_ARG, "NULL argument");
   if (!L->has_links) return fail(QCD_ERR_STATE, "no links yet");
   if (bytes != canonical_bytes(L)) return fail(QCD_ERR_INVALID_ARG, "bytes must equal V*D*N*N*2*sizeof(real)");
   if (dst_is_device && ((uintptr_t)dst & 15u)) return fail(QCD_ERR_INVALID_ARG, "device pointer must be 16-byte aligned");
-  void* canon = dst;
-  if (!dst_is_device) {
-    if (!L->d_canon && cudaMalloc(&L->d_canon, bytes) != cudaSuccess) { L->d_canon = nullptr; cudaGetLastError(); return fail(QCD_ERR_ALLOC, "staging buffer"); }
-    canon = L->d_canon;
-  }
-  LayoutOp op{L, canon, false};
-  int rc = dispatch(L, op);
-  if (rc == QCD_OK && !dst_is_device) {
-    CUDA_TRY(cudaMemcpyAsync(dst, canon, bytes, cudaMemcpyDeviceToHost, L->stream));
-    CUDA_TRY(cudaStreamSynchronize(L->stream));
-  }
-  return rc;
+  if (!dst_is_device) return stage_chunks(L, (char*)dst, false);
+  LayoutOp op{L, dst, false, 0u, L->g.V};
+  return dispatch(L, op);
 }
 
 int qcd_set_links(qcd_lattice_t* L, const void* src, size_t bytes, int src_is_device) {
   if (!L || !src) return fail(QCD_ERR_INVALID_ARG, "NULL argument");
   if (bytes != canonical_bytes(L)) return fail(QCD_ERR_INVALID_ARG, "bytes must equal V*D*N*N*2*sizeof(real)");
   if (src_is_device && ((uintptr_t)src & 15u)) return fail(QCD_ERR_INVALID_ARG, "device pointer must be 16-byte aligned");
-  void* canon = const_cast<void*>(src);
+  int rc;
   if (!src_is_device) {
-    if (!L->d_canon && cudaMalloc(&L->d_canon, bytes) != cudaSuccess) { L->d_canon = nullptr; cudaGetLastError(); return fail(QCD_ERR_ALLOC, "staging buffer"); }
-    canon = L->d_canon;
-    // stream-ordered: a later call reuses the staging buffer only after this kernel, on the same stream; the host
-    // buffer may be pageable, in which case cudaMemcpyAsync returns after it has been staged by the driver
-    CUDA_TRY(cudaMemcpyAsync(canon, src, bytes, cudaMemcpyHostToDevice, L->stream));
+    rc = stage_chunks(L, (char*)const_cast<void*>(src), true);
+  } else {
+    LayoutOp op{L, const_cast<void*>(src), true, 0u, L->g.V};
+    rc = dispatch(L, op);
   }
-  LayoutOp op{L, canon, true};
-  int rc = dispatch(L, op);
   if (rc == QCD_OK) L->has_links = true;
   return rc;
 }
@@ -604,7 +617,6 @@ int qcd_set_option(qcd_lattice_t* L, int key, int value) {
       L->max_trials = value; return QCD_OK;
     case QCD_OPT_DEBUG_TRIALS: L->debug_trials = value != 0; return QCD_OK;
     case QCD_OPT_PROFILE: L->profile = value != 0; return QCD_OK;
-    case QCD_OPT_USE_GRAPH: L->use_graph = value != 0; return QCD_OK;
   }
   return fail(QCD_ERR_INVALID_ARG, "unknown option key");
 }

@@ -151,7 +151,10 @@ __global__ void __launch_bounds__(128) init_kernel(Geom g, typename LinkIO<NC, R
 template <typename R> struct LayoutShape { static constexpr int BL = sizeof(R) == 4 ? 128 : 64; };
 
 template <int NC, int D, typename R, bool COMP, bool TO_INTERNAL>
-__global__ void __launch_bounds__(LayoutShape<R>::BL) layout_kernel(Geom g, typename LinkIO<NC, R, COMP>::Vec* links, R* canon) {
+__global__ void __launch_bounds__(LayoutShape<R>::BL) layout_kernel(Geom g, typename LinkIO<NC, R, COMP>::Vec* links, R* canon,
+                                                                    uint32_t lex_begin, uint32_t lex_end) {
+  // sites [lex_begin, lex_end); `canon` is the canonical address of site lex_begin (a chunk of a host transfer, or the
+  // whole array when lex_begin = 0, lex_end = V)
   // One thread per site in LEX order (both parities in one CTA).  A CTA owns BL consecutive sites, i.e. one contiguous
   // block of BL * D * N*N complex numbers of the canonical array, and moves it through shared memory: the global side is
   // a flat, fully coalesced copy (consecutive threads, consecutive complex numbers), the per-site side (a thread's D
@@ -162,10 +165,10 @@ __global__ void __launch_bounds__(LayoutShape<R>::BL) layout_kernel(Geom g, type
   typedef typename std::conditional<sizeof(R) == 4, float2, double2>::type C2;   // one complex number of the canonical array
   constexpr int BL = LayoutShape<R>::BL, NCX = D * NC * NC, PITCH = NCX + 1;
   __shared__ C2 buf[BL * PITCH];
-  const uint32_t lex0 = blockIdx.x * BL, t = threadIdx.x;
-  const uint32_t nsite = (g.V - lex0 < (uint32_t)BL) ? g.V - lex0 : (uint32_t)BL;
+  const uint32_t lex0 = lex_begin + blockIdx.x * BL, t = threadIdx.x;
+  const uint32_t nsite = (lex_end - lex0 < (uint32_t)BL) ? lex_end - lex0 : (uint32_t)BL;
   const uint32_t nel = nsite * NCX;
-  C2* gc = reinterpret_cast<C2*>(canon) + (size_t)lex0 * NCX;
+  C2* gc = reinterpret_cast<C2*>(canon) + (size_t)(lex0 - lex_begin) * NCX;
   if (TO_INTERNAL) {
     for (uint32_t i = t; i < nel; i += BL) buf[(i / NCX) * PITCH + (i % NCX)] = gc[i];
     __syncthreads();

@@ -158,13 +158,8 @@ __device__ __forceinline__ void store_reals(typename PlaneTraits<R, NREAL>::Vec*
 // that does not touch the links (site decoding, neighbour offsets, the heatbath's random numbers) and then block in
 // pdl_wait() until the previous grid has completed and its stores are visible.  pdl_trigger() at the top of a kernel lets
 // the next one do the same.  Without the attribute both are no-ops.
-#ifndef QCD_NO_PDL
 __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
-#else
-__device__ __forceinline__ void pdl_trigger() {}
-__device__ __forceinline__ void pdl_wait() {}
-#endif
 template <typename... KArgs, typename... Args>
 inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
   cudaLaunchConfig_t cfg;
@@ -173,11 +168,7 @@ inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, siz
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
-#ifndef QCD_NO_PDL
   cfg.numAttrs = 1;
-#else
-  cfg.numAttrs = 0;
-#endif
   return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
 }
 

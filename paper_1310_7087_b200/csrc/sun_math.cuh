@@ -51,7 +51,6 @@ template <typename R> __device__ __forceinline__ Cx<R> cdot2_nn(const Cx<R>& a0,
 //     T1 = sum_k a_k.re * (b_k.re, b_k.im)        T2 = sum_k a_k.im * (b_k.im, b_k.re)
 // and the signs are applied once per dot product:  NN (T1.x - T2.x, T1.y + T2.y)   ND (T1.x + T2.x, T2.y - T1.y)
 // DN (T1.x + T2.x, T1.y - T2.y):  8 issue slots per 3-term dot product instead of 12.
-#ifndef QCD_NO_FFMA2
 __device__ __forceinline__ float2 f2_bcast(float x) { return make_float2(x, x); }
 __device__ __forceinline__ float2 f2_of(const Cx<float>& c) { return make_float2(c.re, c.im); }
 __device__ __forceinline__ float2 f2_swap(const Cx<float>& c) { return make_float2(c.im, c.re); }
@@ -84,7 +83,6 @@ __device__ __forceinline__ Cx<float> cdot2_nn(const Cx<float>& a0, const Cx<floa
   t2 = __ffma2_rn(f2_bcast(a1.im), f2_swap(b1), t2);
   return f2_signs<CD_NN>(t1, t2);
 }
-#endif
 
 template <typename R> struct M3 { Cx<R> e[3][3]; };
 
@@ -100,7 +98,6 @@ template <typename R> __device__ __forceinline__ void m3_complete_row2(M3<R>& a)
   }
 }
 
-#ifndef QCD_NO_FFMA2
 // fp32: each component conj(p*q - r*s) as two packed accumulators, 6 issue slots instead of 8
 __device__ __forceinline__ void m3_complete_row2(M3<float>& a) {
 #pragma unroll
@@ -116,7 +113,6 @@ __device__ __forceinline__ void m3_complete_row2(M3<float>& a) {
     a.e[2][c].im = v.y;
   }
 }
-#endif
 
 // The three product shapes, rows [0,NR) of acc += op(a) op(b), written as outer-product accumulation over k: the six
 // consecutive multiply-adds that follow share the scalar a.re (then a.im) in the same operand slot, which lets the
@@ -145,7 +141,6 @@ template <int NR, int MODE, typename R> __device__ __forceinline__ void m3_mad(M
       }
     }
 }
-#if !defined(QCD_NO_FFMA2) && !defined(QCD_OUTER_SCALAR)
 // fp32 packed: per (i,j) two accumulators T1 += a.re * (b.re, b.im), T2 += a.im * (b.im, b.re), same k-outer order
 template <int NR, int MODE> __device__ __forceinline__ void m3_mad(M3<float>& acc, const M3<float>& a, const M3<float>& b) {
   float2 t1[NR][3], t2[NR][3];
@@ -176,7 +171,6 @@ template <int NR, int MODE> __device__ __forceinline__ void m3_mad(M3<float>& ac
       acc.e[i][j] = f2_signs<MODE>(t1[i][j], t2[i][j]);
     }
 }
-#endif
 template <typename R, int NR> __device__ __forceinline__ void m3_mad_nn(M3<R>& acc, const M3<R>& a, const M3<R>& b) { m3_mad<NR, CD_NN>(acc, a, b); }
 // rows [0,NR) of acc += a * b^dagger      (needs rows [0,NR) of a and ALL rows of b)
 template <typename R, int NR> __device__ __forceinline__ void m3_mad_nd(M3<R>& acc, const M3<R>& a, const M3<R>& b) { m3_mad<NR, CD_ND>(acc, a, b); }

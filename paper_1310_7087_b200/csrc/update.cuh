@@ -29,8 +29,9 @@ struct UpdateArgs {
   double beta;
   double inv_c;      // N / (2 beta): delta = E / alpha = E * inv_c / k   (host-computed; inf when beta = 0 -> every trial fails)
   int parity, mu, hit, max_trials;
-  int prev_parity, prev_mu;   // the update kernel launched just before this one on the stream (-1: none): its output array
-                              // (prev_parity, prev_mu) is the only one that may not be read before griddepcontrol.wait
+  int prev_parity, prev_mu;   // the kernel launched just before this one on the stream: an update kernel (its output array
+                              // (prev_parity, prev_mu) is the only one that may not be read before griddepcontrol.wait),
+                              // -1: a kernel that writes no links, -2: a kernel that writes all of them (init, set_links)
   uint32_t sweep, key0, key1;
   uint8_t* trials;   // NULL or [lex][3] debug trial codes
   TileMap tm;        // thread -> site mapping of the SU(3) kernels (set by the launcher)
@@ -50,13 +51,11 @@ template <int I, int N, typename F> __device__ __forceinline__ void static_for(F
 template <int BYTES> __device__ __forceinline__ void cp_async_vec(void* smem_dst, const void* gmem_src) {
   static_assert(BYTES == 8 || BYTES == 16, "plane vectors are 8 or 16 bytes");
   const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
-#ifndef QCD_CP_ASYNC_CA
   if constexpr (BYTES == 16) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem_src) : "memory");
-    return;
+  } else {                                                          // 8-byte vectors (fp32 x18): .cg needs 16 bytes
+    asm volatile("cp.async.ca.shared.global [%0], [%1], %2;\n" ::"r"(s), "l"(gmem_src), "n"(BYTES) : "memory");
   }
-#endif
-  asm volatile("cp.async.ca.shared.global [%0], [%1], %2;\n" ::"r"(s), "l"(gmem_src), "n"(BYTES) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
@@ -254,7 +253,6 @@ template <typename R> __device__ __forceinline__ void su3_scale_rows(M3<R>& m, c
     for (int j = 0; j < 3; ++j) m.e[r][j] = cmul(m.e[r][j], ph);
   }
 }
-#ifndef QCD_NO_FFMA2
 __device__ __forceinline__ void m3_add(M3<float>& a, const M3<float>& s) {
 #pragma unroll
   for (int r = 0; r < 3; ++r)
@@ -264,7 +262,6 @@ __device__ __forceinline__ void m3_add(M3<float>& a, const M3<float>& s) {
       a.e[r][c].re = v.x; a.e[r][c].im = v.y;
     }
 }
-#endif
 template <typename R> __device__ __forceinline__ void m3_add(M3<R>& a, const M3<R>& s) {
 #pragma unroll
   for (int r = 0; r < 3; ++r)
@@ -324,39 +321,38 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
   int fo[D], bo[D];
 #pragma unroll
   for (int d = 0; d < D; ++d) nbr_offsets(g, sc, d, fo[d], bo[d]);
-  const uint32_t arr = (uint32_t)NP * g.Vh_pad;                    // vectors per (parity, direction) array
-  const uint32_t own_base = (uint32_t)(p * D + MU) * arr;         // array bases (vectors); elements at base + blk_off(h')
-  const uint32_t qmu_base = (uint32_t)((1 - p) * D + MU) * arr;
-  auto at = [&](uint32_t base, int off) -> uint32_t { return base + blk_off<NP>(h + (uint32_t)off); };
+  // A (parity, direction) array holds arr = NP * Vh_pad vectors (< 2^32, checked at creation); its base is a 64-bit,
+  // warp-uniform pointer and elements are addressed by the 32-bit in-array offset blk_off(h').
+  const size_t arr = (size_t)NP * g.Vh_pad;
+  Vec* const own_ptr = links + (size_t)(p * D + MU) * arr;
+  const Vec* const qmu_ptr = links + (size_t)((1 - p) * D + MU) * arr;
+  auto at = [&](const Vec* base, int off) -> const Vec* { return base + blk_off<NP>(h + (uint32_t)off); };
 
-  struct Dir { uint32_t p_idx, q_idx; int f, b, nu; };             // per-direction addressing (array bases), run-time nu
+  struct Dir { const Vec *pp, *qp; int f, b, nu; };                // per-direction addressing (array bases), run-time nu
   auto make_dir = [&](int i) {
     Dir d;
     d.nu = i + (i >= MU ? 1 : 0);
     d.f = fo[0]; d.b = bo[0];
 #pragma unroll
     for (int k = 1; k < D; ++k) if (d.nu == k) { d.f = fo[k]; d.b = bo[k]; }
-    d.p_idx = (uint32_t)(p * D + d.nu) * arr;
-    d.q_idx = (uint32_t)((1 - p) * D + d.nu) * arr;
+    d.pp = links + (size_t)(p * D + d.nu) * arr;
+    d.qp = links + (size_t)((1 - p) * D + d.nu) * arr;
     return d;
   };
-  // vector index of plane 0 of link j of direction d (j = 6: the own link)
-  auto link_idx = [&](auto jc, const Dir& d) -> uint32_t {
+  // plane 0 of link j of direction d (j = 6: the own link)
+  auto link_ptr = [&](auto jc, const Dir& d) -> const Vec* {
     constexpr int J = decltype(jc)::value;
-    if constexpr (J == 0) return at(qmu_base, d.f);
-    else if constexpr (J == 1) return at(d.p_idx, 0);
-    else if constexpr (J == 2) return at(d.q_idx, fo[MU]);
-    else if constexpr (J == 3) return at(d.p_idx, fo[MU] + d.b);
-    else if constexpr (J == 4) return at(qmu_base, d.b);
-    else if constexpr (J == 5) return at(d.q_idx, d.b);
-    else return at(own_base, 0);
+    if constexpr (J == 0) return at(qmu_ptr, d.f);
+    else if constexpr (J == 1) return at(d.pp, 0);
+    else if constexpr (J == 2) return at(d.qp, fo[MU]);
+    else if constexpr (J == 3) return at(d.pp, fo[MU] + d.b);
+    else if constexpr (J == 4) return at(qmu_ptr, d.b);
+    else if constexpr (J == 5) return at(d.qp, d.b);
+    else return at(own_ptr, 0);
   };
   auto issue = [&](auto jc, const Dir& d, int n) {                  // cp.async link J (n-th of the sequence) into ring slot n % K
     constexpr int J = decltype(jc)::value;
-#ifdef QCD_EXP_NOLOAD
-    return;
-#endif
-    const Vec* src = links + link_idx(jc, d);
+    const Vec* src = link_ptr(jc, d);
     Vec* dst = ring + (n % KR) * NP * B;
     // Links that enter only as the LEFT factor of a product whose third row is rebuilt anyway (U3, U1, U2': J = 1, 2, 4)
     // and the own link (J = 6) contribute rows 0,1 only: with 18-real storage the planes of their third row are not
@@ -369,18 +365,12 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
   auto fetch = [&](auto jc, const Dir& d, M3<R>& u, bool row2, int n) {
     constexpr int J = decltype(jc)::value;
     R r[NREAL];
-#ifdef QCD_EXP_NOLOAD
-    if (true) {
-#pragma unroll
-      for (int k = 0; k < NREAL; ++k) r[k] = (R)((h + J) & 7u) * R(0.01) + R(0.1) * (R)k + (R)d.f * R(1e-9);
-    } else
-#endif
     if constexpr (K > 0) {
       const Vec* src = ring + (n % KR) * NP * B;
 #pragma unroll
       for (int k = 0; k < NP; ++k) vec_unpack(src[k * B], r + k * T::VW);
     } else {
-      const Vec* src = links + link_idx(jc, d);
+      const Vec* src = link_ptr(jc, d);
       // the own-link array is written by this kernel (each thread its own element): plain load; the rest is read-only
 #pragma unroll
       for (int k = 0; k < NP; ++k) vec_unpack(J == 6 ? src[k * PLANE_STRIDE] : __ldg(src + k * PLANE_STRIDE), r + k * T::VW);
@@ -413,7 +403,9 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
   // while that kernel drains (in sweep order the previous kernel writes (p, mu-1): only mu = 1 has to wait).  The trigger
   // for the next kernel comes after this kernel's own wait, so at most one earlier update kernel is ever in flight.
   Dir cur = make_dir(0);
-  const bool early = !((a.prev_parity == 1 - p && (a.prev_mu == MU || a.prev_mu == cur.nu)) || (a.prev_parity == p && a.prev_mu == cur.nu));
+  // prev_parity = -2: the kernel before this one wrote every array (init, set_links): nothing may be read early.
+  const bool early = a.prev_parity != -2 &&
+                     !((a.prev_parity == 1 - p && (a.prev_mu == MU || a.prev_mu == cur.nu)) || (a.prev_parity == p && a.prev_mu == cur.nu));
   auto prologue = [&]() {
     if constexpr (K > 0) static_for<0, KR - 1>([&](auto jc) { issue(jc, cur, decltype(jc)::value); cp_async_commit(); });
   };
@@ -443,15 +435,6 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
         cp_async_commit();                                         // one group per step, possibly empty
         cp_async_wait<KR - 1>();                                   // link (i, J) has landed
       }
-#ifdef QCD_EXP_NOCOMPUTE
-      if (true) {
-        M3<R> Ux;
-        m3_zero(Ux);
-        fetch(jc, cur, Ux, false, n0 + decltype(jc)::value);
-        m3_add(A, Ux);
-        return;
-      }
-#endif
       if constexpr (J == 0) {
         fetch(jc, cur, P, true, n0 + decltype(jc)::value);                                   // U2, all rows
       } else if constexpr (J == 1) {
@@ -507,14 +490,6 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
   M3<R> U;
   fetch(std::integral_constant<int, 6>{}, cur, U, true, ROLL ? 6 : 6 * (D - 1));
 
-#if defined(QCD_EXP_NOCOMPUTE) || defined(QCD_EXP_NOHIT)
-  if (true) {
-#pragma unroll
-    for (int r = 0; r < 3; ++r)
-#pragma unroll
-      for (int c = 0; c < 3; ++c) { U.e[r][c].re += R(1e-30) * A.e[r][c].re; U.e[r][c].im += R(1e-30) * A.e[r][c].im; }
-  } else
-#endif
   if constexpr (KIND == 1) {
     int c;
     HbDraw<R> none;
@@ -556,9 +531,7 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
       }
     }
   }
-#ifndef QCD_EXP_NOHIT
   m3_reunitarise(U);
-#endif
 
   R r[NREAL];
   m3_to_reals<R, NREAL>(U, r);

@@ -77,10 +77,10 @@ su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* 
   int fo[D], bo[D];
 #pragma unroll
   for (int d = 0; d < D; ++d) nbr_offsets(g, sc, d, fo[d], bo[d]);
-  const uint32_t arr = (uint32_t)NP * g.Vh_pad;
-  const uint32_t own_base = (uint32_t)(p * D + MU) * arr;                     // array bases; elements at base + blk_off(h')
-  const uint32_t qmu_base = (uint32_t)((1 - p) * D + MU) * arr;
-  auto at = [&](uint32_t base, int off) -> uint32_t { return base + blk_off<NP>(h + (uint32_t)off); };
+  const size_t arr = (size_t)NP * g.Vh_pad;                                   // vectors per array (< 2^32); 64-bit uniform bases
+  Vec* const own_ptr = links + (size_t)(p * D + MU) * arr;
+  const Vec* const qmu_ptr = links + (size_t)((1 - p) * D + MU) * arr;
+  auto at = [&](const Vec* base, int off) -> const Vec* { return base + blk_off<NP>(h + (uint32_t)off); };
   const uint32_t lex = 2u * h + (uint32_t)s;
   const int lin = (int)threadIdx.x;                                          // slot of box element c
   // index of c inside the face of direction d (the d-th coordinate dropped)
@@ -95,50 +95,48 @@ su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* 
   // kernel running just before this one writes the array (q, mu) -- in sweep order it never does -- the region is fetched
   // before griddepcontrol.wait, while that kernel drains.
   auto stage_resident = [&]() {
-    auto stage = [&](int slot, uint32_t src_idx) {
-      const Vec* src = links + src_idx;
+    auto stage = [&](int slot, const Vec* src) {
 #pragma unroll
       for (int k = 0; k < NP; ++k) cp_async_vec<(int)sizeof(Vec)>(res + k * RES + slot, src + k * PLANE_STRIDE);
     };
-    stage(lin, at(qmu_base, 0));
+    stage(lin, at(qmu_ptr, 0));
 #pragma unroll
     for (int d = 0; d < D; ++d) {
       if (d == MU) continue;
       const int fb = TD::face_base(MU, d), l3 = lin3(d);
       if (d == 0) {
         // a row with s = 0 needs j-1 of its first site, a row with s = 1 needs j+1 of its last site
-        if (c[0] == 0 && s == 0) stage(fb + l3, at(qmu_base, bo[0]));
-        if (c[0] == TD::T0 - 1 && s == 1) stage(fb + l3, at(qmu_base, fo[0]));
+        if (c[0] == 0 && s == 0) stage(fb + l3, at(qmu_ptr, bo[0]));
+        if (c[0] == TD::T0 - 1 && s == 1) stage(fb + l3, at(qmu_ptr, fo[0]));
       } else {
-        if (c[d] == 0) stage(fb + l3, at(qmu_base, bo[d]));
-        if (c[d] == TD::T(d) - 1) stage(fb + B / TD::T(d) + l3, at(qmu_base, fo[d]));
+        if (c[d] == 0) stage(fb + l3, at(qmu_ptr, bo[d]));
+        if (c[d] == TD::T(d) - 1) stage(fb + B / TD::T(d) + l3, at(qmu_ptr, fo[d]));
       }
     }
     cp_async_commit();
   };
 
   // ---- ring
-  struct Dir { uint32_t p_idx, q_idx; int b, nu; };
+  struct Dir { const Vec *pp, *qp; int b, nu; };
   auto make_dir = [&](int i) {
     Dir d;
     d.nu = i + (i >= MU ? 1 : 0);
     d.b = bo[0];
 #pragma unroll
     for (int k = 1; k < D; ++k) if (d.nu == k) d.b = bo[k];
-    d.p_idx = (uint32_t)(p * D + d.nu) * arr;
-    d.q_idx = (uint32_t)((1 - p) * D + d.nu) * arr;
+    d.pp = links + (size_t)(p * D + d.nu) * arr;
+    d.qp = links + (size_t)((1 - p) * D + d.nu) * arr;
     return d;
   };
-  auto ring_idx = [&](auto rc, const Dir& d) -> uint32_t {
+  auto ring_idx = [&](auto rc, const Dir& d) -> const Vec* {
     constexpr int RR = decltype(rc)::value;
-    if constexpr (RR == 0) return at(d.p_idx, 0);
-    else if constexpr (RR == 1) return at(d.q_idx, fo[MU]);
-    else if constexpr (RR == 2) return at(d.p_idx, fo[MU] + d.b);
-    else if constexpr (RR == 3) return at(d.q_idx, d.b);
-    else return at(own_base, 0);
+    if constexpr (RR == 0) return at(d.pp, 0);
+    else if constexpr (RR == 1) return at(d.qp, fo[MU]);
+    else if constexpr (RR == 2) return at(d.pp, fo[MU] + d.b);
+    else if constexpr (RR == 3) return at(d.qp, d.b);
+    else return at(own_ptr, 0);
   };
-  auto issue = [&](int n, uint32_t src_idx) {                   // link n of the sequence -> slot n % K
-    const Vec* src = links + src_idx;
+  auto issue = [&](int n, const Vec* src) {                     // link n of the sequence -> slot n % K
     Vec* dst = ring + (n % K) * NP * B;
 #pragma unroll
     for (int k = 0; k < NP; ++k) cp_async_vec<(int)sizeof(Vec)>(dst + k * B, src + k * PLANE_STRIDE);
@@ -162,7 +160,7 @@ su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* 
   // The first K-1 ring links come from the arrays (p, nu0), (q, nu0) of the first direction: same rule.
   Dir cur = make_dir(0);
   auto prologue = [&]() { static_for<0, K - 1>([&](auto rc) { issue(decltype(rc)::value, ring_idx(rc, cur)); cp_async_commit(); }); };
-  const bool early_res = !(a.prev_parity == 1 - p && a.prev_mu == MU);
+  const bool early_res = a.prev_parity != -2 && !(a.prev_parity == 1 - p && a.prev_mu == MU);   // -2: every array was just written
   const bool early_ring = early_res && a.prev_mu != cur.nu;
   if (early_res) stage_resident();
   if (early_ring) prologue();
@@ -184,7 +182,7 @@ su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* 
         issue(4 * i + RA, ring_idx(std::integral_constant<int, RA>{}, cur));
       } else {
         if (!last) issue(4 * i + RA, ring_idx(std::integral_constant<int, RA - 4>{}, nxt));
-        else if (RA == 4) issue(4 * i + RA, at(own_base, 0));          // the own link, once, after the last direction
+        else if (RA == 4) issue(4 * i + RA, at(own_ptr, 0));          // the own link, once, after the last direction
       }
       cp_async_commit();                                       // one group per step, possibly empty
       cp_async_wait<K - 1>();

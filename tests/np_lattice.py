@@ -74,3 +74,26 @@ def unitarity_defect(links):
     N = links.shape[-1]
     uu = links @ dag(links) - np.eye(N)
     return float(np.max(np.abs(uu))), float(np.max(np.abs(np.linalg.det(links) - 1.0)))
+
+
+def staple_dependents(mask, dims, mu):
+    """Sites whose U_mu update reads a marked link.  mask: (V, D) bool of marked links; returns (V,) bool: True at x if the
+    own link U_mu(x) or any of the 6(D-1) links of its staples -- U_nu(x), U_nu(x+mu), U_mu(x+nu), U_nu(x-nu), U_mu(x-nu),
+    U_nu(x+mu-nu) for nu != mu -- is marked.  (Pure index bookkeeping: used to fence off the links a heatbath accept/reject
+    disagreement can reach in later, un-resynced sub-steps.)"""
+    D = len(dims)
+    g = mask.reshape(tuple(reversed(dims)) + (D,))
+    dep = g[..., mu].copy()
+    for nu in range(D):
+        if nu == mu:
+            continue
+        gn, gm = g[..., nu], g[..., mu]
+        dep |= gn | shift(gn, dims, mu) | shift(gm, dims, nu)
+        dep |= shift(gn, dims, nu, -1) | shift(gm, dims, nu, -1) | shift(shift(gn, dims, mu), dims, nu, -1)
+    return dep.reshape(-1)
+
+
+def site_parity(dims):
+    """(V,) parity (sum of coordinates) & 1 in lex order"""
+    V = int(np.prod(dims))
+    return np.stack(np.unravel_index(np.arange(V), tuple(reversed(dims))), axis=-1).sum(axis=1) & 1

@@ -39,9 +39,12 @@ def test_lattice_bytes(q):
     assert q.qcd_lattice_bytes((32, 32, 32, 32), 3, q.QCD_FP64, 0) == 4 * 32 ** 4 * 144
     assert q.qcd_lattice_bytes((48, 48, 48, 8), 2, q.QCD_FP32, 0) == 4 * 48 ** 3 * 8 * 16
     assert q.qcd_lattice_bytes((64, 64, 64, 64), 3, q.QCD_FP64, 0) == 4 * 64 ** 4 * 144
-    # 128^4: 51.5 GB of 12-real fp32 links are addressable with the kernels' 32-bit vector indices, 154.6 GB of fp64 are not
+    # 128^4: each (parity, direction) array is addressed with 32 bits, the array bases are 64-bit: 51.5 GB of 12-real fp32
+    # links and 154.6 GB of 18-real fp64 links (the largest lattice of one B200) are both within the indexing; V > 2^31 is not
     assert q.qcd_lattice_bytes((128, 128, 128, 128), 3, q.QCD_FP32, q.QCD_FLAG_COMPRESS12) == 4 * 128 ** 4 * 48
-    assert q.qcd_lattice_bytes((128, 128, 128, 128), 3, q.QCD_FP64, 0) == 0
+    assert q.qcd_lattice_bytes((128, 128, 128, 128), 3, q.QCD_FP64, 0) == 4 * 128 ** 4 * 144
+    assert q.qcd_lattice_bytes((256, 256, 256, 128), 2, q.QCD_FP32, 0) == 4 * 2 ** 31 * 16
+    assert q.qcd_lattice_bytes((256, 256, 256, 256), 2, q.QCD_FP32, 0) == 0
     assert q.qcd_lattice_bytes((6, 4), 2, q.QCD_FP64, 0) == 2 * 2 * 2 * 32 * 16       # V/2 = 12 padded to 32
     for bad in [((5, 4), 2, 1, 0), ((4,), 2, 1, 0), ((4, 4, 4, 4, 4), 2, 1, 0), ((4, 4), 4, 1, 0), ((4, 4), 2, 2, 0),
                 ((4, 4), 2, 1, 1), ((0, 4), 2, 1, 0), ((4, 4), 3, 1, 2)]:

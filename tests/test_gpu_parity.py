@@ -10,25 +10,10 @@ import pytest
 import oracle
 from tests import np_lattice as npl
 from tests.inputs import random_links, round_to_fp32
+# the bars and the arithmetic they come from (conditioning rule with its ceiling, Haar expectation, un-resynced bar)
+from tests.tolerances import K_COND, MEAS_TOL, TOL, illcond_bound, link_tol, unresynced_bar
 
 pytestmark = pytest.mark.gpu
-
-TOL = {0: 2e-5, 1: 1e-12}          # per-element max abs, by precision (0 = fp32, 1 = fp64)
-# Conditioning rule: the update maps the projected staple v to v/|v|, whose Lipschitz constant
-# is 1/k, k = |v|.  fp32 rounding of v is ~3e-7 absolute whatever k is, so a link whose smallest subgroup norm is
-# k < K_COND (only met on hot / Haar-random configurations, never on thermalised ones where k ~ 4) gets the bar
-# TOL * K_COND / k.  The oracle reports k per link (substep_diag); fp64 needs no such rule at these sizes.
-K_COND = 0.25
-
-
-def link_tol(prec, kmin):
-    """per-link tolerance array from the oracle's conditioning numbers kmin (inf where the link was not updated)"""
-    t = np.full(kmin.shape, TOL[prec])
-    if prec == 0:
-        small = kmin < K_COND
-        t[small] = TOL[prec] * K_COND / np.maximum(kmin[small], 1e-6)
-    return t
-MEAS_TOL = {0: 2e-6, 1: 1e-12}     # observables (means over the lattice)
 
 # (Nc, precision, flags)
 VARIANTS = [(3, 1, 0), (3, 0, 1), (3, 0, 0), (3, 1, 1), (2, 1, 0), (2, 0, 0)]
@@ -200,6 +185,8 @@ def test_overrelaxation_substeps(qcd, variant, dims, fld):
     assert compared > 0
     print("OR worst diff/tol %.3f; links under the conditioning rule: %d of %d" % (worst, illcond, compared))
     assert worst < 1.0, worst
+    # Haar inputs: how many links may fall under the conditioning rule is bounded by the derived expectation
+    assert illcond <= illcond_bound(variant[0], len(dims), compared), (illcond, compared)
 
 
 @pytest.mark.parametrize("variant", VARIANTS, ids=VARIANT_IDS)
@@ -213,6 +200,8 @@ def test_heatbath_substeps(qcd, variant, dims, fld, spread):
     assert worst < 1.0, worst
     if spread is not None:
         assert illcond == 0          # thermalised links are well conditioned: the plain north_star bar applied
+    else:
+        assert illcond <= illcond_bound(variant[0], len(dims), compared), (illcond, compared)
     # north_star: accept/reject disagreements at most 1e-6 of links (reported); on these small lattices that is zero
     print("heatbath disagreements: %d of %d links" % (disagreements, compared))
     assert disagreements <= max(0, int(1e-6 * compared)), (disagreements, compared)
@@ -240,9 +229,86 @@ def test_heatbath_trial_cap_and_exhaustion(qcd):
 
 
 # ----------------------------------------------------------------------------- whole sweeps without resync
+def _unresynced_sequence(qcd, G, O, dims, Nc, prec, flags, beta, sequence, fg=None, fo=None):
+    """Run `sequence` = [(kind, hit, parity, mu), ...] on both sides WITHOUT resync from the state both already hold.
+    Heatbath accept/reject codes are compared per sub-step; a disagreement changes that link by O(1) and reaches, in later
+    sub-steps, the links whose staples contain it: those links (the dependency cone, tests/np_lattice.staple_dependents) are
+    fenced off, every other link must stay within the un-resynced bar (tests/tolerances.unresynced_bar).  Returns
+    (flips, fenced links, worst diff outside the fence, median conditioning number k, min k, GPU links)."""
+    V, D = int(np.prod(dims)), len(dims)
+    par = npl.site_parity(dims)
+    fence = np.zeros((V, D), dtype=bool)
+    flips, kmed, kmin_all = 0, [], np.inf
+    G.qcd_set_option(qcd.QCD_OPT_DEBUG_TRIALS, 1)
+    for kind, hit, parity, mu in sequence:
+        tr_o, kmin = O.substep_diag(beta, kind, hit, parity, mu, fo)
+        k = kmin[np.isfinite(kmin)]
+        kmed.append(float(np.median(k)))
+        kmin_all = min(kmin_all, float(k.min()))
+        G.qcd_debug_substep(beta, kind, hit, parity, mu, fg)
+        # links of this sub-step that read a fenced link join the fence
+        dep = npl.staple_dependents(fence, dims, mu) & (par == parity)
+        fence[dep, mu] = True
+        if kind == 0:
+            tr_g = G.qcd_debug_get_trials()
+            bad = np.any(tr_g != tr_o, axis=1) & (par == parity)
+            flips += int(bad.sum())
+            fence[bad, mu] = True
+    got = G.qcd_get_links().astype(np.complex128)
+    diff = np.max(np.abs(got - O.get_links()), axis=(-1, -2))
+    worst = float(diff[~fence].max()) if (~fence).any() else 0.0
+    return flips, int(fence.sum()), worst, float(np.median(kmed)), kmin_all, got
+
+
+def _sweep_sequence(D, n_hb, n_or):
+    return [(0 if s < n_hb else 1, s if s < n_hb else 0, p, mu) for s in range(n_hb + n_or) for p in (0, 1) for mu in range(D)]
+
+
 @pytest.mark.parametrize("variant", VARIANTS, ids=VARIANT_IDS)
-def test_full_sweep_unresynced(qcd, variant):
-    # config 2 shape for SU(3), config-4-like shape for SU(2); one sweep of 1 HB + 2 OR from the hot start
+def test_full_sweep_unresynced_from_thermal_state(qcd, variant):
+    """One whole sweep (1 HB + 2 OR, 24 sub-steps) without resync, config-2 shape for SU(3) and a config-4-like shape for
+    SU(2), from a thermal-like configuration (well conditioned: the plain bars apply).  Bar: every link-hit adds at most the
+    single-sub-step bar and passes on what its 18 staple links carry with the RMS gain sqrt(18)/k (tests/tolerances.py).
+    qcd_sweep itself must then reproduce, bit for bit, the sequence of debug sub-steps that was compared with the oracle."""
+    Nc, prec, flags = variant
+    dims = (16, 16, 16, 4) if Nc == 3 else (12, 12, 12, 8)
+    beta = 5.7 if Nc == 3 else 2.5
+    D = len(dims)
+    links = prep_links(dims, Nc, prec, seed=29, spread=0.35)
+    O = oracle_lattice(dims, Nc, prec, links)
+    O.set_seed(7)
+    with gpu_lattice(qcd, dims, Nc, prec, flags) as G:
+        G.qcd_set_seed(7)
+        G.qcd_set_links(links)
+        flips, fenced, worst, kmed, kmin, got = _unresynced_sequence(qcd, G, O, dims, Nc, prec, flags, beta, _sweep_sequence(D, 1, 2))
+        bar = unresynced_bar(prec, 3, kmed)
+        print("un-resynced sweep: flips %d, fenced links %d of %d, worst %.3e (bar %.3e), k median %.2f min %.2f"
+              % (flips, fenced, got.shape[0] * D, worst, bar, kmed, kmin))
+        assert kmin > K_COND                       # no link under the conditioning rule on this state
+        assert flips <= 1 and fenced <= 20000 * flips      # north_star: <= 1e-6 of links; one flip reaches < 20000 links in 2 passes
+        assert worst < bar, (worst, bar)
+        uni, det = npl.unitarity_defect(got)
+        assert uni < (1e-12 if prec == 1 else 5e-6) and det < (1e-12 if prec == 1 else 5e-6)
+        # qcd_sweep = the same 24 launches
+        G.qcd_set_links(links)
+        G.qcd_set_sweep_counter(0)
+        G.qcd_sweep(beta, 1, 2)
+        assert G.qcd_get_sweep_counter() == 1
+        again = G.qcd_get_links().astype(np.complex128)
+        assert np.array_equal(again, got)
+        m_g, m_o = G.qcd_measure(), O.measure()
+        if flips == 0:
+            assert abs(m_g[0] - m_o[0]) < 10 * MEAS_TOL[prec]
+
+
+@pytest.mark.parametrize("variant", VARIANTS, ids=VARIANT_IDS)
+def test_full_sweep_unresynced_from_hot_start(qcd, variant):
+    """The same from the HOT start of config 2 (seed 7).  fp64: links agree to the un-resynced bar scaled by the worst
+    conditioning met (k ~ 0.01 occurs among 65536 Haar links: 1e-12 * K_COND / k per hit).  fp32: links under the
+    conditioning rule (tests/tolerances.expected_illcond_fraction: ~0.6 % per sub-step) lose digits at each of the 24
+    sub-steps and pass that on, so link-by-link agreement of an un-resynced sweep is not defined from this state -- per
+    sub-step parity from Haar inputs and un-resynced parity from a thermal state are the tests above; here the observables
+    and the group property must agree."""
     Nc, prec, flags = variant
     dims = (16, 16, 16, 4) if Nc == 3 else (12, 12, 12, 8)
     beta = 5.7 if Nc == 3 else 2.5
@@ -261,18 +327,15 @@ def test_full_sweep_unresynced(qcd, variant):
         got = G.qcd_get_links().astype(np.complex128)
         assert G.qcd_get_sweep_counter() == 1
         m_g = G.qcd_measure()
-    diff = np.max(np.abs(got - ref), axis=(-1, -2))
-    # an accept/reject disagreement changes a link by O(1) and contaminates its neighbours in later sub-steps:
-    # report how many links are off, require (almost) all of them within tolerance
-    # (24 un-resynced sub-steps from a hot start amplify rounding: looser bar than the per-sub-step one)
-    bar = 1e-9 if prec == 1 else 1e-3
-    off = int(np.sum(diff > bar))
-    print("links off after an un-resynced sweep: %d of %d, worst in-bar %.3e" % (off, diff.size, float(diff[diff <= bar].max())))
-    # fp32 from a hot start: ill-conditioned links (k << 1, see K_COND) lose digits at each of the 24 sub-steps and spread
-    # to their neighbours; the count is reported, bounded at 0.2 % of links, and the observables must still agree
-    assert off <= (0 if prec == 1 else diff.size // 500)
     m_o = O.measure()
+    if prec == 1:
+        diff = np.max(np.abs(got - ref), axis=(-1, -2))
+        print("fp64 hot un-resynced sweep: worst link diff %.3e" % float(diff.max()))
+        # Haar links: k is typically |sum of 6 Haar staples| ~ 1.5 (gain sqrt(18)/1.5 per hit) and the worst of the 2.6e5
+        # link-hits is amplified by up to K_COND / K_FLOOR = 100 (the ceiling of the conditioning rule): 1.2e-9
+        assert float(diff.max()) < unresynced_bar(1, 3, 1.5) * 100.0
     assert abs(m_g[0] - m_o[0]) < (1e-11 if prec == 1 else 1e-4)
+    assert abs(m_g[2] - m_o[2]) < (1e-10 if prec == 1 else 2e-3)
     uni, det = npl.unitarity_defect(got)
     assert uni < (1e-12 if prec == 1 else 5e-6) and det < (1e-12 if prec == 1 else 5e-6)
 
@@ -283,15 +346,20 @@ def test_substeps_back_to_back_in_any_order(qcd, variant):
     write (prev_parity / prev_mu in the launch arguments).  qcd_sweep always launches (p, mu-1) before (p, mu); here the
     sub-steps follow each other WITHOUT a resync in orders a sweep never uses -- in particular (1-p, mu) right before
     (p, mu), whose output is the resident U_mu box of the tiled kernel, and (p, nu0) / (1-p, nu0) right before (p, mu),
-    whose outputs are the first ring links -- and the result must equal the oracle's run of the same sequence."""
+    whose outputs are the first ring links, and the first sub-step right after qcd_set_links (every array just written) --
+    and the result must equal the oracle's run of the same sequence."""
     Nc, prec, flags = variant
     dims, beta = (16, 8, 8, 4), 5.7                       # the CTA boxes of the tiled kernel divide this lattice
     links = prep_links(dims, Nc, prec, seed=21, spread=0.35)
     order = [(1, 2), (0, 2), (0, 0), (1, 1), (0, 1), (1, 0), (0, 1), (0, 0), (1, 3), (0, 3), (1, 0), (0, 1), (0, 1), (1, 1)]
     O = oracle_lattice(dims, Nc, prec, links)
+    kmed = []
     for parity, mu in order:
-        O.substep(beta, oracle.KIND_OR, 0, parity, mu)
+        _, kmin = O.substep_diag(beta, oracle.KIND_OR, 0, parity, mu)
+        kmed.append(float(np.median(kmin[np.isfinite(kmin)])))
+        assert kmin.min() > K_COND
     ref = O.get_links()
+    bar = unresynced_bar(prec, len(order), float(np.median(kmed)))     # dependency chains are at most len(order) hits deep
     with gpu_lattice(qcd, dims, Nc, prec, flags) as G:
         for rep in range(3):                              # timing-dependent hazards would not show every time
             G.qcd_set_links(links)
@@ -299,8 +367,7 @@ def test_substeps_back_to_back_in_any_order(qcd, variant):
                 G.qcd_debug_substep(beta, qcd.QCD_KIND_OR, 0, parity, mu)
             got = G.qcd_get_links().astype(np.complex128)
             diff = float(np.max(np.abs(got - ref)))
-            # 14 un-resynced deterministic sub-steps on a thermal configuration (k ~ 4): rounding grows mildly
-            assert diff < (1e-11 if prec == 1 else 2e-4), (rep, diff)
+            assert diff < bar, (rep, diff, bar)
 
 
 @pytest.mark.parametrize("dims,Nc,fld", [((8, 8, 8, 4), 3, None), ((8, 8, 8, 4), 3, (0, 1)), ((16, 16), 2, None), ((6, 4, 10), 3, (0, 2))])
@@ -570,6 +637,79 @@ def test_config3_sampled_links_at_full_size(qcd, prec, flags):
                                 [(0, 0, 0), (0, 1, 3), (1, 1, 1), (1, 0, 2)])
 
 
+@pytest.mark.parametrize("prec,flags", [(0, 1), (1, 0)], ids=["f32x12", "f64x18"])
+def test_config3_thermalised_state_at_full_size(qcd, prec, flags):
+    """BASELINE.json configs[2] on the state bench.py TIMES: SU(3) 32^4, beta 6.0, hot seed 42, then 10 thermalising sweeps
+    of 1 HB + 4 OR (the GPU produces that configuration; both sides start from the same downloaded copy).
+    sec 3.1 (the CPU regenerates configurations from the same random numbers) is the protocol.
+      (i)  heatbath and overrelaxation sub-steps in the bench launch configuration, 1000 sampled links each against the
+           oracle's update_one_link at the PLAIN north_star bars (2e-5 / 1e-12): no link of the sample is under the
+           conditioning rule (asserted), all other links bit-unchanged;
+      (ii) one whole un-resynced sweep (40 sub-steps, all 4.2 M links compared): accept/reject disagreements <= 1e-6 of the
+           heatbath link-hits, every link outside the dependency cone of a disagreement within the derived un-resynced bar;
+           qcd_sweep reproduces that sequence bit for bit."""
+    dims, Nc, beta, seed, therm = (32, 32, 32, 32), 3, 6.0, 42, 10
+    D, V = 4, 32 ** 4
+    par = npl.site_parity(dims)
+    coords = np.stack(np.unravel_index(np.arange(V), dims[::-1]), axis=-1)[:, ::-1]
+    on_edge = np.any((coords == 0) | (coords == np.array(dims) - 1), axis=1)
+    rng = np.random.Generator(np.random.PCG64(11))
+    with gpu_lattice(qcd, dims, Nc, prec, flags) as G:
+        G.qcd_init(qcd.QCD_HOT, seed)
+        for _ in range(therm):
+            G.qcd_sweep(beta, 1, 4)
+        assert G.qcd_get_sweep_counter() == therm
+        p_therm = G.qcd_measure()[0]
+        assert 0.58 < p_therm < 0.61                               # thermalised at beta = 6 (sanity, not a pin)
+        start = G.qcd_get_links().astype(np.complex128)
+        O = oracle_lattice(dims, Nc, prec, start)
+        O.set_seed(seed)
+        O.sweep_counter = therm
+        G.qcd_set_option(qcd.QCD_OPT_DEBUG_TRIALS, 1)
+        # (i) sampled links per sub-step at the plain bars
+        bad = 0
+        for kind, parity, mu in [(0, 0, 0), (0, 1, 3), (1, 1, 1), (1, 0, 2), (0, 1, 2), (1, 0, 0)]:
+            G.qcd_set_links(start)
+            G.qcd_debug_substep(beta, kind, 0, parity, mu)
+            got = G.qcd_get_links()
+            tr = G.qcd_debug_get_trials() if kind == 0 else None
+            cand = np.flatnonzero(par == parity)
+            edge = cand[on_edge[cand]]
+            sample = np.concatenate([rng.choice(edge, 300, replace=False), rng.choice(cand, 700, replace=False)])
+            worst, kworst = 0.0, np.inf
+            for lex in sample:
+                ref, codes = O.update_one_link(beta, kind, 0, int(lex), mu)
+                kworst = min(kworst, O.last_kmin)
+                if kind == 0 and not np.array_equal(codes, tr[lex]):
+                    bad += 1
+                    continue
+                worst = max(worst, float(np.max(np.abs(got[lex, mu].astype(np.complex128) - ref))))
+            print("thermal 32^4 %s p=%d mu=%d: worst |diff| %.3e (bar %.0e), smallest k %.2f" % ("HB" if kind == 0 else "OR", parity, mu, worst, TOL[prec], kworst))
+            assert kworst > K_COND                                  # illcond == 0: the plain bar is the bar
+            assert worst < TOL[prec], (kind, parity, mu, worst)
+            other = np.ones((V, D), dtype=bool)
+            other[par == parity, mu] = False
+            cmp_a = got if flags == 0 else got[..., :2, :]
+            cmp_b = start if flags == 0 else start[..., :2, :]
+            assert np.array_equal(cmp_a[other], cmp_b[other].astype(cmp_a.dtype))
+            del got
+        assert bad == 0, bad
+        # (ii) the whole working sweep without resync
+        G.qcd_set_links(start)
+        flips, fenced, worst, kmed, kmin, got = _unresynced_sequence(qcd, G, O, dims, Nc, prec, flags, beta, _sweep_sequence(D, 1, 4))
+        bar = unresynced_bar(prec, 5, kmed)
+        print("thermal 32^4 un-resynced sweep: flips %d, fenced %d of %d links, worst %.3e (bar %.3e), k median %.2f min %.3f"
+              % (flips, fenced, V * D, worst, bar, kmed, kmin))
+        assert flips <= max(1, int(1e-6 * V * D)), flips           # north_star: at most 1e-6 of links
+        assert fenced <= 120000 * max(flips, 0)                    # a disagreement reaches < (2*4+1)^4 * 4 * ... links in 4 passes
+        assert worst < bar * (1.0 if kmin > K_COND else K_COND / max(kmin, 2.5e-3)), (worst, bar, kmin)
+        G.qcd_set_links(start)
+        G.qcd_set_sweep_counter(therm)
+        G.qcd_sweep(beta, 1, 4)
+        again = G.qcd_get_links().astype(np.complex128)
+        assert np.array_equal(again, got)
+
+
 def test_config4_su2_background_field_at_full_size(qcd):
     # BASELINE.json configs[3]: SU(2) 48^3 x 8, beta 2.5, fp32, constant abelian field along sigma_3 on the x-y plane,
     # every x-y plaquette times exp(i phi sigma_3 / 2), phi = 2 pi n_f / (Lx Ly), n_f = 4; hot seed 99
@@ -653,6 +793,76 @@ def test_config5_su3_64to4_fp64_properties_at_full_size(qcd):
         assert abs(p2 - p1) < 1e-12, (p1, p2)
 
 
+def _mem_available_gb():
+    try:
+        for line in open("/proc/meminfo"):
+            if line.startswith("MemAvailable:"):
+                return int(line.split()[1]) / 2 ** 20
+    except OSError:
+        pass
+    return 0.0
+
+
+def test_config5_su3_64to4_fp64_heatbath_sampled_vs_oracle(qcd):
+    """BASELINE.json configs[4], fp64 arm, the HEATBATH at full size: the 9.66 GB configuration is handed to the oracle (one
+    host copy inside it), the GPU runs whole heatbath sub-steps at 64^4 (Philox counter c0 = lex up to 1.7e7, 64^4 strides,
+    fp64 x18 trial loop), and sampled links -- wrap-around boundary sites, the top of the lex range, random sites -- are
+    recomputed one by one by the oracle's update_one_link: trial codes equal, links within 1e-12."""
+    import torch
+    if _mem_available_gb() < 48.0:
+        pytest.skip("host MemAvailable %.0f GB < 48 GB: the oracle needs 2 x 9.66 GB for the 64^4 configuration" % _mem_available_gb())
+    dims, Nc, seed, beta = (64, 64, 64, 64), 3, 2024, 6.2
+    V, dev = 64 ** 4, torch.device("cuda:0")
+    rng = np.random.Generator(np.random.PCG64(3))
+    with gpu_lattice(qcd, dims, Nc, 1, 0) as G:
+        G.qcd_init(qcd.QCD_HOT, seed)
+        G.qcd_sweep(beta, 1, 1)                                    # off the hot start: staple norms k ~ 3
+        start_dev = torch.empty((V, 4, 3, 3), dtype=torch.complex128, device=dev)
+        G.qcd_get_links_ptr(start_dev.data_ptr(), start_dev.numel() * 16, 1)
+        start = G.qcd_get_links()
+        O = oracle.OracleLattice(dims, Nc)
+        O.set_links(start)
+        del start
+        O.set_seed(seed)
+        O.sweep_counter = G.qcd_get_sweep_counter()
+        G.qcd_set_option(qcd.QCD_OPT_DEBUG_TRIALS, 1)
+        res = torch.empty_like(start_dev)
+        bad, total = 0, 0
+        for parity, mu in [(0, 0), (1, 3), (1, 1)]:
+            G.qcd_set_links_ptr(start_dev.data_ptr(), start_dev.numel() * 16, 1)
+            G.qcd_debug_substep(beta, qcd.QCD_KIND_HB, 0, parity, mu)
+            G.qcd_get_links_ptr(res.data_ptr(), res.numel() * 16, 1)
+            tr = G.qcd_debug_get_trials()
+            # candidate sites: random, forced onto a wrap-around boundary, and from the top 1 % of the lex range
+            c = rng.integers(0, 64, size=(1500, 4))
+            for i in range(500, 1000):
+                c[i, i % 4] = 0 if (i // 4) % 2 else 63
+            c[1000:, 3] = 63
+            c[1000:, 2] = rng.integers(60, 64, size=500)
+            c = c[(c.sum(axis=1) & 1) == parity][:600]
+            lexs = c[:, 0] + 64 * (c[:, 1] + 64 * (c[:, 2] + 64 * c[:, 3]))
+            got = res[torch.from_numpy(lexs).to(dev), mu].cpu().numpy()
+            worst = 0.0
+            for i, lex in enumerate(lexs):
+                ref, codes = O.update_one_link(beta, oracle.KIND_HB, 0, int(lex), mu)
+                assert O.last_kmin > K_COND
+                if not np.array_equal(codes, tr[lex]):
+                    bad += 1
+                    continue
+                worst = max(worst, float(np.max(np.abs(got[i] - ref))))
+            total += len(lexs)
+            print("64^4 fp64 HB p=%d mu=%d: %d sampled links (max lex %d), worst |diff| %.3e" % (parity, mu, len(lexs), int(lexs.max()), worst))
+            assert worst < TOL[1], (parity, mu, worst)
+            assert len(lexs) >= 400 and lexs.max() > 0.98 * V
+            # sites of the other parity did not move (trial code 0 and bit-unchanged), sampled
+            other = rng.integers(0, V, size=2000)
+            oc = np.stack([other % 64, other // 64 % 64, other // 4096 % 64, other // 262144], axis=1)
+            other = other[(oc.sum(axis=1) & 1) != parity]
+            idx = torch.from_numpy(other).to(dev)
+            assert torch.equal(res[idx], start_dev[idx]) and not tr[other].any()
+        assert bad == 0, (bad, total)
+
+
 def test_largest_indexable_lattice_128to4_fp32(qcd):
     """Edge of the 32-bit vector indexing: SU(3) 128^4 with 12-real fp32 links (51.5 GB, 3.2e9 vectors).  Too large for any
     host-side comparison; checked by what holds at any size: the cold start measures plaquette = Polyakov loop = 1 exactly,
@@ -672,6 +882,31 @@ def test_largest_indexable_lattice_128to4_fp32(qcd):
         G.qcd_sweep(6.0, 0, 2)
         p2, planes2, _ = G.qcd_measure()
         assert abs(p2 - p1) < 3e-6, (p1, p2)
+
+
+def test_largest_lattice_of_one_b200_128to4_fp64(qcd):
+    """SU(3) 128^4 in fp64 x18: 154.6 GB of links, the largest lattice one B200 holds (no slab streaming
+    needed below this size).  Each (parity, direction) array has 1.2e9 vectors (32-bit in-array offsets), the array bases are
+    64-bit.  Checked by what holds at any size, like the fp32 case above; skipped when the device has less free memory."""
+    import torch
+    free, _ = torch.cuda.mem_get_info()
+    need = 4 * 128 ** 4 * 144
+    if free < need + (4 << 30):
+        pytest.skip("device has %.1f GB free, the lattice needs %.1f GB" % (free / 1e9, need / 1e9))
+    with gpu_lattice(qcd, (128, 128, 128, 128), 3, 1, 0) as G:
+        G.qcd_init(qcd.QCD_COLD, 1)
+        tot, planes, poly = G.qcd_measure()
+        assert tot == 1.0 and np.all(planes == 1.0) and poly == 1.0
+        G.qcd_init(qcd.QCD_HOT, 1)
+        tot, planes, poly = G.qcd_measure()
+        assert abs(tot) < 1e-4 and np.max(np.abs(planes)) < 1e-4 and abs(poly) < 1.5e-3
+        G.qcd_sweep(6.0, 1, 0)
+        G.qcd_sweep(6.0, 1, 0)
+        p1, planes, _ = G.qcd_measure()
+        assert 0.3 < p1 < 0.62 and np.max(np.abs(planes - p1)) < 2e-2
+        G.qcd_sweep(6.0, 0, 2)
+        p2, _, _ = G.qcd_measure()
+        assert abs(p2 - p1) < 1e-12, (p1, p2)
 
 
 # ----------------------------------------------------------------------------- ABI error paths on a live device

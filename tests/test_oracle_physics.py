@@ -224,6 +224,71 @@ def test_kennedy_pendleton_trial_cap_and_acceptance():
     assert np.mean(codes >= 0x80) < 5e-3 and codes[codes < 0x80].max() <= 10
 
 
+@pytest.mark.parametrize("mode", [0, 1], ids=["u32", "u23"])
+def test_heatbath_direction_is_isotropic(mode):
+    """row "KP sampler", direction part: <g_vec> = 0, isotropy (the draw is SURVEY 8(c)-2.6
+    `ct = 1 - 2 u1, phi = 2 pi u2, g = (g0, r st cos phi, r st sin phi, r ct)`).
+
+    The draw is exercised through the oracle's own update path, not a re-typed formula: on a COLD SU(2) lattice the staple
+    sum of every link is A = 2(D-1) * 1, so W = U A = 6 * 1 (D = 4), v = (6,0,0,0), v~ = 1 and the new link a = g * v~^+ IS
+    the drawn quaternion g = (g0, sqrt(1-g0^2) n), n the unit direction.  What is pinned: n uniform on S^2 -- first moments 0,
+    second moments delta_ij / 3, cos(theta) = n3 uniform on [-1,1] (chi-square), azimuth atan2(n2, n1) uniform on (-pi, pi]
+    (chi-square) and independent of cos(theta); and g0 keeps the Kennedy-Pendleton mean I2/I1 at alpha = beta k = 6 beta."""
+    dims, beta = (16, 16, 16, 8), 0.5                      # alpha = 3: r = sqrt(1-g0^2) is of order 1, no direction is lost
+    samples = []
+    for mu in range(4):
+        for parity in (0, 1):
+            L = make(dims, 2)
+            L.init(oracle.COLD, 77 + mu)
+            if mode == 1:
+                L.set_fp32_shadow(True)
+            L.set_max_trials(100)
+            L.sweep_counter = 3 * mu + parity
+            L.substep(beta, oracle.KIND_HB, 0, parity, mu)
+            u = L.get_links()[:, mu]                       # (V, 2, 2); only sites of this parity moved off the identity
+            g = np.stack([u[:, 0, 0].real, u[:, 0, 1].imag, u[:, 0, 1].real, u[:, 0, 0].imag], axis=1)   # (a0, a1, a2, a3)
+            moved = np.abs(g[:, 0] - 1.0) + np.abs(g[:, 1:]).sum(axis=1) > 0
+            assert moved.sum() == L.V // 2
+            samples.append(g[moved])
+    g = np.concatenate(samples)
+    n_s = len(g)
+    assert n_s >= 100000
+    tol32 = 1e-6 if mode == 1 else 1e-12                   # fp32 shadow rounds the stored link
+    assert np.max(np.abs((g ** 2).sum(axis=1) - 1.0)) < tol32
+    r = np.sqrt((g[:, 1:] ** 2).sum(axis=1))
+    n = g[:, 1:] / r[:, None]
+    # first and second moments of a uniform direction: <n_i> = 0 (sigma = 1/sqrt(3 N)), <n_i n_j> = delta_ij / 3
+    assert np.max(np.abs(n.mean(axis=0))) < 4.5 / np.sqrt(3 * n_s), n.mean(axis=0)
+    second = n.T @ n / n_s
+    # var(n_i^2) = 1/5 - 1/9 = 4/45, var(n_i n_j) = 1/15
+    assert np.max(np.abs(np.diag(second) - 1.0 / 3)) < 4.5 * np.sqrt(4.0 / 45 / n_s), second
+    assert np.max(np.abs(second - np.diag(np.diag(second)))) < 4.5 * np.sqrt(1.0 / 15 / n_s), second
+
+    def chi2_uniform(x, lo, hi, bins=64):
+        obs = np.histogram(x, bins=np.linspace(lo, hi, bins + 1))[0].astype(float)
+        exp = len(x) / bins
+        return np.sum((obs - exp) ** 2 / exp), bins - 1
+
+    for name, x, lo, hi in [("cos(theta)", n[:, 2], -1.0, 1.0), ("azimuth", np.arctan2(n[:, 1], n[:, 0]), -np.pi, np.pi)]:
+        chi2, dof = chi2_uniform(x, lo, hi)
+        assert chi2 < dof + 5 * np.sqrt(2 * dof), (name, chi2, dof)
+    # azimuth independent of the polar angle: 8 x 8 contingency table
+    a = np.digitize(np.arctan2(n[:, 1], n[:, 0]), np.linspace(-np.pi, np.pi, 9)[1:-1])
+    b = np.digitize(n[:, 2], np.linspace(-1, 1, 9)[1:-1])
+    table = np.zeros((8, 8))
+    np.add.at(table, (a, b), 1.0)
+    chi2 = np.sum((table - n_s / 64.0) ** 2 / (n_s / 64.0))
+    assert chi2 < 63 + 5 * np.sqrt(2 * 63), chi2
+    # the direction is independent of g0 and g0 keeps its law: <g0> = I2(alpha)/I1(alpha), alpha = beta * 6
+    alpha = 6.0 * beta
+    dens = lambda x: np.sqrt(1 - x * x) * np.exp(alpha * (x - 1))
+    norm = integrate.quad(dens, -1, 1)[0]
+    mean = special.iv(2, alpha) / special.iv(1, alpha)
+    var = integrate.quad(lambda x: x * x * dens(x), -1, 1)[0] / norm - mean ** 2
+    assert abs(g[:, 0].mean() - mean) < 4.5 * np.sqrt(var / n_s)
+    assert np.max(np.abs((n * (g[:, :1] - mean)).mean(axis=0))) < 4.5 * np.sqrt(var / 3 / n_s)
+
+
 # ----------------------------------------------------------------------------- hot start
 @pytest.mark.parametrize("N", [2, 3])
 def test_hot_start_haar_moments(N):
