@@ -6,9 +6,9 @@
         bench.py --gpus N --steps K --warmup W
 
 Workload (BASELINE.json configs[2], the configuration the metric is quoted on): SU(3), D = 4, 32^4 periodic, beta = 6.0,
-hot start seed 42.  One STEP = one pass of the whole hot path = qcd_sweep(beta, 1 heatbath, 4 overrelaxation)
-+ qcd_measure(plaquette per plane, Polyakov loop)  (the paper's "working sweep",
-PAPER.md:134).  metric = composite link updates/s = D*V*steps / time (reading R13).
+hot start seed 42.  One STEP = one pass of the whole hot path = qcd_sweep_measure(beta, 1 heatbath, 4 overrelaxation):
+the sweep and the plaquette per plane + Polyakov loop of the new configuration, the plaquette folded into the last pass
+(the paper's "working sweep").  metric = composite link updates/s = D*V*steps / time (reading R13).
 
 The line's `value` is the --precision arm (default fp32, 12-real compressed links); the other arm (fp64, 18 reals) is
 measured in the same run and reported under "other_precision".  N > 1: independent replicas, one lattice per GPU, no
@@ -173,6 +173,10 @@ def time_arm(q, torch, prec_name, steps, warmup, therm, seed, dist, sampler):
         state = {}
 
         def working_sweep():
+            # update + observables of the new configuration; the plaquette is folded into the last pass (qcd_sweep_measure)
+            state["obs"] = G.qcd_sweep_measure(BETA, N_HB, N_OR)
+
+        def separate_calls():
             G.qcd_sweep(BETA, N_HB, N_OR)
             state["obs"] = G.qcd_measure()
 
@@ -195,10 +199,11 @@ def time_arm(q, torch, prec_name, steps, warmup, therm, seed, dist, sampler):
         G.qcd_accum_reset()
 
         def accumulate_sweep():
-            G.qcd_sweep(BETA, N_HB, N_OR)
-            G.qcd_measure_accumulate()
+            G.qcd_sweep_measure_accumulate(BETA, N_HB, N_OR)
 
         out["accum"] = timed_reps(torch, dist, sampler, accumulate_sweep, steps, min_total_ms=500.0)
+        # (3b) the working sweep as two calls, with the stand-alone plaquette kernel (what the fusion saves)
+        out["separate"] = timed_reps(torch, dist, sampler, separate_calls, steps, min_total_ms=0.0)
         n_acc, s1, _ = G.qcd_accum_get()
         out["acc_plaquette_mean"] = float(s1[:6].mean() / max(n_acc, 1))
         # (4) end to end through the C ABI with HOST buffers: every step uploads the configuration from pinned host
@@ -209,8 +214,7 @@ def time_arm(q, torch, prec_name, steps, warmup, therm, seed, dist, sampler):
 
         def e2e_step():
             G.qcd_set_links_ptr(host.data_ptr(), nbytes, 0)
-            G.qcd_sweep(BETA, N_HB, N_OR)
-            state["obs"] = G.qcd_measure()
+            state["obs"] = G.qcd_sweep_measure(BETA, N_HB, N_OR)
             G.qcd_get_links_ptr(host.data_ptr(), nbytes, 0)
 
         for _ in range(2):
@@ -301,7 +305,7 @@ def run_ours(args):
         for name in (primary, other):
             value, ms_step, roof, work, upd = summarise(arms[name], name, args.steps, world, hbm_peak, fma[name])
             a = arms[name]
-            e2e, acc = rep_stats(a["e2e"], args.steps), rep_stats(a["accum"], args.steps)
+            e2e, acc, sep = rep_stats(a["e2e"], args.steps), rep_stats(a["accum"], args.steps), rep_stats(a["separate"], args.steps)
             frag[name] = {"value": value, "ms_per_step": ms_step, "reps": work, "roofline": roof,
                           "update_only_sweep": {"ms_per_step": upd["median_ms_per_step"], "reps": upd,
                                                 "value": aggregate_value(world, a["links"], 1, upd["median_ms_per_step"])},
@@ -311,6 +315,7 @@ def run_ours(args):
                           "accumulate_on_device": {"ms_per_step": acc["median_ms_per_step"], "reps": acc,
                                                    "value": aggregate_value(world, a["links"], 1, acc["median_ms_per_step"]),
                                                    "plaquette_mean": a["acc_plaquette_mean"]},
+                          "qcd_sweep_then_qcd_measure": {"ms_per_step": sep["median_ms_per_step"], "reps": sep},
                           "gpu_launches": a["launches_per_rep"], "plaquette": a["plaquette"], "polyakov_abs": a["polyakov_abs"],
                           "dtype": name, "storage": "12 reals/link" if name == "f32" else "18 reals/link"}
         p = frag[primary]
@@ -326,6 +331,7 @@ def run_ours(args):
                                      % (MIN_REPS, args.steps, MIN_DEVICE_MS)},
                 "reps": p["reps"], "e2e": p["e2e"], "gpu_launches": p["gpu_launches"], "roofline": p["roofline"], "clocks": clocks,
                 "update_only_sweep": p["update_only_sweep"], "accumulate_on_device": p["accumulate_on_device"],
+                "qcd_sweep_then_qcd_measure": p["qcd_sweep_then_qcd_measure"],
                 "observables": {"plaquette": p["plaquette"], "polyakov_abs": p["polyakov_abs"]},
                 "other_precision": frag[other]}
         if world == 1 and not args.no_cpu_baseline:

@@ -88,6 +88,19 @@ int qcd_sweep(qcd_lattice_t* lat, double beta, int n_hb, int n_or, const qcd_fie
  * Site arithmetic in the lattice's precision, accumulation in fp64, deterministic.  Synchronises the stream. */
 int qcd_measure(qcd_lattice_t* lat, const qcd_field_t* field, double* plaq_total, double* plaq_planes, double* polyakov_re_im);
 
+/* Working sweep ("working sweeps" = update + measurements): qcd_sweep followed by the
+ * observables of the NEW configuration, with the plaquette measurement folded into the last pass of the sweep: there the
+ * sub-steps (parity 1, mu >= 1) already hold every plaquette of the planes (nu, mu), nu < mu, in its final state as
+ * Re Tr[U'_mu(x) A_nu(x)], so no separate pass over the links is made for it (the Polyakov loop keeps its own small
+ * kernel).  Results equal qcd_sweep + qcd_measure up to rounding (another summation order for the observables; the
+ * measuring kernels are separate instantiations of the update kernels, so the links agree to a few units in the last
+ * place); each call is deterministic on its own.  Arguments and errors as for those two calls; synchronises the stream.
+ * n_hb + n_or = 0 measures the unchanged configuration. */
+int qcd_sweep_measure(qcd_lattice_t* lat, double beta, int n_hb, int n_or, const qcd_field_t* field, double* plaq_total,
+                      double* plaq_planes, double* polyakov_re_im);
+/* The same with the observables added to the on-device accumulators (see below) instead of returned: asynchronous. */
+int qcd_sweep_measure_accumulate(qcd_lattice_t* lat, double beta, int n_hb, int n_or, const qcd_field_t* field);
+
 /* On-device accumulation over configurations (the paper keeps its measurements on the device until
  * the end of a run).  qcd_measure_accumulate measures like qcd_measure and adds the NQ = D(D-1)/2 + 3
  * quantities (plane plaquettes in qcd_measure's order, Re L, Im L, |L|) and their squares to accumulators in device

@@ -23,7 +23,7 @@ SYMBOLS = [
     "qcd_lattice_bytes", "qcd_lattice_create", "qcd_lattice_destroy", "qcd_init", "qcd_sweep", "qcd_measure",
     "qcd_get_links", "qcd_set_links", "qcd_get_sweep_counter", "qcd_set_sweep_counter", "qcd_get_seed", "qcd_set_seed",
     "qcd_set_option", "qcd_debug_substep", "qcd_debug_get_trials", "qcd_debug_philox", "qcd_get_profile",
-    "qcd_reset_profile", "qcd_get_launch_count", "qcd_measure_accumulate", "qcd_accum_get", "qcd_accum_reset", "qcd_probe_fma_tflops", "qcd_probe_copy_gbs", "qcd_last_error",
+    "qcd_reset_profile", "qcd_get_launch_count", "qcd_measure_accumulate", "qcd_sweep_measure", "qcd_sweep_measure_accumulate", "qcd_accum_get", "qcd_accum_reset", "qcd_probe_fma_tflops", "qcd_probe_copy_gbs", "qcd_last_error",
     "qcd_version",
 ]
 
@@ -61,6 +61,8 @@ def lib():
     L.qcd_sweep.argtypes = [p, d, i, i, fp]
     L.qcd_measure.argtypes = [p, fp, dp, dp, dp]
     L.qcd_measure_accumulate.argtypes = [p, fp]
+    L.qcd_sweep_measure.argtypes = [p, d, i, i, fp, dp, dp, dp]
+    L.qcd_sweep_measure_accumulate.argtypes = [p, d, i, i, fp]
     L.qcd_accum_get.argtypes = [p, C.POINTER(C.c_uint64), dp, dp, i]
     L.qcd_accum_reset.argtypes = [p]
     L.qcd_get_links.argtypes = [p, p, sz, i]
@@ -188,6 +190,18 @@ class Lattice:
         _check(lib().qcd_measure(self._h, _fref(field), C.byref(tot) if plaquette else None, planes if plaquette else None,
                                  poly if polyakov else None))
         return tot.value, np.array(planes[:]), complex(poly[0], poly[1])
+
+    def qcd_sweep_measure(self, beta, n_hb, n_or, field=None):
+        """one working sweep: qcd_sweep + the observables of the new configuration (plaquette fused into the last pass)"""
+        npl = self.D * (self.D - 1) // 2
+        tot = C.c_double(0.0)
+        planes = (C.c_double * npl)()
+        poly = (C.c_double * 2)()
+        _check(lib().qcd_sweep_measure(self._h, float(beta), int(n_hb), int(n_or), _fref(field), C.byref(tot), planes, poly))
+        return tot.value, np.array(planes[:]), complex(poly[0], poly[1])
+
+    def qcd_sweep_measure_accumulate(self, beta, n_hb, n_or, field=None):
+        _check(lib().qcd_sweep_measure_accumulate(self._h, float(beta), int(n_hb), int(n_or), _fref(field)))
 
     def qcd_measure_accumulate(self, field=None):
         _check(lib().qcd_measure_accumulate(self._h, _fref(field)))

@@ -44,6 +44,8 @@ struct qcd_lattice {
   int max_trials;
   bool debug_trials, profile;
   uint8_t* d_trials;
+  // per-block / per-warp partial sums of the reductions, one allocation of three regions (sizes fixed by the geometry):
+  // [fused plaquette: NPL x np_warp][plaquette kernel: NPL x nb_plaq][Polyakov: 2 x nb_poly]
   double* d_partials;
   size_t partials_cap;   // doubles
   double* d_results;     // 48 doubles: last measurement + accumulator (see qcd_lattice_create)
@@ -133,6 +135,7 @@ FieldArgs make_field_args(const qcd_field_t* f, bool on, int Nc) {
 
 cudaError_t launch_update(qcd_lattice* L, int kind, bool field, const UpdateArgs& a0) {
   UpdateSel s; s.Nc = L->Nc; s.D = L->D; s.precision = L->precision; s.comp = L->comp; s.kind = kind; s.field = field;
+  s.meas = a0.meas != nullptr;
   UpdateArgs a = a0;
   a.prev_parity = L->last_parity; a.prev_mu = L->last_mu;
   const cudaError_t e = (L->Nc == 2)                ? launch_update_su2(s, L->g, L->mem, a, L->stream)
@@ -158,10 +161,48 @@ int prof_end(qcd_lattice* L, EventPair* ep, int n) {
 }
 
 // bracket: time this single launch with its own event pair (qcd_debug_substep); qcd_sweep brackets whole passes instead
+// sizes of the three regions of d_partials
+struct MeasLayout {
+  uint32_t npl, np_warp, nb_plaq, nb_poly;
+  bool boxed;
+  size_t off_plaq, off_poly, need;
+};
+MeasLayout meas_layout(const qcd_lattice* L) {
+  MeasLayout m;
+  const Geom& g = L->g;
+  m.npl = (uint32_t)(L->D * (L->D - 1) / 2);
+  // fused measurement: one partial per warp of an update launch; every launch shape has <= Vh_pad/32 + 8 warps (CTAs of
+  // <= 256 threads); entries beyond a launch's warps are never written and stay zero from the allocation
+  m.np_warp = g.Vh_pad / 32u + 8u;
+  m.boxed = (L->D == 4 && g.Lh0 % 8 == 0 && g.L[1] % 2 == 0 && g.L[2] % 2 == 0 && g.L[3] % 2 == 0);
+  m.nb_plaq = m.boxed ? g.V / 128u : ((g.Vh + 127u) / 128u) * 2u;
+  m.nb_poly = (g.V / (uint32_t)g.L[L->D - 1] + 127u) / 128u;
+  m.off_plaq = (size_t)m.npl * m.np_warp;
+  m.off_poly = m.off_plaq + (size_t)m.npl * m.nb_plaq;
+  m.need = m.off_poly + 2 * (size_t)m.nb_poly;
+  return m;
+}
+int ensure_partials(qcd_lattice* L) {
+  const MeasLayout m = meas_layout(L);
+  if (L->d_partials && L->partials_cap >= m.need) return QCD_OK;
+  if (L->d_partials) CUDA_TRY(cudaFree(L->d_partials));
+  L->d_partials = nullptr; L->partials_cap = 0;
+  CUDA_TRY(cudaMalloc(&L->d_partials, m.need * sizeof(double)));
+  CUDA_TRY(cudaMemsetAsync(L->d_partials, 0, m.need * sizeof(double), L->stream));
+  L->partials_cap = m.need;
+  return QCD_OK;
+}
+int plane_index(int D, int nu, int mu) { return nu * D - nu * (nu + 1) / 2 + (mu - nu - 1); }   // nu < mu; order (0,1),(0,2),..
+
+// meas: the fused-measurement form of the sub-step (partials of the planes (nu, mu), nu < mu, into d_partials)
 int substep(qcd_lattice* L, double beta, int kind, int hit, int parity, int mu, const qcd_field_t* f, bool field_on, uint8_t* trials,
-            bool bracket) {
+            bool bracket, bool meas = false) {
   UpdateArgs a;
   memset(&a, 0, sizeof(a));
+  if (meas) {
+    a.meas = L->d_partials; a.meas_stride = meas_layout(L).np_warp;
+    for (int nu = 0; nu < mu && nu < 3; ++nu) a.meas_plane[nu] = plane_index(L->D, nu, mu);
+  }
   a.beta = beta; a.inv_c = (double)L->Nc / (2.0 * beta); a.parity = parity; a.mu = mu; a.hit = hit; a.max_trials = L->max_trials;
   a.sweep = L->sweep; a.key0 = (uint32_t)(L->seed & 0xFFFFFFFFull); a.key1 = (uint32_t)(L->seed >> 32);
   a.trials = trials;
@@ -235,31 +276,30 @@ struct LayoutOp {
 };
 
 struct MeasureOp {
-  qcd_lattice* L; MeasureField mf; bool want_plaq, want_poly;
+  // fused: the plaquette partials are already in the fused region of d_partials (written by the MEAS update kernels of the
+  // sweep just enqueued); only their second-stage reduction is launched here
+  qcd_lattice* L; MeasureField mf; bool want_plaq, want_poly, fused;
   template <int NC, int D, typename R, bool COMP> int operator()() {
     typedef typename LinkIO<NC, R, COMP>::Vec Vec;
     constexpr int NPL = D * (D - 1) / 2;
+    int rc = ensure_partials(L);
+    if (rc != QCD_OK) return rc;
+    const MeasLayout m = meas_layout(L);
     // boxed thread mapping of the plaquette kernel (aux_kernels.cuh, MeasureField): one grid row of V / 128 CTAs
-    mf.boxed = (D == 4 && L->g.Lh0 % 8 == 0 && L->g.L[1] % 2 == 0) ? 1 : 0;
+    mf.boxed = m.boxed ? 1 : 0;
     if (mf.boxed) {
       mf.n0 = make_fastdiv((uint32_t)(L->g.Lh0 / 8)); mf.n1 = make_fastdiv((uint32_t)(L->g.L[1] / 2)); mf.n2 = make_fastdiv((uint32_t)(L->g.L[2] / 2));
     }
-    const uint32_t nb_plaq = mf.boxed ? L->g.V / 128u : ((L->g.Vh + 127) / 128) * 2;
     const uint32_t Vs = L->g.V / (uint32_t)L->g.L[D - 1];
-    const uint32_t nb_poly = (Vs + 127) / 128;
-    const size_t need = (size_t)NPL * nb_plaq + 2 * (size_t)nb_poly;
-    if (need > L->partials_cap) {
-      if (L->d_partials) CUDA_TRY(cudaFree(L->d_partials));
-      L->d_partials = nullptr; L->partials_cap = 0;
-      CUDA_TRY(cudaMalloc(&L->d_partials, need * sizeof(double)));
-      L->partials_cap = need;
-    }
-    double* pp = L->d_partials;
-    double* pq = L->d_partials + (size_t)NPL * nb_plaq;
-    auto plaq_grid = [&]() { return mf.boxed ? dim3(L->g.V / 128, 1) : dim3((L->g.Vh + 127) / 128, 2); };
-    if (want_plaq && want_poly) {
-      // fork: the Polyakov kernel (one thread per spatial site, bound by the latency of its L_t dependent loads) goes first
-      // on a side stream and runs beside the plaquette kernel; join before the D2H copy of the results
+    double* pf = L->d_partials;
+    double* pp = L->d_partials + m.off_plaq;
+    double* pq = L->d_partials + m.off_poly;
+    const dim3 plaq_grid = mf.boxed ? dim3(L->g.V / 128, 1) : dim3((L->g.Vh + 127) / 128, 2);
+    const double plaq_scale = 1.0 / ((double)L->g.V * NC), poly_scale = 1.0 / ((double)Vs * NC);
+    const bool fork = want_plaq && want_poly;
+    if (fork) {
+      // the Polyakov kernel (one thread per spatial site, bound by the latency of its L_t dependent loads) goes first on a
+      // side stream and runs beside the plaquette work; join before the results are read
       if (!L->side) {
         CUDA_TRY(cudaStreamCreateWithFlags(&L->side, cudaStreamNonBlocking));
         CUDA_TRY(cudaEventCreateWithFlags(&L->ev_fork, cudaEventDisableTiming));
@@ -267,29 +307,26 @@ struct MeasureOp {
       }
       CUDA_TRY(cudaEventRecord(L->ev_fork, L->stream));
       CUDA_TRY(cudaStreamWaitEvent(L->side, L->ev_fork, 0));
-      polyakov_kernel<NC, D, R, COMP><<<nb_poly, 128, 0, L->side>>>(L->g, (const Vec*)L->mem, pq);
-      final_reduce_kernel<<<2, 256, 0, L->side>>>(pq, nb_poly, L->d_results + 8, 1.0 / ((double)Vs * NC));
-      CUDA_TRY(cudaEventRecord(L->ev_join, L->side));
-      plaquette_kernel<NC, D, R, COMP><<<plaq_grid(), 128, 0, L->stream>>>(L->g, (const Vec*)L->mem, mf, pp);
-      final_reduce_kernel<<<NPL, 256, 0, L->stream>>>(pp, nb_plaq, L->d_results, 1.0 / ((double)L->g.V * NC));
-      CUDA_TRY(cudaStreamWaitEvent(L->stream, L->ev_join, 0));
-      L->launches += 4;
-      L->last_parity = L->last_mu = -1;
-      CUDA_TRY(cudaGetLastError());
-      return QCD_OK;
-    }
-    if (want_plaq) {
-      plaquette_kernel<NC, D, R, COMP><<<plaq_grid(), 128, 0, L->stream>>>(L->g, (const Vec*)L->mem, mf, pp);
-      final_reduce_kernel<<<NPL, 256, 0, L->stream>>>(pp, nb_plaq, L->d_results, 1.0 / ((double)L->g.V * NC));
-      L->launches += 2;
-      L->last_parity = L->last_mu = -1;
     }
     if (want_poly) {
-      polyakov_kernel<NC, D, R, COMP><<<nb_poly, 128, 0, L->stream>>>(L->g, (const Vec*)L->mem, pq);
-      final_reduce_kernel<<<2, 256, 0, L->stream>>>(pq, nb_poly, L->d_results + 8, 1.0 / ((double)Vs * NC));
+      cudaStream_t ps = fork ? L->side : L->stream;
+      polyakov_kernel<NC, D, R, COMP><<<m.nb_poly, 128, 0, ps>>>(L->g, (const Vec*)L->mem, pq);
+      final_reduce_kernel<<<2, 256, 0, ps>>>(pq, m.nb_poly, L->d_results + 8, poly_scale);
       L->launches += 2;
-      L->last_parity = L->last_mu = -1;
+      if (fork) CUDA_TRY(cudaEventRecord(L->ev_join, L->side));
     }
+    if (want_plaq) {
+      if (fused) {
+        final_reduce_kernel<<<NPL, 256, 0, L->stream>>>(pf, m.np_warp, L->d_results, plaq_scale);
+        L->launches += 1;
+      } else {
+        plaquette_kernel<NC, D, R, COMP><<<plaq_grid, 128, 0, L->stream>>>(L->g, (const Vec*)L->mem, mf, pp);
+        final_reduce_kernel<<<NPL, 256, 0, L->stream>>>(pp, m.nb_plaq, L->d_results, plaq_scale);
+        L->launches += 2;
+      }
+    }
+    if (fork) CUDA_TRY(cudaStreamWaitEvent(L->stream, L->ev_join, 0));
+    L->last_parity = L->last_mu = -1;
     CUDA_TRY(cudaGetLastError());
     return QCD_OK;
   }
@@ -419,7 +456,8 @@ int qcd_init(qcd_lattice_t* L, int start, uint64_t seed) {
   return rc;
 }
 
-int qcd_sweep(qcd_lattice_t* L, double beta, int n_hb, int n_or, const qcd_field_t* field) {
+// fused: the last pass's (parity 1, mu >= 1) sub-steps run in the fused-measurement form (update.cuh, meas_store)
+static int sweep_core(qcd_lattice_t* L, double beta, int n_hb, int n_or, const qcd_field_t* field, bool fused) {
   if (!L) return fail(QCD_ERR_INVALID_ARG, "lattice is NULL");
   if (!L->has_links) return fail(QCD_ERR_STATE, "qcd_sweep before qcd_init / qcd_set_links");
   if (!std::isfinite(beta) || beta < 0.0) return fail(QCD_ERR_INVALID_ARG, "beta must be finite and >= 0");
@@ -427,24 +465,33 @@ int qcd_sweep(qcd_lattice_t* L, double beta, int n_hb, int n_or, const qcd_field
   bool fon;
   int rc = check_field(L, field, &fon);
   if (rc != QCD_OK) return rc;
+  if (fused) { rc = ensure_partials(L); if (rc != QCD_OK) return rc; }
   // profiling brackets the run of heatbath launches and the run of overrelaxation launches with one event pair each
   // (3 events per sweep), so the timed stream is not perturbed between kernels
   EventPair ep;
-  for (int pass = 0; pass < n_hb + n_or; ++pass) {
+  bool ep_open = false;
+  const int n_pass = n_hb + n_or;
+  for (int pass = 0; pass < n_pass; ++pass) {
     const int kind = pass < n_hb ? QCD_KIND_HB : QCD_KIND_OR, hit = pass < n_hb ? pass : 0;
-    if (L->profile && (pass == 0 || pass == n_hb)) { rc = prof_begin(L, kind, &ep); if (rc != QCD_OK) return rc; }
+    if (L->profile && (pass == 0 || pass == n_hb)) { rc = prof_begin(L, kind, &ep); if (rc != QCD_OK) return rc; ep_open = true; }
     for (int p = 0; p < 2; ++p)
       for (int mu = 0; mu < L->D; ++mu) {
-        rc = substep(L, beta, kind, hit, p, mu, field, fon, nullptr, false);
-        if (rc != QCD_OK) return rc;
+        const bool meas = fused && pass == n_pass - 1 && p == 1 && mu >= 1;
+        rc = substep(L, beta, kind, hit, p, mu, field, fon, nullptr, false, meas);
+        if (rc != QCD_OK) { if (ep_open) L->ev_free.push_back(ep); return rc; }
       }
-    if (L->profile && (pass == n_hb - 1 || pass == n_hb + n_or - 1)) {
+    if (L->profile && (pass == n_hb - 1 || pass == n_pass - 1)) {
       rc = prof_end(L, &ep, 2 * L->D * (kind == QCD_KIND_HB ? n_hb : n_or));
+      ep_open = false;
       if (rc != QCD_OK) return rc;
     }
   }
   L->sweep += 1;
   return QCD_OK;
+}
+
+int qcd_sweep(qcd_lattice_t* L, double beta, int n_hb, int n_or, const qcd_field_t* field) {
+  return sweep_core(L, beta, n_hb, n_or, field, false);
 }
 
 int qcd_debug_substep(qcd_lattice_t* L, double beta, int kind, int hit, int parity, int mu, const qcd_field_t* field) {
@@ -475,14 +522,14 @@ int qcd_debug_get_trials(qcd_lattice_t* L, uint8_t* dst, size_t bytes) {
 }
 
 // enqueue the measurement kernels (results land in d_results); no synchronisation
-static int enqueue_measure(qcd_lattice_t* L, const qcd_field_t* field, bool want_plaq, bool want_poly) {
+static int enqueue_measure(qcd_lattice_t* L, const qcd_field_t* field, bool want_plaq, bool want_poly, bool fused = false) {
   if (!L) return fail(QCD_ERR_INVALID_ARG, "lattice is NULL");
   if (!L->has_links) return fail(QCD_ERR_STATE, "no links yet");
   bool fon;
   int rc = check_field(L, field, &fon);
   if (rc != QCD_OK) return rc;
   MeasureOp op;
-  op.L = L; op.want_plaq = want_plaq; op.want_poly = want_poly;
+  op.L = L; op.want_plaq = want_plaq; op.want_poly = want_poly; op.fused = fused;
   memset(&op.mf, 0, sizeof(op.mf));
   FieldArgs fa = make_field_args(field, fon, L->Nc);
   op.mf.enabled = fon ? 1 : 0; op.mf.mu = fa.mu; op.mf.nu = fa.nu;
@@ -527,20 +574,50 @@ int qcd_accum_get(qcd_lattice_t* L, uint64_t* count, double* sum, double* sumsq,
   return QCD_OK;
 }
 
-int qcd_measure(qcd_lattice_t* L, const qcd_field_t* field, double* plaq_total, double* plaq_planes, double* polyakov) {
-  struct { bool want_plaq, want_poly; } op = {plaq_total || plaq_planes, polyakov != nullptr};
-  int rc = enqueue_measure(L, field, op.want_plaq, op.want_poly);
-  if (rc != QCD_OK) return rc;
-  if (!op.want_plaq && !op.want_poly) return QCD_OK;
+// copy the last measurement to the host and hand it out (synchronises)
+static int fetch_results(qcd_lattice_t* L, bool want_plaq, double* plaq_total, double* plaq_planes, double* polyakov) {
   CUDA_TRY(cudaMemcpyAsync(L->h_results, L->d_results, 16 * sizeof(double), cudaMemcpyDeviceToHost, L->stream));
   CUDA_TRY(cudaStreamSynchronize(L->stream));
   const int npl = L->D * (L->D - 1) / 2;
-  if (op.want_plaq) {
+  if (want_plaq) {
     double tot = 0.0;
     for (int k = 0; k < npl; ++k) { tot += L->h_results[k]; if (plaq_planes) plaq_planes[k] = L->h_results[k]; }
     if (plaq_total) *plaq_total = tot / npl;
   }
   if (polyakov) { polyakov[0] = L->h_results[8]; polyakov[1] = L->h_results[9]; }
+  return QCD_OK;
+}
+
+int qcd_measure(qcd_lattice_t* L, const qcd_field_t* field, double* plaq_total, double* plaq_planes, double* polyakov) {
+  const bool want_plaq = plaq_total || plaq_planes, want_poly = polyakov != nullptr;
+  int rc = enqueue_measure(L, field, want_plaq, want_poly);
+  if (rc != QCD_OK) return rc;
+  if (!want_plaq && !want_poly) return QCD_OK;
+  return fetch_results(L, want_plaq, plaq_total, plaq_planes, polyakov);
+}
+
+// working sweep = update + measurement of the new configuration, the plaquette folded into the last pass
+int qcd_sweep_measure(qcd_lattice_t* L, double beta, int n_hb, int n_or, const qcd_field_t* field, double* plaq_total, double* plaq_planes,
+                      double* polyakov) {
+  const bool want_plaq = plaq_total || plaq_planes, want_poly = polyakov != nullptr;
+  const bool fused = want_plaq && n_hb + n_or > 0;
+  int rc = sweep_core(L, beta, n_hb, n_or, field, fused);
+  if (rc != QCD_OK) return rc;
+  rc = enqueue_measure(L, field, want_plaq, want_poly, fused);
+  if (rc != QCD_OK) return rc;
+  if (!want_plaq && !want_poly) return QCD_OK;
+  return fetch_results(L, want_plaq, plaq_total, plaq_planes, polyakov);
+}
+
+int qcd_sweep_measure_accumulate(qcd_lattice_t* L, double beta, int n_hb, int n_or, const qcd_field_t* field) {
+  const bool fused = n_hb + n_or > 0;
+  int rc = sweep_core(L, beta, n_hb, n_or, field, fused);
+  if (rc != QCD_OK) return rc;
+  rc = enqueue_measure(L, field, true, true, fused);
+  if (rc != QCD_OK) return rc;
+  accum_kernel<<<1, 32, 0, L->stream>>>(L->d_results, L->d_results + 16, L->D * (L->D - 1) / 2);
+  CUDA_TRY(cudaGetLastError());
+  L->launches += 1;
   return QCD_OK;
 }
 

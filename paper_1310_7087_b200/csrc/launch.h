@@ -10,6 +10,7 @@ struct UpdateSel {
   bool comp;
   int kind;               // 0 HB, 1 OR
   bool field;
+  bool meas;              // fused plaquette measurement (UpdateArgs::meas set; mu >= 1)
 };
 
 // returns cudaErrorInvalidValue for an unsupported combination
@@ -17,6 +18,8 @@ cudaError_t launch_update_su3_f32(const UpdateSel& s, const Geom& g, void* links
 cudaError_t launch_update_su3_f64(const UpdateSel& s, const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st);
 cudaError_t launch_update_su3_f32_d4(const UpdateSel& s, const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st);
 cudaError_t launch_update_su3_f64_d4(const UpdateSel& s, const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st);
+cudaError_t launch_update_su3_f32_d4_meas(const UpdateSel& s, const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st);
+cudaError_t launch_update_su3_f64_d4_meas(const UpdateSel& s, const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st);
 cudaError_t launch_update_su2(const UpdateSel& s, const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st);
 
 }  // namespace qcd

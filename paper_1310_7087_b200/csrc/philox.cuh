@@ -39,8 +39,9 @@ __host__ __device__ __forceinline__ uint32_t philox_c2(int mu, int parity, int s
 // word -> uniform strictly inside (0,1), exactly representable in the target precision (reading R8)
 __device__ __forceinline__ double uniform64(uint32_t w) { return ((double)w + 0.5) * 2.3283064365386963e-10; }          // 2^-32
 __device__ __forceinline__ double uniform23(uint32_t w) { return ((double)(w >> 9) + 0.5) * 1.1920928955078125e-07; }   // 2^-23
-// the same fp32-mode uniform computed in float: (w>>9) + 0.5 has 24 significant bits, so this is exact
-__device__ __forceinline__ float uniform23f(uint32_t w) { return ((float)(w >> 9) + 0.5f) * 1.1920928955078125e-07f; }
+// the same fp32-mode uniform computed in float without an integer conversion: 1.m with m = w >> 9 is 1 + (w>>9) 2^-23,
+// and subtracting 1 - 2^-24 gives (2 (w>>9) + 1) 2^-24, which has 24 significant bits: the subtraction is exact
+__device__ __forceinline__ float uniform23f(uint32_t w) { return __uint_as_float(0x3F800000u | (w >> 9)) - 0.99999994f; }
 template <typename R> __device__ __forceinline__ R uniform_real(uint32_t w);
 template <> __device__ __forceinline__ float uniform_real<float>(uint32_t w) { return uniform23f(w); }
 template <> __device__ __forceinline__ double uniform_real<double>(uint32_t w) { return uniform64(w); }

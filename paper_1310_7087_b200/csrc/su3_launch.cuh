@@ -79,7 +79,7 @@ template <typename Kern> static cudaError_t ensure_smem(Kern kern, size_t smem, 
   return e;
 }
 
-template <typename R, int MU, bool COMP, int KIND, bool FIELD>
+template <typename R, int MU, bool COMP, int KIND, bool FIELD, bool MEAS>
 static cudaError_t su3_go_tiled(const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st) {
   typedef PlaneTraits<R, (COMP ? 12 : 18)> T;
   typedef typename T::Vec Vec;
@@ -87,7 +87,7 @@ static cudaError_t su3_go_tiled(const Geom& g, void* links, const UpdateArgs& a,
   constexpr int K = TiledCfg<R, COMP, KIND>::K, MINB = TiledCfg<R, COMP, KIND>::MINB;
   constexpr bool ROLL = LoopCfg<R, KIND>::ROLL && (4 % K == 0);
   constexpr size_t smem = (size_t)(TD::res_slots(MU) + K * TD::B) * T::NP * sizeof(Vec);
-  auto kern = su3_update_tiled_kernel<R, MU, COMP, KIND, FIELD, TD, K, MINB, ROLL>;
+  auto kern = su3_update_tiled_kernel<R, MU, COMP, KIND, FIELD, TD, K, MINB, ROLL, MEAS>;
   static std::atomic<uint64_t> done{0};
   cudaError_t e = ensure_smem(kern, smem, done);
   if (e != cudaSuccess) return e;
@@ -99,20 +99,20 @@ static cudaError_t su3_go_tiled(const Geom& g, void* links, const UpdateArgs& a,
   return launch_pdl(kern, dim3(g.Vh / TD::B), dim3(TD::B), smem, st, g, (Vec*)links, a2);
 }
 
-template <typename R, int D, int MU, bool COMP, int KIND, bool FIELD>
+template <typename R, int D, int MU, bool COMP, int KIND, bool FIELD, bool MEAS>
 static cudaError_t su3_go(const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st) {
   typedef PlaneTraits<R, (COMP ? 12 : 18)> T;
   typedef typename T::Vec Vec;
   if constexpr (D == 4 && TiledCfg<R, COMP, KIND>::ON) {
     typedef typename TileFor<MU>::TD TD;
     if (g.Lh0 % TD::T0 == 0 && g.L[1] % TD::T1 == 0 && g.L[2] % TD::T2 == 0 && g.L[3] % TD::T3 == 0)
-      return su3_go_tiled<R, MU, COMP, KIND, FIELD>(g, links, a, st);
+      return su3_go_tiled<R, MU, COMP, KIND, FIELD, MEAS>(g, links, a, st);
   }
   constexpr bool ROLL = LoopCfg<R, KIND>::ROLL, PRE = LoopCfg<R, KIND>::PRE;
   constexpr int B = RingCfg<R, COMP>::B, MINB = RingCfg<R, COMP>::MINB;
   constexpr int K = (KIND == 1 && !ROLL && RingKOr<R, COMP>::K >= 0) ? RingKOr<R, COMP>::K : RingCfg<R, COMP>::K;
   constexpr size_t smem = (size_t)K * T::NP * B * sizeof(Vec) + ((KIND == 0 && PRE) ? (size_t)15 * B * sizeof(R) : 0);
-  auto kern = su3_update_kernel<R, D, MU, COMP, KIND, FIELD, B, K, MINB, ROLL, PRE>;
+  auto kern = su3_update_kernel<R, D, MU, COMP, KIND, FIELD, B, K, MINB, ROLL, PRE, MEAS>;
   static std::atomic<uint64_t> done{0};
   cudaError_t e = ensure_smem(kern, smem, done);
   if (e != cudaSuccess) return e;
@@ -121,22 +121,28 @@ static cudaError_t su3_go(const Geom& g, void* links, const UpdateArgs& a, cudaS
   a2.tm = choose_tile(g, B);
   return launch_pdl(kern, dim3(grid), dim3(B), smem, st, g, (Vec*)links, a2);
 }
-template <typename R, int D, int MU, bool COMP>
+// MEAS = the fused-measurement variants (update.cuh, meas_store): instantiated by their own translation units; they exist
+// for mu >= 1 only (the planes (nu, mu), nu < mu)
+template <typename R, int D, int MU, bool COMP, bool MEAS>
 static cudaError_t su3_sel_kind(const UpdateSel& s, const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st) {
-  if (s.kind == 0) return s.field ? su3_go<R, D, MU, COMP, 0, true>(g, links, a, st) : su3_go<R, D, MU, COMP, 0, false>(g, links, a, st);
-  return s.field ? su3_go<R, D, MU, COMP, 1, true>(g, links, a, st) : su3_go<R, D, MU, COMP, 1, false>(g, links, a, st);
+  if constexpr (MEAS && MU == 0) {
+    return cudaErrorInvalidValue;
+  } else {
+    if (s.kind == 0) return s.field ? su3_go<R, D, MU, COMP, 0, true, MEAS>(g, links, a, st) : su3_go<R, D, MU, COMP, 0, false, MEAS>(g, links, a, st);
+    return s.field ? su3_go<R, D, MU, COMP, 1, true, MEAS>(g, links, a, st) : su3_go<R, D, MU, COMP, 1, false, MEAS>(g, links, a, st);
+  }
 }
-template <typename R, int D, int MU>
+template <typename R, int D, int MU, bool MEAS>
 static cudaError_t su3_sel_comp(const UpdateSel& s, const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st) {
-  return s.comp ? su3_sel_kind<R, D, MU, true>(s, g, links, a, st) : su3_sel_kind<R, D, MU, false>(s, g, links, a, st);
+  return s.comp ? su3_sel_kind<R, D, MU, true, MEAS>(s, g, links, a, st) : su3_sel_kind<R, D, MU, false, MEAS>(s, g, links, a, st);
 }
-template <typename R, int D>
+template <typename R, int D, bool MEAS>
 static cudaError_t su3_sel_mu(const UpdateSel& s, const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st) {
   switch (a.mu) {
-    case 0: return su3_sel_comp<R, D, 0>(s, g, links, a, st);
-    case 1: return su3_sel_comp<R, D, 1>(s, g, links, a, st);
-    case 2: if constexpr (D > 2) return su3_sel_comp<R, D, 2>(s, g, links, a, st); break;
-    case 3: if constexpr (D > 3) return su3_sel_comp<R, D, 3>(s, g, links, a, st); break;
+    case 0: return su3_sel_comp<R, D, 0, MEAS>(s, g, links, a, st);
+    case 1: return su3_sel_comp<R, D, 1, MEAS>(s, g, links, a, st);
+    case 2: if constexpr (D > 2) return su3_sel_comp<R, D, 2, MEAS>(s, g, links, a, st); break;
+    case 3: if constexpr (D > 3) return su3_sel_comp<R, D, 3, MEAS>(s, g, links, a, st); break;
   }
   return cudaErrorInvalidValue;
 }

@@ -34,9 +34,44 @@ struct UpdateArgs {
                               // -1: a kernel that writes no links, -2: a kernel that writes all of them (init, set_links)
   uint32_t sweep, key0, key1;
   uint8_t* trials;   // NULL or [lex][3] debug trial codes
+  // fused plaquette measurement (MEAS kernels, see meas_store below): per-warp partial sums of Re Tr[U' A_nu] for the
+  // staple directions nu < mu go to meas[meas_plane[nu] * meas_stride + global warp index]
+  double* meas;
+  uint32_t meas_stride;
+  int meas_plane[3];
   TileMap tm;        // thread -> site mapping of the SU(3) kernels (set by the launcher)
   FieldArgs f;
 };
+
+// ------------------------------------------------------------------ fused plaquette measurement
+// In the LAST pass of a sweep the sub-step (parity 1, mu) leaves every plaquette of the planes (nu, mu), nu < mu, in its
+// final state: the links U_nu (nu < mu) and U_mu on parity 0 were updated earlier in the pass, U_mu on parity 1 is being
+// written, and no later sub-step touches a link of these planes.  Each such plaquette contains exactly one U_mu link on an
+// odd site (U_mu(x) and U_mu(x + nu) have opposite parities), so it is seen exactly once, by that link's thread, as a term
+// of Re Tr[U'_mu(x) A_nu(x)], A_nu = the two staples of direction nu (with the field factor: the dressed plaquette of
+// reading R10).  The kernels keep the cumulative staple sums after the first directions, take Re Tr with the NEW link,
+// difference them per direction in double and reduce per warp (shuffles, fixed order: deterministic); a second kernel sums
+// the per-warp partials.  The three launches (1, mu >= 1) of the last pass thus measure all D(D-1)/2 planes: the "working
+// sweep" of PAPER.md:134 without a separate pass over the links.
+template <int NREC> __device__ __forceinline__ void meas_store(const UpdateArgs& a, const double (&t)[NREC]) {
+  const uint32_t w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+#pragma unroll
+  for (int j = 0; j < NREC; ++j) {
+    double x = t[j];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) x += __shfl_down_sync(0xffffffffu, x, o);
+    if ((threadIdx.x & 31) == 0) a.meas[(size_t)a.meas_plane[j] * a.meas_stride + w] = x;
+  }
+}
+// Re Tr[U S]
+template <typename R> __device__ __forceinline__ R m3_retr(const M3<R>& U, const M3<R>& S) {
+  R t = R(0);
+#pragma unroll
+  for (int i = 0; i < 3; ++i)
+#pragma unroll
+    for (int j = 0; j < 3; ++j) t += U.e[i][j].re * S.e[j][i].re - U.e[i][j].im * S.e[j][i].im;
+  return t;
+}
 
 // ------------------------------------------------------------------ compile-time loops and cp.async
 template <int I, int N, typename F> __device__ __forceinline__ void static_for(F&& f) {
@@ -117,29 +152,34 @@ __device__ __forceinline__ HbDraw<R> hb_first_draw(uint32_t lex, const UpdateArg
   return d;
 }
 
-// the whole trial in double from the Philox block (guard-band path of the fp32 kernels; out of line, rarely taken)
-static __device__ __noinline__ bool kp_trial_f64_cold(double alpha, uint32_t x, uint32_t y, uint32_t z, uint32_t w, double* g0) {
-  const double r1 = uniform23(x), r2 = uniform23(y), r3 = uniform23(z), r4 = uniform23(w);
+// Which Philox block a trial comes from: (lex, sweep, c2, draw = 1 + t) under the launch's key
+struct KpKey { uint32_t lex, sweep, c2, key0, key1; };
+// the whole trial in double from its regenerated Philox block (guard-band path of the fp32 kernels; out of line, rarely taken)
+static __device__ __noinline__ bool kp_trial_f64_cold(double alpha, uint32_t lex, uint32_t sweep, uint32_t c2, uint32_t draw, uint32_t key0,
+                                                      uint32_t key1, double* g0) {
+  const Philox4 b = philox4x32_10(lex, sweep, c2, draw, key0, key1);
+  const double r1 = uniform23(b.x), r2 = uniform23(b.y), r3 = uniform23(b.z), r4 = uniform23(b.w);
   const double c = cospi(2.0 * r2);
   const double delta = -(log(r1) + c * c * log(r3)) / alpha;
   *g0 = 1.0 - delta;
   return r4 * r4 <= 1.0 - 0.5 * delta;
 }
-// accept test of one trial given its random part (E, w); blk = the Philox block the pair came from
-__device__ __forceinline__ bool kp_accept(double inv_alpha, double E, double w, const Philox4&, double& g0) {
+// accept test of trial `draw` given its random part (E, w)
+__device__ __forceinline__ bool kp_accept(double inv_alpha, double E, double w, const KpKey&, uint32_t, double& g0) {
   const double delta = E * inv_alpha;
   g0 = 1.0 - delta;
   return w <= 1.0 - 0.5 * delta;
 }
 // fp32: |error of delta| < (4e-6 E + 2.5e-6) / alpha, so outside the guard band below the float decision is the fp64 one;
-// inside it (probability ~1e-5 per trial) the trial is recomputed in double.
-__device__ __forceinline__ bool kp_accept(float inv, float E, float w, const Philox4& blk, float& g0) {
+// inside it (probability ~1e-5 per trial) the trial is recomputed in double from its own Philox block.  The band is decided
+// here, once, from one rounding of the margin.
+__device__ __forceinline__ bool kp_accept(float inv, float E, float w, const KpKey& k, uint32_t draw, float& g0) {
   const float delta = E * inv;
   const float margin = (1.0f - 0.5f * delta) - w;
   g0 = 1.0f - delta;
   if (fabsf(margin) < (6e-6f * E + 4e-6f) * inv + 5e-7f) {
     double g0d;
-    const bool acc = kp_trial_f64_cold(1.0 / (double)inv, blk.x, blk.y, blk.z, blk.w, &g0d);
+    const bool acc = kp_trial_f64_cold(1.0 / (double)inv, k.lex, k.sweep, k.c2, draw, k.key0, k.key1, &g0d);
     g0 = (float)g0d;
     return acc;
   }
@@ -161,26 +201,17 @@ __device__ __forceinline__ bool subgroup_quaternion(const Q4<R>& v, R k2, uint32
   } else {
     const R rk = q_rsqrt(k2);
     const R inv_alpha = (R)a.inv_c * rk;                 // 1 / alpha, alpha = 2 beta k / N
-    const uint32_t c2 = philox_c2(mu, a.parity, sg, a.hit, 0);
+    KpKey key;
+    key.lex = lex; key.sweep = a.sweep; key.c2 = philox_c2(mu, a.parity, sg, a.hit, 0); key.key0 = a.key0; key.key1 = a.key1;
     R g0;
-    // trial 0 from the precomputed random part; its Philox block is regenerated only inside the fp32 guard band
-    Philox4 blk; blk.x = blk.y = blk.z = blk.w = 0u;
-    bool acc;
-    if (sizeof(R) == 4) {
-      // cheap pre-test, so that the common case does not pay for the Philox block
-      const float inv = (float)inv_alpha;
-      const float margin = (1.0f - 0.5f * (float)d0.E * inv) - (float)d0.w;
-      if (fabsf(margin) < (6e-6f * (float)d0.E + 4e-6f) * inv + 5e-7f) blk = philox4x32_10(lex, a.sweep, c2, 1u, a.key0, a.key1);
-    }
-    acc = kp_accept(inv_alpha, d0.E, d0.w, blk, g0);
+    bool acc = kp_accept(inv_alpha, d0.E, d0.w, key, 1u, g0);     // trial 0 from the precomputed random part
     code = 1;
     if (!acc) {
       code = 0x80 | a.max_trials;
       for (int t = 1; t < a.max_trials; ++t) {
-        const Philox4 x = philox4x32_10(lex, a.sweep, c2, 1u + (uint32_t)t, a.key0, a.key1);
         R E, w;
-        KpRand<R>::run(x, E, w);
-        if (kp_accept(inv_alpha, E, w, x, g0)) { acc = true; code = t + 1; break; }
+        KpRand<R>::run(philox4x32_10(lex, a.sweep, key.c2, 1u + (uint32_t)t, a.key0, a.key1), E, w);
+        if (kp_accept(inv_alpha, E, w, key, 1u + (uint32_t)t, g0)) { acc = true; code = t + 1; break; }
       }
     }
     // fp32: no early return: the lanes that needed further trials re-join the warp here, so what follows is executed
@@ -296,12 +327,17 @@ template <typename R, int R1, int R2> __device__ __forceinline__ void su3_swap_f
 // the third rows of the RIGHT factors U2, U1', U3' (J = 0, 3, 5), which are read in full.
 template <bool COMP> __host__ __device__ constexpr bool rows01_only_t(int J) { return !COMP && (J == 1 || J == 2 || J == 4 || J == 6); }
 
-template <typename R, int D, int MU, bool COMP, int KIND, bool FIELD, int B, int K, int MINB, bool ROLL, bool PRE>
+// MEAS: fused plaquette measurement (see meas_store above); whole warps stay alive for the warp reduction.
+template <typename R, int D, int MU, bool COMP, int KIND, bool FIELD, int B, int K, int MINB, bool ROLL, bool PRE, bool MEAS>
 __global__ void __launch_bounds__(B, MINB)
 su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links, UpdateArgs a) {
   typedef PlaneTraits<R, (COMP ? 12 : 18)> T;
   typedef typename T::Vec Vec;
-  constexpr int NREAL = COMP ? 12 : 18, NP = T::NP, NR = COMP ? 2 : 3;
+  constexpr int NREAL = COMP ? 12 : 18, NP = T::NP;
+  static_assert(!MEAS || MU >= 1, "planes (nu, mu), nu < mu");
+  // cumulative staple sums kept for the measurement: after directions nu = 0 .. NSNAP-1 (the last cumulative sum of
+  // mu = D-1 is A itself)
+  constexpr int NSNAP = !MEAS ? 0 : (MU == D - 1 ? MU - 1 : MU);
   // link n = 6 i + J of the sequence goes to slot n % K; with the rolled direction loop the slot must not depend on i
   static_assert(K == 0 || (K >= 2 && K <= 7 && (!ROLL || 6 % K == 0)), "ring slots: K | 6 when the direction loop is rolled");
   constexpr int KR = K > 0 ? K : 1;
@@ -311,11 +347,17 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
   const int p = a.parity;
   uint32_t h;
   SiteCoord sc;
+  bool active = true;
   if (a.tm.on) {
     sc = decode_site_tiled(g, a.tm, p, h);                         // the tiles cover the lattice exactly
   } else {
     h = blockIdx.x * B + threadIdx.x;
-    if (h >= g.Vh) return;                                         // no block barrier anywhere below
+    if constexpr (MEAS) {
+      active = h < g.Vh;                                           // a surplus thread shadows the last site: it neither
+      if (!active) h = g.Vh - 1;                                   // stores nor contributes, but stays for the shuffles
+    } else {
+      if (h >= g.Vh) return;                                       // no block barrier anywhere below
+    }
     sc = decode_site(g, h, p);
   }
   int fo[D], bo[D];
@@ -416,6 +458,7 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
 
   M3<R> A, P, Q;      // A: staple sum; P: the link kept for the next product (U2 / U1'); Q: X = U3 U2 or Y = U2' U1'
   m3_zero(A);
+  M3<R> snap[NSNAP > 0 ? NSNAP : 1];
   auto direction_step = [&](int i) {
     const bool last = (i == D - 2);
     const int n0 = ROLL ? 0 : 6 * i;                               // sequence number of this direction's first link
@@ -476,6 +519,10 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
       }
     });
     cur = nxt;
+    if constexpr (NSNAP > 0) {
+#pragma unroll
+      for (int k = 0; k < NSNAP; ++k) if (i == k) snap[k] = A;   // directions come in the order nu = 0 .. mu-1, mu+1 ..
+    }
   };
   if constexpr (ROLL) {
 #pragma unroll 1
@@ -521,6 +568,10 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
       // frame (1,2,0) back to (0,1,2): row 0 <- cur 2, row 1 <- cur 0, row 2 <- cur 1
 #pragma unroll
       for (int c = 0; c < 3; ++c) { const Cx<R> t = U.e[2][c]; U.e[2][c] = U.e[1][c]; U.e[1][c] = U.e[0][c]; U.e[0][c] = t; }
+      if constexpr (MEAS && MU == D - 1) {                         // the measurement takes A in the original frame too
+#pragma unroll
+        for (int r = 0; r < 3; ++r) { const Cx<R> t = A.e[r][2]; A.e[r][2] = A.e[r][1]; A.e[r][1] = A.e[r][0]; A.e[r][0] = t; }
+      }
     } else {
       int c0, c1, c2;
       su3_subgroup_hit<R, KIND, 0, 1>(U, A, lex, a, MU, 0, first_draw(0), c0);
@@ -533,6 +584,18 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
   }
   m3_reunitarise(U);
 
+  if constexpr (MEAS) {
+    double t[MU];
+    R prev = R(0);
+#pragma unroll
+    for (int j = 0; j < MU; ++j) {
+      const R c = m3_retr(U, j < NSNAP ? snap[j < NSNAP ? j : 0] : A);
+      t[j] = active ? (double)c - (double)prev : 0.0;
+      prev = c;
+    }
+    meas_store<MU>(a, t);
+    if (!active) return;
+  }
   R r[NREAL];
   m3_to_reals<R, NREAL>(U, r);
   store_reals<R, NREAL>(links, g, (size_t)(p * D + MU) * arr, h, r);
@@ -549,12 +612,18 @@ __device__ __forceinline__ Q4<R> su2_load(const typename PlaneTraits<R, 4>::Vec*
   return q4<R>(r[0], r[1], r[2], r[3]);
 }
 
-template <typename R, int D, int KIND, bool FIELD>
+template <typename R, int D, int KIND, bool FIELD, bool MEAS>
 __global__ void __launch_bounds__(256)
 su2_update_kernel(Geom g, typename PlaneTraits<R, 4>::Vec* links, UpdateArgs a) {
   typedef PlaneTraits<R, 4> T;
-  const uint32_t h = blockIdx.x * blockDim.x + threadIdx.x;
-  if (h >= g.Vh) { pdl_wait(); pdl_trigger(); return; }
+  uint32_t h = blockIdx.x * blockDim.x + threadIdx.x;
+  bool active = true;
+  if constexpr (MEAS) {
+    active = h < g.Vh;
+    if (!active) h = g.Vh - 1;                             // surplus threads stay for the warp reduction (see su3_update_kernel)
+  } else {
+    if (h >= g.Vh) { pdl_wait(); pdl_trigger(); return; }
+  }
   const int p = a.parity, mu = a.mu, q = 1 - p;
   const SiteCoord sc = decode_site(g, h, p);
   int fmu, bmu;
@@ -563,6 +632,7 @@ su2_update_kernel(Geom g, typename PlaneTraits<R, 4>::Vec* links, UpdateArgs a) 
   pdl_trigger();
   const typename T::Vec* __restrict__ ro = links;
   Q4<R> A = q4<R>(0, 0, 0, 0);
+  Q4<R> cum[D - 1];                                        // MEAS: cumulative staple sums after each direction
 #pragma unroll
   for (int i = 0; i < D - 1; ++i) {
     const int nu = i + (i >= mu ? 1 : 0);
@@ -587,6 +657,7 @@ su2_update_kernel(Geom g, typename PlaneTraits<R, 4>::Vec* links, UpdateArgs a) 
       const Q4<R> S = q4_mul(q4_mul(q4_conj(U1), q4_conj(U2)), U3);
       A = q4_add(A, S);
     }
+    if constexpr (MEAS) cum[i] = A;
   }
   const size_t own = array_base<T::NP>(g, D, p, mu);
   Q4<R> U = su2_load<R, false>(links, g, own, h);
@@ -603,6 +674,26 @@ su2_update_kernel(Geom g, typename PlaneTraits<R, 4>::Vec* links, UpdateArgs a) 
   }
   const R n = q_rsqrt(U.a0 * U.a0 + U.a1 * U.a1 + U.a2 * U.a2 + U.a3 * U.a3);
   R r[4] = {U.a0 * n, U.a1 * n, U.a2 * n, U.a3 * n};
+  if constexpr (MEAS) {
+    // Re Tr[U' A_nu] = 2 (U' . A_nu)_0 in the quaternion algebra; directions nu = 0 .. mu-1 come first
+    double t[D - 1];
+    R prev = R(0);
+#pragma unroll
+    for (int j = 0; j < D - 1; ++j) {
+      const R c = R(2) * (r[0] * cum[j].a0 - r[1] * cum[j].a1 - r[2] * cum[j].a2 - r[3] * cum[j].a3);
+      t[j] = (active && j < mu) ? (double)c - (double)prev : 0.0;
+      prev = c;
+    }
+    const uint32_t w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+#pragma unroll
+    for (int j = 0; j < D - 1; ++j) {
+      double x = t[j];
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) x += __shfl_down_sync(0xffffffffu, x, o);
+      if ((threadIdx.x & 31) == 0 && j < mu) a.meas[(size_t)a.meas_plane[j] * a.meas_stride + w] = x;
+    }
+    if (!active) return;
+  }
   store_reals<R, 4>(links, g, own, h, r);
   if (KIND == 0 && a.trials) {
     a.trials[(size_t)lex * 3 + 0] = (uint8_t)code; a.trials[(size_t)lex * 3 + 1] = 0; a.trials[(size_t)lex * 3 + 2] = 0;

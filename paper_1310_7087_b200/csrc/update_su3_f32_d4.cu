@@ -3,6 +3,6 @@
 
 namespace qcd {
 cudaError_t launch_update_su3_f32_d4(const UpdateSel& s, const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st) {
-  return su3_sel_mu<float, 4>(s, g, links, a, st);
+  return su3_sel_mu<float, 4, false>(s, g, links, a, st);
 }
 }  // namespace qcd

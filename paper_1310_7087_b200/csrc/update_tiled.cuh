@@ -38,12 +38,15 @@ template <int T0_, int T1_, int T2_, int T3_> struct TileDims {
 // K ring slots per thread (K-1 links in flight); the ring carries, per direction nu, the four links
 //   r=0  U3  = U_nu(x)      r=1  U1  = U_nu(x+mu)      r=2  U1' = U_nu(x+mu-nu)      r=3  U3' = U_nu(x-nu)
 // and last the own link; link n = 4 i + r goes to slot n % K (ROLL, the rolled loop over nu, needs K | 4).
-template <typename R, int MU, bool COMP, int KIND, bool FIELD, typename TD, int K, int MINB, bool ROLL>
+// MEAS: fused plaquette measurement of the planes (nu, MU), nu < MU (update.cuh, meas_store).
+template <typename R, int MU, bool COMP, int KIND, bool FIELD, typename TD, int K, int MINB, bool ROLL, bool MEAS>
 __global__ void __launch_bounds__(TD::B, MINB)
 su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links, UpdateArgs a) {
   typedef PlaneTraits<R, (COMP ? 12 : 18)> T;
   typedef typename T::Vec Vec;
   constexpr int D = 4, NREAL = COMP ? 12 : 18, NP = T::NP, NR = COMP ? 2 : 3, B = TD::B, RES = TD::res_slots(MU);
+  static_assert(!MEAS || MU >= 1, "planes (nu, mu), nu < mu");
+  constexpr int NSNAP = !MEAS ? 0 : (MU == D - 1 ? MU - 1 : MU);   // cumulative staple sums kept for the measurement
   static_assert(K >= 2 && K <= 5 && (!ROLL || 4 % K == 0), "ring slots");
   extern __shared__ __align__(16) unsigned char tile_raw[];
   Vec* const res = reinterpret_cast<Vec*>(tile_raw);                        // [plane][RES]
@@ -171,6 +174,7 @@ su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* 
 
   M3<R> A, P, Q;
   m3_zero(A);
+  M3<R> snap[NSNAP > 0 ? NSNAP : 1];
   auto phase = [&](int i) {
     const bool last = (i == D - 2);
     const Dir nxt = make_dir(last ? i : i + 1);
@@ -246,6 +250,10 @@ su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* 
       }
     }
     cur = nxt;
+    if constexpr (NSNAP > 0) {
+#pragma unroll
+      for (int k = 0; k < NSNAP; ++k) if (i == k) snap[k] = A;
+    }
   };
   if constexpr (ROLL) {
 #pragma unroll 1
@@ -279,6 +287,10 @@ su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* 
     }
 #pragma unroll
     for (int k = 0; k < 3; ++k) { const Cx<R> t = U.e[2][k]; U.e[2][k] = U.e[1][k]; U.e[1][k] = U.e[0][k]; U.e[0][k] = t; }
+    if constexpr (MEAS && MU == D - 1) {
+#pragma unroll
+      for (int r = 0; r < 3; ++r) { const Cx<R> t = A.e[r][2]; A.e[r][2] = A.e[r][1]; A.e[r][1] = A.e[r][0]; A.e[r][0] = t; }
+    }
   } else {
     int c0, c1, c2;
     su3_subgroup_hit<R, KIND, 0, 1>(U, A, lex, a, MU, 0, hb_first_draw<R>(lex, a, MU, 0), c0);
@@ -290,6 +302,17 @@ su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* 
   }
   m3_reunitarise(U);
 
+  if constexpr (MEAS) {
+    double t[MU];
+    R prev = R(0);
+#pragma unroll
+    for (int j = 0; j < MU; ++j) {
+      const R c = m3_retr(U, j < NSNAP ? snap[j < NSNAP ? j : 0] : A);
+      t[j] = (double)c - (double)prev;
+      prev = c;
+    }
+    meas_store<MU>(a, t);
+  }
   R r[NREAL];
   m3_to_reals<R, NREAL>(U, r);
   store_reals<R, NREAL>(links, g, (size_t)(p * D + MU) * arr, h, r);

@@ -97,3 +97,18 @@ def site_parity(dims):
     """(V,) parity (sum of coordinates) & 1 in lex order"""
     V = int(np.prod(dims))
     return np.stack(np.unravel_index(np.arange(V), tuple(reversed(dims))), axis=-1).sum(axis=1) & 1
+
+
+def staple_rms(B, dims, mu):
+    """For every site x: sqrt of the sum of squares of B over the 6(D-1) links of the staples of U_mu(x) (same index
+    bookkeeping as staple_dependents).  B: (V, D) float.  Used to carry per-link error BOUNDS through un-resynced sub-steps."""
+    D = len(dims)
+    g = (B * B).reshape(tuple(reversed(dims)) + (D,))
+    acc = np.zeros(g.shape[:-1])
+    for nu in range(D):
+        if nu == mu:
+            continue
+        gn, gm = g[..., nu], g[..., mu]
+        acc += gn + shift(gn, dims, mu) + shift(gm, dims, nu)
+        acc += shift(gn, dims, nu, -1) + shift(gm, dims, nu, -1) + shift(shift(gn, dims, mu), dims, nu, -1)
+    return np.sqrt(acc.reshape(-1))

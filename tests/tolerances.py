@@ -58,3 +58,19 @@ def unresynced_bar(prec, n_hits, k_typ=3.5):
         bar = TOL * sum_{i<n} g^i"""
     g = np.sqrt(18.0) / k_typ
     return TOL[prec] * sum(g ** i for i in range(n_hits))
+
+
+def carry_bound(B, rms_nbr, k, tol, updated, mu):
+    """Per-link error bound after one more un-resynced sub-step.  B: (V, D) bounds so far; rms_nbr: (V,)
+    RMS-combined bounds of the 18 staple links (tests/np_lattice.staple_rms); k: (V,) the oracle's smallest subgroup norm of
+    this hit; `updated`: (V,) bool, the sites of this sub-step.  A hit computes U' = a(v) U with v = proj(U A), |v| = k:
+        * its own rounding: at most the single-sub-step bar tol (north_star);
+        * the staple sum inherits sqrt(sum B_nbr^2) (independent errors, every factor unitary), the old link its own B and
+          moves v by at most |A| B_own <= 6 B_own (A is a sum of 6 unitary matrices); the normalisation v -> v/k passes a
+          perturbation of v on with gain 1/k, and U itself enters U' once more directly:
+              B' = tol + (rms_nbr + 6 B_own) / k + B_own."""
+    out = B.copy()
+    own = B[:, mu]
+    new = tol + (rms_nbr + 6.0 * own) / np.where(updated, k, 1.0) + own
+    out[updated, mu] = new[updated]
+    return out
