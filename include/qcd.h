@@ -153,6 +153,61 @@ int qcd_get_launch_count(qcd_lattice_t* lat, uint64_t* out);
 int qcd_probe_fma_tflops(int precision, double* tflops);
 int qcd_probe_copy_gbs(size_t bytes, int reps, double* gbs);
 
+/* ---------------------------------------------------------------------------------------------------------------------
+ * A lattice divided into parts.  PAPER.md:124-128 sec 4: "dividing lattice is made into unequal parts
+ * ... in first spatial coordinate direction ... Divided lattice simulation differs from a full lattice simulation only in
+ * necessity to carry out the exchanging values of boundary sites"; used for several devices and when one device's memory
+ * is not enough.  Here the split direction is the slowest SPATIAL direction, dims[D-2] (D >= 3), so that a part holds whole
+ * time lines (the Polyakov loop stays local).  A part ("slab") of `extent` layers starting at global coordinate `offset`
+ * (both even) is a qcd_lattice_t of local extent extent + 2 along that direction: its own layers, then a copy of the next
+ * part's first layer and a copy of the previous part's last layer (one-site link halos: a staple reaches one site).
+ * After every (parity, mu) sub-step the two boundary layers of the array that sub-step wrote are copied to the neighbours.
+ * The Philox counters use the GLOBAL site index, so a divided lattice reproduces the undivided one bit for bit.
+ *
+ * Slab primitives (one part per handle; the parts may live in different processes, one per GPU, and exchange the packed
+ * layers through any transport, e.g. torch.distributed / NCCL):
+ *   qcd_slab_bytes / qcd_slab_create   like qcd_lattice_bytes / qcd_lattice_create, dims = GLOBAL extents.
+ *   qcd_init, qcd_set_links / qcd_get_links (canonical layout of the part's own block, lex order of its own extents),
+ *   qcd_debug_substep (updates the part's own sites), qcd_set/get_seed, qcd_set/get_sweep_counter work on a slab;
+ *   qcd_sweep, qcd_sweep_measure, qcd_measure, qcd_measure_accumulate return QCD_ERR_UNSUPPORTED on it.
+ *   qcd_slab_halo_bytes                bytes of one boundary layer of one (parity, mu) array.
+ *   qcd_slab_halo_pack(side)           side 0: the first own layer, side 1: the last own layer -> DEVICE buffer.
+ *   qcd_slab_halo_unpack(side)         DEVICE buffer -> side 0: the copy of the previous part's last layer,
+ *                                      side 1: the copy of the next part's first layer.  Both asynchronous on the stream.
+ *   qcd_slab_measure_sums              SUMS over the part's own sites of (1/N) Re Tr plaquette per plane and of
+ *                                      (1/N) Tr Polyakov line (either may be NULL); synchronises.  The caller adds the
+ *                                      parts and divides by V resp. V / dims[D-1].
+ * Split driver (all parts in this process; devices[k] = CUDA device of part k, NULL = the current device for all; parts on
+ * different devices need peer access and write each other's halo layers directly over NVLink):
+ *   qcd_split_create(extents = NULL: parts as equal as even extents allow), qcd_split_init, qcd_split_sweep,
+ *   qcd_split_substep, qcd_split_measure, qcd_split_get_links / qcd_split_set_links (HOST, global canonical layout),
+ *   qcd_split_set_seed, qcd_split_set/get_sweep_counter, qcd_split_parts, qcd_split_halo_bytes (bytes copied between
+ *   parts per sub-step), qcd_split_synchronize, qcd_split_destroy.  Same argument rules and errors as the undivided calls.
+ * ------------------------------------------------------------------------------------------------------------------- */
+typedef struct qcd_split qcd_split_t;
+size_t qcd_slab_bytes(int D, const int* dims, int Nc, int precision, unsigned flags, int offset, int extent);
+int qcd_slab_create(int D, const int* dims, int Nc, int precision, unsigned flags, int offset, int extent, void* device_mem,
+                    size_t bytes, void* cuda_stream, qcd_lattice_t** out);
+size_t qcd_slab_halo_bytes(qcd_lattice_t* lat);
+int qcd_slab_halo_pack(qcd_lattice_t* lat, int parity, int mu, int side, void* device_buf, size_t bytes);
+int qcd_slab_halo_unpack(qcd_lattice_t* lat, int parity, int mu, int side, const void* device_buf, size_t bytes);
+int qcd_slab_measure_sums(qcd_lattice_t* lat, const qcd_field_t* field, double* plaq_sums, double* polyakov_sum);
+int qcd_split_create(int D, const int* dims, int Nc, int precision, unsigned flags, int n_parts, const int* extents,
+                     const int* devices, qcd_split_t** out);
+int qcd_split_destroy(qcd_split_t* s);
+int qcd_split_parts(qcd_split_t* s, int* n_parts, int* offsets, int* extents, int capacity);
+int qcd_split_halo_bytes(qcd_split_t* s, size_t* per_substep);
+int qcd_split_init(qcd_split_t* s, int start, uint64_t seed);
+int qcd_split_sweep(qcd_split_t* s, double beta, int n_hb, int n_or, const qcd_field_t* field);
+int qcd_split_substep(qcd_split_t* s, double beta, int kind, int hit, int parity, int mu, const qcd_field_t* field);
+int qcd_split_measure(qcd_split_t* s, const qcd_field_t* field, double* plaq_total, double* plaq_planes, double* polyakov_re_im);
+int qcd_split_get_links(qcd_split_t* s, void* dst, size_t bytes);
+int qcd_split_set_links(qcd_split_t* s, const void* src, size_t bytes);
+int qcd_split_set_seed(qcd_split_t* s, uint64_t seed);
+int qcd_split_set_sweep_counter(qcd_split_t* s, uint32_t value);
+int qcd_split_get_sweep_counter(qcd_split_t* s, uint32_t* out);
+int qcd_split_synchronize(qcd_split_t* s);
+
 const char* qcd_last_error(void);
 const char* qcd_version(void);
 

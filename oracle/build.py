@@ -9,6 +9,8 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "qcd_oracle.cpp")
 LIB = os.path.join(HERE, "libqcd_oracle.so")
+ON_SRC = os.path.join(HERE, "on_oracle.cpp")       # the O(N) model oracle
+ON_LIB = os.path.join(HERE, "libqcd_on_oracle.so")
 
 
 def build_oracle(force: bool = False) -> str:
@@ -19,5 +21,13 @@ def build_oracle(force: bool = False) -> str:
     return LIB
 
 
+def build_on_oracle(force: bool = False) -> str:
+    if not force and os.path.exists(ON_LIB) and os.path.getmtime(ON_LIB) >= os.path.getmtime(ON_SRC):
+        return ON_LIB
+    subprocess.run(["g++", "-O2", "-std=c++17", "-fopenmp", "-fPIC", "-shared", "-o", ON_LIB, ON_SRC], check=True)
+    return ON_LIB
+
+
 if __name__ == "__main__":
     print(build_oracle(force=True))
+    print(build_on_oracle(force=True))

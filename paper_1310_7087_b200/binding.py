@@ -25,6 +25,10 @@ SYMBOLS = [
     "qcd_set_option", "qcd_debug_substep", "qcd_debug_get_trials", "qcd_debug_philox", "qcd_get_profile",
     "qcd_reset_profile", "qcd_get_launch_count", "qcd_measure_accumulate", "qcd_sweep_measure", "qcd_sweep_measure_accumulate", "qcd_accum_get", "qcd_accum_reset", "qcd_probe_fma_tflops", "qcd_probe_copy_gbs", "qcd_last_error",
     "qcd_version",
+    "qcd_slab_bytes", "qcd_slab_create", "qcd_slab_halo_bytes", "qcd_slab_halo_pack", "qcd_slab_halo_unpack", "qcd_slab_measure_sums",
+    "qcd_split_create", "qcd_split_destroy", "qcd_split_parts", "qcd_split_halo_bytes", "qcd_split_init", "qcd_split_sweep",
+    "qcd_split_substep", "qcd_split_measure", "qcd_split_get_links", "qcd_split_set_links", "qcd_split_set_seed",
+    "qcd_split_set_sweep_counter", "qcd_split_get_sweep_counter", "qcd_split_synchronize",
 ]
 
 
@@ -80,6 +84,28 @@ def lib():
     L.qcd_get_launch_count.argtypes = [p, C.POINTER(C.c_uint64)]
     L.qcd_probe_fma_tflops.argtypes = [i, dp]
     L.qcd_probe_copy_gbs.argtypes = [sz, i, dp]
+    L.qcd_slab_bytes.restype = sz
+    L.qcd_slab_bytes.argtypes = [i, ip, i, i, u, i, i]
+    L.qcd_slab_create.argtypes = [i, ip, i, i, u, i, i, p, sz, p, C.POINTER(p)]
+    L.qcd_slab_halo_bytes.restype = sz
+    L.qcd_slab_halo_bytes.argtypes = [p]
+    L.qcd_slab_halo_pack.argtypes = [p, i, i, i, p, sz]
+    L.qcd_slab_halo_unpack.argtypes = [p, i, i, i, p, sz]
+    L.qcd_slab_measure_sums.argtypes = [p, fp, dp, dp]
+    L.qcd_split_create.argtypes = [i, ip, i, i, u, i, ip, ip, C.POINTER(p)]
+    L.qcd_split_destroy.argtypes = [p]
+    L.qcd_split_parts.argtypes = [p, ip, ip, ip, i]
+    L.qcd_split_halo_bytes.argtypes = [p, C.POINTER(sz)]
+    L.qcd_split_init.argtypes = [p, i, C.c_uint64]
+    L.qcd_split_sweep.argtypes = [p, d, i, i, fp]
+    L.qcd_split_substep.argtypes = [p, d, i, i, i, i, fp]
+    L.qcd_split_measure.argtypes = [p, fp, dp, dp, dp]
+    L.qcd_split_get_links.argtypes = [p, p, sz]
+    L.qcd_split_set_links.argtypes = [p, p, sz]
+    L.qcd_split_set_seed.argtypes = [p, C.c_uint64]
+    L.qcd_split_set_sweep_counter.argtypes = [p, C.c_uint32]
+    L.qcd_split_get_sweep_counter.argtypes = [p, C.POINTER(C.c_uint32)]
+    L.qcd_split_synchronize.argtypes = [p]
     L.qcd_last_error.restype = C.c_char_p
     L.qcd_version.restype = C.c_char_p
     _lib = L
@@ -131,16 +157,23 @@ def qcd_debug_philox(ctr, key, impl=0):
 
 
 class Lattice:
-    """One lattice handle.  Device memory comes from a torch uint8 tensor, the stream from torch."""
+    """One lattice handle.  Device memory comes from a torch uint8 tensor, the stream from torch.
+    slab = (offset, extent): a part of the lattice of global extents `dims`, split along direction D-2 (qcd_slab_create);
+    then dims / V describe the part's own block and global_dims the whole lattice."""
 
-    def __init__(self, dims, Nc, precision=QCD_FP64, flags=0, device="cuda:0", library_alloc=False):
+    def __init__(self, dims, Nc, precision=QCD_FP64, flags=0, device="cuda:0", library_alloc=False, slab=None):
         import torch
-        self.dims = tuple(int(x) for x in dims)
-        self.D, self.Nc, self.precision, self.flags = len(self.dims), int(Nc), int(precision), int(flags)
+        self.global_dims = tuple(int(x) for x in dims)
+        self.D, self.Nc, self.precision, self.flags = len(self.global_dims), int(Nc), int(precision), int(flags)
+        self.slab = None if slab is None else (int(slab[0]), int(slab[1]))
+        self.dims = self.global_dims if slab is None else tuple(self.slab[1] if k == self.D - 2 else x for k, x in enumerate(self.global_dims))
         self.V = int(np.prod(self.dims))
         self._h = C.c_void_p()
-        arr = (C.c_int * self.D)(*self.dims)
-        nbytes = lib().qcd_lattice_bytes(self.D, arr, self.Nc, self.precision, self.flags)
+        arr = (C.c_int * self.D)(*self.global_dims)
+        if slab is None:
+            nbytes = lib().qcd_lattice_bytes(self.D, arr, self.Nc, self.precision, self.flags)
+        else:
+            nbytes = lib().qcd_slab_bytes(self.D, arr, self.Nc, self.precision, self.flags, self.slab[0], self.slab[1])
         self._torch = torch
         self._mem = None
         self._device = torch.device(device)
@@ -152,8 +185,12 @@ class Lattice:
                 stream_ptr = torch.cuda.current_stream().cuda_stream
         elif nbytes:
             torch.cuda.set_device(self._device)
-        _check(lib().qcd_lattice_create(self.D, arr, self.Nc, self.precision, self.flags, mem_ptr, int(nbytes), stream_ptr,
-                                        C.byref(self._h)))
+        if slab is None:
+            _check(lib().qcd_lattice_create(self.D, arr, self.Nc, self.precision, self.flags, mem_ptr, int(nbytes), stream_ptr,
+                                            C.byref(self._h)))
+        else:
+            _check(lib().qcd_slab_create(self.D, arr, self.Nc, self.precision, self.flags, self.slab[0], self.slab[1], mem_ptr,
+                                         int(nbytes), stream_ptr, C.byref(self._h)))
         self.np_real = np.float32 if self.precision == QCD_FP32 else np.float64
         self.np_complex = np.complex64 if self.precision == QCD_FP32 else np.complex128
 
@@ -265,6 +302,23 @@ class Lattice:
         _check(lib().qcd_debug_get_trials(self._h, out.ctypes.data, out.nbytes))
         return out
 
+    # ---- slab primitives (a part of a divided lattice)
+    def qcd_slab_halo_bytes(self):
+        return int(lib().qcd_slab_halo_bytes(self._h))
+
+    def qcd_slab_halo_pack(self, parity, mu, side, device_ptr, nbytes):
+        _check(lib().qcd_slab_halo_pack(self._h, int(parity), int(mu), int(side), int(device_ptr), int(nbytes)))
+
+    def qcd_slab_halo_unpack(self, parity, mu, side, device_ptr, nbytes):
+        _check(lib().qcd_slab_halo_unpack(self._h, int(parity), int(mu), int(side), int(device_ptr), int(nbytes)))
+
+    def qcd_slab_measure_sums(self, field=None):
+        npl = self.D * (self.D - 1) // 2
+        planes = (C.c_double * npl)()
+        poly = (C.c_double * 2)()
+        _check(lib().qcd_slab_measure_sums(self._h, _fref(field), planes, poly))
+        return np.array(planes[:]), complex(poly[0], poly[1])
+
     def qcd_get_profile(self, kind):
         ms = C.c_double(0.0)
         n = C.c_uint64(0)
@@ -278,3 +332,89 @@ class Lattice:
         n = C.c_uint64(0)
         _check(lib().qcd_get_launch_count(self._h, C.byref(n)))
         return int(n.value)
+
+
+class SplitLattice:
+    """A lattice divided into parts along direction D-2, all parts in this process (qcd_split_*): one part per entry of
+    `devices` (CUDA device ordinals; default: n_parts parts on the current device)."""
+
+    def __init__(self, dims, Nc, precision=QCD_FP64, flags=0, n_parts=2, extents=None, devices=None):
+        self.dims = tuple(int(x) for x in dims)
+        self.D, self.Nc, self.precision, self.flags = len(self.dims), int(Nc), int(precision), int(flags)
+        self.V = int(np.prod(self.dims))
+        self._h = C.c_void_p()
+        arr = (C.c_int * self.D)(*self.dims)
+        ext = (C.c_int * n_parts)(*[int(e) for e in extents]) if extents is not None else None
+        dev = (C.c_int * n_parts)(*[int(e) for e in devices]) if devices is not None else None
+        _check(lib().qcd_split_create(self.D, arr, self.Nc, self.precision, self.flags, int(n_parts), ext, dev, C.byref(self._h)))
+        self.np_complex = np.complex64 if self.precision == QCD_FP32 else np.complex128
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h:
+            lib().qcd_split_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    def qcd_split_parts(self):
+        n = C.c_int(0)
+        _check(lib().qcd_split_parts(self._h, C.byref(n), None, None, 0))
+        off, ext = (C.c_int * n.value)(), (C.c_int * n.value)()
+        _check(lib().qcd_split_parts(self._h, C.byref(n), off, ext, n.value))
+        return list(off), list(ext)
+
+    def qcd_split_halo_bytes(self):
+        out = C.c_size_t(0)
+        _check(lib().qcd_split_halo_bytes(self._h, C.byref(out)))
+        return int(out.value)
+
+    def qcd_split_init(self, start, seed):
+        _check(lib().qcd_split_init(self._h, int(start), int(seed)))
+
+    def qcd_split_sweep(self, beta, n_hb, n_or, field=None):
+        _check(lib().qcd_split_sweep(self._h, float(beta), int(n_hb), int(n_or), _fref(field)))
+
+    def qcd_split_substep(self, beta, kind, hit, parity, mu, field=None):
+        _check(lib().qcd_split_substep(self._h, float(beta), int(kind), int(hit), int(parity), int(mu), _fref(field)))
+
+    def qcd_split_measure(self, field=None):
+        npl = self.D * (self.D - 1) // 2
+        tot = C.c_double(0.0)
+        planes = (C.c_double * npl)()
+        poly = (C.c_double * 2)()
+        _check(lib().qcd_split_measure(self._h, _fref(field), C.byref(tot), planes, poly))
+        return tot.value, np.array(planes[:]), complex(poly[0], poly[1])
+
+    def qcd_split_get_links(self):
+        out = np.zeros((self.V, self.D, self.Nc, self.Nc), dtype=self.np_complex)
+        _check(lib().qcd_split_get_links(self._h, out.ctypes.data, out.nbytes))
+        return out
+
+    def qcd_split_set_links(self, links):
+        a = np.ascontiguousarray(links, dtype=self.np_complex)
+        assert a.shape == (self.V, self.D, self.Nc, self.Nc), a.shape
+        _check(lib().qcd_split_set_links(self._h, a.ctypes.data, a.nbytes))
+
+    def qcd_split_set_seed(self, seed):
+        _check(lib().qcd_split_set_seed(self._h, int(seed)))
+
+    def qcd_split_set_sweep_counter(self, v):
+        _check(lib().qcd_split_set_sweep_counter(self._h, int(v)))
+
+    def qcd_split_get_sweep_counter(self):
+        out = C.c_uint32(0)
+        _check(lib().qcd_split_get_sweep_counter(self._h, C.byref(out)))
+        return out.value
+
+    def qcd_split_synchronize(self):
+        _check(lib().qcd_split_synchronize(self._h))

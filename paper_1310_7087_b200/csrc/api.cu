@@ -30,7 +30,9 @@ struct EventPair { cudaEvent_t a, b; int kind; int n; };   // n = update-kernel 
 }  // namespace
 
 struct qcd_lattice {
-  int D, dims[4], Nc, precision;
+  int D, dims[4], Nc, precision;   // dims: the local extents (a slab: n_int + 2 along the split direction)
+  // slab of a larger lattice (Geom::sd >= 0): global extents, and the global coordinate of the first own layer
+  int gdims[4], slab_off;
   unsigned flags;
   bool comp;
   Geom g;
@@ -96,19 +98,35 @@ bool valid_shape(int D, const int* dims, int Nc, int precision, unsigned flags, 
   return true;
 }
 
-Geom make_geom(int D, const int* dims) {
+// dims: local extents.  Not a slab: sd = -1.  Slab: dims[sd] = n_int + 2, gdims = global extents, off = global coordinate of
+// the slab's first own layer (common.cuh, Geom).
+Geom make_geom(int D, const int* dims, int sd = -1, const int* gdims = nullptr, int off = 0) {
   Geom g;
   memset(&g, 0, sizeof(g));
   g.D = D;
-  uint64_t V = 1;
-  for (int d = 0; d < 4; ++d) { g.L[d] = (d < D) ? dims[d] : 1; V *= g.L[d]; }
+  uint64_t V = 1, Vi = 1;
+  for (int d = 0; d < 4; ++d) {
+    g.L[d] = (d < D) ? dims[d] : 1;
+    g.Li[d] = (d == sd) ? g.L[d] - 2 : g.L[d];
+    V *= g.L[d]; Vi *= g.Li[d];
+  }
   g.Lh0 = g.L[0] / 2;
   g.stride[0] = 0; g.stride[1] = g.Lh0; g.stride[2] = g.Lh0 * g.L[1]; g.stride[3] = g.Lh0 * g.L[1] * g.L[2];
   g.V = (uint32_t)V; g.Vh = (uint32_t)(V / 2);
   g.Vh_pad = (g.Vh + 31u) & ~31u;
   g.dLh0 = make_fastdiv((uint32_t)g.Lh0); g.dL1 = make_fastdiv((uint32_t)g.L[1]); g.dL2 = make_fastdiv((uint32_t)g.L[2]);
+  g.sd = sd;
+  g.Vh_int = (uint32_t)(Vi / 2);
+  g.iLh0 = g.dLh0; g.iL1 = make_fastdiv((uint32_t)g.Li[1]); g.iL2 = make_fastdiv((uint32_t)g.Li[2]);
+  uint32_t st = 1;
+  for (int d = 0; d < 4; ++d) {
+    g.lexS[d] = st;
+    st *= (uint32_t)((sd >= 0 && d < D) ? gdims[d] : g.L[d]);
+  }
+  g.lex0 = sd >= 0 ? (uint32_t)off * g.lexS[sd] : 0u;
   return g;
 }
+inline uint32_t own_sites(const qcd_lattice* L) { return 2u * L->g.Vh_int; }   // V, or the interior of a slab
 
 int check_field(const qcd_lattice* L, const qcd_field_t* f, bool* on) {
   *on = false;
@@ -174,9 +192,9 @@ MeasLayout meas_layout(const qcd_lattice* L) {
   // fused measurement: one partial per warp of an update launch; every launch shape has <= Vh_pad/32 + 8 warps (CTAs of
   // <= 256 threads); entries beyond a launch's warps are never written and stay zero from the allocation
   m.np_warp = g.Vh_pad / 32u + 8u;
-  m.boxed = (L->D == 4 && g.Lh0 % 8 == 0 && g.L[1] % 2 == 0 && g.L[2] % 2 == 0 && g.L[3] % 2 == 0);
-  m.nb_plaq = m.boxed ? g.V / 128u : ((g.Vh + 127u) / 128u) * 2u;
-  m.nb_poly = (g.V / (uint32_t)g.L[L->D - 1] + 127u) / 128u;
+  m.boxed = (L->D == 4 && g.Lh0 % 8 == 0 && g.Li[1] % 2 == 0 && g.Li[2] % 2 == 0 && g.Li[3] % 2 == 0);
+  m.nb_plaq = m.boxed ? 2u * g.Vh_int / 128u : ((g.Vh_int + 127u) / 128u) * 2u;
+  m.nb_poly = (2u * g.Vh_int / (uint32_t)g.L[L->D - 1] + 127u) / 128u;
   m.off_plaq = (size_t)m.npl * m.np_warp;
   m.off_poly = m.off_plaq + (size_t)m.npl * m.nb_plaq;
   m.need = m.off_poly + 2 * (size_t)m.nb_poly;
@@ -249,7 +267,7 @@ struct InitOp {
   qcd_lattice* L; int hot;
   template <int NC, int D, typename R, bool COMP> int operator()() {
     typedef typename LinkIO<NC, R, COMP>::Vec Vec;
-    dim3 grid((L->g.Vh + 127) / 128, 2);
+    dim3 grid((L->g.Vh_int + 127) / 128, 2);
     init_kernel<NC, D, R, COMP><<<grid, 128, 0, L->stream>>>(L->g, (Vec*)L->mem, hot, (uint32_t)(L->seed & 0xFFFFFFFFull), (uint32_t)(L->seed >> 32));
     CUDA_TRY(cudaGetLastError());
     L->launches += 1;
@@ -278,7 +296,7 @@ struct LayoutOp {
 struct MeasureOp {
   // fused: the plaquette partials are already in the fused region of d_partials (written by the MEAS update kernels of the
   // sweep just enqueued); only their second-stage reduction is launched here
-  qcd_lattice* L; MeasureField mf; bool want_plaq, want_poly, fused;
+  qcd_lattice* L; MeasureField mf; bool want_plaq, want_poly, fused, sums;
   template <int NC, int D, typename R, bool COMP> int operator()() {
     typedef typename LinkIO<NC, R, COMP>::Vec Vec;
     constexpr int NPL = D * (D - 1) / 2;
@@ -288,14 +306,15 @@ struct MeasureOp {
     // boxed thread mapping of the plaquette kernel (aux_kernels.cuh, MeasureField): one grid row of V / 128 CTAs
     mf.boxed = m.boxed ? 1 : 0;
     if (mf.boxed) {
-      mf.n0 = make_fastdiv((uint32_t)(L->g.Lh0 / 8)); mf.n1 = make_fastdiv((uint32_t)(L->g.L[1] / 2)); mf.n2 = make_fastdiv((uint32_t)(L->g.L[2] / 2));
+      mf.n0 = make_fastdiv((uint32_t)(L->g.Lh0 / 8)); mf.n1 = make_fastdiv((uint32_t)(L->g.Li[1] / 2)); mf.n2 = make_fastdiv((uint32_t)(L->g.Li[2] / 2));
     }
-    const uint32_t Vs = L->g.V / (uint32_t)L->g.L[D - 1];
+    const uint32_t Vs = own_sites(L) / (uint32_t)L->g.L[D - 1];
     double* pf = L->d_partials;
     double* pp = L->d_partials + m.off_plaq;
     double* pq = L->d_partials + m.off_poly;
-    const dim3 plaq_grid = mf.boxed ? dim3(L->g.V / 128, 1) : dim3((L->g.Vh + 127) / 128, 2);
-    const double plaq_scale = 1.0 / ((double)L->g.V * NC), poly_scale = 1.0 / ((double)Vs * NC);
+    const dim3 plaq_grid = mf.boxed ? dim3(own_sites(L) / 128, 1) : dim3((L->g.Vh_int + 127) / 128, 2);
+    // a slab reports SUMS over its own sites (scale 1 / N): the parts' sums are added and divided by the global volume
+    const double plaq_scale = sums ? 1.0 / NC : 1.0 / ((double)L->g.V * NC), poly_scale = sums ? 1.0 / NC : 1.0 / ((double)Vs * NC);
     const bool fork = want_plaq && want_poly;
     if (fork) {
       // the Polyakov kernel (one thread per spatial site, bound by the latency of its L_t dependent loads) goes first on a
@@ -333,7 +352,7 @@ struct MeasureOp {
 };
 
 size_t canonical_bytes(const qcd_lattice* L) {
-  return (size_t)L->g.V * L->D * L->Nc * L->Nc * 2 * (L->precision == QCD_FP32 ? 4 : 8);
+  return (size_t)own_sites(L) * L->D * L->Nc * L->Nc * 2 * (L->precision == QCD_FP32 ? 4 : 8);
 }
 
 // ---- probes
@@ -387,22 +406,19 @@ size_t qcd_lattice_bytes(int D, const int* dims, int Nc, int precision, unsigned
   return (size_t)2 * D * np * (size_t)g.Vh_pad * vb;
 }
 
-int qcd_lattice_create(int D, const int* dims, int Nc, int precision, unsigned flags, void* device_mem, size_t bytes, void* cuda_stream,
-                       qcd_lattice_t** out) {
-  if (!out) return fail(QCD_ERR_INVALID_ARG, "out is NULL");
-  *out = nullptr;
-  int why;
-  if (!valid_shape(D, dims, Nc, precision, flags, &why))
-    return fail(why, why == QCD_ERR_UNSUPPORTED ? "COMPRESS12 needs Nc = 3" : "invalid D / dims (even, >= 2) / Nc / precision / flags");
+// common part of qcd_lattice_create / qcd_slab_create: dims = LOCAL extents (validated by the caller)
+static int create_lattice(int D, const int* dims, int Nc, int precision, unsigned flags, int sd, const int* gdims, int off, void* device_mem,
+                          size_t bytes, void* cuda_stream, qcd_lattice_t** out) {
   const size_t need = qcd_lattice_bytes(D, dims, Nc, precision, flags);
   if (device_mem) {
-    if (bytes < need) return fail(QCD_ERR_INVALID_ARG, "device_mem smaller than qcd_lattice_bytes()");
+    if (bytes < need) return fail(QCD_ERR_INVALID_ARG, "device_mem smaller than the workspace size");
     if (((uintptr_t)device_mem) & 255u) return fail(QCD_ERR_INVALID_ARG, "device_mem must be 256-byte aligned");
   }
   qcd_lattice* L = new qcd_lattice();
   L->D = D; L->Nc = Nc; L->precision = precision; L->flags = flags; L->comp = (flags & QCD_FLAG_COMPRESS12) != 0;
-  for (int d = 0; d < 4; ++d) L->dims[d] = d < D ? dims[d] : 1;
-  L->g = make_geom(D, dims);
+  for (int d = 0; d < 4; ++d) { L->dims[d] = d < D ? dims[d] : 1; L->gdims[d] = d < D ? (gdims ? gdims[d] : dims[d]) : 1; }
+  L->slab_off = off;
+  L->g = make_geom(D, dims, sd, gdims, off);
   L->bytes = need; L->mem = device_mem; L->owns_mem = false;
   L->stream = (cudaStream_t)cuda_stream;
   L->seed = 0; L->sweep = 0; L->has_links = false; L->max_trials = 10;
@@ -426,6 +442,46 @@ int qcd_lattice_create(int D, const int* dims, int Nc, int precision, unsigned f
   if (e != cudaSuccess) { std::string m = cudaGetErrorString(e); qcd_lattice_destroy(L); return fail(QCD_ERR_CUDA, "create: " + m); }
   *out = L;
   return QCD_OK;
+}
+
+int qcd_lattice_create(int D, const int* dims, int Nc, int precision, unsigned flags, void* device_mem, size_t bytes, void* cuda_stream,
+                       qcd_lattice_t** out) {
+  if (!out) return fail(QCD_ERR_INVALID_ARG, "out is NULL");
+  *out = nullptr;
+  int why;
+  if (!valid_shape(D, dims, Nc, precision, flags, &why))
+    return fail(why, why == QCD_ERR_UNSUPPORTED ? "COMPRESS12 needs Nc = 3" : "invalid D / dims (even, >= 2) / Nc / precision / flags");
+  return create_lattice(D, dims, Nc, precision, flags, -1, nullptr, 0, device_mem, bytes, cuda_stream, out);
+}
+
+// ---- slab of a larger lattice
+static int slab_local_dims(int D, const int* gdims, int Nc, int precision, unsigned flags, int offset, int extent, int* ldims) {
+  int why;
+  if (!valid_shape(D, gdims, Nc, precision, flags, &why)) return fail(why, "invalid global D / dims / Nc / precision / flags");
+  if (D < 3) return fail(QCD_ERR_UNSUPPORTED, "a lattice is split along its slowest spatial direction D-2: D >= 3");
+  const int sd = D - 2;
+  if (extent < 2 || (extent & 1) || offset < 0 || (offset & 1) || offset + extent > gdims[sd])
+    return fail(QCD_ERR_INVALID_ARG, "slab offset and extent must be even, extent >= 2, offset + extent <= dims[D-2]");
+  for (int d = 0; d < D; ++d) ldims[d] = gdims[d];
+  ldims[sd] = extent + 2;
+  if (!valid_shape(D, ldims, Nc, precision, flags, &why)) return fail(why, "slab too large for the kernels' indexing");
+  return QCD_OK;
+}
+
+size_t qcd_slab_bytes(int D, const int* dims, int Nc, int precision, unsigned flags, int offset, int extent) {
+  int ld[4];
+  if (slab_local_dims(D, dims, Nc, precision, flags, offset, extent, ld) != QCD_OK) return 0;
+  return qcd_lattice_bytes(D, ld, Nc, precision, flags);
+}
+
+int qcd_slab_create(int D, const int* dims, int Nc, int precision, unsigned flags, int offset, int extent, void* device_mem, size_t bytes,
+                    void* cuda_stream, qcd_lattice_t** out) {
+  if (!out) return fail(QCD_ERR_INVALID_ARG, "out is NULL");
+  *out = nullptr;
+  int ld[4];
+  int rc = slab_local_dims(D, dims, Nc, precision, flags, offset, extent, ld);
+  if (rc != QCD_OK) return rc;
+  return create_lattice(D, ld, Nc, precision, flags, D - 2, dims, offset, device_mem, bytes, cuda_stream, out);
 }
 
 int qcd_lattice_destroy(qcd_lattice_t* L) {
@@ -460,6 +516,7 @@ int qcd_init(qcd_lattice_t* L, int start, uint64_t seed) {
 static int sweep_core(qcd_lattice_t* L, double beta, int n_hb, int n_or, const qcd_field_t* field, bool fused) {
   if (!L) return fail(QCD_ERR_INVALID_ARG, "lattice is NULL");
   if (!L->has_links) return fail(QCD_ERR_STATE, "qcd_sweep before qcd_init / qcd_set_links");
+  if (L->g.sd >= 0) return fail(QCD_ERR_UNSUPPORTED, "a slab is swept sub-step by sub-step with halo exchanges in between (qcd_split_sweep)");
   if (!std::isfinite(beta) || beta < 0.0) return fail(QCD_ERR_INVALID_ARG, "beta must be finite and >= 0");
   if (n_hb < 0 || n_or < 0 || n_hb > 65535 || n_or > 65535) return fail(QCD_ERR_INVALID_ARG, "n_hb, n_or must be in 0..65535");
   bool fon;
@@ -504,6 +561,7 @@ int qcd_debug_substep(qcd_lattice_t* L, double beta, int kind, int hit, int pari
   int rc = check_field(L, field, &fon);
   if (rc != QCD_OK) return rc;
   uint8_t* trials = nullptr;
+  if (L->debug_trials && L->g.sd >= 0) return fail(QCD_ERR_UNSUPPORTED, "trial codes are indexed by the global site: not recorded on a slab");
   if (L->debug_trials && kind == QCD_KIND_HB) {
     if (!L->d_trials) CUDA_TRY(cudaMalloc(&L->d_trials, (size_t)L->g.V * 3));
     CUDA_TRY(cudaMemsetAsync(L->d_trials, 0, (size_t)L->g.V * 3, L->stream));
@@ -529,7 +587,7 @@ static int enqueue_measure(qcd_lattice_t* L, const qcd_field_t* field, bool want
   int rc = check_field(L, field, &fon);
   if (rc != QCD_OK) return rc;
   MeasureOp op;
-  op.L = L; op.want_plaq = want_plaq; op.want_poly = want_poly; op.fused = fused;
+  op.L = L; op.want_plaq = want_plaq; op.want_poly = want_poly; op.fused = fused; op.sums = L->g.sd >= 0;
   memset(&op.mf, 0, sizeof(op.mf));
   FieldArgs fa = make_field_args(field, fon, L->Nc);
   op.mf.enabled = fon ? 1 : 0; op.mf.mu = fa.mu; op.mf.nu = fa.nu;
@@ -549,6 +607,7 @@ __global__ void accum_kernel(const double* res, double* acc, int npl) {
 }
 
 int qcd_measure_accumulate(qcd_lattice_t* L, const qcd_field_t* field) {
+  if (L && L->g.sd >= 0) return fail(QCD_ERR_UNSUPPORTED, "not available on a slab");
   int rc = enqueue_measure(L, field, true, true);
   if (rc != QCD_OK) return rc;
   accum_kernel<<<1, 32, 0, L->stream>>>(L->d_results, L->d_results + 16, L->D * (L->D - 1) / 2);
@@ -589,6 +648,7 @@ static int fetch_results(qcd_lattice_t* L, bool want_plaq, double* plaq_total, d
 }
 
 int qcd_measure(qcd_lattice_t* L, const qcd_field_t* field, double* plaq_total, double* plaq_planes, double* polyakov) {
+  if (L && L->g.sd >= 0) return fail(QCD_ERR_UNSUPPORTED, "a slab has sums, not means: qcd_slab_measure_sums / qcd_split_measure");
   const bool want_plaq = plaq_total || plaq_planes, want_poly = polyakov != nullptr;
   int rc = enqueue_measure(L, field, want_plaq, want_poly);
   if (rc != QCD_OK) return rc;
@@ -625,14 +685,14 @@ int qcd_sweep_measure_accumulate(qcd_lattice_t* L, double beta, int n_hb, int n_
 // copy and layout kernel alternate on the lattice's stream, which orders the reuse of the buffer.
 static const size_t STAGE_BYTES = (size_t)64 << 20;
 static int stage_chunks(qcd_lattice_t* L, char* host, bool to_internal) {
-  const size_t site_bytes = canonical_bytes(L) / L->g.V;
+  const size_t site_bytes = canonical_bytes(L) / own_sites(L);
   const size_t per = std::max<size_t>(128, (STAGE_BYTES / site_bytes) / 128 * 128);     // sites per chunk, a multiple of every BL
   if (!L->d_canon && cudaMalloc(&L->d_canon, per * site_bytes) != cudaSuccess) {
     L->d_canon = nullptr; cudaGetLastError();
     return fail(QCD_ERR_ALLOC, "staging buffer");
   }
-  for (size_t lex0 = 0; lex0 < L->g.V; lex0 += per) {
-    const size_t lex1 = std::min<size_t>(L->g.V, lex0 + per), n = (lex1 - lex0) * site_bytes;
+  for (size_t lex0 = 0; lex0 < own_sites(L); lex0 += per) {
+    const size_t lex1 = std::min<size_t>(own_sites(L), lex0 + per), n = (lex1 - lex0) * site_bytes;
     if (to_internal) CUDA_TRY(cudaMemcpyAsync(L->d_canon, host + lex0 * site_bytes, n, cudaMemcpyHostToDevice, L->stream));
     LayoutOp op{L, L->d_canon, to_internal, (uint32_t)lex0, (uint32_t)lex1};
     const int rc = dispatch(L, op);
@@ -650,7 +710,7 @@ int qcd_get_links(qcd_lattice_t* L, void* dst, size_t bytes, int dst_is_device) 
   if (bytes != canonical_bytes(L)) return fail(QCD_ERR_INVALID_ARG, "bytes must equal V*D*N*N*2*sizeof(real)");
   if (dst_is_device && ((uintptr_t)dst & 15u)) return fail(QCD_ERR_INVALID_ARG, "device pointer must be 16-byte aligned");
   if (!dst_is_device) return stage_chunks(L, (char*)dst, false);
-  LayoutOp op{L, dst, false, 0u, L->g.V};
+  LayoutOp op{L, dst, false, 0u, own_sites(L)};
   return dispatch(L, op);
 }
 
@@ -662,7 +722,7 @@ int qcd_set_links(qcd_lattice_t* L, const void* src, size_t bytes, int src_is_de
   if (!src_is_device) {
     rc = stage_chunks(L, (char*)const_cast<void*>(src), true);
   } else {
-    LayoutOp op{L, const_cast<void*>(src), true, 0u, L->g.V};
+    LayoutOp op{L, const_cast<void*>(src), true, 0u, own_sites(L)};
     rc = dispatch(L, op);
   }
   if (rc == QCD_OK) L->has_links = true;
@@ -791,6 +851,376 @@ int qcd_probe_copy_gbs(size_t bytes, int reps, double* gbs) {
   cudaEventDestroy(a); cudaEventDestroy(b); cudaFree(src); cudaFree(dst);
   if (e != cudaSuccess) return fail(QCD_ERR_CUDA, std::string("copy probe: ") + cudaGetErrorString(e));
   *gbs = best;
+  return QCD_OK;
+}
+
+
+// =====================================================================================
+// Slabs and the split driver (sec 4: the lattice divided into parts along one
+// spatial direction, boundary values exchanged between the parts)
+// =====================================================================================
+}  // extern "C"
+
+namespace {
+
+struct HaloOp {
+  // mode 0: layer `src_layer` of S -> contiguous buffer; 1: buffer -> layer `dst_layer` of T; 2: layer of S -> layer of T
+  int mode; qcd_lattice* S; int src_layer; qcd_lattice* T; int dst_layer; void* buf; int parity, mu; cudaStream_t st;
+  template <int NC, int D, typename R, bool COMP> int operator()() {
+    typedef typename LinkIO<NC, R, COMP>::Vec Vec;
+    constexpr int NP = LinkIO<NC, R, COMP>::T::NP;
+    const qcd_lattice* E = mode == 1 ? T : S;
+    const uint32_t count = E->g.Vh / (uint32_t)E->g.L[E->g.sd];          // half-indices of one layer
+    const dim3 grid((count + 127) / 128);
+    if (mode == 0) halo_kernel<Vec, NP, 0><<<grid, 128, 0, st>>>(S->g, (const Vec*)S->mem, src_layer, S->g, (Vec*)buf, 0, parity, mu, D, count);
+    else if (mode == 1) halo_kernel<Vec, NP, 1><<<grid, 128, 0, st>>>(T->g, (const Vec*)buf, 0, T->g, (Vec*)T->mem, dst_layer, parity, mu, D, count);
+    else halo_kernel<Vec, NP, 2><<<grid, 128, 0, st>>>(S->g, (const Vec*)S->mem, src_layer, T->g, (Vec*)T->mem, dst_layer, parity, mu, D, count);
+    CUDA_TRY(cudaGetLastError());
+    return QCD_OK;
+  }
+};
+
+bool same_format(const qcd_lattice* a, const qcd_lattice* b) {
+  if (a->D != b->D || a->Nc != b->Nc || a->precision != b->precision || a->comp != b->comp || a->g.sd != b->g.sd) return false;
+  for (int d = 0; d < a->D; ++d) if (d != a->g.sd && a->dims[d] != b->dims[d]) return false;
+  return true;
+}
+
+struct DeviceGuard {
+  int prev;
+  explicit DeviceGuard(int dev) : prev(-1) { cudaGetDevice(&prev); if (dev != prev) cudaSetDevice(dev); else prev = -1; }
+  ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+}  // namespace
+
+struct qcd_split {
+  int D, Nc, precision, n;
+  unsigned flags;
+  int dims[4];
+  std::vector<qcd_lattice*> part;
+  std::vector<int> dev, off, ext;
+  std::vector<cudaStream_t> stream;
+  std::vector<cudaEvent_t> ev_upd, ev_halo;    // per part: its last update kernel done / its last halo writes done
+  uint32_t sweep;
+};
+
+namespace {
+
+// refresh, in both neighbours, the copies of part k's boundary layers of the (parity, mu) array.  Part k's stream does the
+// copies after (i) its own update (stream order) and (ii) the neighbours' updates of the same sub-step (they may still read
+// the old copies); the neighbours' next launches wait for ev_halo[k].
+int split_push_halos(qcd_split* S, int k, int parity, int mu) {
+  DeviceGuard dg(S->dev[k]);
+  const int prev = (k + S->n - 1) % S->n, next = (k + 1) % S->n;
+  qcd_lattice* P = S->part[k];
+  if (prev != k) CUDA_TRY(cudaStreamWaitEvent(S->stream[k], S->ev_upd[prev], 0));
+  if (next != k && next != prev) CUDA_TRY(cudaStreamWaitEvent(S->stream[k], S->ev_upd[next], 0));
+  // first own layer -> the previous part's "next" copy (its layer n_int); last own layer -> the next part's "previous" copy
+  HaloOp lo{2, P, 0, S->part[prev], S->ext[prev], nullptr, parity, mu, S->stream[k]};
+  int rc = dispatch(P, lo);
+  if (rc != QCD_OK) return rc;
+  HaloOp hi{2, P, S->ext[k] - 1, S->part[next], S->ext[next] + 1, nullptr, parity, mu, S->stream[k]};
+  rc = dispatch(P, hi);
+  if (rc != QCD_OK) return rc;
+  P->launches += 2;
+  CUDA_TRY(cudaEventRecord(S->ev_halo[k], S->stream[k]));
+  return QCD_OK;
+}
+
+// every part waits for the halo writes of its neighbours before its next launch
+int split_wait_halos(qcd_split* S, int k) {
+  DeviceGuard dg(S->dev[k]);
+  const int prev = (k + S->n - 1) % S->n, next = (k + 1) % S->n;
+  if (prev != k) CUDA_TRY(cudaStreamWaitEvent(S->stream[k], S->ev_halo[prev], 0));
+  if (next != k && next != prev) CUDA_TRY(cudaStreamWaitEvent(S->stream[k], S->ev_halo[next], 0));
+  return QCD_OK;
+}
+
+int split_refresh_all(qcd_split* S) {
+  for (int k = 0; k < S->n; ++k) { DeviceGuard dg(S->dev[k]); CUDA_TRY(cudaEventRecord(S->ev_upd[k], S->stream[k])); }
+  for (int p = 0; p < 2; ++p)
+    for (int mu = 0; mu < S->D; ++mu)
+      for (int k = 0; k < S->n; ++k) { int rc = split_push_halos(S, k, p, mu); if (rc != QCD_OK) return rc; }
+  for (int k = 0; k < S->n; ++k) { int rc = split_wait_halos(S, k); if (rc != QCD_OK) return rc; }
+  return QCD_OK;
+}
+
+int split_substep(qcd_split* S, double beta, int kind, int hit, int parity, int mu, const qcd_field_t* field) {
+  for (int k = 0; k < S->n; ++k) {
+    DeviceGuard dg(S->dev[k]);
+    qcd_lattice* P = S->part[k];
+    P->sweep = S->sweep;
+    bool fon;
+    int rc = check_field(P, field, &fon);
+    if (rc != QCD_OK) return rc;
+    rc = substep(P, beta, kind, hit, parity, mu, field, fon, nullptr, false);
+    if (rc != QCD_OK) return rc;
+    CUDA_TRY(cudaEventRecord(S->ev_upd[k], S->stream[k]));
+  }
+  for (int k = 0; k < S->n; ++k) { int rc = split_push_halos(S, k, parity, mu); if (rc != QCD_OK) return rc; }
+  for (int k = 0; k < S->n; ++k) { int rc = split_wait_halos(S, k); if (rc != QCD_OK) return rc; }
+  return QCD_OK;
+}
+
+// sites per layer of the split direction below it (contiguous run in lex order) and number of such runs
+void split_runs(const qcd_split* S, size_t* run_sites, size_t* n_runs) {
+  const int sd = S->D - 2;
+  size_t lo = 1, hi = 1;
+  for (int d = 0; d < sd; ++d) lo *= (size_t)S->dims[d];
+  for (int d = sd + 1; d < S->D; ++d) hi *= (size_t)S->dims[d];
+  *run_sites = lo; *n_runs = hi;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t qcd_slab_halo_bytes(qcd_lattice_t* L) {
+  if (!L || L->g.sd < 0) return 0;
+  int nreal, vb, np;
+  plane_params(L->Nc, L->precision, L->comp, &nreal, &vb, &np);
+  return (size_t)(L->g.Vh / (uint32_t)L->g.L[L->g.sd]) * np * vb;
+}
+
+int qcd_slab_halo_pack(qcd_lattice_t* L, int parity, int mu, int side, void* device_buf, size_t bytes) {
+  if (!L || !device_buf) return fail(QCD_ERR_INVALID_ARG, "NULL argument");
+  if (L->g.sd < 0) return fail(QCD_ERR_STATE, "not a slab");
+  if ((parity != 0 && parity != 1) || mu < 0 || mu >= L->D || (side != 0 && side != 1)) return fail(QCD_ERR_INVALID_ARG, "bad parity / mu / side");
+  if (bytes != qcd_slab_halo_bytes(L) || ((uintptr_t)device_buf & 15u)) return fail(QCD_ERR_INVALID_ARG, "buffer must hold qcd_slab_halo_bytes() bytes, 16-byte aligned");
+  HaloOp op{0, L, side == 0 ? 0 : L->g.Li[L->g.sd] - 1, L, 0, device_buf, parity, mu, L->stream};
+  int rc = dispatch(L, op);
+  if (rc == QCD_OK) L->launches += 1;
+  return rc;
+}
+
+int qcd_slab_halo_unpack(qcd_lattice_t* L, int parity, int mu, int side, const void* device_buf, size_t bytes) {
+  if (!L || !device_buf) return fail(QCD_ERR_INVALID_ARG, "NULL argument");
+  if (L->g.sd < 0) return fail(QCD_ERR_STATE, "not a slab");
+  if ((parity != 0 && parity != 1) || mu < 0 || mu >= L->D || (side != 0 && side != 1)) return fail(QCD_ERR_INVALID_ARG, "bad parity / mu / side");
+  if (bytes != qcd_slab_halo_bytes(L) || ((uintptr_t)device_buf & 15u)) return fail(QCD_ERR_INVALID_ARG, "buffer must hold qcd_slab_halo_bytes() bytes, 16-byte aligned");
+  const int n = L->g.Li[L->g.sd];
+  HaloOp op{1, L, 0, L, side == 0 ? n + 1 : n, const_cast<void*>(device_buf), parity, mu, L->stream};
+  int rc = dispatch(L, op);
+  // the halo layers of the (parity, mu) array were written: an update kernel may not fetch that array early
+  if (rc == QCD_OK) { L->launches += 1; if (!(L->last_parity == parity && L->last_mu == mu)) L->last_parity = L->last_mu = -2; }
+  return rc;
+}
+
+int qcd_slab_measure_sums(qcd_lattice_t* L, const qcd_field_t* field, double* plaq_sums, double* polyakov_sum) {
+  if (!L) return fail(QCD_ERR_INVALID_ARG, "lattice is NULL");
+  if (L->g.sd < 0) return fail(QCD_ERR_STATE, "not a slab");
+  const bool want_plaq = plaq_sums != nullptr, want_poly = polyakov_sum != nullptr;
+  int rc = enqueue_measure(L, field, want_plaq, want_poly);
+  if (rc != QCD_OK) return rc;
+  if (!want_plaq && !want_poly) return QCD_OK;
+  CUDA_TRY(cudaMemcpyAsync(L->h_results, L->d_results, 16 * sizeof(double), cudaMemcpyDeviceToHost, L->stream));
+  CUDA_TRY(cudaStreamSynchronize(L->stream));
+  if (want_plaq) for (int k = 0; k < L->D * (L->D - 1) / 2; ++k) plaq_sums[k] = L->h_results[k];
+  if (want_poly) { polyakov_sum[0] = L->h_results[8]; polyakov_sum[1] = L->h_results[9]; }
+  return QCD_OK;
+}
+
+int qcd_split_create(int D, const int* dims, int Nc, int precision, unsigned flags, int n_parts, const int* extents, const int* devices,
+                     qcd_split_t** out) {
+  if (!out) return fail(QCD_ERR_INVALID_ARG, "out is NULL");
+  *out = nullptr;
+  int why;
+  if (!valid_shape(D, dims, Nc, precision, flags, &why)) return fail(why, "invalid D / dims / Nc / precision / flags");
+  if (D < 3) return fail(QCD_ERR_UNSUPPORTED, "a lattice is split along its slowest spatial direction D-2: D >= 3");
+  const int sd = D - 2;
+  if (n_parts < 1 || 2 * n_parts > dims[sd]) return fail(QCD_ERR_INVALID_ARG, "n_parts must be in 1 .. dims[D-2] / 2");
+  qcd_split* S = new qcd_split();
+  S->D = D; S->Nc = Nc; S->precision = precision; S->flags = flags; S->n = n_parts; S->sweep = 0;
+  for (int d = 0; d < 4; ++d) S->dims[d] = d < D ? dims[d] : 1;
+  int cur = 0;
+  cudaGetDevice(&cur);
+  int sum = 0;
+  for (int k = 0; k < n_parts; ++k) {
+    // default: parts as equal as even extents allow (in general the parts are unequal)
+    int e = extents ? extents[k] : 2 * ((dims[sd] / 2) / n_parts + (k < (dims[sd] / 2) % n_parts ? 1 : 0));
+    S->off.push_back(sum); S->ext.push_back(e); S->dev.push_back(devices ? devices[k] : cur);
+    sum += e;
+    if (e < 2 || (e & 1)) { delete S; return fail(QCD_ERR_INVALID_ARG, "part extents must be even and >= 2"); }
+  }
+  if (sum != dims[sd]) { delete S; return fail(QCD_ERR_INVALID_ARG, "part extents must add up to dims[D-2]"); }
+  int rc = QCD_OK;
+  for (int k = 0; k < n_parts && rc == QCD_OK; ++k) {
+    DeviceGuard dg(S->dev[k]);
+    cudaStream_t st = nullptr;
+    cudaEvent_t eu = nullptr, eh = nullptr;
+    if (cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking) != cudaSuccess || cudaEventCreateWithFlags(&eu, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&eh, cudaEventDisableTiming) != cudaSuccess) {
+      rc = fail(QCD_ERR_CUDA, std::string("split: stream / event creation: ") + cudaGetErrorString(cudaGetLastError()));
+    }
+    S->stream.push_back(st); S->ev_upd.push_back(eu); S->ev_halo.push_back(eh);
+    qcd_lattice* P = nullptr;
+    if (rc == QCD_OK) rc = qcd_slab_create(D, dims, Nc, precision, flags, S->off[k], S->ext[k], nullptr, 0, st, &P);
+    S->part.push_back(P);
+  }
+  // parts on different devices write each other's halo layers directly: peer access in both directions
+  for (int k = 0; k < n_parts && rc == QCD_OK; ++k) {
+    const int nb[2] = {(k + n_parts - 1) % n_parts, (k + 1) % n_parts};
+    for (int t = 0; t < 2 && rc == QCD_OK; ++t) {
+      if (S->dev[nb[t]] == S->dev[k]) continue;
+      DeviceGuard dg(S->dev[k]);
+      int can = 0;
+      cudaDeviceCanAccessPeer(&can, S->dev[k], S->dev[nb[t]]);
+      if (!can) { rc = fail(QCD_ERR_UNSUPPORTED, "split: no peer access between the devices of neighbouring parts"); break; }
+      cudaError_t e = cudaDeviceEnablePeerAccess(S->dev[nb[t]], 0);
+      if (e != cudaSuccess && e != cudaErrorPeerAccessAlreadyEnabled) rc = fail(QCD_ERR_CUDA, std::string("cudaDeviceEnablePeerAccess: ") + cudaGetErrorString(e));
+      cudaGetLastError();
+    }
+  }
+  if (rc != QCD_OK) { std::string m = g_err; qcd_split_destroy(S); g_err = m; return rc; }
+  *out = S;
+  return QCD_OK;
+}
+
+int qcd_split_destroy(qcd_split_t* S) {
+  if (!S) return QCD_OK;
+  for (size_t k = 0; k < S->part.size(); ++k) {
+    DeviceGuard dg(S->dev[k]);
+    if (S->part[k]) qcd_lattice_destroy(S->part[k]);
+    if (k < S->ev_upd.size() && S->ev_upd[k]) cudaEventDestroy(S->ev_upd[k]);
+    if (k < S->ev_halo.size() && S->ev_halo[k]) cudaEventDestroy(S->ev_halo[k]);
+    if (k < S->stream.size() && S->stream[k]) cudaStreamDestroy(S->stream[k]);
+  }
+  delete S;
+  return QCD_OK;
+}
+
+int qcd_split_parts(qcd_split_t* S, int* n_parts, int* offsets, int* extents, int capacity) {
+  if (!S || !n_parts) return fail(QCD_ERR_INVALID_ARG, "NULL argument");
+  *n_parts = S->n;
+  if (offsets || extents) {
+    if (capacity < S->n) return fail(QCD_ERR_INVALID_ARG, "capacity < number of parts");
+    for (int k = 0; k < S->n; ++k) { if (offsets) offsets[k] = S->off[k]; if (extents) extents[k] = S->ext[k]; }
+  }
+  return QCD_OK;
+}
+
+int qcd_split_halo_bytes(qcd_split_t* S, size_t* per_substep) {
+  if (!S || !per_substep) return fail(QCD_ERR_INVALID_ARG, "NULL argument");
+  *per_substep = 2 * (size_t)S->n * qcd_slab_halo_bytes(S->part[0]);     // two boundary layers per part and sub-step
+  return QCD_OK;
+}
+
+int qcd_split_init(qcd_split_t* S, int start, uint64_t seed) {
+  if (!S) return fail(QCD_ERR_INVALID_ARG, "split lattice is NULL");
+  for (int k = 0; k < S->n; ++k) {
+    DeviceGuard dg(S->dev[k]);
+    int rc = qcd_init(S->part[k], start, seed);
+    if (rc != QCD_OK) return rc;
+  }
+  S->sweep = 0;
+  return split_refresh_all(S);
+}
+
+int qcd_split_substep(qcd_split_t* S, double beta, int kind, int hit, int parity, int mu, const qcd_field_t* field) {
+  if (!S) return fail(QCD_ERR_INVALID_ARG, "split lattice is NULL");
+  if (!S->part[0]->has_links) return fail(QCD_ERR_STATE, "no links yet");
+  if (!std::isfinite(beta) || beta < 0.0) return fail(QCD_ERR_INVALID_ARG, "beta must be finite and >= 0");
+  if ((kind != QCD_KIND_HB && kind != QCD_KIND_OR) || hit < 0 || hit > 65535 || (parity != 0 && parity != 1) || mu < 0 || mu >= S->D)
+    return fail(QCD_ERR_INVALID_ARG, "bad kind / hit / parity / mu");
+  return split_substep(S, beta, kind, hit, parity, mu, field);
+}
+
+int qcd_split_sweep(qcd_split_t* S, double beta, int n_hb, int n_or, const qcd_field_t* field) {
+  if (!S) return fail(QCD_ERR_INVALID_ARG, "split lattice is NULL");
+  if (!S->part[0]->has_links) return fail(QCD_ERR_STATE, "qcd_split_sweep before qcd_split_init / qcd_split_set_links");
+  if (!std::isfinite(beta) || beta < 0.0) return fail(QCD_ERR_INVALID_ARG, "beta must be finite and >= 0");
+  if (n_hb < 0 || n_or < 0 || n_hb > 65535 || n_or > 65535) return fail(QCD_ERR_INVALID_ARG, "n_hb, n_or must be in 0..65535");
+  for (int pass = 0; pass < n_hb + n_or; ++pass) {
+    const int kind = pass < n_hb ? QCD_KIND_HB : QCD_KIND_OR, hit = pass < n_hb ? pass : 0;
+    for (int p = 0; p < 2; ++p)
+      for (int mu = 0; mu < S->D; ++mu) {
+        int rc = split_substep(S, beta, kind, hit, p, mu, field);
+        if (rc != QCD_OK) return rc;
+      }
+  }
+  S->sweep += 1;
+  for (int k = 0; k < S->n; ++k) S->part[k]->sweep = S->sweep;
+  return QCD_OK;
+}
+
+int qcd_split_measure(qcd_split_t* S, const qcd_field_t* field, double* plaq_total, double* plaq_planes, double* polyakov) {
+  if (!S) return fail(QCD_ERR_INVALID_ARG, "split lattice is NULL");
+  const int npl = S->D * (S->D - 1) / 2;
+  double ps[8] = {0, 0, 0, 0, 0, 0, 0, 0}, pl[2] = {0, 0};
+  const bool want_plaq = plaq_total || plaq_planes;
+  // enqueue on every part first, then collect: the parts measure concurrently
+  for (int k = 0; k < S->n; ++k) {
+    DeviceGuard dg(S->dev[k]);
+    int rc = enqueue_measure(S->part[k], field, want_plaq, polyakov != nullptr);
+    if (rc != QCD_OK) return rc;
+    qcd_lattice* P = S->part[k];
+    CUDA_TRY(cudaMemcpyAsync(P->h_results, P->d_results, 16 * sizeof(double), cudaMemcpyDeviceToHost, P->stream));
+  }
+  for (int k = 0; k < S->n; ++k) {                          // fixed order of the parts: deterministic sums
+    DeviceGuard dg(S->dev[k]);
+    qcd_lattice* P = S->part[k];
+    CUDA_TRY(cudaStreamSynchronize(P->stream));
+    for (int i = 0; i < npl; ++i) ps[i] += P->h_results[i];
+    pl[0] += P->h_results[8]; pl[1] += P->h_results[9];
+  }
+  double V = 1.0;
+  for (int d = 0; d < S->D; ++d) V *= S->dims[d];
+  if (want_plaq) {
+    double tot = 0.0;
+    for (int i = 0; i < npl; ++i) { const double v = ps[i] / V; tot += v; if (plaq_planes) plaq_planes[i] = v; }
+    if (plaq_total) *plaq_total = tot / npl;
+  }
+  if (polyakov) { const double Vs = V / S->dims[S->D - 1]; polyakov[0] = pl[0] / Vs; polyakov[1] = pl[1] / Vs; }
+  return QCD_OK;
+}
+
+// global canonical layout on the HOST: the parts' own blocks are runs of ext * (sites below the split direction) sites
+static int split_links(qcd_split_t* S, char* host, size_t bytes, bool set) {
+  if (!S || !host) return fail(QCD_ERR_INVALID_ARG, "NULL argument");
+  size_t V = 1;
+  for (int d = 0; d < S->D; ++d) V *= (size_t)S->dims[d];
+  const size_t site_bytes = (size_t)S->D * S->Nc * S->Nc * 2 * (S->precision == QCD_FP32 ? 4 : 8);
+  if (bytes != V * site_bytes) return fail(QCD_ERR_INVALID_ARG, "bytes must equal V*D*N*N*2*sizeof(real)");
+  size_t lo, hi;
+  split_runs(S, &lo, &hi);
+  const size_t grow = (size_t)S->dims[S->D - 2] * lo * site_bytes;      // bytes between runs of the global array
+  std::vector<char> tmp;
+  for (int k = 0; k < S->n; ++k) {
+    DeviceGuard dg(S->dev[k]);
+    const size_t run = (size_t)S->ext[k] * lo * site_bytes, goff = (size_t)S->off[k] * lo * site_bytes;
+    tmp.resize(run * hi);
+    if (set) for (size_t r = 0; r < hi; ++r) memcpy(tmp.data() + r * run, host + r * grow + goff, run);
+    int rc = set ? qcd_set_links(S->part[k], tmp.data(), tmp.size(), 0) : qcd_get_links(S->part[k], tmp.data(), tmp.size(), 0);
+    if (rc != QCD_OK) return rc;
+    if (!set) for (size_t r = 0; r < hi; ++r) memcpy(host + r * grow + goff, tmp.data() + r * run, run);
+  }
+  return set ? split_refresh_all(S) : QCD_OK;
+}
+int qcd_split_get_links(qcd_split_t* S, void* dst, size_t bytes) {
+  if (S && !S->part[0]->has_links) return fail(QCD_ERR_STATE, "no links yet");
+  return split_links(S, (char*)dst, bytes, false);
+}
+int qcd_split_set_links(qcd_split_t* S, const void* src, size_t bytes) { return split_links(S, (char*)const_cast<void*>(src), bytes, true); }
+
+int qcd_split_set_seed(qcd_split_t* S, uint64_t seed) {
+  if (!S) return fail(QCD_ERR_INVALID_ARG, "NULL argument");
+  for (int k = 0; k < S->n; ++k) S->part[k]->seed = seed;
+  return QCD_OK;
+}
+int qcd_split_set_sweep_counter(qcd_split_t* S, uint32_t v) {
+  if (!S) return fail(QCD_ERR_INVALID_ARG, "NULL argument");
+  S->sweep = v;
+  for (int k = 0; k < S->n; ++k) S->part[k]->sweep = v;
+  return QCD_OK;
+}
+int qcd_split_get_sweep_counter(qcd_split_t* S, uint32_t* out) {
+  if (!S || !out) return fail(QCD_ERR_INVALID_ARG, "NULL argument");
+  *out = S->sweep; return QCD_OK;
+}
+int qcd_split_synchronize(qcd_split_t* S) {
+  if (!S) return fail(QCD_ERR_INVALID_ARG, "NULL argument");
+  for (int k = 0; k < S->n; ++k) { DeviceGuard dg(S->dev[k]); CUDA_TRY(cudaStreamSynchronize(S->stream[k])); }
   return QCD_OK;
 }
 

@@ -84,11 +84,12 @@ __device__ __forceinline__ void box_muller4(const Philox4& w, double* z) {
 template <int NC, int D, typename R, bool COMP>
 __global__ void __launch_bounds__(128) init_kernel(Geom g, typename LinkIO<NC, R, COMP>::Vec* links, int hot, uint32_t key0, uint32_t key1) {
   typedef LinkIO<NC, R, COMP> IO;
-  const uint32_t h = blockIdx.x * blockDim.x + threadIdx.x;
+  const uint32_t hl = blockIdx.x * blockDim.x + threadIdx.x;
   const int p = blockIdx.y;
-  if (h >= g.Vh) return;
-  const SiteCoord sc = decode_site(g, h, p);
-  const uint32_t lex = 2u * h + (uint32_t)sc.s;
+  if (hl >= g.Vh_int) return;                              // a slab initialises its own sites; the halo layers are exchanged
+  uint32_t h;
+  const SiteCoord sc = decode_launch(g, hl, p, h);
+  const uint32_t lex = lex_global(g, sc);
 #pragma unroll
   for (int mu = 0; mu < D; ++mu) {
     Cx<R> m[NC][NC];
@@ -174,12 +175,14 @@ __global__ void __launch_bounds__(LayoutShape<R>::BL) layout_kernel(Geom g, type
     __syncthreads();
   }
   if (t < nsite) {
-    const uint32_t lex = lex0 + t, h = lex >> 1;
-    const uint32_t row = fd_div(h, g.dLh0);
-    const uint32_t r2 = fd_div(row, g.dL1);
-    const uint32_t x1 = row - r2 * (uint32_t)g.L[1];
-    const uint32_t r3 = fd_div(r2, g.dL2);
-    const uint32_t x2 = r2 - r3 * (uint32_t)g.L[2], x3 = r3;
+    // lex runs over the lattice's own sites in lex order of their extents Li (a slab: its interior block)
+    const uint32_t lex = lex0 + t, hl = lex >> 1;
+    const uint32_t row = fd_div(hl, g.iLh0);
+    const uint32_t r2 = fd_div(row, g.iL1);
+    const uint32_t x1 = row - r2 * (uint32_t)g.Li[1];
+    const uint32_t r3 = fd_div(r2, g.iL2);
+    const uint32_t x2 = r2 - r3 * (uint32_t)g.Li[2], x3 = r3;
+    const uint32_t h = ((x3 * (uint32_t)g.L[2] + x2) * (uint32_t)g.L[1] + x1) * (uint32_t)g.Lh0 + (hl - row * (uint32_t)g.Lh0);
     const int p = (int)(((lex & 1u) + x1 + x2 + x3) & 1u);         // x0 & 1 = lex & 1 (L0 even)
 #pragma unroll
     for (int mu = 0; mu < D; ++mu) {
@@ -205,6 +208,42 @@ __global__ void __launch_bounds__(LayoutShape<R>::BL) layout_kernel(Geom g, type
     __syncthreads();
     for (uint32_t i = t; i < nel; i += BL) gc[i] = buf[(i / NCX) * PITCH + (i % NCX)];
   }
+}
+
+// ------------------------------------------------------------------ halo layers of a slab
+// Copy one layer (coordinate `layer` of the split direction sd) of the (parity, mu) link array: the boundary exchange of a
+// lattice divided into parts ("exchanging values of boundary sites").  One thread per half-index of the layer,
+// all NP planes.  MODE 0: lattice layer -> contiguous buffer [plane][site of the layer] (pack, for a message to another
+// process); 1: buffer -> lattice layer (unpack); 2: layer of one part -> layer of another part directly (same process; the
+// destination may be peer memory of another GPU reached over NVLink).  The half-index of a site does not depend on its
+// parity, and part extents are even, so source and destination enumerate the same sites.
+template <typename Vec, int NP, int MODE>
+__global__ void __launch_bounds__(128) halo_kernel(Geom gs, const Vec* __restrict__ src, int src_layer, Geom gd, Vec* __restrict__ dst, int dst_layer,
+                                                   int parity, int mu, int D, uint32_t count) {
+  const uint32_t idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= count) return;
+  const Geom& g = (MODE == 1) ? gd : gs;                  // the geometry that enumerates the layer (both agree off the split direction)
+  const int sd = g.sd;
+  uint32_t rest = idx / (uint32_t)g.Lh0;
+  const uint32_t j = idx - rest * (uint32_t)g.Lh0;
+  uint32_t x[4] = {0, 0, 0, 0};
+#pragma unroll
+  for (int d = 1; d < 4; ++d) {
+    if (d == sd) continue;
+    const uint32_t q = rest / (uint32_t)g.L[d];
+    x[d] = rest - q * (uint32_t)g.L[d];
+    rest = q;
+  }
+  auto half_index = [&](const Geom& gg, int layer) -> uint32_t {
+    uint32_t y[4] = {0, x[1], x[2], x[3]};
+    y[sd] = (uint32_t)layer;
+    return ((y[3] * (uint32_t)gg.L[2] + y[2]) * (uint32_t)gg.L[1] + y[1]) * (uint32_t)gg.Lh0 + j;
+  };
+  const Vec* ps = (MODE == 1) ? src + idx : src + array_base<NP>(gs, D, parity, mu) + blk_off<NP>(half_index(gs, src_layer));
+  Vec* pd = (MODE == 0) ? dst + idx : dst + array_base<NP>(gd, D, parity, mu) + blk_off<NP>(half_index(gd, dst_layer));
+  const size_t ss = (MODE == 1) ? (size_t)count : (size_t)PLANE_STRIDE, ds = (MODE == 0) ? (size_t)count : (size_t)PLANE_STRIDE;
+#pragma unroll
+  for (int k = 0; k < NP; ++k) pd[k * ds] = ps[k * ss];
 }
 
 // ------------------------------------------------------------------ reductions
@@ -280,10 +319,11 @@ __global__ void __launch_bounds__(128) plaquette_kernel(Geom g, const typename L
     h = (uint32_t)(((sc.x3 * g.L[2] + sc.x2) * g.L[1] + sc.x1) * g.Lh0 + sc.j);
     active = true;
   } else {
-    h = blockIdx.x * blockDim.x + threadIdx.x;
+    const uint32_t hl = blockIdx.x * blockDim.x + threadIdx.x;
     p = blockIdx.y;
-    active = h < g.Vh;
-    if (active) sc = decode_site(g, h, p);
+    active = hl < g.Vh_int;
+    h = 0;
+    if (active) sc = decode_launch(g, hl, p, h);
   }
   const int q = 1 - p;
   double acc[NPL];
@@ -373,17 +413,19 @@ template <int NC, int D, typename R, bool COMP>
 __global__ void __launch_bounds__(128) polyakov_kernel(Geom g, const typename LinkIO<NC, R, COMP>::Vec* __restrict__ links, double* partials) {
   typedef LinkIO<NC, R, COMP> IO;
   const uint32_t Lt = (uint32_t)g.L[D - 1];
-  const uint32_t Vs = g.V / Lt;
+  const uint32_t Vs = g.V / Lt;                            // spatial sites of the local lattice (time stride)
+  const uint32_t Vs_int = 2u * g.Vh_int / Lt;              // ... of which the lattice's own (a slab is split along a spatial direction)
   const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
   double acc[2] = {0.0, 0.0};
-  if (s < Vs) {
-    // spatial coordinates of the t = 0 site with lex index s; its parity is (x0 + x1 + x2) & 1 with x0 & 1 = s & 1
-    // (L0 even); x1, x2 decode to 0 when they are not spatial directions (D < 4), because s < Vs.
-    const uint32_t hs = s >> 1;
-    const uint32_t row = fd_div(hs, g.dLh0);
-    const uint32_t r2 = fd_div(row, g.dL1);
-    const int x1 = (int)(row - r2 * (uint32_t)g.L[1]);
+  if (s < Vs_int) {
+    // spatial coordinates of the t = 0 site with interior lex index s; its parity is (x0 + x1 + x2) & 1 with x0 & 1 = s & 1
+    // (L0 even); x1, x2 decode to 0 when they are not spatial directions (D < 4), because s < Vs_int.
+    const uint32_t hl = s >> 1;
+    const uint32_t row = fd_div(hl, g.iLh0);
+    const uint32_t r2 = fd_div(row, g.iL1);
+    const int x1 = (int)(row - r2 * (uint32_t)g.Li[1]);
     const int x2 = (D == 4) ? (int)r2 : 0;
+    const uint32_t hs = (uint32_t)((x2 * g.L[1] + x1) * g.Lh0) + (hl - row * (uint32_t)g.Lh0);
     const int par0 = ((int)(s & 1u) + x1 + x2) & 1;
     Cx<R> P[NC][NC];
 #pragma unroll

@@ -37,6 +37,18 @@ struct Geom {
   uint32_t Vh_pad;   // plane length in vectors
   uint32_t V;
   FastDiv dLh0, dL1, dL2;
+  // ---- slab of a larger lattice ("dividing lattice into parts ... exchanging values of
+  // boundary sites").  The local lattice is a part split off along direction sd (sd = -1: not a slab).  Its layers
+  // [0, n_int) of direction sd are the part's own sites (global coordinate off + layer); layer n_int holds a copy of the next
+  // part's first layer and layer n_int + 1 a copy of the previous part's last layer, so the local periodic wrap of the
+  // extent L[sd] = n_int + 2 lands on the right neighbours.  Kernels visit the interior only: the launch index runs over
+  // the extents Li[d] (= L[d], except Li[sd] = n_int).  Part extents and offsets are even, so local and global parity
+  // coincide.  The Philox counter takes the GLOBAL lex index: lex_g = x0 + x1 lexS[1] + x2 lexS[2] + x3 lexS[3] + lex0.
+  int sd;
+  int Li[4];
+  uint32_t Vh_int;   // interior sites of one parity
+  uint32_t lexS[4], lex0;
+  FastDiv iLh0, iL1, iL2;     // launch-index decoding (interior extents); equal to dLh0, dL1, dL2 when sd < 0
 };
 
 struct SiteCoord {
@@ -54,6 +66,26 @@ __device__ __forceinline__ SiteCoord decode_site(const Geom& g, uint32_t h, int 
   c.x3 = (int)r3;
   c.s = (parity + c.x1 + c.x2 + c.x3) & 1;
   return c;
+}
+
+// launch index hl in [0, Vh_int) of one parity -> site coordinates and local half-index h (h = hl unless the lattice is a slab)
+__device__ __forceinline__ SiteCoord decode_launch(const Geom& g, uint32_t hl, int parity, uint32_t& h) {
+  if (g.sd < 0) { h = hl; return decode_site(g, hl, parity); }
+  SiteCoord c;
+  uint32_t row = fd_div(hl, g.iLh0);
+  c.j = (int)(hl - row * (uint32_t)g.Lh0);
+  uint32_t r2 = fd_div(row, g.iL1);
+  c.x1 = (int)(row - r2 * (uint32_t)g.Li[1]);
+  uint32_t r3 = fd_div(r2, g.iL2);
+  c.x2 = (int)(r2 - r3 * (uint32_t)g.Li[2]);
+  c.x3 = (int)r3;
+  c.s = (parity + c.x1 + c.x2 + c.x3) & 1;
+  h = (uint32_t)(((c.x3 * g.L[2] + c.x2) * g.L[1] + c.x1) * g.Lh0 + c.j);
+  return c;
+}
+// global lex index of a site (the Philox counter word c0, reading R7): the local one unless the lattice is a slab
+__device__ __forceinline__ uint32_t lex_global(const Geom& g, const SiteCoord& c) {
+  return (uint32_t)(2 * c.j + c.s) + (uint32_t)c.x1 * g.lexS[1] + (uint32_t)c.x2 * g.lexS[2] + (uint32_t)c.x3 * g.lexS[3] + g.lex0;
 }
 
 // ------------------------------------------------------------------ CTA tile mapping

@@ -49,7 +49,8 @@ static inline TileMap choose_tile(const Geom& g, int B) {
   int lb = 0;
   while ((1 << lb) < B) ++lb;
   auto pow2_part = [](int x) { int s = 0; while (!(x & 1)) { x >>= 1; ++s; } return s; };
-  const int m[4] = {pow2_part(g.Lh0), pow2_part(g.L[1]), pow2_part(g.L[2]), pow2_part(g.L[3])};
+  // the tiles cover the sites the launch visits: the interior extents Li (= L unless the lattice is a slab)
+  const int m[4] = {pow2_part(g.Lh0), pow2_part(g.Li[1]), pow2_part(g.Li[2]), pow2_part(g.Li[3])};
   int s[4] = {m[0] < 3 ? m[0] : 3, 0, 0, 0};
   int left = lb - s[0];
   for (int d = 1; left > 0; d = d % 3 + 1) {
@@ -61,7 +62,7 @@ static inline TileMap choose_tile(const Geom& g, int B) {
   if (left > 0) s[0] += left;
   for (int d = 0; d < 4; ++d) if (s[d] > m[d]) return tm;
   tm.on = 1; tm.s0 = s[0]; tm.s1 = s[1]; tm.s2 = s[2];
-  tm.n0 = make_fastdiv((uint32_t)(g.Lh0 >> s[0])); tm.n1 = make_fastdiv((uint32_t)(g.L[1] >> s[1])); tm.n2 = make_fastdiv((uint32_t)(g.L[2] >> s[2]));
+  tm.n0 = make_fastdiv((uint32_t)(g.Lh0 >> s[0])); tm.n1 = make_fastdiv((uint32_t)(g.Li[1] >> s[1])); tm.n2 = make_fastdiv((uint32_t)(g.Li[2] >> s[2]));
   return tm;
 }
 
@@ -94,9 +95,9 @@ static cudaError_t su3_go_tiled(const Geom& g, void* links, const UpdateArgs& a,
   UpdateArgs a2 = a;
   memset(&a2.tm, 0, sizeof(a2.tm));
   a2.tm.on = 1;
-  a2.tm.n0 = make_fastdiv((uint32_t)(g.Lh0 / TD::T0)); a2.tm.n1 = make_fastdiv((uint32_t)(g.L[1] / TD::T1));
-  a2.tm.n2 = make_fastdiv((uint32_t)(g.L[2] / TD::T2));
-  return launch_pdl(kern, dim3(g.Vh / TD::B), dim3(TD::B), smem, st, g, (Vec*)links, a2);
+  a2.tm.n0 = make_fastdiv((uint32_t)(g.Lh0 / TD::T0)); a2.tm.n1 = make_fastdiv((uint32_t)(g.Li[1] / TD::T1));
+  a2.tm.n2 = make_fastdiv((uint32_t)(g.Li[2] / TD::T2));
+  return launch_pdl(kern, dim3(g.Vh_int / TD::B), dim3(TD::B), smem, st, g, (Vec*)links, a2);
 }
 
 template <typename R, int D, int MU, bool COMP, int KIND, bool FIELD, bool MEAS>
@@ -105,7 +106,7 @@ static cudaError_t su3_go(const Geom& g, void* links, const UpdateArgs& a, cudaS
   typedef typename T::Vec Vec;
   if constexpr (D == 4 && TiledCfg<R, COMP, KIND>::ON) {
     typedef typename TileFor<MU>::TD TD;
-    if (g.Lh0 % TD::T0 == 0 && g.L[1] % TD::T1 == 0 && g.L[2] % TD::T2 == 0 && g.L[3] % TD::T3 == 0)
+    if (g.Lh0 % TD::T0 == 0 && g.Li[1] % TD::T1 == 0 && g.Li[2] % TD::T2 == 0 && g.Li[3] % TD::T3 == 0)
       return su3_go_tiled<R, MU, COMP, KIND, FIELD, MEAS>(g, links, a, st);
   }
   constexpr bool ROLL = LoopCfg<R, KIND>::ROLL, PRE = LoopCfg<R, KIND>::PRE;
@@ -116,7 +117,7 @@ static cudaError_t su3_go(const Geom& g, void* links, const UpdateArgs& a, cudaS
   static std::atomic<uint64_t> done{0};
   cudaError_t e = ensure_smem(kern, smem, done);
   if (e != cudaSuccess) return e;
-  const unsigned grid = (g.Vh + B - 1) / B;
+  const unsigned grid = (g.Vh_int + B - 1) / B;
   UpdateArgs a2 = a;
   a2.tm = choose_tile(g, B);
   return launch_pdl(kern, dim3(grid), dim3(B), smem, st, g, (Vec*)links, a2);

@@ -351,14 +351,14 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
   if (a.tm.on) {
     sc = decode_site_tiled(g, a.tm, p, h);                         // the tiles cover the lattice exactly
   } else {
-    h = blockIdx.x * B + threadIdx.x;
+    uint32_t hl = blockIdx.x * B + threadIdx.x;                    // launch index over the interior (= h unless a slab)
     if constexpr (MEAS) {
-      active = h < g.Vh;                                           // a surplus thread shadows the last site: it neither
-      if (!active) h = g.Vh - 1;                                   // stores nor contributes, but stays for the shuffles
+      active = hl < g.Vh_int;                                      // a surplus thread shadows the last site: it neither
+      if (!active) hl = g.Vh_int - 1;                              // stores nor contributes, but stays for the shuffles
     } else {
-      if (h >= g.Vh) return;                                       // no block barrier anywhere below
+      if (hl >= g.Vh_int) return;                                  // no block barrier anywhere below
     }
-    sc = decode_site(g, h, p);
+    sc = decode_launch(g, hl, p, h);
   }
   int fo[D], bo[D];
 #pragma unroll
@@ -426,7 +426,7 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
     }
   };
 
-  const uint32_t lex = 2u * h + (uint32_t)sc.s;
+  const uint32_t lex = lex_global(g, sc);
   // heatbath: the random-number-only part of trial 0 and the direction of each subgroup, parked in shared memory behind
   // the ring ([subgroup][5][B] reals, this thread's column).  It does not touch the links, so it runs before pdl_wait():
   // in the tail of the previous sub-step's kernel when this CTA became resident early.
@@ -616,16 +616,16 @@ template <typename R, int D, int KIND, bool FIELD, bool MEAS>
 __global__ void __launch_bounds__(256)
 su2_update_kernel(Geom g, typename PlaneTraits<R, 4>::Vec* links, UpdateArgs a) {
   typedef PlaneTraits<R, 4> T;
-  uint32_t h = blockIdx.x * blockDim.x + threadIdx.x;
+  uint32_t hl = blockIdx.x * blockDim.x + threadIdx.x, h;  // launch index over the interior (= h unless a slab)
   bool active = true;
   if constexpr (MEAS) {
-    active = h < g.Vh;
-    if (!active) h = g.Vh - 1;                             // surplus threads stay for the warp reduction (see su3_update_kernel)
+    active = hl < g.Vh_int;
+    if (!active) hl = g.Vh_int - 1;                        // surplus threads stay for the warp reduction (see su3_update_kernel)
   } else {
-    if (h >= g.Vh) { pdl_wait(); pdl_trigger(); return; }
+    if (hl >= g.Vh_int) { pdl_wait(); pdl_trigger(); return; }
   }
   const int p = a.parity, mu = a.mu, q = 1 - p;
-  const SiteCoord sc = decode_site(g, h, p);
+  const SiteCoord sc = decode_launch(g, hl, p, h);
   int fmu, bmu;
   nbr_offsets(g, sc, mu, fmu, bmu);
   pdl_wait();
@@ -661,7 +661,7 @@ su2_update_kernel(Geom g, typename PlaneTraits<R, 4>::Vec* links, UpdateArgs a) 
   }
   const size_t own = array_base<T::NP>(g, D, p, mu);
   Q4<R> U = su2_load<R, false>(links, g, own, h);
-  const uint32_t lex = 2u * h + (uint32_t)sc.s;
+  const uint32_t lex = lex_global(g, sc);
   const Q4<R> v = q4_mul(U, A);                       // proj(W) = W itself in the quaternion algebra
   const R k2 = v.a0 * v.a0 + v.a1 * v.a1 + v.a2 * v.a2 + v.a3 * v.a3;
   int code = 0;

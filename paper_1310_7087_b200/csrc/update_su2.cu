@@ -6,7 +6,7 @@ namespace qcd {
 template <typename R, int D, int KIND, bool FIELD, bool MEAS>
 static cudaError_t go(const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st) {
   typedef typename PlaneTraits<R, 4>::Vec Vec;
-  const unsigned block = 256, grid = (g.Vh + block - 1) / block;
+  const unsigned block = 256, grid = (g.Vh_int + block - 1) / block;
   return launch_pdl(su2_update_kernel<R, D, KIND, FIELD, MEAS>, dim3(grid), dim3(block), 0, st, g, (Vec*)links, a);
 }
 template <typename R, int D, bool MEAS>

@@ -84,7 +84,7 @@ su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* 
   Vec* const own_ptr = links + (size_t)(p * D + MU) * arr;
   const Vec* const qmu_ptr = links + (size_t)((1 - p) * D + MU) * arr;
   auto at = [&](const Vec* base, int off) -> const Vec* { return base + blk_off<NP>(h + (uint32_t)off); };
-  const uint32_t lex = 2u * h + (uint32_t)s;
+  const uint32_t lex = lex_global(g, sc);
   const int lin = (int)threadIdx.x;                                          // slot of box element c
   // index of c inside the face of direction d (the d-th coordinate dropped)
   auto lin3 = [&](int d) -> int {
