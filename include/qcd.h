@@ -208,6 +208,37 @@ int qcd_split_set_sweep_counter(qcd_split_t* s, uint32_t value);
 int qcd_split_get_sweep_counter(qcd_split_t* s, uint32_t* out);
 int qcd_split_synchronize(qcd_split_t* s);
 
+/* ---------------------------------------------------------------------------------------------------------------------
+ * The O(N) scalar model on lattice sites, the paper's second workload: "In case of O(N)
+ * models the fields are set with N-vectors, which are associated with lattice sites", :108 "Improved Metropolis algorithm
+ * [7] is used for O(N) update", :134 "For O(4) model NHIT=100 tries were used to update each lattice site".  Ref [7] (the
+ * N-component lambda phi^4 model) is not available; readings R16-R19 of DESIGN.md:
+ *   action  S = sum_x [ -2 kappa sum_mu phi(x).phi(x+mu) + phi(x).phi(x) + lambda (phi(x).phi(x) - 1)^2 ]
+ *   sweep   for parity in (0, 1): every site of that parity makes nhit Metropolis tries phi' = phi + delta (2u - 1) per
+ *           component, accepted iff u' < exp(-(S(phi') - S(phi))), each from its current value, all nhit made; then the sweep
+ *           counter is incremented.  One Philox4x32-10 block per try, counter (lex site, sweep counter,
+ *           parity<<4 | try<<8 | 2<<24, 0): five 23-bit numbers, u = (k + 1/2) 2^-23.  N = 1..4, D = 2..4, extents even.
+ *   starts  QCD_COLD: phi = (1, 0, .., 0); QCD_HOT: components uniform in (-1, 1) from Philox domain 3.
+ * Canonical field layout (get/set): [lex site][component] in the lattice's precision.  Handles, memory, streams, status codes
+ * and asynchrony as for qcd_lattice_t; qcd_on_measure, qcd_on_get_counts and host transfers synchronise the stream.
+ * qcd_on_measure: phi2 = (1/V) sum phi.phi, link = (1/(V D)) sum_x sum_mu phi(x).phi(x+mu), mag[N] = (1/V) sum phi (any may be
+ * NULL).  qcd_on_get_counts: accepted and made tries since qcd_on_init.  qcd_on_half_sweep: one parity, counter unchanged.
+ * ------------------------------------------------------------------------------------------------------------------- */
+typedef struct qcd_on qcd_on_t;
+size_t qcd_on_bytes(int D, const int* dims, int N, int precision);
+int qcd_on_create(int D, const int* dims, int N, int precision, void* device_mem, size_t bytes, void* cuda_stream, qcd_on_t** out);
+int qcd_on_destroy(qcd_on_t* lat);
+int qcd_on_init(qcd_on_t* lat, int start, uint64_t seed);
+int qcd_on_sweep(qcd_on_t* lat, double kappa, double lambda, double delta, int nhit);
+int qcd_on_half_sweep(qcd_on_t* lat, int parity, double kappa, double lambda, double delta, int nhit);
+int qcd_on_measure(qcd_on_t* lat, double* phi2, double* link, double* mag);
+int qcd_on_get_counts(qcd_on_t* lat, uint64_t* accepted, uint64_t* tried);
+int qcd_on_get_field(qcd_on_t* lat, void* dst, size_t bytes, int dst_is_device);
+int qcd_on_set_field(qcd_on_t* lat, const void* src, size_t bytes, int src_is_device);
+int qcd_on_set_seed(qcd_on_t* lat, uint64_t seed);
+int qcd_on_set_sweep_counter(qcd_on_t* lat, uint32_t value);
+int qcd_on_get_sweep_counter(qcd_on_t* lat, uint32_t* out);
+
 const char* qcd_last_error(void);
 const char* qcd_version(void);
 

@@ -29,6 +29,8 @@ SYMBOLS = [
     "qcd_split_create", "qcd_split_destroy", "qcd_split_parts", "qcd_split_halo_bytes", "qcd_split_init", "qcd_split_sweep",
     "qcd_split_substep", "qcd_split_measure", "qcd_split_get_links", "qcd_split_set_links", "qcd_split_set_seed",
     "qcd_split_set_sweep_counter", "qcd_split_get_sweep_counter", "qcd_split_synchronize",
+    "qcd_on_bytes", "qcd_on_create", "qcd_on_destroy", "qcd_on_init", "qcd_on_sweep", "qcd_on_half_sweep", "qcd_on_measure",
+    "qcd_on_get_counts", "qcd_on_get_field", "qcd_on_set_field", "qcd_on_set_seed", "qcd_on_set_sweep_counter", "qcd_on_get_sweep_counter",
 ]
 
 
@@ -106,6 +108,20 @@ def lib():
     L.qcd_split_set_sweep_counter.argtypes = [p, C.c_uint32]
     L.qcd_split_get_sweep_counter.argtypes = [p, C.POINTER(C.c_uint32)]
     L.qcd_split_synchronize.argtypes = [p]
+    L.qcd_on_bytes.restype = sz
+    L.qcd_on_bytes.argtypes = [i, ip, i, i]
+    L.qcd_on_create.argtypes = [i, ip, i, i, p, sz, p, C.POINTER(p)]
+    L.qcd_on_destroy.argtypes = [p]
+    L.qcd_on_init.argtypes = [p, i, C.c_uint64]
+    L.qcd_on_sweep.argtypes = [p, d, d, d, i]
+    L.qcd_on_half_sweep.argtypes = [p, i, d, d, d, i]
+    L.qcd_on_measure.argtypes = [p, dp, dp, dp]
+    L.qcd_on_get_counts.argtypes = [p, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
+    L.qcd_on_get_field.argtypes = [p, p, sz, i]
+    L.qcd_on_set_field.argtypes = [p, p, sz, i]
+    L.qcd_on_set_seed.argtypes = [p, C.c_uint64]
+    L.qcd_on_set_sweep_counter.argtypes = [p, C.c_uint32]
+    L.qcd_on_get_sweep_counter.argtypes = [p, C.POINTER(C.c_uint32)]
     L.qcd_last_error.restype = C.c_char_p
     L.qcd_version.restype = C.c_char_p
     _lib = L
@@ -418,3 +434,84 @@ class SplitLattice:
 
     def qcd_split_synchronize(self):
         _check(lib().qcd_split_synchronize(self._h))
+
+
+class OnLattice:
+    """The O(N) scalar model on lattice sites (qcd_on_*): N-vectors, multi-hit Metropolis on the checkerboard."""
+
+    def __init__(self, dims, N, precision=QCD_FP64, device="cuda:0"):
+        import torch
+        self.dims = tuple(int(x) for x in dims)
+        self.D, self.N, self.precision = len(self.dims), int(N), int(precision)
+        self.V = int(np.prod(self.dims))
+        self._h = C.c_void_p()
+        arr = (C.c_int * self.D)(*self.dims)
+        nbytes = lib().qcd_on_bytes(self.D, arr, self.N, self.precision)
+        self._mem, mem_ptr, stream_ptr = None, None, None
+        dev = torch.device(device)
+        if nbytes:
+            with torch.cuda.device(dev):
+                self._mem = torch.empty(int(nbytes), dtype=torch.uint8, device=dev)
+                mem_ptr = self._mem.data_ptr()
+                stream_ptr = torch.cuda.current_stream().cuda_stream
+        _check(lib().qcd_on_create(self.D, arr, self.N, self.precision, mem_ptr, int(nbytes), stream_ptr, C.byref(self._h)))
+        self.np_real = np.float32 if self.precision == QCD_FP32 else np.float64
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h:
+            lib().qcd_on_destroy(self._h)
+            self._h = C.c_void_p()
+        self._mem = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    def qcd_on_init(self, start, seed):
+        _check(lib().qcd_on_init(self._h, int(start), int(seed)))
+
+    def qcd_on_sweep(self, kappa, lam, delta, nhit):
+        _check(lib().qcd_on_sweep(self._h, float(kappa), float(lam), float(delta), int(nhit)))
+
+    def qcd_on_half_sweep(self, parity, kappa, lam, delta, nhit):
+        _check(lib().qcd_on_half_sweep(self._h, int(parity), float(kappa), float(lam), float(delta), int(nhit)))
+
+    def qcd_on_measure(self):
+        p2, lk = C.c_double(0.0), C.c_double(0.0)
+        mag = (C.c_double * self.N)()
+        _check(lib().qcd_on_measure(self._h, C.byref(p2), C.byref(lk), mag))
+        return p2.value, lk.value, np.array(mag[:])
+
+    def qcd_on_get_counts(self):
+        a, t = C.c_uint64(0), C.c_uint64(0)
+        _check(lib().qcd_on_get_counts(self._h, C.byref(a), C.byref(t)))
+        return int(a.value), int(t.value)
+
+    def qcd_on_get_field(self):
+        out = np.zeros((self.V, self.N), dtype=self.np_real)
+        _check(lib().qcd_on_get_field(self._h, out.ctypes.data, out.nbytes, 0))
+        return out
+
+    def qcd_on_set_field(self, phi):
+        a = np.ascontiguousarray(phi, dtype=self.np_real)
+        assert a.shape == (self.V, self.N), a.shape
+        _check(lib().qcd_on_set_field(self._h, a.ctypes.data, a.nbytes, 0))
+
+    def qcd_on_set_seed(self, seed):
+        _check(lib().qcd_on_set_seed(self._h, int(seed)))
+
+    def qcd_on_set_sweep_counter(self, v):
+        _check(lib().qcd_on_set_sweep_counter(self._h, int(v)))
+
+    def qcd_on_get_sweep_counter(self):
+        out = C.c_uint32(0)
+        _check(lib().qcd_on_get_sweep_counter(self._h, C.byref(out)))
+        return out.value

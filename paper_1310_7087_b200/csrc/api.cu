@@ -19,6 +19,10 @@ namespace {
 
 thread_local std::string g_err;
 int fail(int code, const std::string& msg) { g_err = msg; return code; }
+}  // namespace
+// the other translation units of the library (on_model.cu) report errors through the same thread-local message
+namespace qcd { int set_error(int code, const std::string& msg) { return fail(code, msg); } }
+namespace {
 #define CUDA_TRY(expr)                                                                                   \
   do {                                                                                                   \
     cudaError_t e_ = (expr);                                                                             \
@@ -879,12 +883,6 @@ struct HaloOp {
     return QCD_OK;
   }
 };
-
-bool same_format(const qcd_lattice* a, const qcd_lattice* b) {
-  if (a->D != b->D || a->Nc != b->Nc || a->precision != b->precision || a->comp != b->comp || a->g.sd != b->g.sd) return false;
-  for (int d = 0; d < a->D; ++d) if (d != a->g.sd && a->dims[d] != b->dims[d]) return false;
-  return true;
-}
 
 struct DeviceGuard {
   int prev;

@@ -1,0 +1,181 @@
+"""GPU-vs-oracle parity of the O(N) model (qcd_on_*) through the C ABI, and the GPU sampler against the
+closed forms that pin the oracle (decoupled sites, free field).  Tolerances: fp64 field 1e-12 per half sweep with identical
+accept/reject decisions; fp32 2e-5 with decision disagreements reported and at most 1e-6 of the tries (the fp32 kernel takes
+a try's decision in double inside a guard band, from the same float-valued operands the fp32-shadow oracle uses)."""
+import numpy as np
+import pytest
+from scipy import integrate
+
+from oracle import on
+
+pytestmark = pytest.mark.gpu
+
+CASES = [((4, 6), 1), ((8, 8), 2), ((6, 4, 10), 3), ((6, 4, 10, 2), 4), ((2, 2, 2, 2), 4), ((16, 8, 8, 4), 4), ((12, 6, 4, 8), 2)]
+
+
+def _oracle(dims, N, prec):
+    O = on.OnOracle(dims, N)
+    if prec == 0:
+        O.set_fp32_shadow(True)
+    return O
+
+
+@pytest.mark.parametrize("prec", [1, 0], ids=["f64", "f32"])
+@pytest.mark.parametrize("dims,N", CASES)
+def test_starts_roundtrip_and_measure(qcd, prec, dims, N):
+    O = _oracle(dims, N, prec)
+    with qcd.OnLattice(dims, N, prec) as G:
+        G.qcd_on_init(qcd.QCD_COLD, 1)
+        O.init(on.COLD, 1)
+        assert np.array_equal(G.qcd_on_get_field(), O.get_field())
+        p2, lk, mag = G.qcd_on_measure()
+        assert p2 == 1.0 and lk == 1.0 and mag[0] == 1.0 and not mag[1:].any()
+        G.qcd_on_init(qcd.QCD_HOT, 42)
+        O.init(on.HOT, 42)
+        assert np.array_equal(G.qcd_on_get_field().astype(np.float64), O.get_field())   # exactly representable numbers
+        rng = np.random.default_rng(2)
+        phi = rng.uniform(-1.5, 1.5, size=(O.V, N))
+        if prec == 0:
+            phi = phi.astype(np.float32).astype(np.float64)
+        G.qcd_on_set_field(phi)
+        O.set_field(phi)
+        assert np.array_equal(G.qcd_on_get_field().astype(np.float64), phi)
+        a, b = G.qcd_on_measure(), O.measure()
+        tol = 1e-12 if prec == 1 else 1e-6
+        assert abs(a[0] - b[0]) < tol and abs(a[1] - b[1]) < tol and np.max(np.abs(a[2] - b[2])) < tol
+        again = G.qcd_on_measure()
+        assert again[0] == a[0] and again[1] == a[1] and np.array_equal(again[2], a[2])
+
+
+@pytest.mark.parametrize("prec", [1, 0], ids=["f64", "f32"])
+@pytest.mark.parametrize("dims,N", CASES)
+def test_half_sweeps_match_the_oracle(qcd, prec, dims, N):
+    kappa, lam, delta, nhit = 0.12, 0.6, 0.75, 12
+    O = _oracle(dims, N, prec)
+    rng = np.random.default_rng(5)
+    phi = rng.uniform(-1.2, 1.2, size=(O.V, N))
+    if prec == 0:
+        phi = phi.astype(np.float32).astype(np.float64)
+    tries, flips, worst = 0, 0, 0.0
+    with qcd.OnLattice(dims, N, prec) as G:
+        for sweep_ctr, parity in [(0, 0), (0, 1), (9, 1), (9, 0)]:
+            G.qcd_on_init(qcd.QCD_COLD, 31)                            # resets the counters; the seed is 31
+            G.qcd_on_set_field(phi)
+            G.qcd_on_set_sweep_counter(sweep_ctr)
+            O.init(on.COLD, 31)
+            O.set_field(phi)
+            O.sweep_counter = sweep_ctr
+            G.qcd_on_half_sweep(parity, kappa, lam, delta, nhit)
+            O.half_sweep(parity, kappa, lam, delta, nhit)
+            got, ref = G.qcd_on_get_field().astype(np.float64), O.get_field()
+            diff = np.max(np.abs(got - ref), axis=1)
+            acc_g, tried_g = G.qcd_on_get_counts()
+            acc_o, tried_o = O.counts()
+            assert tried_g == tried_o == (O.V // 2) * nhit
+            tries += tried_g
+            if prec == 1:
+                assert acc_g == acc_o
+                assert diff.max() < 1e-12, diff.max()
+            else:
+                bad = diff > 2e-5                                      # a disagreeing decision moves a site by O(delta)
+                flips += int(bad.sum())
+                worst = max(worst, float(diff[~bad].max()))
+            par = np.stack(np.unravel_index(np.arange(O.V), dims[::-1]), axis=-1).sum(1) & 1
+            assert np.array_equal(got[par != parity], phi[par != parity])
+    if prec == 0:
+        print("fp32 O(N) half sweeps: %d disagreeing sites in %d tries, worst other diff %.2e" % (flips, tries, worst))
+        assert flips <= max(0, int(1e-6 * tries)), (flips, tries)
+
+
+def test_o4_full_size_half_sweep_nhit100(qcd):
+    """the paper's O(4) workload (Table 1: O(4) 32^4, NHIT = 100) at full size: one half sweep, every site
+    against the oracle (fp64), from the hot start"""
+    dims, N = (32, 32, 32, 32), 4
+    O = on.OnOracle(dims, N)
+    O.init(on.HOT, 2013)
+    with qcd.OnLattice(dims, N, 1) as G:
+        G.qcd_on_init(qcd.QCD_HOT, 2013)
+        assert np.array_equal(G.qcd_on_get_field(), O.get_field())
+        G.qcd_on_half_sweep(0, 0.15, 0.5, 0.5, 100)
+        O.half_sweep(0, 0.15, 0.5, 0.5, 100)
+        assert np.max(np.abs(G.qcd_on_get_field() - O.get_field())) < 1e-12
+        assert G.qcd_on_get_counts() == O.counts()
+        a, b = G.qcd_on_measure(), O.measure()
+        assert abs(a[0] - b[0]) < 1e-12 and abs(a[1] - b[1]) < 1e-12 and np.max(np.abs(a[2] - b[2])) < 1e-12
+
+
+@pytest.mark.parametrize("prec", [1, 0], ids=["f64", "f32"])
+@pytest.mark.parametrize("N,lam", [(1, 0.0), (4, 0.5), (3, 10.0)])
+def test_gpu_sampler_decoupled_sites_against_radial_quadrature(qcd, prec, N, lam):
+    w = lambda r: r ** (N - 1) * np.exp(-r * r - lam * (r * r - 1.0) ** 2)
+    exact = integrate.quad(lambda r: r * r * w(r), 0, np.inf)[0] / integrate.quad(w, 0, np.inf)[0]
+    dims = (16, 16, 16)
+    with qcd.OnLattice(dims, N, prec) as G:
+        G.qcd_on_init(qcd.QCD_HOT, 11)
+        per_site = 0.0
+        n = 0
+        for s in range(70):
+            G.qcd_on_sweep(0.0, lam, 1.0 if lam < 5 else 0.4, 10)
+            if s >= 10:
+                per_site = per_site + (G.qcd_on_get_field().astype(np.float64) ** 2).sum(1)
+                n += 1
+        x = per_site / n                                   # independent sites: one time average each
+        assert abs(x.mean() - exact) < 4.5 * x.std(ddof=1) / np.sqrt(len(x)), (x.mean(), exact)
+
+
+@pytest.mark.parametrize("prec", [1, 0], ids=["f64", "f32"])
+def test_gpu_sampler_free_field_against_the_lattice_propagator(qcd, prec):
+    dims, N, kappa = (8, 8, 8, 8), 4, 0.1
+    D = len(dims)
+    grids = np.meshgrid(*[2 * np.pi * np.arange(L) / L for L in dims], indexing="ij")
+    csum = sum(np.cos(g) for g in grids)
+    denom = 2.0 * (1.0 - 2.0 * kappa * csum)
+    V = int(np.prod(dims))
+    phi2_exact, link_exact = N * np.sum(1.0 / denom) / V, N * np.sum(csum / D / denom) / V
+    with qcd.OnLattice(dims, N, prec) as G:
+        G.qcd_on_init(qcd.QCD_HOT, 5)
+        p2, lk = [], []
+        for s in range(900):
+            G.qcd_on_sweep(kappa, 0.0, 1.2, 4)
+            if s >= 100:
+                a, b, _ = G.qcd_on_measure()
+                p2.append(a)
+                lk.append(b)
+        acc, tried = G.qcd_on_get_counts()
+        assert tried == 900 * V * 4 and 0.2 < acc / tried < 0.8
+
+    def err(x, nb=20):
+        b = np.asarray(x)[: len(x) // nb * nb].reshape(nb, -1).mean(1)
+        return b.std(ddof=1) / np.sqrt(nb)
+
+    assert abs(np.mean(p2) - phi2_exact) < 4.5 * err(p2), (np.mean(p2), phi2_exact, err(p2))
+    assert abs(np.mean(lk) - link_exact) < 4.5 * err(lk), (np.mean(lk), link_exact, err(lk))
+
+
+def test_on_resume_and_errors(qcd):
+    dims, N = (8, 8, 4, 4), 4
+    with qcd.OnLattice(dims, N, 1) as A, qcd.OnLattice(dims, N, 1) as B, qcd.OnLattice(dims, N, 1) as C2:
+        A.qcd_on_init(qcd.QCD_HOT, 8)
+        B.qcd_on_init(qcd.QCD_HOT, 8)
+        for _ in range(4):
+            A.qcd_on_sweep(0.12, 0.5, 0.6, 5)
+        for _ in range(2):
+            B.qcd_on_sweep(0.12, 0.5, 0.6, 5)
+        C2.qcd_on_set_field(B.qcd_on_get_field())
+        C2.qcd_on_set_seed(8)
+        C2.qcd_on_set_sweep_counter(B.qcd_on_get_sweep_counter())
+        for _ in range(2):
+            C2.qcd_on_sweep(0.12, 0.5, 0.6, 5)
+        assert np.array_equal(A.qcd_on_get_field(), C2.qcd_on_get_field()) and A.qcd_on_get_sweep_counter() == 4
+        with pytest.raises(qcd.QcdError) as e:
+            A.qcd_on_sweep(0.1, -1.0, 0.5, 5)
+        assert e.value.code == qcd.QCD_ERR_INVALID_ARG
+        with pytest.raises(qcd.QcdError):
+            A.qcd_on_sweep(0.1, 0.5, 0.0, 5)
+    with pytest.raises(qcd.QcdError) as e:
+        qcd.OnLattice((8, 8), 5, 1)
+    assert e.value.code == qcd.QCD_ERR_INVALID_ARG
+    with qcd.OnLattice((4, 4), 2, 0) as G:
+        with pytest.raises(qcd.QcdError) as e:
+            G.qcd_on_sweep(0.1, 0.5, 0.5, 5)
+        assert e.value.code == qcd.QCD_ERR_STATE

@@ -957,7 +957,10 @@ def test_largest_lattice_of_one_b200_128to4_fp64(qcd):
     """SU(3) 128^4 in fp64 x18: 154.6 GB of links, the largest lattice one B200 holds (no slab streaming
     needed below this size).  Each (parity, direction) array has 1.2e9 vectors (32-bit in-array offsets), the array bases are
     64-bit.  Checked by what holds at any size, like the fp32 case above; skipped when the device has less free memory."""
+    import gc
     import torch
+    gc.collect()
+    torch.cuda.empty_cache()                                     # blocks cached by earlier tests count as used otherwise
     free, _ = torch.cuda.mem_get_info()
     need = 4 * 128 ** 4 * 144
     if free < need + (4 << 30):
