@@ -226,6 +226,45 @@ def time_arm(q, torch, prec_name, steps, warmup, therm, seed, dist, sampler):
     return out
 
 
+def time_on_model(q, torch, dist, sampler, with_oracle):
+    """The paper's second workload beside the headline (Table 1): O(4) on 32^4, NHIT = 100
+    tries per site visit, hot start; one step = qcd_on_sweep + qcd_on_measure (a "working sweep").  Instruction-bound."""
+    dims, N, kappa, lam, delta, nhit = DIMS, 4, 0.15, 0.5, 0.5, 100
+    V = 1
+    for d in dims:
+        V *= d
+    out = {"workload": "O(4) phi^4 model 32^4, kappa 0.15, lambda 0.5, delta 0.5, NHIT 100, hot start (readings R16-R19)",
+           "paper_context": "PAPER.md Table 1: O(4) 32^4 working sweep 0.72 s (single) / 0.99 s (double) on a GeForce GTX 560 Ti"}
+    for name, prec in (("f32", q.QCD_FP32), ("f64", q.QCD_FP64)):
+        with q.OnLattice(dims, N, prec, device=torch.device("cuda", torch.cuda.current_device())) as G:
+            G.qcd_on_init(q.QCD_HOT, SEED)
+            state = {}
+
+            def step():
+                G.qcd_on_sweep(kappa, lam, delta, nhit)
+                state["obs"] = G.qcd_on_measure()
+
+            for _ in range(5):
+                step()
+            st = rep_stats(timed_reps(torch, dist, sampler, step, 10, min_total_ms=100.0), 10)
+            acc, tried = G.qcd_on_get_counts()
+            # issue floor: instructions per try x tries / (148 SMs x 4 schedulers x 32 lanes) is not known a priori; report the rate
+            out[name] = {"ms_per_sweep": st["median_ms_per_step"], "reps": st, "site_visits_per_s": V / (st["median_ms_per_step"] * 1e-3),
+                         "tries_per_s": V * nhit / (st["median_ms_per_step"] * 1e-3), "acceptance": acc / max(tried, 1),
+                         "phi2": state["obs"][0], "link": state["obs"][1]}
+    if with_oracle:
+        from oracle import on
+        small = (16, 16, 16, 16)
+        O = on.OnOracle(small, N)
+        O.init(on.HOT, SEED)
+        t0 = time.time()
+        O.sweep(kappa, lam, delta, nhit)
+        dt = time.time() - t0
+        out["cpu_baseline"] = {"value": 16 ** 4 / dt, "unit": "site visits/s", "cores": on.num_threads(), "kind": "oracle",
+                               "sample": "one sweep of the same model on 16^4 (%.2f s)" % dt}
+    return out
+
+
 def replica_seed(rank):
     """every rank runs an independent lattice of the same workload: same recipe, its own Philox seed"""
     return SEED + rank
@@ -298,6 +337,7 @@ def run_ours(args):
     arms = {}
     for name in (primary, other):
         arms[name] = time_arm(q, torch, name, args.steps, args.warmup, args.therm, replica_seed(rank), dist, sampler)
+    on_model = time_on_model(q, torch, dist, sampler, with_oracle=(world == 1 and rank == 0 and not args.no_cpu_baseline))
     clocks = sampler.stop()
     line = None
     if rank == 0:
@@ -333,7 +373,7 @@ def run_ours(args):
                 "update_only_sweep": p["update_only_sweep"], "accumulate_on_device": p["accumulate_on_device"],
                 "qcd_sweep_then_qcd_measure": p["qcd_sweep_then_qcd_measure"],
                 "observables": {"plaquette": p["plaquette"], "polyakov_abs": p["polyakov_abs"]},
-                "other_precision": frag[other]}
+                "other_precision": frag[other], "on_model": on_model}
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline_sample()
     if dist is not None:
