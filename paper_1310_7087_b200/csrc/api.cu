@@ -48,7 +48,7 @@ struct qcd_lattice {
   uint32_t sweep;
   bool has_links;
   int max_trials;
-  bool debug_trials, profile;
+  bool debug_trials, profile, bulk_copy;
   uint8_t* d_trials;
   // per-block / per-warp partial sums of the reductions, one allocation of three regions (sizes fixed by the geometry):
   // [fused plaquette: NPL x np_warp][plaquette kernel: NPL x nb_plaq][Polyakov: 2 x nb_poly]
@@ -185,7 +185,7 @@ int prof_end(qcd_lattice* L, EventPair* ep, int n) {
 // bracket: time this single launch with its own event pair (qcd_debug_substep); qcd_sweep brackets whole passes instead
 // sizes of the three regions of d_partials
 struct MeasLayout {
-  uint32_t npl, np_warp, nb_plaq, nb_poly;
+  uint32_t npl, np_warp, nb_plaq, nb_poly, poly_seg;
   bool boxed;
   size_t off_plaq, off_poly, need;
 };
@@ -198,7 +198,9 @@ MeasLayout meas_layout(const qcd_lattice* L) {
   m.np_warp = g.Vh_pad / 32u + 8u;
   m.boxed = (L->D == 4 && g.Lh0 % 8 == 0 && g.Li[1] % 2 == 0 && g.Li[2] % 2 == 0 && g.Li[3] % 2 == 0);
   m.nb_plaq = m.boxed ? 2u * g.Vh_int / 128u : ((g.Vh_int + 127u) / 128u) * 2u;
-  m.nb_poly = (2u * g.Vh_int / (uint32_t)g.L[L->D - 1] + 127u) / 128u;
+  // Polyakov kernel: SEG lanes per spatial site, SEG = the largest of 4, 2, 1 that divides Lt
+  m.poly_seg = (g.L[L->D - 1] % 4 == 0) ? 4u : (g.L[L->D - 1] % 2 == 0) ? 2u : 1u;
+  m.nb_poly = (2u * g.Vh_int / (uint32_t)g.L[L->D - 1] * m.poly_seg + 127u) / 128u;
   m.off_plaq = (size_t)m.npl * m.np_warp;
   m.off_poly = m.off_plaq + (size_t)m.npl * m.nb_plaq;
   m.need = m.off_poly + 2 * (size_t)m.nb_poly;
@@ -228,6 +230,7 @@ int substep(qcd_lattice* L, double beta, int kind, int hit, int parity, int mu, 
   a.beta = beta; a.inv_c = (double)L->Nc / (2.0 * beta); a.parity = parity; a.mu = mu; a.hit = hit; a.max_trials = L->max_trials;
   a.sweep = L->sweep; a.key0 = (uint32_t)(L->seed & 0xFFFFFFFFull); a.key1 = (uint32_t)(L->seed >> 32);
   a.trials = trials;
+  a.use_bulk = L->bulk_copy ? 1 : 0;
   a.f = make_field_args(f, field_on, L->Nc);
   EventPair ep;
   const bool prof = L->profile && bracket;
@@ -333,7 +336,9 @@ struct MeasureOp {
     }
     if (want_poly) {
       cudaStream_t ps = fork ? L->side : L->stream;
-      polyakov_kernel<NC, D, R, COMP><<<m.nb_poly, 128, 0, ps>>>(L->g, (const Vec*)L->mem, pq);
+      if (m.poly_seg == 4) polyakov_kernel<NC, D, R, COMP, 4><<<m.nb_poly, 128, 0, ps>>>(L->g, (const Vec*)L->mem, pq);
+      else if (m.poly_seg == 2) polyakov_kernel<NC, D, R, COMP, 2><<<m.nb_poly, 128, 0, ps>>>(L->g, (const Vec*)L->mem, pq);
+      else polyakov_kernel<NC, D, R, COMP, 1><<<m.nb_poly, 128, 0, ps>>>(L->g, (const Vec*)L->mem, pq);
       final_reduce_kernel<<<2, 256, 0, ps>>>(pq, m.nb_poly, L->d_results + 8, poly_scale);
       L->launches += 2;
       if (fork) CUDA_TRY(cudaEventRecord(L->ev_join, L->side));
@@ -426,7 +431,7 @@ static int create_lattice(int D, const int* dims, int Nc, int precision, unsigne
   L->bytes = need; L->mem = device_mem; L->owns_mem = false;
   L->stream = (cudaStream_t)cuda_stream;
   L->seed = 0; L->sweep = 0; L->has_links = false; L->max_trials = 10;
-  L->debug_trials = false; L->profile = false;
+  L->debug_trials = false; L->profile = false; L->bulk_copy = false;
   L->d_trials = nullptr; L->d_partials = nullptr; L->partials_cap = 0; L->d_results = nullptr; L->h_results = nullptr;
   L->prof_ms[0] = L->prof_ms[1] = 0.0; L->prof_n[0] = L->prof_n[1] = 0; L->launches = 0; L->last_parity = L->last_mu = -2; L->d_canon = nullptr;
   L->side = nullptr; L->ev_fork = nullptr; L->ev_join = nullptr;
@@ -758,6 +763,7 @@ int qcd_set_option(qcd_lattice_t* L, int key, int value) {
       L->max_trials = value; return QCD_OK;
     case QCD_OPT_DEBUG_TRIALS: L->debug_trials = value != 0; return QCD_OK;
     case QCD_OPT_PROFILE: L->profile = value != 0; return QCD_OK;
+    case QCD_OPT_BULK_COPY: L->bulk_copy = value != 0; return QCD_OK;
   }
   return fail(QCD_ERR_INVALID_ARG, "unknown option key");
 }

@@ -408,16 +408,32 @@ __global__ void __launch_bounds__(128) plaquette_kernel(Geom g, const typename L
   block_reduce_store<NPL, 128>(acc, partials, gridDim.x * gridDim.y, blockIdx.y * gridDim.x + blockIdx.x);
 }
 
-// Polyakov loop: one thread per spatial site, ordered product over t of U_{D-1}
-template <int NC, int D, typename R, bool COMP>
+// Polyakov loop: ordered product over t of U_{D-1}.  SEG lanes per spatial site: lane g multiplies the links of the time
+// segment [g Lt/SEG, (g+1) Lt/SEG) -- the kernel is bound by the latency of its dependent loads, and the segments' loads are
+// independent -- then the SEG partial products are combined in order by shuffles (P0 P1)(P2 P3).  SEG = 1: one thread per
+// spatial site walks all of Lt.  SEG must divide Lt and 32.
+template <int NC, typename R> __device__ __forceinline__ void mat_shfl_down(Cx<R> (&dst)[NC][NC], const Cx<R> (&src)[NC][NC], int delta) {
+#pragma unroll
+  for (int i = 0; i < NC; ++i)
+#pragma unroll
+    for (int j = 0; j < NC; ++j) {
+      dst[i][j].re = __shfl_down_sync(0xffffffffu, src[i][j].re, delta);
+      dst[i][j].im = __shfl_down_sync(0xffffffffu, src[i][j].im, delta);
+    }
+}
+template <int NC, int D, typename R, bool COMP, int SEG>
 __global__ void __launch_bounds__(128) polyakov_kernel(Geom g, const typename LinkIO<NC, R, COMP>::Vec* __restrict__ links, double* partials) {
   typedef LinkIO<NC, R, COMP> IO;
   const uint32_t Lt = (uint32_t)g.L[D - 1];
   const uint32_t Vs = g.V / Lt;                            // spatial sites of the local lattice (time stride)
   const uint32_t Vs_int = 2u * g.Vh_int / Lt;              // ... of which the lattice's own (a slab is split along a spatial direction)
-  const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
+  const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x;
+  const uint32_t seg = tid % SEG;
+  const uint32_t s_raw = tid / SEG;
+  const bool live = s_raw < Vs_int;
+  const uint32_t s = live ? s_raw : Vs_int - 1;            // surplus lanes shadow the last site (whole warps do the shuffles)
   double acc[2] = {0.0, 0.0};
-  if (s < Vs_int) {
+  {
     // spatial coordinates of the t = 0 site with interior lex index s; its parity is (x0 + x1 + x2) & 1 with x0 & 1 = s & 1
     // (L0 even); x1, x2 decode to 0 when they are not spatial directions (D < 4), because s < Vs_int.
     const uint32_t hl = s >> 1;
@@ -432,7 +448,8 @@ __global__ void __launch_bounds__(128) polyakov_kernel(Geom g, const typename Li
     for (int i = 0; i < NC; ++i)
 #pragma unroll
       for (int j = 0; j < NC; ++j) P[i][j] = cx<R>(i == j ? R(1) : R(0), R(0));
-    for (uint32_t t = 0; t < Lt; ++t) {
+    const uint32_t nt = Lt / SEG, t0 = seg * nt;
+    for (uint32_t t = t0; t < t0 + nt; ++t) {
       const int p = (par0 + (int)t) & 1;
       const uint32_t h = hs + t * (Vs >> 1);
       Cx<R> u[NC][NC], n[NC][NC];
@@ -443,8 +460,21 @@ __global__ void __launch_bounds__(128) polyakov_kernel(Geom g, const typename Li
 #pragma unroll
         for (int j = 0; j < NC; ++j) P[i][j] = n[i][j];
     }
+    // combine the segments in time order: lanes seg, seg + delta hold consecutive runs of segments
 #pragma unroll
-    for (int i = 0; i < NC; ++i) { acc[0] += (double)P[i][i].re; acc[1] += (double)P[i][i].im; }
+    for (int delta = 1; delta < SEG; delta <<= 1) {
+      Cx<R> o[NC][NC], n[NC][NC];
+      mat_shfl_down<NC, R>(o, P, delta);
+      mm_nn<NC, R>(n, P, o);
+#pragma unroll
+      for (int i = 0; i < NC; ++i)
+#pragma unroll
+        for (int j = 0; j < NC; ++j) P[i][j] = n[i][j];
+    }
+    if (live && seg == 0) {
+#pragma unroll
+      for (int i = 0; i < NC; ++i) { acc[0] += (double)P[i][i].re; acc[1] += (double)P[i][i].im; }
+    }
   }
   block_reduce_store<2, 128>(acc, partials, gridDim.x, blockIdx.x);
 }

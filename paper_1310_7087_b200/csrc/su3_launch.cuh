@@ -6,7 +6,7 @@
 #include <cstring>
 
 #include "launch.h"
-#include "update_tiled.cuh"
+#include "update_bulk.cuh"
 
 namespace qcd {
 
@@ -21,6 +21,15 @@ template <> struct TileFor<3> { typedef TileDims<8, 4, 4, 1> TD; };
 // the occupancy the region costs than they gain from the lighter L2 traffic.  K ring slots, MINB CTAs per SM.
 template <typename R, bool COMP, int KIND> struct TiledCfg { static constexpr bool ON = false; static constexpr int K = 2, MINB = 1; };
 template <> struct TiledCfg<float, true, 1> { static constexpr bool ON = true; static constexpr int K = 5, MINB = 4; };
+
+// ---- bulk-copy kernel (update_bulk.cuh), D = 4, L0 = 32, fp32 x12 overrelaxation without field: producer warp + mbarriers.
+// Instantiated, but run only on request (QCD_OPT_BULK_COPY): it is slower than the tiled kernel (DESIGN.md sec 6.10,
+// profiles/r2_bulk_copy.md) and is kept so that the measurement can be repeated.
+template <typename R, bool COMP, int KIND, bool FIELD, bool MEAS> struct BulkCfg { static constexpr bool ON = false; static constexpr int K = 5, MINB = 4; };
+template <> struct BulkCfg<float, true, 1, false, false> { static constexpr bool ON = true; static constexpr int K = 5, MINB = 4; };
+// boxes of the bulk kernel: the full x0 row (16 half-indices: L0 = 32) x 8 rows, thin in mu where that keeps T1 = 4
+template <int MU> struct BulkTileFor { typedef TileDims<16, 4, 2, 1> TD; };
+template <> struct BulkTileFor<2> { typedef TileDims<16, 4, 1, 2> TD; };
 
 // ---- ring kernel (update.cuh): B threads per CTA, K link slots per thread (K-1 links in flight; K = 0: direct global
 // loads), MINB = second __launch_bounds__ argument.  Shared memory per CTA = K * (bytes per link) * B.
@@ -100,10 +109,37 @@ static cudaError_t su3_go_tiled(const Geom& g, void* links, const UpdateArgs& a,
   return launch_pdl(kern, dim3(g.Vh_int / TD::B), dim3(TD::B), smem, st, g, (Vec*)links, a2);
 }
 
+template <typename R, int MU, bool COMP, int KIND, bool FIELD>
+static cudaError_t su3_go_bulk(const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st) {
+  typedef PlaneTraits<R, (COMP ? 12 : 18)> T;
+  typedef typename T::Vec Vec;
+  typedef typename BulkTileFor<MU>::TD TD;
+  constexpr int K = BulkCfg<R, COMP, KIND, FIELD, false>::K, MINB = BulkCfg<R, COMP, KIND, FIELD, false>::MINB;
+  constexpr int ROWS = TD::B / TD::T0, ROWV = T::NP * TD::T0;
+  constexpr int RROWS = ROWS + (MU != 1 ? 2 * (ROWS / TD::T1) : 0) + (MU != 2 ? 2 * (ROWS / TD::T2) : 0) + (MU != 3 ? 2 * (ROWS / TD::T3) : 0);
+  constexpr size_t smem = (size_t)(RROWS * ROWV + K * ROWS * ROWV) * sizeof(Vec) + (2 * K + 1) * 8;
+  auto kern = su3_update_bulk_kernel<R, MU, COMP, KIND, FIELD, TD, K, MINB>;
+  static std::atomic<uint64_t> done{0};
+  cudaError_t e = ensure_smem(kern, smem, done);
+  if (e != cudaSuccess) return e;
+  UpdateArgs a2 = a;
+  memset(&a2.tm, 0, sizeof(a2.tm));
+  a2.tm.on = 1;
+  a2.tm.n0 = make_fastdiv(1u); a2.tm.n1 = make_fastdiv((uint32_t)(g.Li[1] / TD::T1));
+  a2.tm.n2 = make_fastdiv((uint32_t)(g.Li[2] / TD::T2));
+  return launch_pdl(kern, dim3(g.Vh_int / TD::B), dim3(TD::B + 32), smem, st, g, (Vec*)links, a2);
+}
+
 template <typename R, int D, int MU, bool COMP, int KIND, bool FIELD, bool MEAS>
 static cudaError_t su3_go(const Geom& g, void* links, const UpdateArgs& a, cudaStream_t st) {
   typedef PlaneTraits<R, (COMP ? 12 : 18)> T;
   typedef typename T::Vec Vec;
+  if constexpr (D == 4 && BulkCfg<R, COMP, KIND, FIELD, MEAS>::ON) {
+    typedef typename BulkTileFor<MU>::TD TD;
+    // the box spans the whole x0 row (L0 = 32); a slab's halo layers are not visited: plain lattices only
+    if (a.use_bulk && g.sd < 0 && g.Lh0 == TD::T0 && g.L[1] % TD::T1 == 0 && g.L[2] % TD::T2 == 0 && g.L[3] % TD::T3 == 0)
+      return su3_go_bulk<R, MU, COMP, KIND, FIELD>(g, links, a, st);
+  }
   if constexpr (D == 4 && TiledCfg<R, COMP, KIND>::ON) {
     typedef typename TileFor<MU>::TD TD;
     if (g.Lh0 % TD::T0 == 0 && g.Li[1] % TD::T1 == 0 && g.Li[2] % TD::T2 == 0 && g.Li[3] % TD::T3 == 0)

@@ -40,6 +40,7 @@ struct UpdateArgs {
   uint32_t meas_stride;
   int meas_plane[3];
   TileMap tm;        // thread -> site mapping of the SU(3) kernels (set by the launcher)
+  int use_bulk;      // host side only: QCD_OPT_BULK_COPY (update_bulk.cuh instead of the tiled kernel where it applies)
   FieldArgs f;
 };
 

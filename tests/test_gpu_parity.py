@@ -479,6 +479,32 @@ def test_sweep_measure_with_no_pass_measures_the_unchanged_configuration(qcd):
         assert np.array_equal(G.qcd_get_links(), links)
 
 
+def test_bulk_copy_overrelaxation_kernel_matches_the_oracle(qcd):
+    """QCD_OPT_BULK_COPY: the kernel that stages every operand with cp.async.bulk + mbarriers (update_bulk.cuh; slower,
+    kept for the measurement of DESIGN.md sec 6.10) on lattices with dims[0] = 32: every (parity, mu) overrelaxation
+    sub-step against the oracle, boxes that wrap onto themselves and several boxes per direction, and after qcd_set_links
+    (no early fetch) as well as back to back"""
+    for dims in [(32, 4, 2, 2), (32, 8, 4, 4), (32, 4, 6, 2)]:
+        links = prep_links(dims, 3, 0, seed=61, spread=0.35)
+        with gpu_lattice(qcd, dims, 3, 0, 1) as G:
+            G.qcd_set_option(qcd.QCD_OPT_BULK_COPY, 1)
+            worst = 0.0
+            for parity in (0, 1):
+                for mu in range(4):
+                    O = oracle_lattice(dims, 3, 0, links)
+                    O.substep(5.7, oracle.KIND_OR, 0, parity, mu)
+                    G.qcd_set_links(links)
+                    G.qcd_debug_substep(5.7, qcd.QCD_KIND_OR, 0, parity, mu)
+                    worst = max(worst, float(np.max(np.abs(G.qcd_get_links().astype(np.complex128) - O.get_links()))))
+            assert worst < TOL[0], (dims, worst)
+            O = oracle_lattice(dims, 3, 0, links)
+            G.qcd_set_links(links)
+            for parity, mu in [(0, 1), (1, 1), (1, 0), (0, 0), (0, 3), (1, 2), (0, 2), (1, 3)]:
+                O.substep(5.7, oracle.KIND_OR, 0, parity, mu)
+                G.qcd_debug_substep(5.7, qcd.QCD_KIND_OR, 0, parity, mu)
+            assert float(np.max(np.abs(G.qcd_get_links().astype(np.complex128) - O.get_links()))) < unresynced_bar(0, 8, 3.5)
+
+
 def test_overrelaxation_conserves_action_on_gpu(qcd):
     dims = (8, 8, 8, 8)
     for Nc, prec, flags, tol in [(3, 1, 0, 1e-12), (3, 0, 1, 3e-6), (2, 1, 0, 1e-12)]:
