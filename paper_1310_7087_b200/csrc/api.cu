@@ -229,6 +229,7 @@ int substep(qcd_lattice* L, double beta, int kind, int hit, int parity, int mu, 
   }
   a.beta = beta; a.inv_c = (double)L->Nc / (2.0 * beta); a.parity = parity; a.mu = mu; a.hit = hit; a.max_trials = L->max_trials;
   a.sweep = L->sweep; a.key0 = (uint32_t)(L->seed & 0xFFFFFFFFull); a.key1 = (uint32_t)(L->seed >> 32);
+  a.rk = philox_round_keys(a.key0, a.key1);
   a.trials = trials;
   a.use_bulk = L->bulk_copy ? 1 : 0;
   a.f = make_field_args(f, field_on, L->Nc);

@@ -13,6 +13,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "hb_math.cuh"
+
 namespace qcd {
 
 // ------------------------------------------------------------------ division by run-time constants
@@ -205,12 +207,17 @@ inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, siz
 }
 
 // ------------------------------------------------------------------ math dispatch
-__device__ __forceinline__ float q_rsqrt(float x) { return rsqrtf(x); }
-__device__ __forceinline__ double q_rsqrt(double x) { return rsqrt(x); }
-__device__ __forceinline__ float q_sqrt(float x) { return sqrtf(x); }
-__device__ __forceinline__ double q_sqrt(double x) { return sqrt(x); }
-__device__ __forceinline__ float q_rcp(float x) { return 1.0f / x; }
-__device__ __forceinline__ double q_rcp(double x) { return 1.0 / x; }
+// The arguments of these calls are positive normal numbers (squared norms guarded by reading R4, radicands 1 - x^2 of
+// numbers strictly inside (-1, 1)), so the special-case paths of the library routines are dead weight.
+//   float:  the SFU approximations (MUFU.RSQ / MUFU.SQRT / MUFU.RCP, 1-2 ulp; the link tolerance is 2e-5) in place of the
+//           IEEE sqrtf and division, whose slow paths put a branch and a call into the hit;
+//   double: seed + Newton forms without branches (hb_math.cuh, ~1e-16 relative; tolerance 1e-12).
+__device__ __forceinline__ float q_rsqrt(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float q_sqrt(float x) { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float q_rcp(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ double q_rsqrt(double x) { return hbm::rsqrt(x); }
+__device__ __forceinline__ double q_sqrt(double x) { return hbm::sqrt_pos(x); }
+__device__ __forceinline__ double q_rcp(double x) { return hbm::rcp(x); }
 __device__ __forceinline__ void q_sincospi(float x, float* s, float* c) { sincospif(x, s, c); }
 __device__ __forceinline__ void q_sincospi(double x, double* s, double* c) { sincospi(x, s, c); }
 __device__ __forceinline__ float q_fma(float a, float b, float c) { return fmaf(a, b, c); }

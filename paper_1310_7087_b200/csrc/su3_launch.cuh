@@ -43,11 +43,10 @@ template <> struct RingCfg<double, false> : RingShape<128, 3, 3> {};
 // heatbath kernels, whose direction loop is rolled, need K | 6 and take the K above.  -1: same as the heatbath kernel.
 template <typename R, bool COMP> struct RingKOr { static constexpr int K = -1; };
 template <> struct RingKOr<double, false> { static constexpr int K = 4; };
-// Loop shape per precision and kind: ROLL = direction / subgroup loops kept rolled (the unrolled heatbath misses the
-// instruction cache), PRE = heatbath random part of trial 0 precomputed into shared memory.
-template <typename R, int KIND> struct LoopCfg;
-template <int KIND> struct LoopCfg<float, KIND> { static constexpr bool ROLL = (KIND == 0), PRE = true; };
-template <int KIND> struct LoopCfg<double, KIND> { static constexpr bool ROLL = (KIND == 0), PRE = false; };
+// Loop shape per kind: ROLL = the direction loop of the heatbath kernels is kept rolled (their straight-line code would
+// be 60+ KB).  The three subgroup hits are unrolled in both precisions (round 2: a rolled hit on a permuted frame cost
+// ~150 register moves per link: fp32 HB 79.5 -> 76.9 us, fp64 HB 190 -> 181 us on the same box).
+template <int KIND> struct LoopCfg { static constexpr bool ROLL = (KIND == 0); };
 
 // Tile of B threads of the ring kernel: 8 half-indices along x0 (one 128-byte line of 16-byte vectors), the rest spread
 // over x1, x2, x3 in powers of two; every extent must divide the lattice, else the linear mapping is used.
@@ -95,7 +94,7 @@ static cudaError_t su3_go_tiled(const Geom& g, void* links, const UpdateArgs& a,
   typedef typename T::Vec Vec;
   typedef typename TileFor<MU>::TD TD;
   constexpr int K = TiledCfg<R, COMP, KIND>::K, MINB = TiledCfg<R, COMP, KIND>::MINB;
-  constexpr bool ROLL = LoopCfg<R, KIND>::ROLL && (4 % K == 0);
+  constexpr bool ROLL = LoopCfg<KIND>::ROLL && (4 % K == 0);
   constexpr size_t smem = (size_t)(TD::res_slots(MU) + K * TD::B) * T::NP * sizeof(Vec);
   auto kern = su3_update_tiled_kernel<R, MU, COMP, KIND, FIELD, TD, K, MINB, ROLL, MEAS>;
   static std::atomic<uint64_t> done{0};
@@ -145,11 +144,11 @@ static cudaError_t su3_go(const Geom& g, void* links, const UpdateArgs& a, cudaS
     if (g.Lh0 % TD::T0 == 0 && g.Li[1] % TD::T1 == 0 && g.Li[2] % TD::T2 == 0 && g.Li[3] % TD::T3 == 0)
       return su3_go_tiled<R, MU, COMP, KIND, FIELD, MEAS>(g, links, a, st);
   }
-  constexpr bool ROLL = LoopCfg<R, KIND>::ROLL, PRE = LoopCfg<R, KIND>::PRE;
+  constexpr bool ROLL = LoopCfg<KIND>::ROLL;
   constexpr int B = RingCfg<R, COMP>::B, MINB = RingCfg<R, COMP>::MINB;
   constexpr int K = (KIND == 1 && !ROLL && RingKOr<R, COMP>::K >= 0) ? RingKOr<R, COMP>::K : RingCfg<R, COMP>::K;
-  constexpr size_t smem = (size_t)K * T::NP * B * sizeof(Vec) + ((KIND == 0 && PRE) ? (size_t)15 * B * sizeof(R) : 0);
-  auto kern = su3_update_kernel<R, D, MU, COMP, KIND, FIELD, B, K, MINB, ROLL, PRE, MEAS>;
+  constexpr size_t smem = (size_t)K * T::NP * B * sizeof(Vec) + (KIND == 0 ? (size_t)15 * B * sizeof(R) : 0);
+  auto kern = su3_update_kernel<R, D, MU, COMP, KIND, FIELD, B, K, MINB, ROLL, MEAS>;
   static std::atomic<uint64_t> done{0};
   cudaError_t e = ensure_smem(kern, smem, done);
   if (e != cudaSuccess) return e;

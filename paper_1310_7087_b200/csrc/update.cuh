@@ -33,6 +33,7 @@ struct UpdateArgs {
                               // (prev_parity, prev_mu) is the only one that may not be read before griddepcontrol.wait),
                               // -1: a kernel that writes no links, -2: a kernel that writes all of them (init, set_links)
   uint32_t sweep, key0, key1;
+  PhiloxKeys rk;     // the round keys of (key0, key1), host-computed (philox.cuh)
   uint8_t* trials;   // NULL or [lex][3] debug trial codes
   // fused plaquette measurement (MEAS kernels, see meas_store below): per-warp partial sums of Re Tr[U' A_nu] for the
   // staple directions nu < mu go to meas[meas_plane[nu] * meas_stride + global warp index]
@@ -108,10 +109,10 @@ template <typename R> struct HbDraw { R E, w, n1, n2, n3; };
 
 template <typename R> struct KpRand;
 template <> struct KpRand<double> {
+  // branch-free forms on the Philox words themselves (hb_math.cuh): ln r1, cos^2(2 pi r2), ln r3 to ~5e-16 absolute
   static __device__ __forceinline__ void run(const Philox4& x, double& E, double& w) {
-    const double r1 = uniform64(x.x), r2 = uniform64(x.y), r3 = uniform64(x.z), r4 = uniform64(x.w);
-    const double c = cospi(2.0 * r2);
-    E = -(log(r1) + c * c * log(r3));
+    const double r4 = uniform64(x.w);
+    E = -(hbm::log_uniform32(x.x) + hbm::cos2_2pi_uniform32(x.y) * hbm::log_uniform32(x.z));
     w = r4 * r4;
   }
 };
@@ -134,6 +135,14 @@ template <typename R> __device__ __forceinline__ void hb_direction(const Philox4
   q_sincospi(R(2) * u2, &sphi, &cphi);
   n1 = st * cphi; n2 = st * sphi; n3 = ct;
 }
+// fp64: sin, cos(2 pi u2) with the octant reduction done on the Philox word (hb_math.cuh)
+template <> __device__ __forceinline__ void hb_direction<double>(const Philox4& x, double& n1, double& n2, double& n3) {
+  const double ct = 1.0 - 2.0 * uniform64(x.x);
+  const double st = hbm::sqrt_pos(1.0 - ct * ct);
+  double sphi, cphi;
+  hbm::sincos_2pi_uniform32(x.y, &sphi, &cphi);
+  n1 = st * cphi; n2 = st * sphi; n3 = ct;
+}
 // fp32: the azimuth from the SFU, argument folded into (-pi, pi) where __sinf / __cosf are good to 2^-21.4 absolute
 // (the link tolerance is 2e-5): sin(2 pi u) = -sin(2 pi (u - 1/2)), cos likewise
 template <> __device__ __forceinline__ void hb_direction<float>(const Philox4& x, float& n1, float& n2, float& n3) {
@@ -148,8 +157,8 @@ template <typename R>
 __device__ __forceinline__ HbDraw<R> hb_first_draw(uint32_t lex, const UpdateArgs& a, int mu, int sg) {
   const uint32_t c2 = philox_c2(mu, a.parity, sg, a.hit, 0);
   HbDraw<R> d;
-  KpRand<R>::run(philox4x32_10(lex, a.sweep, c2, 1u, a.key0, a.key1), d.E, d.w);
-  hb_direction<R>(philox4x32_10(lex, a.sweep, c2, 0u, a.key0, a.key1), d.n1, d.n2, d.n3);
+  KpRand<R>::run(philox4x32_10(lex, a.sweep, c2, 1u, a.rk), d.E, d.w);
+  hb_direction<R>(philox4x32_10(lex, a.sweep, c2, 0u, a.rk), d.n1, d.n2, d.n3);
   return d;
 }
 
@@ -187,6 +196,21 @@ __device__ __forceinline__ bool kp_accept(float inv, float E, float w, const KpK
   return margin >= 0.0f;
 }
 
+// Trials 1 .. max_trials-1 of a subgroup whose trial 0 was rejected (3 % of the lanes at beta = 6, but 60 % of the warps
+// have such a lane).  Inlined into each of the three subgroup hits: one shared out-of-line copy was measured and lost
+// (fp32 HB 79.5 -> 86.5 us, fp64 190 -> 204 us: the call spills the hit's live matrices around it).  Off the hot path,
+// so it derives the round keys from the key itself.
+template <typename R>
+static __device__ __forceinline__ bool kp_retry(R inv_alpha, const KpKey& key, int max_trials, R& g0, int& code) {
+  code = 0x80 | max_trials;
+  for (int t = 1; t < max_trials; ++t) {
+    R E, w;
+    KpRand<R>::run(philox4x32_10(key.lex, key.sweep, key.c2, 1u + (uint32_t)t, key.key0, key.key1), E, w);
+    if (kp_accept(inv_alpha, E, w, key, 1u + (uint32_t)t, g0)) { code = t + 1; return true; }
+  }
+  return false;
+}
+
 // quaternion a of the subgroup update from the projected v = proj(W) (not normalised), k2 = |v|^2;
 // d0 = trial 0 and direction (heatbath only)
 template <typename R, int KIND, int NC>
@@ -207,14 +231,7 @@ __device__ __forceinline__ bool subgroup_quaternion(const Q4<R>& v, R k2, uint32
     R g0;
     bool acc = kp_accept(inv_alpha, d0.E, d0.w, key, 1u, g0);     // trial 0 from the precomputed random part
     code = 1;
-    if (!acc) {
-      code = 0x80 | a.max_trials;
-      for (int t = 1; t < a.max_trials; ++t) {
-        R E, w;
-        KpRand<R>::run(philox4x32_10(lex, a.sweep, key.c2, 1u + (uint32_t)t, a.key0, a.key1), E, w);
-        if (kp_accept(inv_alpha, E, w, key, 1u + (uint32_t)t, g0)) { acc = true; code = t + 1; break; }
-      }
-    }
+    if (!acc) acc = kp_retry<R>(inv_alpha, key, a.max_trials, g0, code);
     // fp32: no early return: the lanes that needed further trials re-join the warp here, so what follows is executed
     // once per warp and not once per divergent path (it was 1.57 times per subgroup at 3 % rejection).  fp64 keeps the
     // early exit (the straight-line form costs it two spilled registers at its 168-register cap).
@@ -301,15 +318,6 @@ template <typename R> __device__ __forceinline__ void m3_add(M3<R>& a, const M3<
     for (int c = 0; c < 3; ++c) { a.e[r][c].re += s.e[r][c].re; a.e[r][c].im += s.e[r][c].im; }
 }
 
-// swap rows r1 <-> r2 of U and columns r1 <-> r2 of A: afterwards the subgroup acting on rows/columns (0,1) of the
-// permuted pair is the subgroup (frame[0], frame[1]) of the original one (W' = P W P^T)
-template <typename R, int R1, int R2> __device__ __forceinline__ void su3_swap_frame(M3<R>& U, M3<R>& A) {
-#pragma unroll
-  for (int c = 0; c < 3; ++c) { const Cx<R> t = U.e[R1][c]; U.e[R1][c] = U.e[R2][c]; U.e[R2][c] = t; }
-#pragma unroll
-  for (int r = 0; r < 3; ++r) { const Cx<R> t = A.e[r][R1]; A.e[r][R1] = A.e[r][R2]; A.e[r][R2] = t; }
-}
-
 // The links a thread consumes, in order.  For the i-th direction nu != MU, slot j = 0..5:
 //   j=0  U2  = U_mu(x+nu)        j=1  U3  = U_nu(x)        j=2  U1  = U_nu(x+mu)          upper staple U1 (U3 U2)^+
 //   j=3  U1' = U_nu(x+mu-nu)     j=4  U2' = U_mu(x-nu)     j=5  U3' = U_nu(x-nu)          lower staple (U2' U1')^+ U3'
@@ -317,11 +325,10 @@ template <typename R, int R1, int R2> __device__ __forceinline__ void su3_swap_f
 //
 // Template parameters: K = ring slots per thread (3 or 6, so that the slot of link (i, j) is j % K whatever i is; K = 0:
 // no ring, every link is loaded from global memory when it is consumed); B threads per CTA; MINB = CTAs per SM the
-// register allocation must allow.  ROLL: the loop over nu and the loop over the SU(2) subgroups of the heatbath are not
-// unrolled (the straight-line code of a fully unrolled link update, 39 KB overrelaxation / 64 KB heatbath, does not fit the
-// 32 KB instruction cache level; the fp32 kernels, which are issue-bound, take it; the fp64 kernels, which run few warps
-// and live on instruction-level parallelism, are faster unrolled).  PRE: heatbath only, park the random-number-only part
-// of trial 0 of every subgroup in shared memory at the start of the kernel instead of computing it inside the hit.
+// register allocation must allow.  ROLL: the loop over nu is not unrolled (heatbath kernels: their straight-line code
+// would be 60+ KB against a 32 KB instruction cache level; the three subgroup hits ARE unrolled, see su3_launch.cuh).
+// Heatbath: the random-number-only part of trial 0 of every subgroup is computed at the start of the kernel, before
+// griddepcontrol.wait, and parked in shared memory.
 // 18-real storage only: the links of which a thread uses rows 0,1 alone (J as in the table above; 6 = the own link, whose
 // third row is rebuilt).  Every product of SU(3) matrices is in SU(3), so the third rows of X = U3 U2, Y = U2' U1' and of
 // the staples are rebuilt as conj(row0 x row1) whatever the storage; what 18-real storage saves is the rebuilding of
@@ -329,7 +336,7 @@ template <typename R, int R1, int R2> __device__ __forceinline__ void su3_swap_f
 template <bool COMP> __host__ __device__ constexpr bool rows01_only_t(int J) { return !COMP && (J == 1 || J == 2 || J == 4 || J == 6); }
 
 // MEAS: fused plaquette measurement (see meas_store above); whole warps stay alive for the warp reduction.
-template <typename R, int D, int MU, bool COMP, int KIND, bool FIELD, int B, int K, int MINB, bool ROLL, bool PRE, bool MEAS>
+template <typename R, int D, int MU, bool COMP, int KIND, bool FIELD, int B, int K, int MINB, bool ROLL, bool MEAS>
 __global__ void __launch_bounds__(B, MINB)
 su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links, UpdateArgs a) {
   typedef PlaneTraits<R, (COMP ? 12 : 18)> T;
@@ -432,7 +439,7 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
   // the ring ([subgroup][5][B] reals, this thread's column).  It does not touch the links, so it runs before pdl_wait():
   // in the tail of the previous sub-step's kernel when this CTA became resident early.
   R* draws = reinterpret_cast<R*>(ring_raw + (size_t)K * NP * B * sizeof(Vec)) + threadIdx.x;
-  if constexpr (KIND == 0 && PRE) {
+  if constexpr (KIND == 0) {
 #pragma unroll 1
     for (int sg = 0; sg < 3; ++sg) {
       const HbDraw<R> d = hb_first_draw<R>(lex, a, MU, sg);
@@ -546,41 +553,20 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
     su3_subgroup_hit<R, KIND, 0, 2>(U, A, lex, a, MU, 1, none, c);
     su3_subgroup_hit<R, KIND, 1, 2>(U, A, lex, a, MU, 2, none, c);
   } else {
+    // trial 0 and the direction of each subgroup were parked in shared memory at kernel start; the three hits are
+    // unrolled (compile-time rows: no frame permutation)
     auto first_draw = [&](int sg) {
       HbDraw<R> d;
-      if constexpr (PRE) {
-        const R* o = draws + sg * 5 * B;
-        d.E = o[0]; d.w = o[B]; d.n1 = o[2 * B]; d.n2 = o[3 * B]; d.n3 = o[4 * B];
-      } else {
-        d = hb_first_draw<R>(lex, a, MU, sg);
-      }
+      const R* o = draws + sg * 5 * B;
+      d.E = o[0]; d.w = o[B]; d.n1 = o[2 * B]; d.n2 = o[3 * B]; d.n3 = o[4 * B];
       return d;
     };
-    if constexpr (ROLL) {
-      // one copy of the heatbath hit, on rows (0,1) of a permuted frame: (0,1,2) -> (0,2,1) -> (1,2,0)   (reading R3)
-#pragma unroll 1
-      for (int sg = 0; sg < 3; ++sg) {
-        int c;
-        su3_subgroup_hit<R, KIND, 0, 1>(U, A, lex, a, MU, sg, first_draw(sg), c);
-        if (a.trials) a.trials[(size_t)lex * 3 + sg] = (uint8_t)c;
-        if (sg == 0) su3_swap_frame<R, 1, 2>(U, A);
-        else if (sg == 1) su3_swap_frame<R, 0, 2>(U, A);
-      }
-      // frame (1,2,0) back to (0,1,2): row 0 <- cur 2, row 1 <- cur 0, row 2 <- cur 1
-#pragma unroll
-      for (int c = 0; c < 3; ++c) { const Cx<R> t = U.e[2][c]; U.e[2][c] = U.e[1][c]; U.e[1][c] = U.e[0][c]; U.e[0][c] = t; }
-      if constexpr (MEAS && MU == D - 1) {                         // the measurement takes A in the original frame too
-#pragma unroll
-        for (int r = 0; r < 3; ++r) { const Cx<R> t = A.e[r][2]; A.e[r][2] = A.e[r][1]; A.e[r][1] = A.e[r][0]; A.e[r][0] = t; }
-      }
-    } else {
-      int c0, c1, c2;
-      su3_subgroup_hit<R, KIND, 0, 1>(U, A, lex, a, MU, 0, first_draw(0), c0);
-      su3_subgroup_hit<R, KIND, 0, 2>(U, A, lex, a, MU, 1, first_draw(1), c1);
-      su3_subgroup_hit<R, KIND, 1, 2>(U, A, lex, a, MU, 2, first_draw(2), c2);
-      if (a.trials) {
-        a.trials[(size_t)lex * 3 + 0] = (uint8_t)c0; a.trials[(size_t)lex * 3 + 1] = (uint8_t)c1; a.trials[(size_t)lex * 3 + 2] = (uint8_t)c2;
-      }
+    int c0, c1, c2;
+    su3_subgroup_hit<R, KIND, 0, 1>(U, A, lex, a, MU, 0, first_draw(0), c0);
+    su3_subgroup_hit<R, KIND, 0, 2>(U, A, lex, a, MU, 1, first_draw(1), c1);
+    su3_subgroup_hit<R, KIND, 1, 2>(U, A, lex, a, MU, 2, first_draw(2), c2);
+    if (a.trials) {
+      a.trials[(size_t)lex * 3 + 0] = (uint8_t)c0; a.trials[(size_t)lex * 3 + 1] = (uint8_t)c1; a.trials[(size_t)lex * 3 + 2] = (uint8_t)c2;
     }
   }
   m3_reunitarise(U);

@@ -275,22 +275,6 @@ su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* 
     su3_subgroup_hit<R, KIND, 0, 1>(U, A, lex, a, MU, 0, none, cd);
     su3_subgroup_hit<R, KIND, 0, 2>(U, A, lex, a, MU, 1, none, cd);
     su3_subgroup_hit<R, KIND, 1, 2>(U, A, lex, a, MU, 2, none, cd);
-  } else if constexpr (ROLL) {
-    // one copy of the heatbath hit, on rows (0,1) of a permuted frame: (0,1,2) -> (0,2,1) -> (1,2,0)   (reading R3)
-#pragma unroll 1
-    for (int sg = 0; sg < 3; ++sg) {
-      int cd;
-      su3_subgroup_hit<R, KIND, 0, 1>(U, A, lex, a, MU, sg, hb_first_draw<R>(lex, a, MU, sg), cd);
-      if (a.trials) a.trials[(size_t)lex * 3 + sg] = (uint8_t)cd;
-      if (sg == 0) su3_swap_frame<R, 1, 2>(U, A);
-      else if (sg == 1) su3_swap_frame<R, 0, 2>(U, A);
-    }
-#pragma unroll
-    for (int k = 0; k < 3; ++k) { const Cx<R> t = U.e[2][k]; U.e[2][k] = U.e[1][k]; U.e[1][k] = U.e[0][k]; U.e[0][k] = t; }
-    if constexpr (MEAS && MU == D - 1) {
-#pragma unroll
-      for (int r = 0; r < 3; ++r) { const Cx<R> t = A.e[r][2]; A.e[r][2] = A.e[r][1]; A.e[r][1] = A.e[r][0]; A.e[r][0] = t; }
-    }
   } else {
     int c0, c1, c2;
     su3_subgroup_hit<R, KIND, 0, 1>(U, A, lex, a, MU, 0, hb_first_draw<R>(lex, a, MU, 0), c0);
