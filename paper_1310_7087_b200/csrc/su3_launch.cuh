@@ -24,7 +24,7 @@ template <> struct TiledCfg<float, true, 1> { static constexpr bool ON = true; s
 
 // ---- bulk-copy kernel (update_bulk.cuh), D = 4, L0 = 32, fp32 x12 overrelaxation without field: producer warp + mbarriers.
 // Instantiated, but run only on request (QCD_OPT_BULK_COPY): it is slower than the tiled kernel (DESIGN.md sec 6.10,
-// profiles/r2_bulk_copy.md) and is kept so that the measurement can be repeated.
+// profiles/r2_a_launches_and_ncu.md) and is kept so that the measurement can be repeated.
 template <typename R, bool COMP, int KIND, bool FIELD, bool MEAS> struct BulkCfg { static constexpr bool ON = false; static constexpr int K = 5, MINB = 4; };
 template <> struct BulkCfg<float, true, 1, false, false> { static constexpr bool ON = true; static constexpr int K = 5, MINB = 4; };
 // boxes of the bulk kernel: the full x0 row (16 half-indices: L0 = 32) x 8 rows, thin in mu where that keeps T1 = 4
