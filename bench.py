@@ -158,7 +158,7 @@ def rep_stats(times, steps):
             "reps": len(t), "device_ms_total": sum(t)}
 
 
-def time_arm(q, torch, prec_name, steps, warmup, therm, seed, dist, sampler, bulk_copy=False):
+def time_arm(q, torch, prec_name, steps, warmup, therm, seed, dist, sampler, bulk_copy=False, alternate=True):
     """device-resident timing + end-to-end timing of one precision arm; returns a dict of raw numbers"""
     prec = q.QCD_FP32 if prec_name == "f32" else q.QCD_FP64
     flags = q.QCD_FLAG_COMPRESS12 if prec_name == "f32" else 0
@@ -169,6 +169,8 @@ def time_arm(q, torch, prec_name, steps, warmup, therm, seed, dist, sampler, bul
     with q.Lattice(DIMS, NC, prec, flags, device=torch.device("cuda", torch.cuda.current_device())) as G:
         if bulk_copy:
             G.qcd_set_option(q.QCD_OPT_BULK_COPY, 1)
+        if not alternate:
+            G.qcd_set_option(q.QCD_OPT_ALTERNATE_ORDER, 0)
         G.qcd_init(q.QCD_HOT, seed)
         for _ in range(therm):                       # setup: move off the hot start (KP acceptance, staple norms)
             G.qcd_sweep(BETA, N_HB, N_OR)
@@ -338,7 +340,7 @@ def run_ours(args):
     other = "f64" if primary == "f32" else "f32"
     arms = {}
     for name in (primary, other):
-        arms[name] = time_arm(q, torch, name, args.steps, args.warmup, args.therm, replica_seed(rank), dist, sampler, args.bulk_copy)
+        arms[name] = time_arm(q, torch, name, args.steps, args.warmup, args.therm, replica_seed(rank), dist, sampler, args.bulk_copy, not args.same_order)
     on_model = time_on_model(q, torch, dist, sampler, with_oracle=(world == 1 and rank == 0 and not args.no_cpu_baseline))
     clocks = sampler.stop()
     line = None
@@ -376,6 +378,8 @@ def run_ours(args):
                 "qcd_sweep_then_qcd_measure": p["qcd_sweep_then_qcd_measure"],
                 "observables": {"plaquette": p["plaquette"], "polyakov_abs": p["polyakov_abs"]},
                 "other_precision": frag[other], "on_model": on_model}
+        if args.same_order:
+            line["config"]["launch_order"] = "QCD_OPT_ALTERNATE_ORDER = 0"
         if args.bulk_copy:
             line["config"]["or_kernel"] = "QCD_OPT_BULK_COPY = 1: su3_update_bulk_kernel (fp32 arm)"
             line["roofline"]["kernel"] = "su3_update_bulk_kernel<float, x12, OR> (and the tiled kernel in the fused last pass)"
@@ -479,6 +483,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--bulk-copy", action="store_true",
                     help="fp32 arm: overrelaxation by the bulk-copy kernel (QCD_OPT_BULK_COPY; the comparison of DESIGN.md sec 6.10)")
+    ap.add_argument("--same-order", action="store_true",
+                    help="every update launch visits the lattice in the same direction (QCD_OPT_ALTERNATE_ORDER = 0; the comparison "
+                         "of DESIGN.md sec 6.5)")
     args = ap.parse_args()
     if args.impl == "reference":
         args.steps = 16 if args.steps is None else args.steps

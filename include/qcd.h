@@ -46,10 +46,13 @@ enum {
   QCD_OPT_DEBUG_TRIALS = 1,  /* 1: qcd_debug_substep records per-(link,subgroup) trial codes (allocates V*3 bytes) */
   QCD_OPT_PROFILE = 2,       /* 1: CUDA events around the update kernels: one pair per run of same-kind launches in qcd_sweep,
                                 one pair per launch in qcd_debug_substep (see qcd_get_profile) */
-  QCD_OPT_BULK_COPY = 3      /* 1: SU(3) fp32 x12 overrelaxation on D = 4 lattices with dims[0] = 32 runs the kernel that stages
+  QCD_OPT_BULK_COPY = 3,     /* 1: SU(3) fp32 x12 overrelaxation on D = 4 lattices with dims[0] = 32 runs the kernel that stages
                                 every operand with bulk asynchronous copies (cp.async.bulk + mbarriers, update_bulk.cuh) instead
                                 of the tiled cp.async kernel.  Same results to rounding; measured SLOWER:
                                 default 0, kept so that the comparison can be repeated (bench.py --bulk-copy) */
+  QCD_OPT_ALTERNATE_ORDER = 4 /* 1 (default): consecutive update launches visit the lattice in opposite directions, so that a
+                                launch starts on the links the previous one touched last and finds them in the L2
+                                (DESIGN.md sec 6.5).  Results are bit-identical either way; 0 restores one direction */
 };
 
 /* Constant abelian background: every plaquette of plane (mu,nu), mu < nu, is multiplied on the left, at its

@@ -16,7 +16,7 @@ QCD_FP32, QCD_FP64 = 0, 1
 QCD_FLAG_COMPRESS12 = 1
 QCD_COLD, QCD_HOT = 0, 1
 QCD_KIND_HB, QCD_KIND_OR = 0, 1
-QCD_OPT_KP_MAX_TRIALS, QCD_OPT_DEBUG_TRIALS, QCD_OPT_PROFILE, QCD_OPT_BULK_COPY = 0, 1, 2, 3
+QCD_OPT_KP_MAX_TRIALS, QCD_OPT_DEBUG_TRIALS, QCD_OPT_PROFILE, QCD_OPT_BULK_COPY, QCD_OPT_ALTERNATE_ORDER = 0, 1, 2, 3, 4
 
 # every symbol include/qcd.h declares (tests check that the library exports all of them)
 SYMBOLS = [

@@ -48,7 +48,7 @@ struct qcd_lattice {
   uint32_t sweep;
   bool has_links;
   int max_trials;
-  bool debug_trials, profile, bulk_copy;
+  bool debug_trials, profile, bulk_copy, alternate_order;
   uint8_t* d_trials;
   // per-block / per-warp partial sums of the reductions, one allocation of three regions (sizes fixed by the geometry):
   // [fused plaquette: NPL x np_warp][plaquette kernel: NPL x nb_plaq][Polyakov: 2 x nb_poly]
@@ -60,6 +60,7 @@ struct qcd_lattice {
   double prof_ms[2];
   uint64_t prof_n[2];
   uint64_t launches;
+  uint32_t order_toggle;   // flips with every update launch (UpdateArgs::rev)
   // What the kernel launched last on the stream wrote: (parity, mu) of an update kernel; -1: no links (measurement,
   // get_links); -2: all links (init, set_links, the create-time memset).  The next update kernel may fetch, before its
   // griddepcontrol.wait, only arrays that kernel does not write (update.cuh)
@@ -160,10 +161,11 @@ cudaError_t launch_update(qcd_lattice* L, int kind, bool field, const UpdateArgs
   s.meas = a0.meas != nullptr;
   UpdateArgs a = a0;
   a.prev_parity = L->last_parity; a.prev_mu = L->last_mu;
+  a.rev = L->alternate_order ? (int)(L->order_toggle & 1u) : 0;
   const cudaError_t e = (L->Nc == 2)                ? launch_update_su2(s, L->g, L->mem, a, L->stream)
                         : L->precision == QCD_FP32 ? launch_update_su3_f32(s, L->g, L->mem, a, L->stream)
                                                    : launch_update_su3_f64(s, L->g, L->mem, a, L->stream);
-  if (e == cudaSuccess) { L->launches += 1; L->last_parity = a.parity; L->last_mu = a.mu; }
+  if (e == cudaSuccess) { L->launches += 1; L->order_toggle ^= 1u; L->last_parity = a.parity; L->last_mu = a.mu; }
   return e;
 }
 
@@ -432,9 +434,9 @@ static int create_lattice(int D, const int* dims, int Nc, int precision, unsigne
   L->bytes = need; L->mem = device_mem; L->owns_mem = false;
   L->stream = (cudaStream_t)cuda_stream;
   L->seed = 0; L->sweep = 0; L->has_links = false; L->max_trials = 10;
-  L->debug_trials = false; L->profile = false; L->bulk_copy = false;
+  L->debug_trials = false; L->profile = false; L->bulk_copy = false; L->alternate_order = true;
   L->d_trials = nullptr; L->d_partials = nullptr; L->partials_cap = 0; L->d_results = nullptr; L->h_results = nullptr;
-  L->prof_ms[0] = L->prof_ms[1] = 0.0; L->prof_n[0] = L->prof_n[1] = 0; L->launches = 0; L->last_parity = L->last_mu = -2; L->d_canon = nullptr;
+  L->prof_ms[0] = L->prof_ms[1] = 0.0; L->prof_n[0] = L->prof_n[1] = 0; L->launches = 0; L->order_toggle = 0; L->last_parity = L->last_mu = -2; L->d_canon = nullptr;
   L->side = nullptr; L->ev_fork = nullptr; L->ev_join = nullptr;
   cudaError_t e = cudaSuccess;
   if (!device_mem) {
@@ -765,6 +767,7 @@ int qcd_set_option(qcd_lattice_t* L, int key, int value) {
     case QCD_OPT_DEBUG_TRIALS: L->debug_trials = value != 0; return QCD_OK;
     case QCD_OPT_PROFILE: L->profile = value != 0; return QCD_OK;
     case QCD_OPT_BULK_COPY: L->bulk_copy = value != 0; return QCD_OK;
+    case QCD_OPT_ALTERNATE_ORDER: L->alternate_order = value != 0; return QCD_OK;
   }
   return fail(QCD_ERR_INVALID_ARG, "unknown option key");
 }

@@ -99,12 +99,12 @@ struct TileMap {
   int s0, s1, s2;      // log2 of the tile extents in directions 0 (half-indices), 1, 2; direction 3 takes the rest of B
   FastDiv n0, n1, n2;  // tiles per direction 0, 1, 2
 };
-__device__ __forceinline__ SiteCoord decode_site_tiled(const Geom& g, const TileMap& tm, int parity, uint32_t& h) {
+// b = the CTA's logical block index (UpdateArgs::rev reverses the launch order, see update.cuh)
+__device__ __forceinline__ SiteCoord decode_site_tiled(const Geom& g, const TileMap& tm, int parity, uint32_t b, uint32_t& h) {
   uint32_t t = threadIdx.x;
   const uint32_t jl = t & ((1u << tm.s0) - 1u); t >>= tm.s0;
   const uint32_t y1 = t & ((1u << tm.s1) - 1u); t >>= tm.s1;
   const uint32_t y2 = t & ((1u << tm.s2) - 1u); t >>= tm.s2;
-  uint32_t b = blockIdx.x;
   uint32_t q = fd_div(b, tm.n0); const uint32_t b0 = b - q * tm.n0.d; b = q;
   q = fd_div(b, tm.n1); const uint32_t b1 = b - q * tm.n1.d; b = q;
   q = fd_div(b, tm.n2); const uint32_t b2 = b - q * tm.n2.d; const uint32_t b3 = q;

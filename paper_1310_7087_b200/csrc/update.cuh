@@ -41,6 +41,9 @@ struct UpdateArgs {
   uint32_t meas_stride;
   int meas_plane[3];
   TileMap tm;        // thread -> site mapping of the SU(3) kernels (set by the launcher)
+  int rev;           // 1: the CTAs visit their boxes in descending order.  Consecutive launches of a sweep alternate, so that a
+                     // launch starts on the part of the lattice the previous one touched last and finds it in the L2
+                     // (the 32^4 lattices are 1.6 / 4.8 times the 126 MB L2: in the same order nothing survives a launch)
   int use_bulk;      // host side only: QCD_OPT_BULK_COPY (update_bulk.cuh instead of the tiled kernel where it applies)
   FieldArgs f;
 };
@@ -55,8 +58,11 @@ struct UpdateArgs {
 // difference them per direction in double and reduce per warp (shuffles, fixed order: deterministic); a second kernel sums
 // the per-warp partials.  The three launches (1, mu >= 1) of the last pass thus measure all D(D-1)/2 planes: the "working
 // sweep" of PAPER.md:134 without a separate pass over the links.
+// logical block index of a CTA: the launch order is reversed when a.rev is set; everything a CTA does (sites, measurement
+// slots) follows the logical index, so results do not depend on the order
+__device__ __forceinline__ uint32_t logical_block(const UpdateArgs& a) { return a.rev ? gridDim.x - 1u - blockIdx.x : blockIdx.x; }
 template <int NREC> __device__ __forceinline__ void meas_store(const UpdateArgs& a, const double (&t)[NREC]) {
-  const uint32_t w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const uint32_t w = (logical_block(a) * blockDim.x + threadIdx.x) >> 5;
 #pragma unroll
   for (int j = 0; j < NREC; ++j) {
     double x = t[j];
@@ -357,9 +363,9 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
   SiteCoord sc;
   bool active = true;
   if (a.tm.on) {
-    sc = decode_site_tiled(g, a.tm, p, h);                         // the tiles cover the lattice exactly
+    sc = decode_site_tiled(g, a.tm, p, logical_block(a), h);       // the tiles cover the lattice exactly
   } else {
-    uint32_t hl = blockIdx.x * B + threadIdx.x;                    // launch index over the interior (= h unless a slab)
+    uint32_t hl = logical_block(a) * B + threadIdx.x;              // launch index over the interior (= h unless a slab)
     if constexpr (MEAS) {
       active = hl < g.Vh_int;                                      // a surplus thread shadows the last site: it neither
       if (!active) hl = g.Vh_int - 1;                              // stores nor contributes, but stays for the shuffles
@@ -603,7 +609,7 @@ template <typename R, int D, int KIND, bool FIELD, bool MEAS>
 __global__ void __launch_bounds__(256)
 su2_update_kernel(Geom g, typename PlaneTraits<R, 4>::Vec* links, UpdateArgs a) {
   typedef PlaneTraits<R, 4> T;
-  uint32_t hl = blockIdx.x * blockDim.x + threadIdx.x, h;  // launch index over the interior (= h unless a slab)
+  uint32_t hl = logical_block(a) * blockDim.x + threadIdx.x, h;  // launch index over the interior (= h unless a slab)
   bool active = true;
   if constexpr (MEAS) {
     active = hl < g.Vh_int;
@@ -671,7 +677,7 @@ su2_update_kernel(Geom g, typename PlaneTraits<R, 4>::Vec* links, UpdateArgs a) 
       t[j] = (active && j < mu) ? (double)c - (double)prev : 0.0;
       prev = c;
     }
-    const uint32_t w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const uint32_t w = (logical_block(a) * blockDim.x + threadIdx.x) >> 5;
 #pragma unroll
     for (int j = 0; j < D - 1; ++j) {
       double x = t[j];

@@ -83,7 +83,7 @@ su3_update_bulk_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* l
 
   const int p = a.parity;
   // CTA -> box origin (the box covers x0 completely)
-  uint32_t bb = blockIdx.x;
+  uint32_t bb = logical_block(a);
   uint32_t qd = fd_div(bb, a.tm.n1); const uint32_t b1 = bb - qd * a.tm.n1.d; bb = qd;
   qd = fd_div(bb, a.tm.n2); const uint32_t b2 = bb - qd * a.tm.n2.d; const uint32_t b3 = qd;
   const int o1 = (int)b1 * TD::T1, o2 = (int)b2 * TD::T2, o3 = (int)b3 * TD::T3;

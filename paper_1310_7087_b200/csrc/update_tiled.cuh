@@ -65,7 +65,7 @@ su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* 
   SiteCoord sc;
   uint32_t h;
   {
-    uint32_t b = blockIdx.x;
+    uint32_t b = logical_block(a);
     uint32_t q = fd_div(b, a.tm.n0); const uint32_t b0 = b - q * a.tm.n0.d; b = q;
     q = fd_div(b, a.tm.n1); const uint32_t b1 = b - q * a.tm.n1.d; b = q;
     q = fd_div(b, a.tm.n2); const uint32_t b2 = b - q * a.tm.n2.d; const uint32_t b3 = q;

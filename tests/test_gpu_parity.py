@@ -505,6 +505,26 @@ def test_bulk_copy_overrelaxation_kernel_matches_the_oracle(qcd):
             assert float(np.max(np.abs(G.qcd_get_links().astype(np.complex128) - O.get_links()))) < unresynced_bar(0, 8, 3.5)
 
 
+def test_launch_order_does_not_change_any_result(qcd):
+    """QCD_OPT_ALTERNATE_ORDER (consecutive update launches visit the lattice in opposite directions, for L2 reuse): the
+    order in which CTAs take their boxes must not show in the links, the trial codes or the fused observables -- bit for bit,
+    every storage format, tiled / ring / SU(2) kernels, a ragged last CTA and a divisible lattice"""
+    cases = [((16, 16, 16, 4), 3, 0, 1), ((16, 16, 16, 4), 3, 1, 0), ((6, 4, 10, 2), 3, 0, 0), ((6, 4, 10, 2), 3, 1, 1),
+             ((12, 6, 4, 8), 2, 0, 0), ((6, 4, 10), 3, 1, 0), ((4, 6), 2, 1, 0)]
+    for dims, Nc, prec, flags in cases:
+        out = []
+        for alt in (1, 0):
+            with gpu_lattice(qcd, dims, Nc, prec, flags) as G:
+                G.qcd_set_option(qcd.QCD_OPT_ALTERNATE_ORDER, alt)
+                G.qcd_init(qcd.QCD_HOT, 11)
+                G.qcd_sweep(5.7, 1, 2)
+                obs = G.qcd_sweep_measure(5.7, 1, 1)
+                out.append((G.qcd_get_links(), obs))
+        (la, oa), (lb, ob) = out
+        assert np.array_equal(la, lb), (dims, Nc, prec, flags)
+        assert oa[0] == ob[0] and np.array_equal(oa[1], ob[1]) and oa[2] == ob[2], (dims, Nc, prec, flags)
+
+
 def test_overrelaxation_conserves_action_on_gpu(qcd):
     dims = (8, 8, 8, 8)
     for Nc, prec, flags, tol in [(3, 1, 0, 1e-12), (3, 0, 1, 3e-6), (2, 1, 0, 1e-12)]:
