@@ -159,7 +159,26 @@ __device__ __forceinline__ size_t array_base(const Geom& g, int D, int parity, i
 // PLANE_STRIDE vectors apart (an immediate offset) and all of a link lies within NP * 128 bytes (page locality on large
 // lattices).  A warp's load of one plane of 8 consecutive half-indices is still one full 128-byte line.
 constexpr int PLANE_STRIDE = 8;
-template <int NP> __device__ __forceinline__ uint32_t blk_off(uint32_t h) { return (h >> 3) * (8u * NP) + (h & 7u); }
+// Written with shifts and adds (the ALU pipe): as a multiply it becomes an IMAD on the FMA pipe, which is the pipe the
+// fp32 kernels are bound by.
+// x * NP (mod 2^32) by shifts and adds
+template <int NP> __device__ __forceinline__ uint32_t mul_planes(uint32_t x) {
+  if constexpr (NP == 1) return x;
+  else if constexpr (NP == 2) return x << 1;
+  else if constexpr (NP == 3) return (x << 1) + x;
+  else if constexpr (NP == 6) return ((x << 1) + x) << 1;
+  else if constexpr (NP == 9) return (x << 3) + x;
+  else return x * (uint32_t)NP;
+}
+template <int NP> __device__ __forceinline__ uint32_t blk_off(uint32_t h) {
+  const uint32_t q = h >> 3, r = h & 7u;
+  if constexpr (NP == 1) return (q << 3) + r;
+  else if constexpr (NP == 2) return (q << 4) + r;
+  else if constexpr (NP == 3) return (((q << 1) + q) << 3) + r;
+  else if constexpr (NP == 6) return (((q << 1) + q) << 4) + r;
+  else if constexpr (NP == 9) return (((q << 3) + q) << 3) + r;
+  else return q * (8u * NP) + r;
+}
 
 // load the NREAL reals of link h of the array starting at `base` (vectors); NC = through the read-only path
 template <typename R, int NREAL, bool NC>

@@ -74,6 +74,15 @@ static inline TileMap choose_tile(const Geom& g, int B) {
   return tm;
 }
 
+// array starts for the kernels (UpdateArgs::pbase / qbase)
+template <typename Vec> static void fill_bases(UpdateArgs& a, const Geom& g, void* links, int NP) {
+  const size_t arr = (size_t)NP * g.Vh_pad;
+  for (int nu = 0; nu < 4; ++nu) {
+    a.pbase[nu] = nu < g.D ? (const void*)((Vec*)links + (size_t)(a.parity * g.D + nu) * arr) : nullptr;
+    a.qbase[nu] = nu < g.D ? (const void*)((Vec*)links + (size_t)((1 - a.parity) * g.D + nu) * arr) : nullptr;
+  }
+}
+
 // opt in to > 48 KB of dynamic shared memory once per (kernel instantiation, device); `done` is a per-instantiation
 // bit mask over device ordinals.  Racing host threads at worst both set the (idempotent) attribute.
 template <typename Kern> static cudaError_t ensure_smem(Kern kern, size_t smem, std::atomic<uint64_t>& done) {
@@ -105,6 +114,7 @@ static cudaError_t su3_go_tiled(const Geom& g, void* links, const UpdateArgs& a,
   a2.tm.on = 1;
   a2.tm.n0 = make_fastdiv((uint32_t)(g.Lh0 / TD::T0)); a2.tm.n1 = make_fastdiv((uint32_t)(g.Li[1] / TD::T1));
   a2.tm.n2 = make_fastdiv((uint32_t)(g.Li[2] / TD::T2));
+  fill_bases<Vec>(a2, g, links, T::NP);
   return launch_pdl(kern, dim3(g.Vh_int / TD::B), dim3(TD::B), smem, st, g, (Vec*)links, a2);
 }
 
@@ -155,6 +165,7 @@ static cudaError_t su3_go(const Geom& g, void* links, const UpdateArgs& a, cudaS
   const unsigned grid = (g.Vh_int + B - 1) / B;
   UpdateArgs a2 = a;
   a2.tm = choose_tile(g, B);
+  fill_bases<Vec>(a2, g, links, T::NP);
   return launch_pdl(kern, dim3(grid), dim3(B), smem, st, g, (Vec*)links, a2);
 }
 // MEAS = the fused-measurement variants (update.cuh, meas_store): instantiated by their own translation units; they exist

@@ -41,6 +41,11 @@ struct UpdateArgs {
   uint32_t meas_stride;
   int meas_plane[3];
   TileMap tm;        // thread -> site mapping of the SU(3) kernels (set by the launcher)
+  // start of every (parity, direction) array, computed by the launcher: pbase[nu] = U_nu on the parity being updated,
+  // qbase[nu] = U_nu on the other parity.  In the kernels they are constant-bank loads; computed there, (p D + nu) * arr is
+  // a 64-bit multiply-add per array on the FMA pipe.
+  const void* pbase[4];
+  const void* qbase[4];
   int rev;           // 1: the CTAs visit their boxes in descending order.  Consecutive launches of a sweep alternate, so that a
                      // launch starts on the part of the lattice the previous one touched last and finds it in the L2
                      // (the 32^4 lattices are 1.6 / 4.8 times the 126 MB L2: in the same order nothing survives a launch)
@@ -379,9 +384,9 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
   for (int d = 0; d < D; ++d) nbr_offsets(g, sc, d, fo[d], bo[d]);
   // A (parity, direction) array holds arr = NP * Vh_pad vectors (< 2^32, checked at creation); its base is a 64-bit,
   // warp-uniform pointer and elements are addressed by the 32-bit in-array offset blk_off(h').
-  const size_t arr = (size_t)NP * g.Vh_pad;
-  Vec* const own_ptr = links + (size_t)(p * D + MU) * arr;
-  const Vec* const qmu_ptr = links + (size_t)((1 - p) * D + MU) * arr;
+
+  Vec* const own_ptr = (Vec*)a.pbase[MU];
+  const Vec* const qmu_ptr = (const Vec*)a.qbase[MU];
   auto at = [&](const Vec* base, int off) -> const Vec* { return base + blk_off<NP>(h + (uint32_t)off); };
 
   struct Dir { const Vec *pp, *qp; int f, b, nu; };                // per-direction addressing (array bases), run-time nu
@@ -391,8 +396,8 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
     d.f = fo[0]; d.b = bo[0];
 #pragma unroll
     for (int k = 1; k < D; ++k) if (d.nu == k) { d.f = fo[k]; d.b = bo[k]; }
-    d.pp = links + (size_t)(p * D + d.nu) * arr;
-    d.qp = links + (size_t)((1 - p) * D + d.nu) * arr;
+    d.pp = (const Vec*)a.pbase[d.nu];
+    d.qp = (const Vec*)a.qbase[d.nu];
     return d;
   };
   // plane 0 of link j of direction d (j = 6: the own link)
@@ -591,7 +596,7 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
   }
   R r[NREAL];
   m3_to_reals<R, NREAL>(U, r);
-  store_reals<R, NREAL>(links, g, (size_t)(p * D + MU) * arr, h, r);
+  store_reals<R, NREAL>(own_ptr, g, 0, h, r);
 }
 
 // =====================================================================================

@@ -80,10 +80,18 @@ su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* 
   int fo[D], bo[D];
 #pragma unroll
   for (int d = 0; d < D; ++d) nbr_offsets(g, sc, d, fo[d], bo[d]);
-  const size_t arr = (size_t)NP * g.Vh_pad;                                   // vectors per array (< 2^32); 64-bit uniform bases
-  Vec* const own_ptr = links + (size_t)(p * D + MU) * arr;
-  const Vec* const qmu_ptr = links + (size_t)((1 - p) * D + MU) * arr;
-  auto at = [&](const Vec* base, int off) -> const Vec* { return base + blk_off<NP>(h + (uint32_t)off); };
+  Vec* const own_ptr = (Vec*)a.pbase[MU];
+  const Vec* const qmu_ptr = (const Vec*)a.qbase[MU];
+  // In-array vector offsets.  The boxes are 8 half-indices wide, so Lh0 and with it every stride of a direction >= 1 is a
+  // multiple of 8: such a step moves whole blocks, blk_off(h + o) = blk_off(h) + NP o.  Only a step along direction 0
+  // (k0 = +1 forward, -1 backward) moves inside the row and takes the full formula -- three evaluations per thread
+  // instead of one per link.
+  const uint32_t vh = blk_off<NP>(h), vf0 = blk_off<NP>(h + (uint32_t)fo[0]), vb0 = blk_off<NP>(h + (uint32_t)bo[0]);
+  auto at = [&](const Vec* base, int k0, int rest) -> const Vec* {
+    return base + ((k0 == 0 ? vh : k0 > 0 ? vf0 : vb0) + mul_planes<NP>((uint32_t)rest));
+  };
+  constexpr int F0 = (MU == 0) ? 1 : 0;                                      // x + mu: direction-0 part ...
+  const int frest = (MU == 0) ? 0 : fo[MU];                                  // ... and the rest
   const uint32_t lex = lex_global(g, sc);
   const int lin = (int)threadIdx.x;                                          // slot of box element c
   // index of c inside the face of direction d (the d-th coordinate dropped)
@@ -102,42 +110,43 @@ su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* 
 #pragma unroll
       for (int k = 0; k < NP; ++k) cp_async_vec<(int)sizeof(Vec)>(res + k * RES + slot, src + k * PLANE_STRIDE);
     };
-    stage(lin, at(qmu_ptr, 0));
+    stage(lin, at(qmu_ptr, 0, 0));
 #pragma unroll
     for (int d = 0; d < D; ++d) {
       if (d == MU) continue;
       const int fb = TD::face_base(MU, d), l3 = lin3(d);
       if (d == 0) {
         // a row with s = 0 needs j-1 of its first site, a row with s = 1 needs j+1 of its last site
-        if (c[0] == 0 && s == 0) stage(fb + l3, at(qmu_ptr, bo[0]));
-        if (c[0] == TD::T0 - 1 && s == 1) stage(fb + l3, at(qmu_ptr, fo[0]));
+        if (c[0] == 0 && s == 0) stage(fb + l3, at(qmu_ptr, -1, 0));
+        if (c[0] == TD::T0 - 1 && s == 1) stage(fb + l3, at(qmu_ptr, 1, 0));
       } else {
-        if (c[d] == 0) stage(fb + l3, at(qmu_ptr, bo[d]));
-        if (c[d] == TD::T(d) - 1) stage(fb + B / TD::T(d) + l3, at(qmu_ptr, fo[d]));
+        if (c[d] == 0) stage(fb + l3, at(qmu_ptr, 0, bo[d]));
+        if (c[d] == TD::T(d) - 1) stage(fb + B / TD::T(d) + l3, at(qmu_ptr, 0, fo[d]));
       }
     }
     cp_async_commit();
   };
 
   // ---- ring
-  struct Dir { const Vec *pp, *qp; int b, nu; };
+  struct Dir { const Vec *pp, *qp; int b0, brest, nu; };              // x - nu: direction-0 part (-1 or 0) and the rest
   auto make_dir = [&](int i) {
     Dir d;
     d.nu = i + (i >= MU ? 1 : 0);
-    d.b = bo[0];
+    d.b0 = (d.nu == 0) ? -1 : 0;
+    d.brest = 0;
 #pragma unroll
-    for (int k = 1; k < D; ++k) if (d.nu == k) d.b = bo[k];
-    d.pp = links + (size_t)(p * D + d.nu) * arr;
-    d.qp = links + (size_t)((1 - p) * D + d.nu) * arr;
+    for (int k = 1; k < D; ++k) if (d.nu == k) d.brest = bo[k];
+    d.pp = (const Vec*)a.pbase[d.nu];
+    d.qp = (const Vec*)a.qbase[d.nu];
     return d;
   };
   auto ring_idx = [&](auto rc, const Dir& d) -> const Vec* {
     constexpr int RR = decltype(rc)::value;
-    if constexpr (RR == 0) return at(d.pp, 0);
-    else if constexpr (RR == 1) return at(d.qp, fo[MU]);
-    else if constexpr (RR == 2) return at(d.pp, fo[MU] + d.b);
-    else if constexpr (RR == 3) return at(d.qp, d.b);
-    else return at(own_ptr, 0);
+    if constexpr (RR == 0) return at(d.pp, 0, 0);
+    else if constexpr (RR == 1) return at(d.qp, F0, frest);
+    else if constexpr (RR == 2) return at(d.pp, F0 + d.b0, frest + d.brest);
+    else if constexpr (RR == 3) return at(d.qp, d.b0, d.brest);
+    else return at(own_ptr, 0, 0);
   };
   auto issue = [&](int n, const Vec* src) {                     // link n of the sequence -> slot n % K
     Vec* dst = ring + (n % K) * NP * B;
@@ -186,7 +195,7 @@ su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* 
         issue(4 * i + RA, ring_idx(std::integral_constant<int, RA>{}, cur));
       } else {
         if (!last) issue(4 * i + RA, ring_idx(std::integral_constant<int, RA - 4>{}, nxt));
-        else if (RA == 4) issue(4 * i + RA, at(own_ptr, 0));          // the own link, once, after the last direction
+        else if (RA == 4) issue(4 * i + RA, at(own_ptr, 0, 0));          // the own link, once, after the last direction
       }
       cp_async_commit();                                       // one group per step, possibly empty
       cp_async_wait<K - 1>();
@@ -299,7 +308,7 @@ su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* 
   }
   R r[NREAL];
   m3_to_reals<R, NREAL>(U, r);
-  store_reals<R, NREAL>(links, g, (size_t)(p * D + MU) * arr, h, r);
+  store_reals<R, NREAL>(own_ptr, g, 0, h, r);
 }
 
 }  // namespace qcd
