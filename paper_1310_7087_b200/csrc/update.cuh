@@ -236,7 +236,9 @@ __device__ __forceinline__ bool subgroup_quaternion(const Q4<R>& v, R k2, uint32
     return true;
   } else {
     const R rk = q_rsqrt(k2);
-    const R inv_alpha = (R)a.inv_c * rk;                 // 1 / alpha, alpha = 2 beta k / N
+    // 1 / alpha, alpha = 2 beta k / N.  The SU(3) hit hands in v = 2 proj(W) (it leaves out the factor 1/2 of the
+    // projection: everything else here is homogeneous of degree 0 in v), so k = |v| / 2 there.
+    const R inv_alpha = (R)a.inv_c * rk * (NC == 3 ? R(2) : R(1));
     KpKey key;
     key.lex = lex; key.sweep = a.sweep; key.c2 = philox_c2(mu, a.parity, sg, a.hit, 0); key.key0 = a.key0; key.key1 = a.key1;
     R g0;
@@ -262,6 +264,25 @@ template <> struct Tiny<double> { static __device__ __forceinline__ double k2() 
 // =====================================================================================
 // SU(3)
 // =====================================================================================
+// twice the SU(2) projection of the 2x2 block (wii wij; wji wjj), and its squared norm
+template <typename R>
+__device__ __forceinline__ void su3_project2(const Cx<R>& wii, const Cx<R>& wij, const Cx<R>& wji, const Cx<R>& wjj, Q4<R>& v, R& k2) {
+  v.a0 = wii.re + wjj.re;
+  v.a1 = wij.im + wji.im;
+  v.a2 = wij.re - wji.re;
+  v.a3 = wii.im - wjj.im;
+  k2 = v.a0 * v.a0 + v.a1 * v.a1 + v.a2 * v.a2 + v.a3 * v.a3;
+}
+__device__ __forceinline__ void su3_project2(const Cx<float>& wii, const Cx<float>& wij, const Cx<float>& wji, const Cx<float>& wjj,
+                                             Q4<float>& v, float& k2) {
+  const float2 p = __ffma2_rn(f2_of(wjj), make_float2(1.0f, -1.0f), f2_of(wii));     // (a0, a3)
+  const float2 q = __ffma2_rn(f2_of(wji), make_float2(-1.0f, 1.0f), f2_of(wij));     // (a2, a1)
+  float2 t = __fmul2_rn(p, p);
+  t = __ffma2_rn(q, q, t);
+  v.a0 = p.x; v.a3 = p.y; v.a2 = q.x; v.a1 = q.y;
+  k2 = t.x + t.y;
+}
+
 // one Cabibbo-Marinari subgroup hit on rows (I,J) of U given the staple sum A
 template <typename R, int KIND, int I, int J>
 __device__ __forceinline__ void su3_subgroup_hit(M3<R>& U, const M3<R>& A, uint32_t lex, const UpdateArgs& a, int mu, int sg,
@@ -271,15 +292,13 @@ __device__ __forceinline__ void su3_subgroup_hit(M3<R>& U, const M3<R>& A, uint3
   cdot3<CD_NN>(wij, U.e[I][0], U.e[I][1], U.e[I][2], A.e[0][J], A.e[1][J], A.e[2][J]);
   cdot3<CD_NN>(wji, U.e[J][0], U.e[J][1], U.e[J][2], A.e[0][I], A.e[1][I], A.e[2][I]);
   cdot3<CD_NN>(wjj, U.e[J][0], U.e[J][1], U.e[J][2], A.e[0][J], A.e[1][J], A.e[2][J]);
+  // v = 2 proj(W): the factor 1/2 of the projection is left out (four multiplies); k2 = 4 k^2
   Q4<R> v;
-  v.a0 = R(0.5) * (wii.re + wjj.re);
-  v.a1 = R(0.5) * (wij.im + wji.im);
-  v.a2 = R(0.5) * (wij.re - wji.re);
-  v.a3 = R(0.5) * (wii.im - wjj.im);
-  const R k2 = v.a0 * v.a0 + v.a1 * v.a1 + v.a2 * v.a2 + v.a3 * v.a3;
+  R k2;
+  su3_project2(wii, wij, wji, wjj, v, k2);
   // reading R4 (k -> 0) and R5 (all trials rejected): the subgroup factor is the identity.  Applied as a = 1 rather than
   // by skipping the row update (1 * u + 0 * u' = u exactly), so that the warp does not diverge around it.
-  const bool tiny = k2 < Tiny<R>::k2();
+  const bool tiny = k2 < R(4) * Tiny<R>::k2();
   if constexpr (sizeof(R) == 8) { if (tiny) { code = 0; return; } }
   Q4<R> q;
   int cd = 0;
