@@ -44,15 +44,16 @@ LINK_SIZES_PER_HIT = 2 * len(DIMS) + 1
 # flops per link-hit EXECUTED by the kernels this file launches: ncu's per-opcode thread-instruction counts
 # (sass__thread_inst_executed_true_per_opcode) of one launch / V/2, weighted FFMA2 4, FMUL2 / FADD2 / FFMA / DFMA 2,
 # FMUL / FADD / DMUL / DADD / MUFU 1  (profiles/r2_flop_count.md; SURVEY 8(d)'s estimates were 4030 / 4270 / 3270 / 3900)
-FLOPS_PER_HIT = {"f32": {"hb": 3932.0, "or": 3707.0}, "f64": {"hb": 3915.0, "or": 3183.0}}
-FLOPS_SOURCE = "profiles/r2_flop_count.md"
+FLOPS_PER_HIT = {"f32": {"hb": 3944.0, "or": 3719.0}, "f64": {"hb": 3909.0, "or": 3171.0}}
+FLOPS_SOURCE = "profiles/r2_d_final.md (weights: profiles/r2_flop_count.md)"
 
 
 # the dominant kernel of each arm (overrelaxation: 32 of the 40 update launches of a step) and its DRAM traffic per launch,
 # dram__bytes_read.sum + dram__bytes_write.sum of one `ncu --set full` capture of this workload (bytes)
 OR_KERNEL = {"f32": "su3_update_tiled_kernel<float, x12, OR>", "f64": "su3_update_kernel<double, x18, OR>"}
-NCU_TRAFFIC = {"f32": {"or": 220620000, "hb": 225480000}, "f64": {"or": 658150000, "hb": 665560000},
-               "source": "profiles/r2_b_heatbath.md"}
+NCU_TRAFFIC = {"f32": {"or": 220570000, "hb": 225180000}, "f64": {"or": 658960000, "hb": 665390000},
+               "source": "profiles/r2_d_final.md (cache flush between ncu replays; 142 + 24 / 534 + 77 MB read + write with the caches "
+                         "left alone, profiles/r2_c_launch_order.md)"}
 
 
 def load_peaks():
