@@ -465,19 +465,6 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
   };
 
   const uint32_t lex = lex_global(g, sc);
-  // heatbath: the random-number-only part of trial 0 and the direction of each subgroup, parked in shared memory behind
-  // the ring ([subgroup][5][B] reals, this thread's column).  It does not touch the links, so it runs before pdl_wait():
-  // in the tail of the previous sub-step's kernel when this CTA became resident early.
-  R* draws = reinterpret_cast<R*>(ring_raw + (size_t)K * NP * B * sizeof(Vec)) + threadIdx.x;
-  if constexpr (KIND == 0) {
-#pragma unroll 1
-    for (int sg = 0; sg < 3; ++sg) {
-      const HbDraw<R> d = hb_first_draw<R>(lex, a, MU, sg);
-      R* o = draws + sg * 5 * B;
-      o[0] = d.E; o[B] = d.w; o[2 * B] = d.n1; o[3 * B] = d.n2; o[4 * B] = d.n3;
-    }
-  }
-
   // Prologue: links 0 .. K-2 of the first direction nu0.  They come from the arrays (q, mu), (p, nu0), (q, nu0); unless the
   // update kernel running just before this one writes one of them, they are fetched before griddepcontrol.wait, i.e.
   // while that kernel drains (in sweep order the previous kernel writes (p, mu-1): only mu = 1 has to wait).  The trigger
@@ -490,6 +477,20 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
     if constexpr (K > 0) static_for<0, KR - 1>([&](auto jc) { issue(jc, cur, decltype(jc)::value); cp_async_commit(); });
   };
   if (early) prologue();
+  // heatbath: the random-number-only part of trial 0 and the direction of each subgroup, parked in shared memory behind
+  // the ring ([subgroup][5][B] reals, this thread's column).  It does not touch the links, so it runs before pdl_wait()
+  // -- in the tail of the previous sub-step's kernel when this CTA became resident early -- and after the early prologue,
+  // whose loads are then in flight meanwhile.
+  R* draws = reinterpret_cast<R*>(ring_raw + (size_t)K * NP * B * sizeof(Vec)) + threadIdx.x;
+  if constexpr (KIND == 0) {
+#pragma unroll 1
+    for (int sg = 0; sg < 3; ++sg) {
+      const HbDraw<R> d = hb_first_draw<R>(lex, a, MU, sg);
+      R* o = draws + sg * 5 * B;
+      o[0] = d.E; o[B] = d.w; o[2 * B] = d.n1; o[3 * B] = d.n2; o[4 * B] = d.n3;
+    }
+  }
+
   pdl_wait();                                                      // the previous sub-step's links are complete and visible
   pdl_trigger();
   if (!early) prologue();
