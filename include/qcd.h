@@ -147,6 +147,11 @@ int qcd_debug_get_trials(qcd_lattice_t* lat, uint8_t* dst, size_t bytes);
  * impl 0: this library's generator; impl 1: cuRAND's curand_Philox4x32_10 compiled into a kernel (cross-check). */
 int qcd_debug_philox(const uint32_t* ctr, const uint32_t* key, size_t n, uint32_t* out, int impl);
 
+/* The fp64 heatbath's elementary functions (csrc/hb_math.cuh) evaluated on the device for n 32-bit words w (host arrays):
+ * out[7 i + 0..6] = ln u, cos^2(2 pi u), sin(2 pi u), cos(2 pi u) with u = (w + 1/2) 2^-32, and sqrt(x), 1/sqrt(x), 1/x
+ * with x = u.  Lets a test compare the device forms (hardware seeds) with libm directly. */
+int qcd_debug_hb_math(const uint32_t* words, size_t n, double* out);
+
 /* Profiling (QCD_OPT_PROFILE = 1): summed device time (ms, CUDA events on the lattice's stream) and launch count of
  * the update kernels of `kind` since the last qcd_reset_profile.  Synchronises the stream. */
 int qcd_get_profile(qcd_lattice_t* lat, int kind, double* total_ms, uint64_t* launches);

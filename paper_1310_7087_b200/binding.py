@@ -22,7 +22,7 @@ QCD_OPT_KP_MAX_TRIALS, QCD_OPT_DEBUG_TRIALS, QCD_OPT_PROFILE, QCD_OPT_BULK_COPY,
 SYMBOLS = [
     "qcd_lattice_bytes", "qcd_lattice_create", "qcd_lattice_destroy", "qcd_init", "qcd_sweep", "qcd_measure",
     "qcd_get_links", "qcd_set_links", "qcd_get_sweep_counter", "qcd_set_sweep_counter", "qcd_get_seed", "qcd_set_seed",
-    "qcd_set_option", "qcd_debug_substep", "qcd_debug_get_trials", "qcd_debug_philox", "qcd_get_profile",
+    "qcd_set_option", "qcd_debug_substep", "qcd_debug_get_trials", "qcd_debug_philox", "qcd_debug_hb_math", "qcd_get_profile",
     "qcd_reset_profile", "qcd_get_launch_count", "qcd_measure_accumulate", "qcd_sweep_measure", "qcd_sweep_measure_accumulate", "qcd_accum_get", "qcd_accum_reset", "qcd_probe_fma_tflops", "qcd_probe_copy_gbs", "qcd_last_error",
     "qcd_version",
     "qcd_slab_bytes", "qcd_slab_create", "qcd_slab_halo_bytes", "qcd_slab_halo_pack", "qcd_slab_halo_unpack", "qcd_slab_measure_sums",
@@ -81,6 +81,7 @@ def lib():
     L.qcd_debug_substep.argtypes = [p, d, i, i, i, i, fp]
     L.qcd_debug_get_trials.argtypes = [p, p, sz]
     L.qcd_debug_philox.argtypes = [p, p, sz, p, i]
+    L.qcd_debug_hb_math.argtypes = [p, sz, p]
     L.qcd_get_profile.argtypes = [p, i, dp, C.POINTER(C.c_uint64)]
     L.qcd_reset_profile.argtypes = [p]
     L.qcd_get_launch_count.argtypes = [p, C.POINTER(C.c_uint64)]
@@ -169,6 +170,14 @@ def qcd_debug_philox(ctr, key, impl=0):
     assert len(ctr) == len(key)
     out = np.zeros_like(ctr)
     _check(lib().qcd_debug_philox(ctr.ctypes.data, key.ctypes.data, len(ctr), out.ctypes.data, int(impl)))
+    return out
+
+
+def qcd_debug_hb_math(words):
+    """rows (ln u, cos^2 2 pi u, sin 2 pi u, cos 2 pi u, sqrt u, 1/sqrt u, 1/u), u = (w + 1/2) 2^-32, computed on the device"""
+    words = np.ascontiguousarray(words, dtype=np.uint32).reshape(-1)
+    out = np.zeros((len(words), 7), dtype=np.float64)
+    _check(lib().qcd_debug_hb_math(words.ctypes.data, len(words), out.ctypes.data))
     return out
 
 

@@ -387,6 +387,17 @@ __global__ void __launch_bounds__(256) copy_probe_kernel(const float4* __restric
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) dst[i] = __ldg(src + i);
 }
 
+__global__ void hb_math_debug_kernel(const uint32_t* w, size_t n, double* out) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const double u = uniform64(w[i]);
+  double sn, cs;
+  hbm::sincos_2pi_uniform32(w[i], &sn, &cs);
+  double* o = out + 7 * i;
+  o[0] = hbm::log_uniform32(w[i]); o[1] = hbm::cos2_2pi_uniform32(w[i]); o[2] = sn; o[3] = cs;
+  o[4] = hbm::sqrt_pos(u); o[5] = hbm::rsqrt(u); o[6] = hbm::rcp(u);
+}
+
 __global__ void philox_debug_kernel(const uint32_t* ctr, const uint32_t* key, size_t n, uint32_t* out, int impl) {
   const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
@@ -807,6 +818,24 @@ int qcd_debug_philox(const uint32_t* ctr, const uint32_t* key, size_t n, uint32_
   if (e == cudaSuccess) e = cudaMemcpy(out, dout, n * 16, cudaMemcpyDeviceToHost);
   cudaFree(dc); cudaFree(dk); cudaFree(dout);
   if (e != cudaSuccess) return fail(QCD_ERR_CUDA, std::string("debug_philox: ") + cudaGetErrorString(e));
+  return QCD_OK;
+}
+
+int qcd_debug_hb_math(const uint32_t* words, size_t n, double* out) {
+  if (!words || !out) return fail(QCD_ERR_INVALID_ARG, "NULL argument");
+  if (n == 0) return QCD_OK;
+  uint32_t* dw = nullptr;
+  double* dout = nullptr;
+  cudaError_t e = cudaMalloc(&dw, n * 4);
+  if (e == cudaSuccess) e = cudaMalloc(&dout, n * 56);
+  if (e == cudaSuccess) e = cudaMemcpy(dw, words, n * 4, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) {
+    hb_math_debug_kernel<<<(unsigned)((n + 255) / 256), 256>>>(dw, n, dout);
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) e = cudaMemcpy(out, dout, n * 56, cudaMemcpyDeviceToHost);
+  cudaFree(dw); cudaFree(dout);
+  if (e != cudaSuccess) return fail(QCD_ERR_CUDA, std::string("debug_hb_math: ") + cudaGetErrorString(e));
   return QCD_OK;
 }
 

@@ -14,7 +14,8 @@
 // remainder is below 1e-17.  Errors, measured by tests/test_hb_math.py (this header compiled for the host, against libm
 // in long double over 10^6 random words and +-2000 words around every fold point): ln u 2.5e-15 absolute (|ln u| <= 22.9,
 // i.e. 0.7 units in the last place of the result), cos^2 / sin / cos 2e-16 absolute, sqrt / rsqrt / rcp 1.4e-16
-// relative.  The link tolerance against the fp64 oracle is 1e-12, and an accept decision changes only if its margin is
+// relative; the same bounds on the device through qcd_debug_hb_math (`test_heatbath_functions_on_the_device_against_libm`).
+// The link tolerance against the fp64 oracle is 1e-12, and an accept decision changes only if its margin is
 // below these errors (probability ~1e-15 per trial).
 #pragma once
 #include <stdint.h>

@@ -525,6 +525,34 @@ def test_launch_order_does_not_change_any_result(qcd):
         assert oa[0] == ob[0] and np.array_equal(oa[1], ob[1]) and oa[2] == ob[2], (dims, Nc, prec, flags)
 
 
+def test_heatbath_functions_on_the_device_against_libm(qcd):
+    """csrc/hb_math.cuh as the GPU evaluates it (MUFU.RCP64H / RSQ64H seeds, constant-bank coefficients) against numpy in
+    extended precision: ln u, cos^2, sin, cos of 2 pi u for u = (w + 1/2) 2^-32, and sqrt / rsqrt / rcp -- random words
+    and the neighbourhood of every fold point of the integer argument reductions.  Same bounds as the host test
+    (tests/test_hb_math.py)."""
+    rng = np.random.default_rng(99)
+    edges = np.array([0x00000000, 0x1fffffff, 0x20000000, 0x3fffffff, 0x40000000, 0x5fffffff, 0x60000000, 0x7fffffff, 0x80000000,
+                      0x9fffffff, 0xa0000000, 0xbfffffff, 0xc0000000, 0xdfffffff, 0xe0000000, 0xffffffff, 0x5a827999, 0xb504f333,
+                      0x6a09e667, 0x2d413ccc], dtype=np.int64)
+    near = ((edges[:, None] + np.arange(-300, 301)[None, :]) % (1 << 32)).reshape(-1)
+    words = np.concatenate([near, rng.integers(0, 1 << 32, size=400000, dtype=np.int64)]).astype(np.uint32)
+    got = qcd.qcd_debug_hb_math(words)
+    ld = np.longdouble
+    u = (words.astype(ld) + ld(0.5)) / ld(4294967296.0)
+    assert np.finfo(ld).eps < 2e-19, "needs an extended-precision long double (x86-64)"
+    ang = 2 * ld("3.14159265358979323846264338327950288") * u
+    err = lambda a, b: float(np.max(np.abs(a.astype(ld) - b)))
+    assert err(got[:, 0], np.log(u)) < 5e-15
+    # reference angle good to ~1e-18 (64-bit mantissa)
+    assert err(got[:, 1], np.cos(ang) ** 2) < 4e-16
+    assert err(got[:, 2], np.sin(ang)) < 4e-16
+    assert err(got[:, 3], np.cos(ang)) < 4e-16
+    rel = lambda a, b: float(np.max(np.abs(a.astype(ld) / b - 1)))
+    assert rel(got[:, 4], np.sqrt(u)) < 3e-16
+    assert rel(got[:, 5], 1 / np.sqrt(u)) < 3e-16
+    assert rel(got[:, 6], 1 / u) < 3e-16
+
+
 def test_overrelaxation_conserves_action_on_gpu(qcd):
     dims = (8, 8, 8, 8)
     for Nc, prec, flags, tol in [(3, 1, 0, 1e-12), (3, 0, 1, 3e-6), (2, 1, 0, 1e-12)]:
