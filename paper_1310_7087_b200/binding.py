@@ -184,9 +184,10 @@ def qcd_debug_hb_math(words):
 class Lattice:
     """One lattice handle.  Device memory comes from a torch uint8 tensor, the stream from torch.
     slab = (offset, extent): a part of the lattice of global extents `dims`, split along direction D-2 (qcd_slab_create);
-    then dims / V describe the part's own block and global_dims the whole lattice."""
+    then dims / V describe the part's own block and global_dims the whole lattice.
+    mem: a torch uint8 CUDA tensor to use as the lattice's memory (at least nbytes long) instead of allocating one."""
 
-    def __init__(self, dims, Nc, precision=QCD_FP64, flags=0, device="cuda:0", library_alloc=False, slab=None):
+    def __init__(self, dims, Nc, precision=QCD_FP64, flags=0, device="cuda:0", library_alloc=False, slab=None, mem=None):
         import torch
         self.global_dims = tuple(int(x) for x in dims)
         self.D, self.Nc, self.precision, self.flags = len(self.global_dims), int(Nc), int(precision), int(flags)
@@ -203,9 +204,14 @@ class Lattice:
         self._mem = None
         self._device = torch.device(device)
         mem_ptr, stream_ptr = None, None
+        self.nbytes = int(nbytes)
         if nbytes and not library_alloc:
             with torch.cuda.device(self._device):
-                self._mem = torch.empty(int(nbytes), dtype=torch.uint8, device=self._device)
+                if mem is None:
+                    self._mem = torch.empty(int(nbytes), dtype=torch.uint8, device=self._device)
+                else:
+                    assert mem.dtype == torch.uint8 and mem.is_cuda and mem.numel() >= int(nbytes) and mem.data_ptr() % 256 == 0
+                    self._mem = mem
                 mem_ptr = self._mem.data_ptr()
                 stream_ptr = torch.cuda.current_stream().cuda_stream
         elif nbytes:

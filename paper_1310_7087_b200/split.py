@@ -165,3 +165,161 @@ class GpuPart:
 
     def set_sweep_counter(self, v):
         self.lat.qcd_set_sweep_counter(v)
+
+
+class StreamedLattice:
+    """A divided lattice whose parts live in pinned HOST memory and pass through ONE device buffer, part by part, in every
+    sub-step: the paper's other use of the division -- "when one device's memory is not enough".  Host-side
+    bookkeeping only; every step runs in the kernels of the slab handles (qcd_slab_*), all created over the same device
+    buffer.  Per sub-step and part: upload the part (its internal layout, halo layers included), unpack the boundary layers
+    its neighbours have produced since its last turn, update, pack its own two boundary layers of the array just written
+    for the neighbours, download.  The messages stay on the device (two layers per array and part).
+    Each sub-step moves the whole lattice over the host link twice, so this is two orders of magnitude slower than a
+    resident lattice: it exists for lattices beyond the 180 GB of one B200, and is tested on small ones,
+    where it must reproduce the undivided sweep bit for bit."""
+
+    def __init__(self, q, dims, Nc, precision, flags=0, n_parts=2, extents=None, device="cuda:0"):
+        import torch
+        self.q, self.torch, self.device = q, torch, torch.device(device)
+        self.dims, self.D = tuple(int(x) for x in dims), len(dims)
+        sd = self.D - 2
+        if extents is None:
+            self.parts = partition(self.dims[sd], n_parts)
+        else:
+            off, self.parts = 0, []
+            for e in extents:
+                self.parts.append((off, int(e)))
+                off += int(e)
+            assert off == self.dims[sd]
+        self.n = len(self.parts)
+        import ctypes
+        arr = (ctypes.c_int * self.D)(*self.dims)
+        probe = [int(q.lib().qcd_slab_bytes(self.D, arr, int(Nc), int(precision), int(flags), o, e)) for o, e in self.parts]
+        with torch.cuda.device(self.device):
+            self.buf = torch.empty(max(probe), dtype=torch.uint8, device=self.device)
+        self.lat = [q.Lattice(self.dims, Nc, precision, flags, device=device, slab=pe, mem=self.buf) for pe in self.parts]
+        self.host = [torch.empty(L.nbytes, dtype=torch.uint8, pin_memory=True) for L in self.lat]
+        self.hbytes = [L.qcd_slab_halo_bytes() for L in self.lat]
+        self.pending = [dict() for _ in range(self.n)]       # per part: {(parity, mu, unpack side): message tensor}
+        self.resident = None
+        self.sweep_counter = 0
+        self.bytes_moved = 0
+
+    def close(self):
+        for L in self.lat:
+            L.close()
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    # ---- residency
+    def _upload(self, k):
+        """part k into the device buffer, then the boundary layers that arrived since it was last there"""
+        L = self.lat[k]
+        self.buf[:L.nbytes].copy_(self.host[k], non_blocking=True)
+        self.bytes_moved += L.nbytes
+        self.resident = k
+        for (parity, mu, side), msg in self.pending[k].items():
+            L.qcd_slab_halo_unpack(parity, mu, side, msg.data_ptr(), self.hbytes[k])
+        # (an unpack tells the handle that its arrays were written behind its back: no early loads in the next kernel)
+        if not self.pending[k]:
+            raise RuntimeError("a part must have received its halo layers before its first turn (call refresh_all)")
+        self.pending[k] = {}
+
+    def _download(self, k):
+        L = self.lat[k]
+        self.host[k].copy_(self.buf[:L.nbytes], non_blocking=True)
+        self.torch.cuda.current_stream().synchronize()      # the buffer is reused by the next part
+        self.bytes_moved += L.nbytes
+
+    def _post(self, k, parity, mu):
+        """the two boundary layers of array (parity, mu) of the resident part k, as messages to its neighbours"""
+        L = self.lat[k]
+        for side, dst, uside in halo_messages(k, self.n):
+            msg = self.torch.empty(self.hbytes[k], dtype=self.torch.uint8, device=self.device)
+            L.qcd_slab_halo_pack(parity, mu, side, msg.data_ptr(), self.hbytes[k])
+            self.pending[dst][(parity, mu, uside)] = msg
+
+    def refresh_all(self):
+        """after the parts were set as a whole: every array's boundary layers to the neighbours"""
+        for k in range(self.n):
+            L = self.lat[k]
+            self.buf[:L.nbytes].copy_(self.host[k], non_blocking=True)
+            for parity in (0, 1):
+                for mu in range(self.D):
+                    self._post(k, parity, mu)
+            self.torch.cuda.current_stream().synchronize()
+
+    # ---- the lattice as a whole
+    def init(self, start, seed):
+        for k, L in enumerate(self.lat):
+            L.qcd_init(start, seed)
+            self._download(k)
+        self.refresh_all()
+
+    def set_seed(self, seed):
+        for L in self.lat:
+            L.qcd_set_seed(seed)
+
+    def set_links(self, links):
+        """canonical [lex][mu][N][N] of the whole lattice"""
+        import numpy as np
+        sd = self.D - 2
+        a = np.asarray(links).reshape(tuple(reversed(self.dims)) + np.asarray(links).shape[1:])
+        for k, (off, ext) in enumerate(self.parts):
+            idx = [slice(None)] * self.D
+            idx[self.D - 1 - sd] = slice(off, off + ext)
+            blk = np.ascontiguousarray(a[tuple(idx)])
+            self.lat[k].qcd_set_links(blk.reshape((-1,) + blk.shape[self.D:]))
+            self._download(k)
+        self.refresh_all()
+
+    def get_links(self):
+        import numpy as np
+        sd = self.D - 2
+        out = None
+        for k, (off, ext) in enumerate(self.parts):
+            L = self.lat[k]
+            self.buf[:L.nbytes].copy_(self.host[k], non_blocking=True)
+            blk = L.qcd_get_links()
+            if out is None:
+                out = np.zeros(tuple(reversed(self.dims)) + blk.shape[1:], dtype=blk.dtype)
+            idx = [slice(None)] * self.D
+            idx[self.D - 1 - sd] = slice(off, off + ext)
+            shape = list(reversed(self.dims))
+            shape[self.D - 1 - sd] = ext
+            out[tuple(idx)] = blk.reshape(tuple(shape) + blk.shape[1:])
+        return out.reshape((-1,) + out.shape[self.D:])
+
+    def substep(self, beta, kind, hit, parity, mu, field=None):
+        for k in range(self.n):
+            self._upload(k)
+            self.lat[k].qcd_debug_substep(beta, kind, hit, parity, mu, field)
+            self._post(k, parity, mu)
+            self._download(k)
+
+    def sweep(self, beta, n_hb, n_or, field=None):
+        for kind, hit, parity, mu in sweep_schedule(self.D, n_hb, n_or):
+            self.substep(beta, kind, hit, parity, mu, field)
+        self.sweep_counter += 1
+        for L in self.lat:
+            L.qcd_set_sweep_counter(self.sweep_counter)
+
+    def measure(self, field=None):
+        import numpy as np
+        planes, poly = None, 0j
+        for k in range(self.n):
+            L = self.lat[k]
+            self.buf[:L.nbytes].copy_(self.host[k], non_blocking=True)
+            for (parity, mu, side), msg in self.pending[k].items():
+                L.qcd_slab_halo_unpack(parity, mu, side, msg.data_ptr(), self.hbytes[k])
+            pk, lk = L.qcd_slab_measure_sums(field)
+            planes = pk if planes is None else planes + pk
+            poly += lk
+        V = int(np.prod(self.dims))
+        planes = planes / V
+        Vs = V // self.dims[-1]
+        return float(planes.mean()), planes, poly / Vs

@@ -194,3 +194,42 @@ def test_split_error_paths(qcd):
         S.qcd_split_init(qcd.QCD_COLD, 1)
         tot, planes, poly = S.qcd_split_measure()
         assert tot == 1.0 and np.all(planes == 1.0) and poly == 1.0
+
+
+@pytest.mark.parametrize("variant", [(3, 1, 0), (3, 0, 1), (2, 0, 0)], ids=["su3-f64x18", "su3-f32x12", "su2-f32"])
+@pytest.mark.parametrize("dims,extents,fld", [((8, 6, 8, 4), [2, 4, 2], (1, 2)), ((8, 6, 8, 4), [8], None), ((6, 8, 4), [4, 4], None)])
+def test_streamed_lattice_reproduces_the_undivided_sweep(qcd, variant, dims, extents, fld):
+    """split.StreamedLattice: the parts live in pinned host memory and pass through one device buffer in every sub-step
+    (the paper's use of the division when one device's memory is not enough).  From the same links and the
+    same hot start it must reproduce qcd_sweep bit for bit (dims[0] = 8 or 6: every kernel is the ring kernel on both sides)
+    and the observables within the measurement bars."""
+    from paper_1310_7087_b200 import split
+    Nc, prec, flags = variant
+    beta = 5.7 if Nc == 3 else 2.5
+    fg, _ = _field(qcd, fld, Nc)
+    links = _prep(dims, Nc, prec)
+    with qcd.Lattice(dims, Nc, prec, flags) as G, split.StreamedLattice(qcd, dims, Nc, prec, flags, extents=extents) as S:
+        G.qcd_set_seed(77)
+        S.set_seed(77)
+        G.qcd_set_links(links)
+        S.set_links(links)
+        cmp = slice(None) if flags == 0 else slice(0, 2)
+        assert np.array_equal(S.get_links().astype(np.complex128)[..., cmp, :], links[..., cmp, :])
+        for _ in range(2):
+            G.qcd_sweep(beta, 1, 1, fg)
+            S.sweep(beta, 1, 1, fg)
+        assert np.array_equal(G.qcd_get_links(), S.get_links())
+        ma, mb = G.qcd_measure(fg), S.measure(fg)
+        tol = MEAS_TOL[prec]
+        assert abs(ma[0] - mb[0]) < tol and np.max(np.abs(ma[1] - mb[1])) < tol and abs(ma[2] - mb[2]) < tol
+        # every sub-step moved every part to the device and back
+        per_substep = 2 * sum(L.nbytes for L in S.lat)
+        assert S.bytes_moved >= 2 * 2 * 2 * len(dims) * per_substep
+    # hot start through the parts = hot start of the whole lattice (Philox counters use the global site index)
+    with qcd.Lattice(dims, Nc, prec, flags) as G, split.StreamedLattice(qcd, dims, Nc, prec, flags, extents=extents) as S:
+        G.qcd_init(qcd.QCD_HOT, 5)
+        S.init(qcd.QCD_HOT, 5)
+        assert np.array_equal(G.qcd_get_links(), S.get_links())
+        G.qcd_sweep(beta, 1, 0, fg)
+        S.sweep(beta, 1, 0, fg)
+        assert np.array_equal(G.qcd_get_links(), S.get_links())
