@@ -159,7 +159,7 @@ def rep_stats(times, steps):
             "reps": len(t), "device_ms_total": sum(t)}
 
 
-def time_arm(q, torch, prec_name, steps, warmup, therm, seed, dist, sampler, bulk_copy=False, alternate=True):
+def time_arm(q, torch, prec_name, steps, warmup, therm, seed, dist, sampler, bulk_copy=False, alternate=True, full_exchange=False):
     """device-resident timing + end-to-end timing of one precision arm; returns a dict of raw numbers"""
     prec = q.QCD_FP32 if prec_name == "f32" else q.QCD_FP64
     flags = q.QCD_FLAG_COMPRESS12 if prec_name == "f32" else 0
@@ -212,7 +212,14 @@ def time_arm(q, torch, prec_name, steps, warmup, therm, seed, dist, sampler, bul
         n_acc, s1, _ = G.qcd_accum_get()
         out["acc_plaquette_mean"] = float(s1[:6].mean() / max(n_acc, 1))
         # (4) end to end through the C ABI with HOST buffers: every step uploads the configuration from pinned host
-        # memory (canonical layout), runs the working sweep, reads the observables and downloads the configuration
+        # memory, runs the working sweep, reads the observables and downloads the configuration.  Exchange layout: the
+        # canonical one; for the 12-real arm its compressed form (rows 0,1 of every link, QCD_OPT_EXCHANGE_ROWS01), i.e.
+        # exactly the reals the lattice stores -- a third less over the host link, nothing lost
+        if flags & q.QCD_FLAG_COMPRESS12 and not full_exchange:
+            G.qcd_set_option(q.QCD_OPT_EXCHANGE_ROWS01, 1)
+            out["exchange"] = "rows 0,1 of every link, [lex][mu][2][3][re,im] (QCD_OPT_EXCHANGE_ROWS01)"
+        else:
+            out["exchange"] = "canonical [lex][mu][3][3][re,im]"
         nbytes = G.canonical_bytes
         host = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
         G.qcd_get_links_ptr(host.data_ptr(), nbytes, 0)
@@ -341,7 +348,7 @@ def run_ours(args):
     other = "f64" if primary == "f32" else "f32"
     arms = {}
     for name in (primary, other):
-        arms[name] = time_arm(q, torch, name, args.steps, args.warmup, args.therm, replica_seed(rank), dist, sampler, args.bulk_copy, not args.same_order)
+        arms[name] = time_arm(q, torch, name, args.steps, args.warmup, args.therm, replica_seed(rank), dist, sampler, args.bulk_copy, not args.same_order, args.full_exchange)
     on_model = time_on_model(q, torch, dist, sampler, with_oracle=(world == 1 and rank == 0 and not args.no_cpu_baseline))
     clocks = sampler.stop()
     line = None
@@ -356,7 +363,7 @@ def run_ours(args):
                                                 "value": aggregate_value(world, a["links"], 1, upd["median_ms_per_step"])},
                           "e2e": {"value": aggregate_value(world, a["links"], 1, e2e["median_ms_per_step"]), "unit": UNIT,
                                   "h2d_bytes_per_step": a["h2d"], "d2h_bytes_per_step": a["d2h"],
-                                  "ms_per_step": e2e["median_ms_per_step"], "reps": e2e},
+                                  "ms_per_step": e2e["median_ms_per_step"], "reps": e2e, "exchange_layout": a["exchange"]},
                           "accumulate_on_device": {"ms_per_step": acc["median_ms_per_step"], "reps": acc,
                                                    "value": aggregate_value(world, a["links"], 1, acc["median_ms_per_step"]),
                                                    "plaquette_mean": a["acc_plaquette_mean"]},
@@ -484,6 +491,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--bulk-copy", action="store_true",
                     help="fp32 arm: overrelaxation by the bulk-copy kernel (QCD_OPT_BULK_COPY; the comparison of DESIGN.md sec 6.10)")
+    ap.add_argument("--full-exchange", action="store_true",
+                    help="e2e of the 12-real arm through the full 3 x 3 canonical layout instead of rows 0,1")
     ap.add_argument("--same-order", action="store_true",
                     help="every update launch visits the lattice in the same direction (QCD_OPT_ALTERNATE_ORDER = 0; the comparison "
                          "of DESIGN.md sec 6.5)")

@@ -50,9 +50,13 @@ enum {
                                 every operand with bulk asynchronous copies (cp.async.bulk + mbarriers, update_bulk.cuh) instead
                                 of the tiled cp.async kernel.  Same results to rounding; measured SLOWER:
                                 default 0, kept so that the comparison can be repeated (bench.py --bulk-copy) */
-  QCD_OPT_ALTERNATE_ORDER = 4 /* 1 (default): consecutive update launches visit the lattice in opposite directions, so that a
+  QCD_OPT_ALTERNATE_ORDER = 4, /* 1 (default): consecutive update launches visit the lattice in opposite directions, so that a
                                 launch starts on the links the previous one touched last and finds them in the L2
                                 (DESIGN.md sec 6.5).  Results are bit-identical either way; 0 restores one direction */
+  QCD_OPT_EXCHANGE_ROWS01 = 5 /* 1: qcd_get_links / qcd_set_links of this lattice exchange rows 0,1 of every link only --
+                                [lex site][mu][2][3][re,im], V*D*12 reals -- i.e. exactly what a 12-real (COMPRESS12) SU(3)
+                                lattice stores: a third less over the host link, nothing lost (row 2 = conj(row0 x row1)).
+                                SU(3) with COMPRESS12 only; default 0 (full 3 x 3) */
 };
 
 /* Constant abelian background: every plaquette of plane (mu,nu), mu < nu, is multiplied on the left, at its

@@ -16,7 +16,7 @@ QCD_FP32, QCD_FP64 = 0, 1
 QCD_FLAG_COMPRESS12 = 1
 QCD_COLD, QCD_HOT = 0, 1
 QCD_KIND_HB, QCD_KIND_OR = 0, 1
-QCD_OPT_KP_MAX_TRIALS, QCD_OPT_DEBUG_TRIALS, QCD_OPT_PROFILE, QCD_OPT_BULK_COPY, QCD_OPT_ALTERNATE_ORDER = 0, 1, 2, 3, 4
+QCD_OPT_KP_MAX_TRIALS, QCD_OPT_DEBUG_TRIALS, QCD_OPT_PROFILE, QCD_OPT_BULK_COPY, QCD_OPT_ALTERNATE_ORDER, QCD_OPT_EXCHANGE_ROWS01 = 0, 1, 2, 3, 4, 5
 
 # every symbol include/qcd.h declares (tests check that the library exports all of them)
 SYMBOLS = [
@@ -222,6 +222,7 @@ class Lattice:
         else:
             _check(lib().qcd_slab_create(self.D, arr, self.Nc, self.precision, self.flags, self.slab[0], self.slab[1], mem_ptr,
                                          int(nbytes), stream_ptr, C.byref(self._h)))
+        self._rows = self.Nc                      # rows of a link in the exchange layout (2 with QCD_OPT_EXCHANGE_ROWS01)
         self.np_real = np.float32 if self.precision == QCD_FP32 else np.float64
         self.np_complex = np.complex64 if self.precision == QCD_FP32 else np.complex128
 
@@ -287,13 +288,13 @@ class Lattice:
 
     def qcd_get_links(self):
         """canonical (V, D, N, N) complex array in the lattice's precision (host)"""
-        out = np.zeros((self.V, self.D, self.Nc, self.Nc), dtype=self.np_complex)
+        out = np.zeros((self.V, self.D, self._rows, self.Nc), dtype=self.np_complex)
         _check(lib().qcd_get_links(self._h, out.ctypes.data, out.nbytes, 0))
         return out
 
     def qcd_set_links(self, links):
         a = np.ascontiguousarray(links, dtype=self.np_complex)
-        assert a.shape == (self.V, self.D, self.Nc, self.Nc), a.shape
+        assert a.shape == (self.V, self.D, self._rows, self.Nc), a.shape
         _check(lib().qcd_set_links(self._h, a.ctypes.data, a.nbytes, 0))
 
     def qcd_get_links_ptr(self, ptr, nbytes, is_device):
@@ -304,7 +305,7 @@ class Lattice:
 
     @property
     def canonical_bytes(self):
-        return self.V * self.D * self.Nc * self.Nc * 2 * (4 if self.precision == QCD_FP32 else 8)
+        return self.V * self.D * self._rows * self.Nc * 2 * (4 if self.precision == QCD_FP32 else 8)
 
     def qcd_get_sweep_counter(self):
         out = C.c_uint32(0)
@@ -324,6 +325,8 @@ class Lattice:
 
     def qcd_set_option(self, key, value):
         _check(lib().qcd_set_option(self._h, int(key), int(value)))
+        if int(key) == QCD_OPT_EXCHANGE_ROWS01:
+            self._rows = 2 if value else self.Nc
 
     def qcd_debug_substep(self, beta, kind, hit, parity, mu, field=None):
         _check(lib().qcd_debug_substep(self._h, float(beta), int(kind), int(hit), int(parity), int(mu), _fref(field)))

@@ -48,7 +48,7 @@ struct qcd_lattice {
   uint32_t sweep;
   bool has_links;
   int max_trials;
-  bool debug_trials, profile, bulk_copy, alternate_order;
+  bool debug_trials, profile, bulk_copy, alternate_order, exchange_rows01;
   uint8_t* d_trials;
   // per-block / per-warp partial sums of the reductions, one allocation of three regions (sizes fixed by the geometry):
   // [fused plaquette: NPL x np_warp][plaquette kernel: NPL x nb_plaq][Polyakov: 2 x nb_poly]
@@ -293,8 +293,18 @@ struct LayoutOp {
     typedef typename LinkIO<NC, R, COMP>::Vec Vec;
     constexpr int BL = LayoutShape<R>::BL;
     dim3 grid((lex_end - lex_begin + BL - 1) / BL, 1);
-    if (to_internal) layout_kernel<NC, D, R, COMP, true><<<grid, BL, 0, L->stream>>>(L->g, (Vec*)L->mem, (R*)canon, lex_begin, lex_end);
-    else layout_kernel<NC, D, R, COMP, false><<<grid, BL, 0, L->stream>>>(L->g, (Vec*)L->mem, (R*)canon, lex_begin, lex_end);
+    if constexpr (NC == 3 && COMP) {
+      if (L->exchange_rows01) {
+        if (to_internal) layout_kernel<NC, D, R, COMP, true, 2><<<grid, BL, 0, L->stream>>>(L->g, (Vec*)L->mem, (R*)canon, lex_begin, lex_end);
+        else layout_kernel<NC, D, R, COMP, false, 2><<<grid, BL, 0, L->stream>>>(L->g, (Vec*)L->mem, (R*)canon, lex_begin, lex_end);
+        CUDA_TRY(cudaGetLastError());
+        L->launches += 1;
+        L->last_parity = L->last_mu = to_internal ? -2 : -1;
+        return QCD_OK;
+      }
+    }
+    if (to_internal) layout_kernel<NC, D, R, COMP, true, NC><<<grid, BL, 0, L->stream>>>(L->g, (Vec*)L->mem, (R*)canon, lex_begin, lex_end);
+    else layout_kernel<NC, D, R, COMP, false, NC><<<grid, BL, 0, L->stream>>>(L->g, (Vec*)L->mem, (R*)canon, lex_begin, lex_end);
     CUDA_TRY(cudaGetLastError());
     L->launches += 1;
     if (to_internal) L->last_parity = L->last_mu = -2;             // link arrays were written
@@ -364,7 +374,7 @@ struct MeasureOp {
 };
 
 size_t canonical_bytes(const qcd_lattice* L) {
-  return (size_t)own_sites(L) * L->D * L->Nc * L->Nc * 2 * (L->precision == QCD_FP32 ? 4 : 8);
+  return (size_t)own_sites(L) * L->D * (L->exchange_rows01 ? 2 : L->Nc) * L->Nc * 2 * (L->precision == QCD_FP32 ? 4 : 8);
 }
 
 // ---- probes
@@ -445,7 +455,7 @@ static int create_lattice(int D, const int* dims, int Nc, int precision, unsigne
   L->bytes = need; L->mem = device_mem; L->owns_mem = false;
   L->stream = (cudaStream_t)cuda_stream;
   L->seed = 0; L->sweep = 0; L->has_links = false; L->max_trials = 10;
-  L->debug_trials = false; L->profile = false; L->bulk_copy = false; L->alternate_order = true;
+  L->debug_trials = false; L->profile = false; L->bulk_copy = false; L->alternate_order = true; L->exchange_rows01 = false;
   L->d_trials = nullptr; L->d_partials = nullptr; L->partials_cap = 0; L->d_results = nullptr; L->h_results = nullptr;
   L->prof_ms[0] = L->prof_ms[1] = 0.0; L->prof_n[0] = L->prof_n[1] = 0; L->launches = 0; L->order_toggle = 0; L->last_parity = L->last_mu = -2; L->d_canon = nullptr;
   L->side = nullptr; L->ev_fork = nullptr; L->ev_join = nullptr;
@@ -730,7 +740,7 @@ static int stage_chunks(qcd_lattice_t* L, char* host, bool to_internal) {
 int qcd_get_links(qcd_lattice_t* L, void* dst, size_t bytes, int dst_is_device) {
   if (!L || !dst) return fail(QCD_ERR_INVALID_ARG, "NULL argument");
   if (!L->has_links) return fail(QCD_ERR_STATE, "no links yet");
-  if (bytes != canonical_bytes(L)) return fail(QCD_ERR_INVALID_ARG, "bytes must equal V*D*N*N*2*sizeof(real)");
+  if (bytes != canonical_bytes(L)) return fail(QCD_ERR_INVALID_ARG, "bytes must equal V*D*N*N*2*sizeof(real) (V*D*2*3*2*sizeof(real) with EXCHANGE_ROWS01)");
   if (dst_is_device && ((uintptr_t)dst & 15u)) return fail(QCD_ERR_INVALID_ARG, "device pointer must be 16-byte aligned");
   if (!dst_is_device) return stage_chunks(L, (char*)dst, false);
   LayoutOp op{L, dst, false, 0u, own_sites(L)};
@@ -779,6 +789,10 @@ int qcd_set_option(qcd_lattice_t* L, int key, int value) {
     case QCD_OPT_PROFILE: L->profile = value != 0; return QCD_OK;
     case QCD_OPT_BULK_COPY: L->bulk_copy = value != 0; return QCD_OK;
     case QCD_OPT_ALTERNATE_ORDER: L->alternate_order = value != 0; return QCD_OK;
+    case QCD_OPT_EXCHANGE_ROWS01:
+      if (value != 0 && !(L->Nc == 3 && L->comp)) return fail(QCD_ERR_UNSUPPORTED, "EXCHANGE_ROWS01 needs SU(3) with COMPRESS12");
+      if ((value != 0) != L->exchange_rows01 && L->d_canon) { cudaFree(L->d_canon); L->d_canon = nullptr; }   // chunk geometry changes
+      L->exchange_rows01 = value != 0; return QCD_OK;
   }
   return fail(QCD_ERR_INVALID_ARG, "unknown option key");
 }

@@ -151,7 +151,9 @@ __global__ void __launch_bounds__(128) init_kernel(Geom g, typename LinkIO<NC, R
 // sites per CTA of layout_kernel: one CTA's block of the canonical array (BL * D * N*N complex numbers) fits 48 KB
 template <typename R> struct LayoutShape { static constexpr int BL = sizeof(R) == 4 ? 128 : 64; };
 
-template <int NC, int D, typename R, bool COMP, bool TO_INTERNAL>
+// NRC = rows of a link in the canonical array: NC, or 2 for the compressed exchange format of 12-real SU(3) lattices
+// (QCD_OPT_EXCHANGE_ROWS01: rows 0,1 only, [lex][mu][2][3][re,im]).
+template <int NC, int D, typename R, bool COMP, bool TO_INTERNAL, int NRC>
 __global__ void __launch_bounds__(LayoutShape<R>::BL) layout_kernel(Geom g, typename LinkIO<NC, R, COMP>::Vec* links, R* canon,
                                                                     uint32_t lex_begin, uint32_t lex_end) {
   // sites [lex_begin, lex_end); `canon` is the canonical address of site lex_begin (a chunk of a host transfer, or the
@@ -164,7 +166,8 @@ __global__ void __launch_bounds__(LayoutShape<R>::BL) layout_kernel(Geom g, type
   // and half-warp.
   typedef LinkIO<NC, R, COMP> IO;
   typedef typename std::conditional<sizeof(R) == 4, float2, double2>::type C2;   // one complex number of the canonical array
-  constexpr int BL = LayoutShape<R>::BL, NCX = D * NC * NC, PITCH = NCX + 1;
+  static_assert(NRC == NC || (NRC == 2 && NC == 3 && COMP), "rows 0,1 only for 12-real SU(3) links");
+  constexpr int BL = LayoutShape<R>::BL, NCX = D * NRC * NC, PITCH = NCX + 1;
   __shared__ C2 buf[BL * PITCH];
   const uint32_t lex0 = lex_begin + blockIdx.x * BL, t = threadIdx.x;
   const uint32_t nsite = (lex_end - lex0 < (uint32_t)BL) ? lex_end - lex0 : (uint32_t)BL;
@@ -186,19 +189,22 @@ __global__ void __launch_bounds__(LayoutShape<R>::BL) layout_kernel(Geom g, type
     const int p = (int)(((lex & 1u) + x1 + x2 + x3) & 1u);         // x0 & 1 = lex & 1 (L0 even)
 #pragma unroll
     for (int mu = 0; mu < D; ++mu) {
-      C2* c = buf + t * PITCH + mu * NC * NC;
+      C2* c = buf + t * PITCH + mu * NRC * NC;
       Cx<R> m[NC][NC];
       const size_t base = array_base<IO::T::NP>(g, D, p, mu);
       if (TO_INTERNAL) {
 #pragma unroll
         for (int i = 0; i < NC; ++i)
 #pragma unroll
-          for (int j = 0; j < NC; ++j) { const C2 v = c[i * NC + j]; m[i][j] = cx<R>(v.x, v.y); }
+          for (int j = 0; j < NC; ++j) {
+            if (i < NRC) { const C2 v = c[i * NC + j]; m[i][j] = cx<R>(v.x, v.y); }
+            else m[i][j] = cx<R>(R(0), R(0));                      // row 2 is not stored by 12-real links
+          }
         IO::store(m, links, g, base, h);
       } else {
         IO::template load<false>(m, links, g, base, h);
 #pragma unroll
-        for (int i = 0; i < NC; ++i)
+        for (int i = 0; i < NRC; ++i)
 #pragma unroll
           for (int j = 0; j < NC; ++j) { C2 v; v.x = m[i][j].re; v.y = m[i][j].im; c[i * NC + j] = v; }
       }

@@ -553,6 +553,40 @@ def test_heatbath_functions_on_the_device_against_libm(qcd):
     assert rel(got[:, 6], 1 / u) < 3e-16
 
 
+def test_exchange_rows01_is_the_compressed_form_of_the_canonical_layout(qcd):
+    """QCD_OPT_EXCHANGE_ROWS01: qcd_get_links / qcd_set_links of a 12-real SU(3) lattice move rows 0,1 only
+    ([lex][mu][2][3]): the same numbers as rows 0,1 of the full canonical array, in both directions and through host and
+    device pointers, whole lattice and chunked staging (a lattice larger than one 64 MiB chunk); refused elsewhere."""
+    import torch
+    for dims, prec in [((6, 4, 10, 2), 0), ((6, 4, 10, 2), 1), ((6, 4, 10), 0), ((48, 32, 32, 32), 0)]:
+        with gpu_lattice(qcd, dims, 3, prec, 1) as G:
+            G.qcd_init(qcd.QCD_HOT, 3)
+            full = G.qcd_get_links()
+            G.qcd_set_option(qcd.QCD_OPT_EXCHANGE_ROWS01, 1)
+            assert G.canonical_bytes == full.nbytes * 2 // 3
+            half = G.qcd_get_links()
+            assert half.shape == full.shape[:2] + (2, 3) and np.array_equal(half, full[:, :, :2, :])
+            # device pointer form
+            dev = torch.empty(G.canonical_bytes, dtype=torch.uint8, device="cuda")
+            G.qcd_get_links_ptr(dev.data_ptr(), G.canonical_bytes, 1)
+            torch.cuda.synchronize()
+            assert np.array_equal(dev.cpu().numpy().view(half.dtype).reshape(half.shape), half)
+            # and back in: a cold lattice takes the rows and returns the same configuration
+            G.qcd_init(qcd.QCD_COLD, 0)
+            G.qcd_set_links(half)
+            G.qcd_set_option(qcd.QCD_OPT_EXCHANGE_ROWS01, 0)
+            assert np.array_equal(G.qcd_get_links(), full)
+            G.qcd_set_option(qcd.QCD_OPT_EXCHANGE_ROWS01, 1)
+            G.qcd_init(qcd.QCD_COLD, 0)
+            G.qcd_set_links_ptr(dev.data_ptr(), G.canonical_bytes, 1)
+            G.qcd_set_option(qcd.QCD_OPT_EXCHANGE_ROWS01, 0)
+            assert np.array_equal(G.qcd_get_links(), full)
+    for Nc, flags in [(3, 0), (2, 0)]:
+        with gpu_lattice(qcd, (4, 4, 4, 4), Nc, 0, flags) as G:
+            with pytest.raises(qcd.QcdError):
+                G.qcd_set_option(qcd.QCD_OPT_EXCHANGE_ROWS01, 1)
+
+
 def test_overrelaxation_conserves_action_on_gpu(qcd):
     dims = (8, 8, 8, 8)
     for Nc, prec, flags, tol in [(3, 1, 0, 1e-12), (3, 0, 1, 3e-6), (2, 1, 0, 1e-12)]:
