@@ -114,6 +114,71 @@ __device__ __forceinline__ void m3_complete_row2(M3<float>& a) {
   }
 }
 
+// ---- staple accumulation with the third row summed in its unreduced form.
+// Every staple S is in SU(3), so its row 2 is conj(S0 x S1); the sum A = sum S needs the sum of those rows.  Instead of
+// rebuilding row 2 of each staple and adding it (per component: the cross product, its sign combination, an add), the
+// products of the cross product are accumulated over the staples directly:
+//   generic:  A[2][c] += conj(S[0][c1] S[1][c2] - S[0][c2] S[1][c1])        8 multiply-adds per component, nothing else
+//   float:    two packed running sums per component; the sign combination is applied ONCE per link (finish)
+// finish() ADDS the accumulated row to A's row 2 (which may already hold directly accumulated contributions).
+template <typename R> struct Row2Sum {
+  __device__ __forceinline__ void zero() {}
+  __device__ __forceinline__ void add(M3<R>& A, const M3<R>& S) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const int c1 = (c + 1) % 3, c2 = (c + 2) % 3;
+      const Cx<R>&p = S.e[0][c1], &q = S.e[1][c2], &r = S.e[0][c2], &s = S.e[1][c1];
+      R re = A.e[2][c].re, im = A.e[2][c].im;
+      re = q_fma(p.re, q.re, re); re = q_fma(-p.im, q.im, re); re = q_fma(-r.re, s.re, re); re = q_fma(r.im, s.im, re);
+      im = q_fma(-p.re, q.im, im); im = q_fma(-p.im, q.re, im); im = q_fma(r.re, s.im, im); im = q_fma(r.im, s.re, im);
+      A.e[2][c].re = re; A.e[2][c].im = im;
+    }
+  }
+  __device__ __forceinline__ void finish(M3<R>&) const {}
+};
+template <> struct Row2Sum<float> {
+  float2 t1[3], t2[3];
+  __device__ __forceinline__ void zero() {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { t1[c] = make_float2(0.0f, 0.0f); t2[c] = make_float2(0.0f, 0.0f); }
+  }
+  __device__ __forceinline__ void add(M3<float>&, const M3<float>& S) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const int c1 = (c + 1) % 3, c2 = (c + 2) % 3;
+      const Cx<float>&p = S.e[0][c1], &q = S.e[1][c2], &r = S.e[0][c2], &s = S.e[1][c1];
+      t1[c] = __ffma2_rn(f2_bcast(p.re), f2_of(q), t1[c]);
+      t1[c] = __ffma2_rn(f2_bcast(-r.re), f2_of(s), t1[c]);
+      t2[c] = __ffma2_rn(f2_bcast(p.im), f2_swap(q), t2[c]);
+      t2[c] = __ffma2_rn(f2_bcast(-r.im), f2_swap(s), t2[c]);
+    }
+  }
+  __device__ __forceinline__ void finish(M3<float>& A) const {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      float2 v = __ffma2_rn(t1[c], make_float2(1.0f, -1.0f), make_float2(-t2[c].x, -t2[c].y));   // (t1.x - t2.x, -t1.y - t2.y)
+      v = __fadd2_rn(v, f2_of(A.e[2][c]));
+      A.e[2][c].re = v.x; A.e[2][c].im = v.y;
+    }
+  }
+};
+// rows 0,1 of a += rows 0,1 of s
+__device__ __forceinline__ void m3_add_rows01(M3<float>& a, const M3<float>& s) {
+#pragma unroll
+  for (int r = 0; r < 2; ++r)
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const float2 v = __fadd2_rn(f2_of(a.e[r][c]), f2_of(s.e[r][c]));
+      a.e[r][c].re = v.x; a.e[r][c].im = v.y;
+    }
+}
+template <typename R> __device__ __forceinline__ void m3_add_rows01(M3<R>& a, const M3<R>& s) {
+#pragma unroll
+  for (int r = 0; r < 2; ++r)
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { a.e[r][c].re += s.e[r][c].re; a.e[r][c].im += s.e[r][c].im; }
+}
+
 // The three product shapes, rows [0,NR) of acc += op(a) op(b), written as outer-product accumulation over k: the six
 // consecutive multiply-adds that follow share the scalar a.re (then a.im) in the same operand slot, which lets the
 // register-operand reuse cache serve it (the FP32 pipe is bounded by register-file reads).

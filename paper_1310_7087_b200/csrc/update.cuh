@@ -497,6 +497,8 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
 
   M3<R> A, P, Q;      // A: staple sum; P: the link kept for the next product (U2 / U1'); Q: X = U3 U2 or Y = U2' U1'
   m3_zero(A);
+  Row2Sum<R> row2;    // third row of the staple sum, accumulated in its unreduced form (sun_math.cuh); without a field only
+  row2.zero();
   M3<R> snap[NSNAP > 0 ? NSNAP : 1];
   auto direction_step = [&](int i) {
     const bool last = (i == D - 2);
@@ -531,9 +533,14 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
         M3<R> Sm;
         m3_zero(Sm);
         m3_mad_nd<R, 2>(Sm, U1, Q);                                // U1 X^+, rows 0,1; the staple is in SU(3): row 2 rebuilt
-        m3_complete_row2(Sm);
-        if (FIELD && fsign != 0) su3_scale_cols(Sm, a.f, fsign < 0);     // first direction: . F ; second: . F^+
-        m3_add(A, Sm);
+        if constexpr (!FIELD) {
+          m3_add_rows01(A, Sm);
+          row2.add(A, Sm);
+        } else {
+          m3_complete_row2(Sm);
+          if (fsign != 0) su3_scale_cols(Sm, a.f, fsign < 0);            // first direction: . F ; second: . F^+
+          m3_add(A, Sm);
+        }
       } else if constexpr (J == 3) {
         fetch(jc, cur, P, true, n0 + decltype(jc)::value);                                   // U1', all rows
       } else if constexpr (J == 4) {
@@ -550,8 +557,13 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
           M3<R> Sm;
           m3_zero(Sm);
           m3_mad_dn<R, 2>(Sm, Q, U3);                              // Y^+ U3'
-          m3_complete_row2(Sm);
-          m3_add(A, Sm);
+          if constexpr (!FIELD) {
+            m3_add_rows01(A, Sm);
+            row2.add(A, Sm);
+          } else {
+            m3_complete_row2(Sm);
+            m3_add(A, Sm);
+          }
         } else {
           m3_mad_dn<R, 3>(A, Q, U3);
         }
@@ -560,7 +572,7 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
     cur = nxt;
     if constexpr (NSNAP > 0) {
 #pragma unroll
-      for (int k = 0; k < NSNAP; ++k) if (i == k) snap[k] = A;   // directions come in the order nu = 0 .. mu-1, mu+1 ..
+      for (int k = 0; k < NSNAP; ++k) if (i == k) { snap[k] = A; row2.finish(snap[k]); }   // directions come in the order nu = 0 .. mu-1, mu+1 ..
     }
   };
   if constexpr (ROLL) {
@@ -571,6 +583,7 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
     for (int i = 0; i < D - 1; ++i) direction_step(i);
   }
 
+  row2.finish(A);
   // own link: the last one through the ring
   if constexpr (K > 0) cp_async_wait<0>();
   M3<R> U;

@@ -183,6 +183,8 @@ su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* 
 
   M3<R> A, P, Q;
   m3_zero(A);
+  Row2Sum<R> row2;                                             // third row of the staple sum, unreduced (sun_math.cuh)
+  row2.zero();
   M3<R> snap[NSNAP > 0 ? NSNAP : 1];
   auto phase = [&](int i) {
     const bool last = (i == D - 2);
@@ -229,9 +231,14 @@ su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* 
         M3<R> Sm;
         m3_zero(Sm);
         m3_mad_nd<R, NR>(Sm, U1, Q);                           // U1 X^+
-        if (COMP) m3_complete_row2(Sm);
-        if (FIELD && fsign != 0) su3_scale_cols(Sm, a.f, fsign < 0);
-        m3_add(A, Sm);
+        if constexpr (COMP && !FIELD) {
+          m3_add_rows01(A, Sm);
+          row2.add(A, Sm);
+        } else {
+          if (COMP) m3_complete_row2(Sm);
+          if (FIELD && fsign != 0) su3_scale_cols(Sm, a.f, fsign < 0);
+          m3_add(A, Sm);
+        }
       } else {
         m3_mad_nd<R, 3>(A, U1, Q);
       }
@@ -252,8 +259,13 @@ su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* 
         M3<R> Sm;
         m3_zero(Sm);
         m3_mad_dn<R, 2>(Sm, Q, U3);                            // Y^+ U3'
-        m3_complete_row2(Sm);
-        m3_add(A, Sm);
+        if constexpr (!FIELD) {
+          m3_add_rows01(A, Sm);
+          row2.add(A, Sm);
+        } else {
+          m3_complete_row2(Sm);
+          m3_add(A, Sm);
+        }
       } else {
         m3_mad_dn<R, 3>(A, Q, U3);
       }
@@ -261,7 +273,7 @@ su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* 
     cur = nxt;
     if constexpr (NSNAP > 0) {
 #pragma unroll
-      for (int k = 0; k < NSNAP; ++k) if (i == k) snap[k] = A;
+      for (int k = 0; k < NSNAP; ++k) if (i == k) { snap[k] = A; row2.finish(snap[k]); }
     }
   };
   if constexpr (ROLL) {
@@ -272,6 +284,7 @@ su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* 
     for (int i = 0; i < D - 1; ++i) phase(i);
   }
 
+  row2.finish(A);
   // own link: the last one through the ring
   cp_async_wait<0>();
   M3<R> U;
