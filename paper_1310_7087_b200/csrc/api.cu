@@ -937,6 +937,19 @@ struct HaloOp {
   }
 };
 
+struct HaloPairOp {
+  qcd_lattice* S; qcd_lattice* Tprev; int dst_prev; qcd_lattice* Tnext; int dst_next; int last_layer; int parity, mu; cudaStream_t st;
+  template <int NC, int D, typename R, bool COMP> int operator()() {
+    typedef typename LinkIO<NC, R, COMP>::Vec Vec;
+    constexpr int NP = LinkIO<NC, R, COMP>::T::NP;
+    const uint32_t count = S->g.Vh / (uint32_t)S->g.L[S->g.sd];          // half-indices of one layer
+    HaloTarget<Vec> t0{Tprev->g, (Vec*)Tprev->mem, 0, dst_prev}, t1{Tnext->g, (Vec*)Tnext->mem, last_layer, dst_next};
+    CUDA_TRY(launch_pdl(halo_pair_kernel<Vec, NP>, dim3((count + 127) / 128, 2), dim3(128), 0, st, S->g, (const Vec*)S->mem, t0, t1, parity, mu,
+                        (int)D, count));
+    return QCD_OK;
+  }
+};
+
 struct DeviceGuard {
   int prev;
   explicit DeviceGuard(int dev) : prev(-1) { cudaGetDevice(&prev); if (dev != prev) cudaSetDevice(dev); else prev = -1; }
@@ -968,13 +981,10 @@ int split_push_halos(qcd_split* S, int k, int parity, int mu) {
   if (prev != k) CUDA_TRY(cudaStreamWaitEvent(S->stream[k], S->ev_upd[prev], 0));
   if (next != k && next != prev) CUDA_TRY(cudaStreamWaitEvent(S->stream[k], S->ev_upd[next], 0));
   // first own layer -> the previous part's "next" copy (its layer n_int); last own layer -> the next part's "previous" copy
-  HaloOp lo{2, P, 0, S->part[prev], S->ext[prev], nullptr, parity, mu, S->stream[k]};
-  int rc = dispatch(P, lo);
+  HaloPairOp op{P, S->part[prev], S->ext[prev], S->part[next], S->ext[next] + 1, S->ext[k] - 1, parity, mu, S->stream[k]};
+  const int rc = dispatch(P, op);
   if (rc != QCD_OK) return rc;
-  HaloOp hi{2, P, S->ext[k] - 1, S->part[next], S->ext[next] + 1, nullptr, parity, mu, S->stream[k]};
-  rc = dispatch(P, hi);
-  if (rc != QCD_OK) return rc;
-  P->launches += 2;
+  P->launches += 1;
   CUDA_TRY(cudaEventRecord(S->ev_halo[k], S->stream[k]));
   return QCD_OK;
 }

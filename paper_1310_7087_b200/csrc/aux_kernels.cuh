@@ -252,6 +252,43 @@ __global__ void __launch_bounds__(128) halo_kernel(Geom gs, const Vec* __restric
   for (int k = 0; k < NP; ++k) pd[k * ds] = ps[k * ss];
 }
 
+// Both boundary layers of one part in ONE launch (the single-process driver qcd_split_*): blockIdx.y = 0 copies the part's
+// first own layer into the previous part's "next" copy, blockIdx.y = 1 its last own layer into the next part's "previous"
+// copy.  Same addressing as halo_kernel<., ., 2>.
+template <typename Vec> struct HaloTarget { Geom g; Vec* mem; int src_layer, dst_layer; };
+template <typename Vec, int NP>
+__global__ void __launch_bounds__(128) halo_pair_kernel(Geom gs, const Vec* __restrict__ src, HaloTarget<Vec> t0, HaloTarget<Vec> t1, int parity, int mu,
+                                                        int D, uint32_t count) {
+  // launched with programmatic stream serialization behind the part's update kernel: resident while that kernel drains,
+  // reads its output only after the wait; the trigger comes after the wait (as in the update kernels: at most one earlier
+  // kernel of the chain is in flight)
+  pdl_wait();
+  pdl_trigger();
+  const uint32_t idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= count) return;
+  const HaloTarget<Vec>& t = blockIdx.y ? t1 : t0;
+  const int sd = gs.sd;
+  uint32_t rest = idx / (uint32_t)gs.Lh0;
+  const uint32_t j = idx - rest * (uint32_t)gs.Lh0;
+  uint32_t x[4] = {0, 0, 0, 0};
+#pragma unroll
+  for (int d = 1; d < 4; ++d) {
+    if (d == sd) continue;
+    const uint32_t q = rest / (uint32_t)gs.L[d];
+    x[d] = rest - q * (uint32_t)gs.L[d];
+    rest = q;
+  }
+  auto half_index = [&](const Geom& gg, int layer) -> uint32_t {
+    uint32_t y[4] = {0, x[1], x[2], x[3]};
+    y[sd] = (uint32_t)layer;
+    return ((y[3] * (uint32_t)gg.L[2] + y[2]) * (uint32_t)gg.L[1] + y[1]) * (uint32_t)gg.Lh0 + j;
+  };
+  const Vec* ps = src + array_base<NP>(gs, D, parity, mu) + blk_off<NP>(half_index(gs, t.src_layer));
+  Vec* pd = t.mem + array_base<NP>(t.g, D, parity, mu) + blk_off<NP>(half_index(t.g, t.dst_layer));
+#pragma unroll
+  for (int k = 0; k < NP; ++k) pd[k * PLANE_STRIDE] = ps[k * PLANE_STRIDE];
+}
+
 // ------------------------------------------------------------------ reductions
 // block-wide sums of NV doubles per thread: warp shuffle, then shared memory, fixed order => deterministic
 template <int NV, int BLOCK>
