@@ -177,7 +177,9 @@ int qcd_probe_copy_gbs(size_t bytes, int reps, double* gbs);
  * time lines (the Polyakov loop stays local).  A part ("slab") of `extent` layers starting at global coordinate `offset`
  * (both even) is a qcd_lattice_t of local extent extent + 2 along that direction: its own layers, then a copy of the next
  * part's first layer and a copy of the previous part's last layer (one-site link halos: a staple reaches one site).
- * After every (parity, mu) sub-step the two boundary layers of the array that sub-step wrote are copied to the neighbours.
+ * After every (parity, mu) sub-step the two boundary layers of the array that sub-step wrote are copied to the neighbours
+ * (qcd_split_*: by the update kernel itself, which stores a boundary link a second time into the neighbouring part's
+ * memory -- a peer GPU's with one part per device; slab primitives: by qcd_slab_halo_pack / unpack).
  * The Philox counters use the GLOBAL site index, so a divided lattice reproduces the undivided one bit for bit.
  *
  * Slab primitives (one part per handle; the parts may live in different processes, one per GPU, and exchange the packed

@@ -61,6 +61,7 @@ struct qcd_lattice {
   uint64_t prof_n[2];
   uint64_t launches;
   uint32_t order_toggle;   // flips with every update launch (UpdateArgs::rev)
+  qcd_lattice *push_prev, *push_next;   // divided lattice, single-process driver: the update kernels write the boundary layers there too
   // What the kernel launched last on the stream wrote: (parity, mu) of an update kernel; -1: no links (measurement,
   // get_links); -2: all links (init, set_links, the create-time memset).  The next update kernel may fetch, before its
   // griddepcontrol.wait, only arrays that kernel does not write (update.cuh)
@@ -162,6 +163,20 @@ cudaError_t launch_update(qcd_lattice* L, int kind, bool field, const UpdateArgs
   UpdateArgs a = a0;
   a.prev_parity = L->last_parity; a.prev_mu = L->last_mu;
   a.rev = L->alternate_order ? (int)(L->order_toggle & 1u) : 0;
+  if (L->push_prev && L->push_next) {
+    int nreal, vb, np;
+    plane_params(L->Nc, L->precision, L->comp, &nreal, &vb, &np);
+    qcd_lattice* T[2] = {L->push_prev, L->push_next};
+    const int sd = L->g.sd, n_int = L->g.Li[sd];
+    a.hp.on = 1; a.hp.last = n_int - 1;
+    for (int t = 0; t < 2; ++t) {
+      // my first own layer is the previous part's copy "next part's first layer" (its layer n_int'), my last own layer the
+      // next part's copy "previous part's last layer" (its layer n_int' + 1)
+      a.hp.layer[t] = T[t]->g.Li[sd] + t;
+      a.hp.L1[t] = T[t]->g.L[1]; a.hp.L2[t] = T[t]->g.L[2];
+      a.hp.base[t] = (char*)T[t]->mem + (size_t)(a.parity * L->D + a.mu) * np * T[t]->g.Vh_pad * (size_t)vb;
+    }
+  }
   const cudaError_t e = (L->Nc == 2)                ? launch_update_su2(s, L->g, L->mem, a, L->stream)
                         : L->precision == QCD_FP32 ? launch_update_su3_f32(s, L->g, L->mem, a, L->stream)
                                                    : launch_update_su3_f64(s, L->g, L->mem, a, L->stream);
@@ -457,7 +472,7 @@ static int create_lattice(int D, const int* dims, int Nc, int precision, unsigne
   L->seed = 0; L->sweep = 0; L->has_links = false; L->max_trials = 10;
   L->debug_trials = false; L->profile = false; L->bulk_copy = false; L->alternate_order = true; L->exchange_rows01 = false;
   L->d_trials = nullptr; L->d_partials = nullptr; L->partials_cap = 0; L->d_results = nullptr; L->h_results = nullptr;
-  L->prof_ms[0] = L->prof_ms[1] = 0.0; L->prof_n[0] = L->prof_n[1] = 0; L->launches = 0; L->order_toggle = 0; L->last_parity = L->last_mu = -2; L->d_canon = nullptr;
+  L->prof_ms[0] = L->prof_ms[1] = 0.0; L->prof_n[0] = L->prof_n[1] = 0; L->launches = 0; L->order_toggle = 0; L->push_prev = L->push_next = nullptr; L->last_parity = L->last_mu = -2; L->d_canon = nullptr;
   L->side = nullptr; L->ev_fork = nullptr; L->ev_join = nullptr;
   cudaError_t e = cudaSuccess;
   if (!device_mem) {
@@ -1007,7 +1022,18 @@ int split_refresh_all(qcd_split* S) {
   return QCD_OK;
 }
 
+// One sub-step of every part.  The update kernels write the boundary layers of the array they update into the neighbouring
+// parts themselves (HaloPush): there is no separate exchange step, and one event per part and sub-step orders everything --
+// a part's kernel of sub-step s+1 starts after both neighbours' kernels of sub-step s, which (i) have then written its halo
+// copies of the array they updated and (ii) no longer read the halo copies it is about to overwrite there.  (A sub-step
+// reads the array it updates only at its own sites, so kernels of the SAME sub-step never conflict.)
 int split_substep(qcd_split* S, double beta, int kind, int hit, int parity, int mu, const qcd_field_t* field) {
+  for (int k = 0; k < S->n; ++k) {                                   // the events of the previous sub-step
+    DeviceGuard dg(S->dev[k]);
+    const int prev = (k + S->n - 1) % S->n, next = (k + 1) % S->n;
+    if (prev != k) CUDA_TRY(cudaStreamWaitEvent(S->stream[k], S->ev_upd[prev], 0));
+    if (next != k && next != prev) CUDA_TRY(cudaStreamWaitEvent(S->stream[k], S->ev_upd[next], 0));
+  }
   for (int k = 0; k < S->n; ++k) {
     DeviceGuard dg(S->dev[k]);
     qcd_lattice* P = S->part[k];
@@ -1017,10 +1043,8 @@ int split_substep(qcd_split* S, double beta, int kind, int hit, int parity, int 
     if (rc != QCD_OK) return rc;
     rc = substep(P, beta, kind, hit, parity, mu, field, fon, nullptr, false);
     if (rc != QCD_OK) return rc;
-    CUDA_TRY(cudaEventRecord(S->ev_upd[k], S->stream[k]));
   }
-  for (int k = 0; k < S->n; ++k) { int rc = split_push_halos(S, k, parity, mu); if (rc != QCD_OK) return rc; }
-  for (int k = 0; k < S->n; ++k) { int rc = split_wait_halos(S, k); if (rc != QCD_OK) return rc; }
+  for (int k = 0; k < S->n; ++k) { DeviceGuard dg(S->dev[k]); CUDA_TRY(cudaEventRecord(S->ev_upd[k], S->stream[k])); }
   return QCD_OK;
 }
 
@@ -1134,6 +1158,11 @@ int qcd_split_create(int D, const int* dims, int Nc, int precision, unsigned fla
     }
   }
   if (rc != QCD_OK) { std::string m = g_err; qcd_split_destroy(S); g_err = m; return rc; }
+  // the update kernels of a part write its boundary layers into the neighbours' copies (HaloPush)
+  for (int k = 0; k < n_parts; ++k) {
+    S->part[k]->push_prev = S->part[(k + n_parts - 1) % n_parts];
+    S->part[k]->push_next = S->part[(k + 1) % n_parts];
+  }
   *out = S;
   return QCD_OK;
 }

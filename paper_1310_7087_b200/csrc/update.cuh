@@ -25,6 +25,19 @@ struct FieldArgs {   // F = diag(exp(i theta_c)) on plane (mu,nu), mu<nu; cos/si
   double c[3], s[3];
 };
 
+// Boundary layers of a part written straight into its neighbours' memory by the update kernel itself (the single-process
+// driver of a divided lattice, qcd_split_*: "exchanging values of boundary sites", here without a separate
+// exchange step).  A thread whose site lies in the part's first (last) own layer stores its new link a second time, into
+// the previous (next) part's copy of that layer -- local memory or a peer GPU's over NVLink.  The destination part may
+// have another extent, so its half-index is rebuilt from the coordinates with the destination's extents.
+struct HaloPush {
+  int on;            // 0: no neighbours to serve
+  int last;          // the part's last own layer (first = 0)
+  int layer[2];      // destination layer in the previous / next part
+  int L1[2], L2[2];  // extents 1 and 2 of the previous / next part's local lattice (only the split extent differs)
+  void* base[2];     // start of the (parity, mu) array being written in the previous / next part
+};
+
 struct UpdateArgs {
   double beta;
   double inv_c;      // N / (2 beta): delta = E / alpha = E * inv_c / k   (host-computed; inf when beta = 0 -> every trial fails)
@@ -46,6 +59,7 @@ struct UpdateArgs {
   // a 64-bit multiply-add per array on the FMA pipe.
   const void* pbase[4];
   const void* qbase[4];
+  HaloPush hp;
   int rev;           // 1: the CTAs visit their boxes in descending order.  Consecutive launches of a sweep alternate, so that a
                      // launch starts on the part of the lattice the previous one touched last and finds it in the L2
                      // (the 32^4 lattices are 1.6 / 4.8 times the 126 MB L2: in the same order nothing survives a launch)
@@ -66,6 +80,21 @@ struct UpdateArgs {
 // logical block index of a CTA: the launch order is reversed when a.rev is set; everything a CTA does (sites, measurement
 // slots) follows the logical index, so results do not depend on the order
 __device__ __forceinline__ uint32_t logical_block(const UpdateArgs& a) { return a.rev ? gridDim.x - 1u - blockIdx.x : blockIdx.x; }
+// second store of a boundary link into the neighbouring part(s) (HaloPush); r = the reals just stored at the own site
+template <typename R, int NREAL>
+__device__ __forceinline__ void halo_push_store(const UpdateArgs& a, const Geom& g, const SiteCoord& sc, const R* r) {
+  typedef typename PlaneTraits<R, NREAL>::Vec Vec;
+  if (!a.hp.on) return;
+  const int xs = g.sd == 1 ? sc.x1 : g.sd == 2 ? sc.x2 : sc.x3;
+#pragma unroll
+  for (int t = 0; t < 2; ++t) {
+    if (xs != (t == 0 ? 0 : a.hp.last)) continue;
+    int y1 = sc.x1, y2 = sc.x2, y3 = sc.x3;
+    if (g.sd == 1) y1 = a.hp.layer[t]; else if (g.sd == 2) y2 = a.hp.layer[t]; else y3 = a.hp.layer[t];
+    const uint32_t hh = (uint32_t)(((y3 * a.hp.L2[t] + y2) * a.hp.L1[t] + y1) * g.Lh0 + sc.j);
+    store_reals<R, NREAL>((Vec*)a.hp.base[t], g, 0, hh, r);
+  }
+}
 template <int NREC> __device__ __forceinline__ void meas_store(const UpdateArgs& a, const double (&t)[NREC]) {
   const uint32_t w = (logical_block(a) * blockDim.x + threadIdx.x) >> 5;
 #pragma unroll
@@ -630,6 +659,7 @@ su3_update_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* links,
   R r[NREAL];
   m3_to_reals<R, NREAL>(U, r);
   store_reals<R, NREAL>(own_ptr, g, 0, h, r);
+  halo_push_store<R, NREAL>(a, g, sc, r);
 }
 
 // =====================================================================================
@@ -726,6 +756,7 @@ su2_update_kernel(Geom g, typename PlaneTraits<R, 4>::Vec* links, UpdateArgs a) 
     if (!active) return;
   }
   store_reals<R, 4>(links, g, own, h, r);
+  halo_push_store<R, 4>(a, g, sc, r);
   if (KIND == 0 && a.trials) {
     a.trials[(size_t)lex * 3 + 0] = (uint8_t)code; a.trials[(size_t)lex * 3 + 1] = 0; a.trials[(size_t)lex * 3 + 2] = 0;
   }

@@ -322,6 +322,7 @@ su3_update_tiled_kernel(Geom g, typename PlaneTraits<R, (COMP ? 12 : 18)>::Vec* 
   R r[NREAL];
   m3_to_reals<R, NREAL>(U, r);
   store_reals<R, NREAL>(own_ptr, g, 0, h, r);
+  halo_push_store<R, NREAL>(a, g, sc, r);
 }
 
 }  // namespace qcd
