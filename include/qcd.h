@@ -122,6 +122,44 @@ int qcd_measure_accumulate(qcd_lattice_t* lat, const qcd_field_t* field);
 int qcd_accum_get(qcd_lattice_t* lat, uint64_t* count, double* sum, double* sumsq, int capacity);
 int qcd_accum_reset(qcd_lattice_t* lat);
 
+/* The plane plaquettes for callers that must not allocate device memory.
+ *
+ * Who that is: a program that has given the whole GPU to an allocator of its own -- typically a PyTorch process whose caching
+ * allocator already holds nearly all of the 180 GB (a 128^4 fp64 lattice alone is 154.6 GB) -- so that a cudaMalloc made by
+ * this library behind the allocator's back can fail although the pool has room, and the library cannot ask the pool (the ABI
+ * carries no torch types); and a program that measures inside a steady-state loop next to other work on the same GPU (other
+ * lattices on other streams), where it cannot afford cudaMalloc / cudaFree, which may stall the whole device.  qcd_measure
+ * is not safe for them: when first called on a lattice it cudaMallocs its buffer of per-CTA partial sums (and creates a side
+ * stream and two events).
+ *
+ * This call computes what qcd_measure returns in plaq_planes -- the same two kernels, launched the same way, so the numbers
+ * are the same bit for bit -- but keeps the partial sums in an array built into the library's device code.  It calls no
+ * cudaMalloc, cudaFree or any other allocating routine, on the first call or later.  The price: that array is
+ * QCD_NOALLOC_MAX_PARTIALS doubles = 8 MiB on every GPU on which the library's device code is loaded, held until the process
+ * exits whether or not this call is ever used, and it bounds the lattice: D(D-1)/2 planes x (own sites / 128, rounded up
+ * per parity) partial sums must fit: in D = 4 that is 22.3 million sites (64^4 = 16.8 million fits, 128^4 does not; the 32^4
+ * headline lattice uses 384 KiB of it).
+ * A larger lattice is refused with QCD_ERR_UNSUPPORTED and a message naming both numbers; nothing is launched.
+ *
+ *   lat         an initialised lattice (not a slab); its links are the input.  Its device must be the CURRENT device.
+ *   field       as for qcd_measure (NULL: none).
+ *   device_out  DEVICE pointer, caller-owned, D(D-1)/2 doubles, 8-byte aligned: the plane plaquettes in qcd_measure's
+ *               order (0,1),(0,2),..,(D-2,D-1); their mean is qcd_measure's plaq_total.
+ * Asynchronous on the lattice's stream: device_out is valid once the work enqueued by this call has completed there.
+ *
+ * Set-up: the first call on each device asks the CUDA runtime for the array's address on that device
+ * (cudaGetSymbolAddress; the result is cached per device).  Make that first call during set-up, before any stream capture
+ * is begun in the process.
+ * Sharing: there is ONE array per GPU, used by every call on every lattice and stream, and it keeps whatever the previous
+ * call left in it.  That is harmless for calls that follow one another (each call overwrites every entry it later reads;
+ * nothing needs to start at zero).  Two calls that can run on the GPU at the same time -- different streams, or different
+ * host threads driving different lattices -- race on it and both results are garbage: order them yourself (one stream, or an
+ * event between them).
+ * Errors: INVALID_ARG (NULL / misaligned pointer, bad field), STATE (no links yet; lattice on another device than the
+ * current one), UNSUPPORTED (slab; lattice beyond the array; device ordinal >= 64), CUDA. */
+enum { QCD_NOALLOC_MAX_PARTIALS = 1 << 20 };
+int qcd_measure_plaquette_noalloc(qcd_lattice_t* lat, const qcd_field_t* field, double* device_out);
+
 /* Copy links out of / into the lattice in the canonical layout.  bytes must equal V*D*N*N*2*sizeof(real).
  * dst_is_device / src_is_device: the pointer is a DEVICE pointer, 16-byte aligned (then the call is asynchronous on the
  * stream).  HOST pointers (pageable or pinned): the transfer is staged through a bounded device buffer (64 MiB, allocated

@@ -17,6 +17,7 @@ QCD_FLAG_COMPRESS12 = 1
 QCD_COLD, QCD_HOT = 0, 1
 QCD_KIND_HB, QCD_KIND_OR = 0, 1
 QCD_OPT_KP_MAX_TRIALS, QCD_OPT_DEBUG_TRIALS, QCD_OPT_PROFILE, QCD_OPT_BULK_COPY, QCD_OPT_ALTERNATE_ORDER, QCD_OPT_EXCHANGE_ROWS01 = 0, 1, 2, 3, 4, 5
+QCD_NOALLOC_MAX_PARTIALS = 1 << 20
 
 # every symbol include/qcd.h declares (tests check that the library exports all of them)
 SYMBOLS = [
@@ -24,7 +25,7 @@ SYMBOLS = [
     "qcd_get_links", "qcd_set_links", "qcd_get_sweep_counter", "qcd_set_sweep_counter", "qcd_get_seed", "qcd_set_seed",
     "qcd_set_option", "qcd_debug_substep", "qcd_debug_get_trials", "qcd_debug_philox", "qcd_debug_hb_math", "qcd_get_profile",
     "qcd_reset_profile", "qcd_get_launch_count", "qcd_measure_accumulate", "qcd_sweep_measure", "qcd_sweep_measure_accumulate", "qcd_accum_get", "qcd_accum_reset", "qcd_probe_fma_tflops", "qcd_probe_copy_gbs", "qcd_last_error",
-    "qcd_version",
+    "qcd_version", "qcd_measure_plaquette_noalloc",
     "qcd_slab_bytes", "qcd_slab_create", "qcd_slab_halo_bytes", "qcd_slab_halo_pack", "qcd_slab_halo_unpack", "qcd_slab_measure_sums",
     "qcd_split_create", "qcd_split_destroy", "qcd_split_parts", "qcd_split_halo_bytes", "qcd_split_init", "qcd_split_sweep",
     "qcd_split_substep", "qcd_split_measure", "qcd_split_get_links", "qcd_split_set_links", "qcd_split_set_seed",
@@ -67,6 +68,7 @@ def lib():
     L.qcd_sweep.argtypes = [p, d, i, i, fp]
     L.qcd_measure.argtypes = [p, fp, dp, dp, dp]
     L.qcd_measure_accumulate.argtypes = [p, fp]
+    L.qcd_measure_plaquette_noalloc.argtypes = [p, fp, p]
     L.qcd_sweep_measure.argtypes = [p, d, i, i, fp, dp, dp, dp]
     L.qcd_sweep_measure_accumulate.argtypes = [p, d, i, i, fp]
     L.qcd_accum_get.argtypes = [p, C.POINTER(C.c_uint64), dp, dp, i]
@@ -259,6 +261,16 @@ class Lattice:
         _check(lib().qcd_measure(self._h, _fref(field), C.byref(tot) if plaquette else None, planes if plaquette else None,
                                  poly if polyakov else None))
         return tot.value, np.array(planes[:]), complex(poly[0], poly[1])
+
+    def qcd_measure_plaquette_noalloc(self, out, field=None):
+        """Plane plaquettes (qcd_measure's `planes`) written to `out`, a float64 CUDA tensor of D(D-1)/2 elements that the
+        caller owns, without any device allocation by the library -- for programs whose own allocator holds the GPU's memory
+        or which cannot afford a cudaMalloc in their loop (include/qcd.h says who and why).  The partial sums live in one
+        8 MiB array per GPU built into the library, shared by all calls: lattices beyond QCD_NOALLOC_MAX_PARTIALS partial sums
+        are refused, and calls that may overlap on the GPU must be ordered by the caller.  Asynchronous on the lattice's
+        stream; the lattice's device must be current.  Call it once during set-up before any stream capture."""
+        assert out.is_cuda and out.dtype == self._torch.float64 and out.is_contiguous() and out.numel() >= self.D * (self.D - 1) // 2
+        _check(lib().qcd_measure_plaquette_noalloc(self._h, _fref(field), out.data_ptr()))
 
     def qcd_sweep_measure(self, beta, n_hb, n_or, field=None):
         """one working sweep: qcd_sweep + the observables of the new configuration (plaquette fused into the last pass)"""

@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -1315,3 +1316,96 @@ int qcd_split_synchronize(qcd_split_t* S) {
 }
 
 }  // extern "C"
+
+// =====================================================================================
+// qcd_measure_plaquette_noalloc: the plaquette measurement for callers that must not allocate (include/qcd.h).
+//
+// qcd_measure keeps the per-CTA partial sums of plaquette_kernel in a buffer it cudaMallocs on first use.  Here the same two
+// kernels run with the partials in the array below instead, which is part of the library's device image: every GPU that
+// loads the library holds these QCD_NOALLOC_MAX_PARTIALS doubles (8 MiB) until the process exits, whether this entry point
+// is ever called or not, and nothing is allocated or freed at call time.
+//
+// g_noalloc_partials is a device symbol.  In the host code of this file the name only identifies the symbol to the runtime;
+// it is not an address a kernel can use, so the device address is looked up with cudaGetSymbolAddress, once per device and
+// with that device current, and kept in g_noalloc_ptr.
+// =====================================================================================
+static __device__ __align__(256) double g_noalloc_partials[QCD_NOALLOC_MAX_PARTIALS];
+
+namespace {
+
+constexpr int NOALLOC_MAX_DEVICES = 64;
+std::mutex g_noalloc_mutex;
+double* g_noalloc_ptr[NOALLOC_MAX_DEVICES];   // device address of g_noalloc_partials on device i; nullptr: not looked up yet
+
+// device address of the array on the CURRENT device (looked up on this device's first call; no allocation)
+int noalloc_scratch(int dev, double** out) {
+  if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return fail(QCD_ERR_UNSUPPORTED, "device ordinal beyond the per-device table of qcd_measure_plaquette_noalloc");
+  std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+  if (!g_noalloc_ptr[dev]) {
+    void* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&p, g_noalloc_partials);
+    if (e != cudaSuccess || !p) return fail(QCD_ERR_CUDA, std::string("cudaGetSymbolAddress(g_noalloc_partials): ") + cudaGetErrorString(e));
+    g_noalloc_ptr[dev] = (double*)p;
+  }
+  *out = g_noalloc_ptr[dev];
+  return QCD_OK;
+}
+
+struct NoAllocPlaquetteOp {
+  qcd_lattice* L; MeasureField mf; double* scratch; double* device_out;
+  template <int NC, int D, typename R, bool COMP> int operator()() {
+    typedef typename LinkIO<NC, R, COMP>::Vec Vec;
+    constexpr int NPL = D * (D - 1) / 2;
+    const MeasLayout m = meas_layout(L);
+    mf.boxed = m.boxed ? 1 : 0;
+    if (mf.boxed) {
+      mf.n0 = make_fastdiv((uint32_t)(L->g.Lh0 / 8)); mf.n1 = make_fastdiv((uint32_t)(L->g.Li[1] / 2)); mf.n2 = make_fastdiv((uint32_t)(L->g.Li[2] / 2));
+    }
+    const dim3 plaq_grid = mf.boxed ? dim3(own_sites(L) / 128, 1) : dim3((L->g.Vh_int + 127) / 128, 2);
+    // Every CTA of plaquette_kernel stores all NPL of its partials and final_reduce_kernel reads exactly those
+    // NPL x nb_plaq entries: nothing in the array has to start at zero, and what an earlier call left beyond them is not read.
+    plaquette_kernel<NC, D, R, COMP><<<plaq_grid, 128, 0, L->stream>>>(L->g, (const Vec*)L->mem, mf, scratch);
+    final_reduce_kernel<<<NPL, 256, 0, L->stream>>>(scratch, m.nb_plaq, device_out, 1.0 / ((double)L->g.V * NC));
+    CUDA_TRY(cudaGetLastError());
+    L->launches += 2;
+    L->last_parity = L->last_mu = -1;
+    return QCD_OK;
+  }
+};
+
+}  // namespace
+
+extern "C" int qcd_measure_plaquette_noalloc(qcd_lattice_t* L, const qcd_field_t* field, double* device_out) {
+  if (!L || !device_out) return fail(QCD_ERR_INVALID_ARG, "NULL argument");
+  if (((uintptr_t)device_out) & 7u) return fail(QCD_ERR_INVALID_ARG, "device_out must be 8-byte aligned");
+  if (!L->has_links) return fail(QCD_ERR_STATE, "no links yet");
+  if (L->g.sd >= 0) return fail(QCD_ERR_UNSUPPORTED, "a slab has sums, not means: qcd_slab_measure_sums / qcd_split_measure");
+  bool fon;
+  int rc = check_field(L, field, &fon);
+  if (rc != QCD_OK) return rc;
+  const MeasLayout m = meas_layout(L);
+  const size_t need = (size_t)m.npl * m.nb_plaq;
+  if (need > (size_t)QCD_NOALLOC_MAX_PARTIALS) {
+    char msg[256];
+    snprintf(msg, sizeof(msg), "lattice too large for qcd_measure_plaquette_noalloc: it needs %zu partial sums (planes x sites/128), the "
+             "built-in scratch array holds QCD_NOALLOC_MAX_PARTIALS = %d; use qcd_measure", need, (int)QCD_NOALLOC_MAX_PARTIALS);
+    return fail(QCD_ERR_UNSUPPORTED, msg);
+  }
+  // the array's address is per device: the lattice's device must be the current one
+  int dev = -1;
+  CUDA_TRY(cudaGetDevice(&dev));
+  cudaPointerAttributes attr;
+  CUDA_TRY(cudaPointerGetAttributes(&attr, L->mem));
+  if ((attr.type != cudaMemoryTypeDevice && attr.type != cudaMemoryTypeManaged) || (attr.type == cudaMemoryTypeDevice && attr.device != dev))
+    return fail(QCD_ERR_STATE, "qcd_measure_plaquette_noalloc: the lattice's device must be the current device");
+  double* scratch = nullptr;
+  rc = noalloc_scratch(dev, &scratch);
+  if (rc != QCD_OK) return rc;
+  NoAllocPlaquetteOp op;
+  op.L = L; op.scratch = scratch; op.device_out = device_out;
+  memset(&op.mf, 0, sizeof(op.mf));
+  const FieldArgs fa = make_field_args(field, fon, L->Nc);
+  op.mf.enabled = fon ? 1 : 0; op.mf.mu = fa.mu; op.mf.nu = fa.nu;
+  for (int c = 0; c < 3; ++c) { op.mf.c[c] = fa.c[c]; op.mf.s[c] = fa.s[c]; }
+  return dispatch(L, op);
+}
