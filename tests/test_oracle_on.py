@@ -91,6 +91,33 @@ def test_action_and_one_hit_against_the_definition(dims, N):
         assert 0 < n_acc < V // 2
 
 
+@pytest.mark.parametrize("dims,N", [((4, 6), 1), ((4, 4, 2), 3), ((4, 2, 6, 2), 4), ((2, 2, 2, 2), 2), ((6, 4, 2), 4)])
+def test_measure_against_the_definitions(dims, N):
+    """R19 on a fixed random field, element-wise: phi2 = (1/V) sum_x phi.phi, link = (1/(V D)) sum_x sum_mu phi(x).phi(x+mu),
+    mag_a = (1/V) sum_x phi_a, each recomputed here with numpy (roll for the neighbour).  The field has a non-zero mean in
+    every component, distinct per component, and the extents differ, so a wrong normalisation (V D for V, a dropped 1/D),
+    a swapped component or a wrong neighbour changes the number."""
+    D, V = len(dims), int(np.prod(dims))
+    rng = np.random.default_rng(17)
+    phi = rng.uniform(-1.0, 1.0, size=(V, N)) + 0.3 * (1.0 + np.arange(N))
+    O = on.OnOracle(dims, N)
+    O.set_field(phi)
+    p2, lk, mag = O.measure()
+    g = phi.reshape(tuple(reversed(dims)) + (N,))
+    assert abs(p2 - (g * g).sum() / V) < 1e-13
+    link = sum((g * np.roll(g, -1, axis=D - 1 - mu)).sum() for mu in range(D)) / (V * D)
+    assert abs(lk - link) < 1e-13
+    assert mag.shape == (N,) and np.max(np.abs(mag - phi.mean(axis=0))) < 1e-13
+    assert np.min(np.abs(np.diff(phi.mean(axis=0)))) > 0.1 if N > 1 else True
+    # the backward neighbour gives the same link sum (periodic lattice); a constant field gives phi2 = link = |c|^2, mag = c
+    link_b = sum((g * np.roll(g, +1, axis=D - 1 - mu)).sum() for mu in range(D)) / (V * D)
+    assert abs(lk - link_b) < 1e-13
+    c = 0.25 * (1.0 + np.arange(N))
+    O.set_field(np.broadcast_to(c, (V, N)).copy())
+    p2, lk, mag = O.measure()
+    assert abs(p2 - c @ c) < 1e-14 and abs(lk - c @ c) < 1e-14 and np.max(np.abs(mag - c)) < 1e-15
+
+
 def _radial_moment(N, lam):
     w = lambda r: r ** (N - 1) * np.exp(-r * r - lam * (r * r - 1.0) ** 2)
     z = integrate.quad(w, 0, np.inf)[0]
