@@ -219,6 +219,9 @@ int qcd_probe_copy_gbs(size_t bytes, int reps, double* gbs);
  * (qcd_split_*: by the update kernel itself, which stores a boundary link a second time into the neighbouring part's
  * memory -- a peer GPU's with one part per device; slab primitives: by qcd_slab_halo_pack / unpack).
  * The Philox counters use the GLOBAL site index, so a divided lattice reproduces the undivided one bit for bit.
+ * A part's halo copies are written by its NEIGHBOURS' kernels on their streams: they are valid on the part's own stream only
+ * behind a wait for the neighbours' last update (qcd_split_substep, qcd_split_sweep and qcd_split_measure enqueue that wait
+ * themselves; qcd_split_destroy drains every part's stream before it frees anything).
  *
  * Slab primitives (one part per handle; the parts may live in different processes, one per GPU, and exchange the packed
  * layers through any transport, e.g. torch.distributed / NCCL):

@@ -1023,18 +1023,27 @@ int split_refresh_all(qcd_split* S) {
   return QCD_OK;
 }
 
+// Every part's stream waits for the last update kernels of both neighbours (ev_upd).  A part's halo layers are written by its
+// NEIGHBOURS' update kernels, on their streams: whatever reads them next on the part's own stream -- the next sub-step's
+// kernel, or a measurement -- has to come behind this wait.
+int split_wait_updates(qcd_split* S) {
+  for (int k = 0; k < S->n; ++k) {
+    DeviceGuard dg(S->dev[k]);
+    const int prev = (k + S->n - 1) % S->n, next = (k + 1) % S->n;
+    if (prev != k) CUDA_TRY(cudaStreamWaitEvent(S->stream[k], S->ev_upd[prev], 0));
+    if (next != k && next != prev) CUDA_TRY(cudaStreamWaitEvent(S->stream[k], S->ev_upd[next], 0));
+  }
+  return QCD_OK;
+}
+
 // One sub-step of every part.  The update kernels write the boundary layers of the array they update into the neighbouring
 // parts themselves (HaloPush): there is no separate exchange step, and one event per part and sub-step orders everything --
 // a part's kernel of sub-step s+1 starts after both neighbours' kernels of sub-step s, which (i) have then written its halo
 // copies of the array they updated and (ii) no longer read the halo copies it is about to overwrite there.  (A sub-step
 // reads the array it updates only at its own sites, so kernels of the SAME sub-step never conflict.)
 int split_substep(qcd_split* S, double beta, int kind, int hit, int parity, int mu, const qcd_field_t* field) {
-  for (int k = 0; k < S->n; ++k) {                                   // the events of the previous sub-step
-    DeviceGuard dg(S->dev[k]);
-    const int prev = (k + S->n - 1) % S->n, next = (k + 1) % S->n;
-    if (prev != k) CUDA_TRY(cudaStreamWaitEvent(S->stream[k], S->ev_upd[prev], 0));
-    if (next != k && next != prev) CUDA_TRY(cudaStreamWaitEvent(S->stream[k], S->ev_upd[next], 0));
-  }
+  int rc0 = split_wait_updates(S);                                   // the events of the previous sub-step
+  if (rc0 != QCD_OK) return rc0;
   for (int k = 0; k < S->n; ++k) {
     DeviceGuard dg(S->dev[k]);
     qcd_lattice* P = S->part[k];
@@ -1170,6 +1179,12 @@ int qcd_split_create(int D, const int* dims, int Nc, int precision, unsigned fla
 
 int qcd_split_destroy(qcd_split_t* S) {
   if (!S) return QCD_OK;
+  // a neighbour's update kernel may still be storing into a part's halo layers (from another stream, or another device,
+  // which cudaFree of this device's memory does not wait for): drain every stream before anything is freed
+  for (size_t k = 0; k < S->stream.size(); ++k) {
+    DeviceGuard dg(S->dev[k]);
+    if (S->stream[k]) cudaStreamSynchronize(S->stream[k]);
+  }
   for (size_t k = 0; k < S->part.size(); ++k) {
     DeviceGuard dg(S->dev[k]);
     if (S->part[k]) qcd_lattice_destroy(S->part[k]);
@@ -1240,6 +1255,9 @@ int qcd_split_measure(qcd_split_t* S, const qcd_field_t* field, double* plaq_tot
   const int npl = S->D * (S->D - 1) / 2;
   double ps[8] = {0, 0, 0, 0, 0, 0, 0, 0}, pl[2] = {0, 0};
   const bool want_plaq = plaq_total || plaq_planes;
+  // the plaquette kernel of a part reads its halo copies, which the neighbours' last update kernels may still be writing
+  int rcw = split_wait_updates(S);
+  if (rcw != QCD_OK) return rcw;
   // enqueue on every part first, then collect: the parts measure concurrently
   for (int k = 0; k < S->n; ++k) {
     DeviceGuard dg(S->dev[k]);

@@ -77,6 +77,24 @@ def test_split_sweep_is_bit_identical_to_the_undivided_sweep(qcd, variant, dims,
         assert abs(ma[0] - mb[0]) < tol and np.max(np.abs(ma[1] - mb[1])) < tol and abs(ma[2] - mb[2]) < tol
 
 
+@pytest.mark.parametrize("variant", [(3, 0, 1), (3, 1, 0)], ids=["su3-f32x12", "su3-f64x18"])
+def test_split_measure_straight_behind_a_sweep(qcd, variant):
+    """qcd_split_measure enqueued directly behind qcd_split_sweep, with no qcd_split_get_links / synchronise in between: the
+    plaquette kernel of a part reads halo copies that the neighbours' last update kernels write from other streams, so the
+    measurement has to wait for them itself.  Repeated, on four parts, against the undivided sweep + measure."""
+    Nc, prec, flags = variant
+    dims, beta = (16, 8, 16, 8), 5.7
+    with qcd.Lattice(dims, Nc, prec, flags) as G, qcd.SplitLattice(dims, Nc, prec, flags, n_parts=4) as S:
+        G.qcd_init(qcd.QCD_HOT, 77)
+        S.qcd_split_init(qcd.QCD_HOT, 77)
+        for it in range(25):
+            G.qcd_sweep(beta, 1, 1)
+            S.qcd_split_sweep(beta, 1, 1)
+            ma, mb = G.qcd_measure(), S.qcd_split_measure()
+            assert abs(ma[0] - mb[0]) < MEAS_TOL[prec] and np.max(np.abs(ma[1] - mb[1])) < MEAS_TOL[prec] and abs(ma[2] - mb[2]) < MEAS_TOL[prec], it
+        assert np.array_equal(G.qcd_get_links(), S.qcd_split_get_links())
+
+
 @pytest.mark.parametrize("variant", VARIANTS, ids=VARIANT_IDS)
 def test_split_hot_start_and_substeps_match_the_oracle(qcd, variant):
     """hot start of the parts = the oracle's (global Philox counters); every (parity, mu) heatbath and overrelaxation sub-step
@@ -112,7 +130,7 @@ def test_split_hot_start_and_substeps_match_the_oracle(qcd, variant):
                     got = S.qcd_split_get_links().astype(np.complex128)
                     worst = max(worst, float(np.max(np.abs(got - Oc.get_links()))))
         # thermal-like links: well conditioned, no accept/reject disagreement expected at this size (it would show as O(1))
-        assert worst < TOL[prec] * (1.0 if flags == 0 else 1.5), worst
+        assert worst < TOL[prec], worst                                      # the bar of the undivided sub-step tests, all storage forms
 
 
 @pytest.mark.parametrize("variant", [(3, 1, 0), (3, 0, 1), (2, 0, 0)], ids=["su3-f64x18", "su3-f32x12", "su2-f32"])
