@@ -87,21 +87,55 @@ def test_half_sweeps_match_the_oracle(qcd, prec, dims, N):
         assert flips <= max(0, int(1e-6 * tries)), (flips, tries)
 
 
-def test_o4_full_size_half_sweep_nhit100(qcd):
-    """the paper's O(4) workload (Table 1: O(4) 32^4, NHIT = 100) at full size: one half sweep, every site
-    against the oracle (fp64), from the hot start"""
-    dims, N = (32, 32, 32, 32), 4
-    O = on.OnOracle(dims, N)
+@pytest.mark.parametrize("prec", [1, 0], ids=["f64", "f32"])
+def test_o4_full_size_half_sweeps_nhit100(qcd, prec):
+    """the paper's O(4) workload (Table 1: O(4) 32^4, NHIT = 100) at the size, NHIT and precisions bench.py
+    times: both half sweeps from the hot start, every site against the oracle.  fp64: 1e-12 and identical accept counts.
+    fp32 (the kernel with the guard-band decision, against the fp32-shadow oracle): sites whose decision sequence differs are
+    counted and at most 1e-6 of the 2 x 5.2e7 tries; every other site within 2e-5; the field is re-synchronised with the
+    oracle's between the half sweeps so that a disagreement does not spread to its neighbours."""
+    dims, N, nhit = (32, 32, 32, 32), 4, 100
+    O = _oracle(dims, N, prec)
     O.init(on.HOT, 2013)
-    with qcd.OnLattice(dims, N, 1) as G:
+    flips, tries, worst = 0, 0, 0.0
+    with qcd.OnLattice(dims, N, prec) as G:
         G.qcd_on_init(qcd.QCD_HOT, 2013)
-        assert np.array_equal(G.qcd_on_get_field(), O.get_field())
-        G.qcd_on_half_sweep(0, 0.15, 0.5, 0.5, 100)
-        O.half_sweep(0, 0.15, 0.5, 0.5, 100)
-        assert np.max(np.abs(G.qcd_on_get_field() - O.get_field())) < 1e-12
-        assert G.qcd_on_get_counts() == O.counts()
+        assert np.array_equal(G.qcd_on_get_field().astype(np.float64), O.get_field())
+        for parity in (0, 1):
+            G.qcd_on_half_sweep(parity, 0.15, 0.5, 0.5, nhit)
+            O.half_sweep(parity, 0.15, 0.5, 0.5, nhit)
+            got, ref = G.qcd_on_get_field().astype(np.float64), O.get_field()
+            diff = np.max(np.abs(got - ref), axis=1)
+            tries += (O.V // 2) * nhit
+            if prec == 1:
+                assert diff.max() < 1e-12, diff.max()
+            else:
+                bad = diff > 2e-5
+                flips += int(bad.sum())
+                worst = max(worst, float(diff[~bad].max()))
+            G.qcd_on_set_field(ref)                                    # both precisions: the measurement below is of the same field
+        assert G.qcd_on_get_counts()[1] == O.counts()[1] == tries
+        if prec == 1:
+            assert G.qcd_on_get_counts() == O.counts()
+        else:
+            print("fp32 O(4) 32^4 NHIT=100: %d disagreeing sites in %d tries, worst other diff %.2e" % (flips, tries, worst))
+            assert flips <= int(1e-6 * tries), (flips, tries)
+            assert abs(G.qcd_on_get_counts()[0] - O.counts()[0]) <= 100 * flips
         a, b = G.qcd_on_measure(), O.measure()
-        assert abs(a[0] - b[0]) < 1e-12 and abs(a[1] - b[1]) < 1e-12 and np.max(np.abs(a[2] - b[2])) < 1e-12
+        # The oracle adds its 4 x 2^20 (phi2) and 16 x 2^20 (link) terms one after the other in double: at this size its OWN
+        # rounding is ~ sqrt(n) ulps of the running sum (measured 1.2e-12 on phi2 = 1.30 from identical fields), so the
+        # small-lattice bar 1e-12 is replaced by 4e-12 here, and the kernel is held to 2e-13 against correctly rounded sums
+        # (math.fsum) of the same field instead.  fp32: site arithmetic in float, 1e-6 as on the small lattices.
+        tol = 4e-12 if prec == 1 else 1e-6
+        assert abs(a[0] - b[0]) < tol and abs(a[1] - b[1]) < tol and np.max(np.abs(a[2] - b[2])) < tol
+        if prec == 1:
+            import math
+            g = ref.reshape(tuple(reversed(dims)) + (N,))
+            D, V = len(dims), O.V
+            p2 = math.fsum((g * g).ravel()) / V
+            lk = math.fsum(np.concatenate([(g * np.roll(g, -1, axis=D - 1 - mu)).ravel() for mu in range(D)])) / (V * D)
+            mag = np.array([math.fsum(g[..., c].ravel()) / V for c in range(N)])
+            assert abs(a[0] - p2) < 2e-13 and abs(a[1] - lk) < 2e-13 and np.max(np.abs(a[2] - mag)) < 2e-13, (a, p2, lk, mag)
 
 
 @pytest.mark.parametrize("prec", [1, 0], ids=["f64", "f32"])
