@@ -86,11 +86,15 @@ template <int N> __device__ __forceinline__ double on_local_action(const double*
   return -2.0 * kappa * ph + pp + lambda * (pp - 1.0) * (pp - 1.0);
 }
 // guard-band path of the fp32 kernel: the decision of one try in double from the float-valued operands (out of line, rare)
-template <int N> static __device__ __noinline__ bool on_accept_f64_cold(const float* p, const float* q, const double* h, double kappa, double lambda, double u) {
+// The operands travel BY VALUE: handed over as pointers, phi and h had to live in local memory, and the hot loop stored
+// phi there on every accepted try (1.7 STL per try, profiles/r3_on_model.md).
+template <int N> struct OnVecF { float v[N]; };
+template <int N> struct OnVecD { double v[N]; };
+template <int N> static __device__ __noinline__ bool on_accept_f64_cold(OnVecF<N> p, OnVecF<N> q, OnVecD<N> h, double kappa, double lambda, double u) {
   double pd[N], qd[N];
 #pragma unroll
-  for (int a = 0; a < N; ++a) { pd[a] = (double)p[a]; qd[a] = (double)q[a]; }
-  const double dS = on_local_action<N>(qd, h, kappa, lambda) - on_local_action<N>(pd, h, kappa, lambda);
+  for (int a = 0; a < N; ++a) { pd[a] = (double)p.v[a]; qd[a] = (double)q.v[a]; }
+  const double dS = on_local_action<N>(qd, h.v, kappa, lambda) - on_local_action<N>(pd, h.v, kappa, lambda);
   return u < exp(-dS);
 }
 
@@ -157,7 +161,13 @@ __global__ void __launch_bounds__(128) on_update_kernel(Geom g, typename OnIO<R>
         // the float error of dS is below 8e-7 (|t1| + |d2| + |t3|) + 1e-6 (roundings of the sums, of h and of the products),
         // __expf adds 2e-6 relative: inside that band around the acceptance boundary the try is decided in double, like
         // the oracle does, from the same float-valued operands
-        if (fabsf(u - e) < (8e-7f * (fabsf(t1) + fabsf(d2) + fabsf(t3)) + 4e-6f) * e) ok = on_accept_f64_cold<N>(ph, qv, hs, a.kappa, a.lambda, (double)u);
+        if (fabsf(u - e) < (8e-7f * (fabsf(t1) + fabsf(d2) + fabsf(t3)) + 4e-6f) * e) {
+          OnVecF<N> pv, qw;
+          OnVecD<N> hv;
+#pragma unroll
+          for (int c = 0; c < N; ++c) { pv.v[c] = ph[c]; qw.v[c] = qv[c]; hv.v[c] = hs[c]; }
+          ok = on_accept_f64_cold<N>(pv, qw, hv, a.kappa, a.lambda, (double)u);
+        }
       } else {
         ok = u < exp(-dS);
       }
