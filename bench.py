@@ -159,7 +159,7 @@ def rep_stats(times, steps):
             "reps": len(t), "device_ms_total": sum(t)}
 
 
-def time_arm(q, torch, prec_name, steps, warmup, therm, seed, dist, sampler, bulk_copy=False, alternate=True, full_exchange=False):
+def time_arm(q, torch, prec_name, steps, warmup, therm, seed, dist, sampler, bulk_copy=False, alternate=True):
     """device-resident timing + end-to-end timing of one precision arm; returns a dict of raw numbers"""
     prec = q.QCD_FP32 if prec_name == "f32" else q.QCD_FP64
     flags = q.QCD_FLAG_COMPRESS12 if prec_name == "f32" else 0
@@ -215,25 +215,28 @@ def time_arm(q, torch, prec_name, steps, warmup, therm, seed, dist, sampler, bul
         # memory, runs the working sweep, reads the observables and downloads the configuration.  Exchange layout: the
         # canonical one; for the 12-real arm its compressed form (rows 0,1 of every link, QCD_OPT_EXCHANGE_ROWS01), i.e.
         # exactly the reals the lattice stores -- a third less over the host link, nothing lost
-        if flags & q.QCD_FLAG_COMPRESS12 and not full_exchange:
-            G.qcd_set_option(q.QCD_OPT_EXCHANGE_ROWS01, 1)
-            out["exchange"] = "rows 0,1 of every link, [lex][mu][2][3][re,im] (QCD_OPT_EXCHANGE_ROWS01)"
-        else:
-            out["exchange"] = "canonical [lex][mu][3][3][re,im]"
-        nbytes = G.canonical_bytes
-        host = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
-        G.qcd_get_links_ptr(host.data_ptr(), nbytes, 0)
-
-        def e2e_step():
-            G.qcd_set_links_ptr(host.data_ptr(), nbytes, 0)
-            state["obs"] = G.qcd_sweep_measure(BETA, N_HB, N_OR)
+        # `e2e` is always the canonical layout ("full N x N always"); the 12-real arm is timed a second time
+        # through its compressed exchange form (e2e_rows01)
+        def e2e_arm(key, rows01):
+            G.qcd_set_option(q.QCD_OPT_EXCHANGE_ROWS01, 1 if rows01 else 0) if flags & q.QCD_FLAG_COMPRESS12 else None
+            nbytes = G.canonical_bytes
+            host = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
             G.qcd_get_links_ptr(host.data_ptr(), nbytes, 0)
 
-        for _ in range(2):
-            e2e_step()
-        out["e2e"] = timed_reps(torch, dist, sampler, e2e_step, steps, min_total_ms=0.0)
-        out["h2d"] = nbytes
-        out["d2h"] = nbytes + 9 * 8
+            def e2e_step():
+                G.qcd_set_links_ptr(host.data_ptr(), nbytes, 0)
+                state["obs"] = G.qcd_sweep_measure(BETA, N_HB, N_OR)
+                G.qcd_get_links_ptr(host.data_ptr(), nbytes, 0)
+
+            for _ in range(2):
+                e2e_step()
+            out[key] = {"times": timed_reps(torch, dist, sampler, e2e_step, steps, min_total_ms=0.0), "h2d": nbytes, "d2h": nbytes + 9 * 8,
+                        "exchange": "rows 0,1 of every link, [lex][mu][2][3][re,im] (QCD_OPT_EXCHANGE_ROWS01)" if rows01
+                        else "canonical [lex][mu][3][3][re,im]"}
+
+        e2e_arm("e2e", False)
+        if flags & q.QCD_FLAG_COMPRESS12:
+            e2e_arm("e2e_rows01", True)
         out["sweep_counter"] = G.qcd_get_sweep_counter()
     return out
 
@@ -277,6 +280,50 @@ def time_on_model(q, torch, dist, sampler, with_oracle):
     return out
 
 
+def time_split(q, torch, steps, therm, seed):
+    """--split: the lattice divided into 1, 2 and 4 parts on THIS GPU (qcd_split_*) beside the undivided
+    lattice, fp32 x12 arm: update-only sweep and sweep + measurement.  The parts run on streams of their own, so a repetition
+    is bracketed by two events on torch's stream with a host synchronisation of all work before the second one (the same
+    procedure for the undivided lattice, so the rows are comparable with each other; a few microseconds of host latency per
+    repetition of >= 40 ms ride along)."""
+    prec, flags = q.QCD_FP32, q.QCD_FLAG_COMPRESS12
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+    def timed(body, sync, reps=7):
+        times = []
+        for _ in range(reps):
+            torch.cuda.synchronize()
+            e0.record()
+            for _ in range(steps):
+                body()
+            sync()
+            e1.record()
+            torch.cuda.synchronize()
+            times.append(e0.elapsed_time(e1))
+        return rep_stats(times, steps)
+
+    out = {"workload": "SU(3) fp32 x12 32^4 beta 6.0, 1 HB + 4 OR per sweep, every part on the same GPU", "steps": steps, "rows": {}}
+    with q.Lattice(DIMS, NC, prec, flags, device=torch.device("cuda", torch.cuda.current_device())) as G:
+        G.qcd_init(q.QCD_HOT, seed)
+        for _ in range(therm + 3):
+            G.qcd_sweep(BETA, N_HB, N_OR)
+        u = timed(lambda: G.qcd_sweep(BETA, N_HB, N_OR), torch.cuda.synchronize)
+        m = timed(lambda: (G.qcd_sweep(BETA, N_HB, N_OR), G.qcd_measure()), torch.cuda.synchronize)
+        out["rows"]["undivided"] = {"sweep_ms": u["median_ms_per_step"], "sweep_measure_ms": m["median_ms_per_step"], "reps": u}
+    base = out["rows"]["undivided"]["sweep_ms"]
+    for n in (1, 2, 4):
+        with q.SplitLattice(DIMS, NC, prec, flags, n_parts=n) as S:
+            S.qcd_split_init(q.QCD_HOT, seed)
+            for _ in range(therm + 3):
+                S.qcd_split_sweep(BETA, N_HB, N_OR)
+            u = timed(lambda: S.qcd_split_sweep(BETA, N_HB, N_OR), S.qcd_split_synchronize)
+            m = timed(lambda: (S.qcd_split_sweep(BETA, N_HB, N_OR), S.qcd_split_measure()), S.qcd_split_synchronize)
+            out["rows"]["%d part%s" % (n, "" if n == 1 else "s")] = {
+                "sweep_ms": u["median_ms_per_step"], "sweep_measure_ms": m["median_ms_per_step"], "reps": u,
+                "overhead_vs_undivided": u["median_ms_per_step"] / base - 1.0, "halo_bytes_per_substep": S.qcd_split_halo_bytes()}
+    return out
+
+
 def replica_seed(rank):
     """every rank runs an independent lattice of the same workload: same recipe, its own Philox seed"""
     return SEED + rank
@@ -303,14 +350,18 @@ def summarise(arm, prec_name, steps, n_gpus, hbm_peak, fma_peak_tflops):
     n_launch = 2 * len(DIMS) * (N_HB + N_OR)
     sweep_bytes = n_launch * bytes_launch
     sweep_flops = hits * 2 * len(DIMS) * (N_HB * FLOPS_PER_HIT[prec_name]["hb"] + N_OR * FLOPS_PER_HIT[prec_name]["or"])
-    roof = {"bound": "hbm", "kernel": OR_KERNEL[prec_name], "achieved": round(achieved, 1), "peak": hbm_peak,
+    sweep_frac = round(sweep_bytes / (ms_step * 1e-3) / 1e9 / hbm_peak, 4)
+    # north_star sets its target on the SWEEP, not on a kernel: it leads the block.  frac / achieved below are the
+    # dominant kernel's, as the roofline contract asks
+    roof = {"target": {"on": "sweep_frac", "value": 0.70, "sweep_frac": sweep_frac, "met": bool(sweep_frac >= 0.70)},
+            "bound": "hbm", "kernel": OR_KERNEL[prec_name], "achieved": round(achieved, 1), "peak": hbm_peak,
             "unit": "GB/s", "frac": round(achieved / hbm_peak, 4), "traffic": NCU_TRAFFIC[prec_name]["or"],
             "traffic_source": NCU_TRAFFIC["source"],
             "bytes_per_launch": bytes_launch, "us_per_launch": round(or_us, 2), "launches_timed": arm["or_n"],
             "hb_us_per_launch": round(hb_us, 2),
             "hb_frac": round(bytes_launch / (hb_us * 1e-6) / 1e9 / hbm_peak, 4) if hb_us > 0 else None,
             # working sweep: update bytes over the whole step (measurement time inside, its bytes not counted)
-            "sweep_frac": round(sweep_bytes / (ms_step * 1e-3) / 1e9 / hbm_peak, 4),
+            "sweep_frac": sweep_frac,
             # update-only sweep (the SURVEY 8(d) headline form)
             "update_sweep_frac": round(sweep_bytes / (upd["median_ms_per_step"] * 1e-3) / 1e9 / hbm_peak, 4),
             "sweep_bytes": sweep_bytes}
@@ -348,8 +399,9 @@ def run_ours(args):
     other = "f64" if primary == "f32" else "f32"
     arms = {}
     for name in (primary, other):
-        arms[name] = time_arm(q, torch, name, args.steps, args.warmup, args.therm, replica_seed(rank), dist, sampler, args.bulk_copy, not args.same_order, args.full_exchange)
+        arms[name] = time_arm(q, torch, name, args.steps, args.warmup, args.therm, replica_seed(rank), dist, sampler, args.bulk_copy, not args.same_order)
     on_model = time_on_model(q, torch, dist, sampler, with_oracle=(world == 1 and rank == 0 and not args.no_cpu_baseline))
+    split = time_split(q, torch, args.steps, args.therm, replica_seed(rank)) if args.split and world == 1 else None
     clocks = sampler.stop()
     line = None
     if rank == 0:
@@ -357,19 +409,25 @@ def run_ours(args):
         for name in (primary, other):
             value, ms_step, roof, work, upd = summarise(arms[name], name, args.steps, world, hbm_peak, fma[name])
             a = arms[name]
-            e2e, acc, sep = rep_stats(a["e2e"], args.steps), rep_stats(a["accum"], args.steps), rep_stats(a["separate"], args.steps)
+            acc, sep = rep_stats(a["accum"], args.steps), rep_stats(a["separate"], args.steps)
+
+            def e2e_block(key):
+                st = rep_stats(a[key]["times"], args.steps)
+                return {"value": aggregate_value(world, a["links"], 1, st["median_ms_per_step"]), "unit": UNIT,
+                        "h2d_bytes_per_step": a[key]["h2d"], "d2h_bytes_per_step": a[key]["d2h"],
+                        "ms_per_step": st["median_ms_per_step"], "reps": st, "exchange_layout": a[key]["exchange"]}
             frag[name] = {"value": value, "ms_per_step": ms_step, "reps": work, "roofline": roof,
                           "update_only_sweep": {"ms_per_step": upd["median_ms_per_step"], "reps": upd,
                                                 "value": aggregate_value(world, a["links"], 1, upd["median_ms_per_step"])},
-                          "e2e": {"value": aggregate_value(world, a["links"], 1, e2e["median_ms_per_step"]), "unit": UNIT,
-                                  "h2d_bytes_per_step": a["h2d"], "d2h_bytes_per_step": a["d2h"],
-                                  "ms_per_step": e2e["median_ms_per_step"], "reps": e2e, "exchange_layout": a["exchange"]},
+                          "e2e": e2e_block("e2e"),
                           "accumulate_on_device": {"ms_per_step": acc["median_ms_per_step"], "reps": acc,
                                                    "value": aggregate_value(world, a["links"], 1, acc["median_ms_per_step"]),
                                                    "plaquette_mean": a["acc_plaquette_mean"]},
                           "qcd_sweep_then_qcd_measure": {"ms_per_step": sep["median_ms_per_step"], "reps": sep},
                           "gpu_launches": a["launches_per_rep"], "plaquette": a["plaquette"], "polyakov_abs": a["polyakov_abs"],
                           "dtype": name, "storage": "12 reals/link" if name == "f32" else "18 reals/link"}
+            if "e2e_rows01" in a:
+                frag[name]["e2e_rows01"] = e2e_block("e2e_rows01")
         p = frag[primary]
         p["roofline"]["peak_source"] = peak_src
         p["roofline"]["copy_probe_gbs_same_run"] = round(copy_gbs, 1)
@@ -386,6 +444,10 @@ def run_ours(args):
                 "qcd_sweep_then_qcd_measure": p["qcd_sweep_then_qcd_measure"],
                 "observables": {"plaquette": p["plaquette"], "polyakov_abs": p["polyakov_abs"]},
                 "other_precision": frag[other], "on_model": on_model}
+        if "e2e_rows01" in p:
+            line["e2e_rows01"] = p["e2e_rows01"]
+        if split is not None:
+            line["split"] = split
         if args.same_order:
             line["config"]["launch_order"] = "QCD_OPT_ALTERNATE_ORDER = 0"
         if args.bulk_copy:
@@ -393,6 +455,11 @@ def run_ours(args):
             line["roofline"]["kernel"] = "su3_update_bulk_kernel<float, x12, OR> (and the tiled kernel in the fused last pass)"
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline_sample()
+            # vs_baseline stays null: BASELINE.md holds the paper's times for ANOTHER sweep (heatbath only, NHIT = 10) on other
+            # hardware.  The ratio to the oracle timed above is reported for what it is (a slow, untuned checker)
+            cb = line["cpu_baseline"]["value"]
+            line["vs_cpu_baseline"] = {"value": line["value"] / cb, "e2e": line["e2e"]["value"] / cb,
+                                       "note": "ratio to the CPU oracle on %d host cores; not a target" % line["cpu_baseline"]["cores"]}
     if dist is not None:
         dist.barrier()
         dist.destroy_process_group()
@@ -491,8 +558,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--bulk-copy", action="store_true",
                     help="fp32 arm: overrelaxation by the bulk-copy kernel (QCD_OPT_BULK_COPY; the comparison of DESIGN.md sec 6.10)")
-    ap.add_argument("--full-exchange", action="store_true",
-                    help="e2e of the 12-real arm through the full 3 x 3 canonical layout instead of rows 0,1")
+    ap.add_argument("--split", action="store_true",
+                    help="also time the lattice divided into 1, 2 and 4 parts on this GPU (qcd_split_sweep; DESIGN.md sec 9)")
     ap.add_argument("--same-order", action="store_true",
                     help="every update launch visits the lattice in the same direction (QCD_OPT_ALTERNATE_ORDER = 0; the comparison "
                          "of DESIGN.md sec 6.5)")
