@@ -238,14 +238,14 @@ __device__ __forceinline__ bool kp_accept(float inv, float E, float w, const KpK
 
 // Trials 1 .. max_trials-1 of a subgroup whose trial 0 was rejected (3 % of the lanes at beta = 6, but 60 % of the warps
 // have such a lane).  Inlined into each of the three subgroup hits: one shared out-of-line copy was measured and lost
-// (fp32 HB 79.5 -> 86.5 us, fp64 190 -> 204 us: the call spills the hit's live matrices around it).  Off the hot path,
-// so it derives the round keys from the key itself.
+// (fp32 HB 79.5 -> 86.5 us, fp64 190 -> 204 us: the call spills the hit's live matrices around it).  Round keys from the
+// launch arguments, like trial 0.
 template <typename R>
-static __device__ __forceinline__ bool kp_retry(R inv_alpha, const KpKey& key, int max_trials, R& g0, int& code) {
+static __device__ __forceinline__ bool kp_retry(R inv_alpha, const KpKey& key, const PhiloxKeys& rk, int max_trials, R& g0, int& code) {
   code = 0x80 | max_trials;
   for (int t = 1; t < max_trials; ++t) {
     R E, w;
-    KpRand<R>::run(philox4x32_10(key.lex, key.sweep, key.c2, 1u + (uint32_t)t, key.key0, key.key1), E, w);
+    KpRand<R>::run(philox4x32_10(key.lex, key.sweep, key.c2, 1u + (uint32_t)t, rk), E, w);
     if (kp_accept(inv_alpha, E, w, key, 1u + (uint32_t)t, g0)) { code = t + 1; return true; }
   }
   return false;
@@ -273,7 +273,7 @@ __device__ __forceinline__ bool subgroup_quaternion(const Q4<R>& v, R k2, uint32
     R g0;
     bool acc = kp_accept(inv_alpha, d0.E, d0.w, key, 1u, g0);     // trial 0 from the precomputed random part
     code = 1;
-    if (!acc) acc = kp_retry<R>(inv_alpha, key, a.max_trials, g0, code);
+    if (!acc) acc = kp_retry<R>(inv_alpha, key, a.rk, a.max_trials, g0, code);
     // fp32: no early return: the lanes that needed further trials re-join the warp here, so what follows is executed
     // once per warp and not once per divergent path (it was 1.57 times per subgroup at 3 % rejection).  fp64 keeps the
     // early exit (the straight-line form costs it two spilled registers at its 168-register cap).
