@@ -44,16 +44,20 @@ LINK_SIZES_PER_HIT = 2 * len(DIMS) + 1
 # flops per link-hit EXECUTED by the kernels this file launches: ncu's per-opcode thread-instruction counts
 # (sass__thread_inst_executed_true_per_opcode) of one launch / V/2, weighted FFMA2 4, FMUL2 / FADD2 / FFMA / DFMA 2,
 # FMUL / FADD / DMUL / DADD / MUFU 1  (profiles/r2_flop_count.md; SURVEY 8(d)'s estimates were 4030 / 4270 / 3270 / 3900)
-FLOPS_PER_HIT = {"f32": {"hb": 3944.0, "or": 3719.0}, "f64": {"hb": 3909.0, "or": 3171.0}}
-FLOPS_SOURCE = "profiles/r2_d_final.md (weights: profiles/r2_flop_count.md)"
+FLOPS_PER_HIT = {"f32": {"hb": 3925.0, "or": 3701.0}, "f64": {"hb": 3909.0, "or": 3166.0}}
+FLOPS_SOURCE = "profiles/r3_final.md: ncu capture of the build at commit 7d96bdb (weights: profiles/r2_flop_count.md)"
 
 
 # the dominant kernel of each arm (overrelaxation: 32 of the 40 update launches of a step) and its DRAM traffic per launch,
 # dram__bytes_read.sum + dram__bytes_write.sum of one `ncu --set full` capture of this workload (bytes)
 OR_KERNEL = {"f32": "su3_update_tiled_kernel<float, x12, OR>", "f64": "su3_update_kernel<double, x18, OR>"}
-NCU_TRAFFIC = {"f32": {"or": 220570000, "hb": 225180000}, "f64": {"or": 658960000, "hb": 665390000},
-               "source": "profiles/r2_d_final.md (cache flush between ncu replays; 142 + 24 / 534 + 77 MB read + write with the caches "
-                         "left alone, profiles/r2_c_launch_order.md)"}
+NCU_TRAFFIC = {"f32": {"or": 222690000, "hb": 223640000}, "f64": {"or": 658940000, "hb": 666810000},
+               "source": "profiles/r3_final.md: ncu --set full of the build at commit 7d96bdb (cache flush between ncu replays; "
+                         "142 + 24 / 534 + 77 MB read + write with the caches left alone, profiles/r2_c_launch_order.md)"}
+# O(N) kernel (instruction-bound): warp-instructions of one half-sweep launch of O(4) 32^4 NHIT = 100, smsp__inst_executed.sum
+# of the same capture
+ON_WARP_INST = {"f32": 194.76e6, "f64": 257.38e6, "source": "profiles/r3_final.md (ncu --set full, commit 7d96bdb)"}
+N_SM, SCHEDULERS_PER_SM = 148, 4          # B200: one warp-instruction per scheduler and cycle is the issue limit
 
 
 def load_peaks():
@@ -401,8 +405,24 @@ def run_ours(args):
     for name in (primary, other):
         arms[name] = time_arm(q, torch, name, args.steps, args.warmup, args.therm, replica_seed(rank), dist, sampler, args.bulk_copy, not args.same_order)
     on_model = time_on_model(q, torch, dist, sampler, with_oracle=(world == 1 and rank == 0 and not args.no_cpu_baseline))
+    sm_mhz = None
     split = time_split(q, torch, args.steps, args.therm, replica_seed(rank)) if args.split and world == 1 else None
     clocks = sampler.stop()
+    # O(N) kernel against its issue limit: bound "alu", peak = 148 SMs x 4 schedulers x 1 warp-instruction per cycle at the
+    # median SM clock sampled under load in this run (the maximum clock if nvidia-smi gave none); achieved counts the two
+    # update launches of a sweep over the WHOLE step time (measurement kernels and the host read inside)
+    sm_mhz = clocks.get("sm_mhz") or clocks.get("sm_max_mhz") or 1965.0
+    for name in ("f32", "f64"):
+        if name in on_model:
+            peak = N_SM * SCHEDULERS_PER_SM * sm_mhz * 1e6 / 1e9
+            ach = 2 * ON_WARP_INST[name] / (on_model[name]["ms_per_sweep"] * 1e-3) / 1e9
+            on_model[name]["roofline"] = {"bound": "alu", "kernel": "on_update_kernel<%s, 4, 4>" % ("float" if name == "f32" else "double"),
+                                          "achieved": round(ach, 1), "peak": round(peak, 1), "unit": "G warp-instructions/s",
+                                          "frac": round(ach / peak, 4), "traffic": None,
+                                          "warp_inst_per_launch": ON_WARP_INST[name],
+                                          "thread_inst_per_try": round(ON_WARP_INST[name] * 32 / (16 ** 4 * 8 * 100), 1),
+                                          "peak_derivation": "148 SMs x 4 schedulers x %.0f MHz (median SM clock under load, this run)" % sm_mhz,
+                                          "source": ON_WARP_INST["source"]}
     line = None
     if rank == 0:
         frag = {}
