@@ -171,12 +171,13 @@ class StreamedLattice:
     """A divided lattice whose parts live in pinned HOST memory and pass through ONE device buffer, part by part, in every
     sub-step: the paper's other use of the division -- "when one device's memory is not enough".  Host-side
     bookkeeping only; every step runs in the kernels of the slab handles (qcd_slab_*), all created over the same device
-    buffer.  Per sub-step and part: upload the part (its internal layout, halo layers included), unpack the boundary layers
-    its neighbours have produced since its last turn, update, pack its own two boundary layers of the array just written
-    for the neighbours, download.  The messages stay on the device (two layers per array and part).
-    Each sub-step moves the whole lattice over the host link twice, so this is two orders of magnitude slower than a
-    resident lattice: it exists for lattices beyond the 180 GB of one B200, and is tested on small ones,
-    where it must reproduce the undivided sweep bit for bit."""
+    buffer.  Per sub-step and part: upload the part (its internal layout), unpack the latest boundary layers of its
+    neighbours (the messages stay on the device: two layers per array and part, each kept until the next one replaces it),
+    update, pack its own two boundary layers of the array just written for the neighbours, and download ONLY that
+    (parity, mu) array -- the one the sub-step wrote, 1 / (2 D) of the part.  Each sub-step moves 1 + 1 / (2 D) times the
+    lattice over the host link, so this is two orders of magnitude slower than a resident lattice: it
+    exists for lattices beyond the 180 GB of one B200, and is tested on small ones, where it must reproduce the undivided
+    sweep bit for bit."""
 
     def __init__(self, q, dims, Nc, precision, flags=0, n_parts=2, extents=None, device="cuda:0"):
         import torch
@@ -200,7 +201,7 @@ class StreamedLattice:
         self.lat = [q.Lattice(self.dims, Nc, precision, flags, device=device, slab=pe, mem=self.buf) for pe in self.parts]
         self.host = [torch.empty(L.nbytes, dtype=torch.uint8, pin_memory=True) for L in self.lat]
         self.hbytes = [L.qcd_slab_halo_bytes() for L in self.lat]
-        self.pending = [dict() for _ in range(self.n)]       # per part: {(parity, mu, unpack side): message tensor}
+        self.pending = [dict() for _ in range(self.n)]       # per part: {(parity, mu, unpack side): latest message tensor}
         self.resident = None
         self.sweep_counter = 0
         self.bytes_moved = 0
@@ -217,7 +218,8 @@ class StreamedLattice:
 
     # ---- residency
     def _upload(self, k):
-        """part k into the device buffer, then the boundary layers that arrived since it was last there"""
+        """part k into the device buffer, then the latest boundary layers of its neighbours for every array (the halo layers
+        of the host copy are not kept up to date: only the array a sub-step wrote travels back)"""
         L = self.lat[k]
         self.buf[:L.nbytes].copy_(self.host[k], non_blocking=True)
         self.bytes_moved += L.nbytes
@@ -225,15 +227,18 @@ class StreamedLattice:
         for (parity, mu, side), msg in self.pending[k].items():
             L.qcd_slab_halo_unpack(parity, mu, side, msg.data_ptr(), self.hbytes[k])
         # (an unpack tells the handle that its arrays were written behind its back: no early loads in the next kernel)
-        if not self.pending[k]:
-            raise RuntimeError("a part must have received its halo layers before its first turn (call refresh_all)")
-        self.pending[k] = {}
+        if len(self.pending[k]) != 4 * self.D:
+            raise RuntimeError("a part must have received all its halo layers before its first turn (call refresh_all)")
 
-    def _download(self, k):
+    def _download(self, k, array=None):
+        """the resident part k back to its host copy: all of it, or only the (parity, mu) array number `array` =
+        parity * D + mu (the internal layout is 2 D equal arrays, one per parity and direction, back to back)"""
         L = self.lat[k]
-        self.host[k].copy_(self.buf[:L.nbytes], non_blocking=True)
+        a = L.nbytes // (2 * self.D)
+        lo, hi = (0, L.nbytes) if array is None else (array * a, (array + 1) * a)
+        self.host[k][lo:hi].copy_(self.buf[lo:hi], non_blocking=True)
         self.torch.cuda.current_stream().synchronize()      # the buffer is reused by the next part
-        self.bytes_moved += L.nbytes
+        self.bytes_moved += hi - lo
 
     def _post(self, k, parity, mu):
         """the two boundary layers of array (parity, mu) of the resident part k, as messages to its neighbours"""
@@ -299,7 +304,7 @@ class StreamedLattice:
             self._upload(k)
             self.lat[k].qcd_debug_substep(beta, kind, hit, parity, mu, field)
             self._post(k, parity, mu)
-            self._download(k)
+            self._download(k, parity * self.D + mu)
 
     def sweep(self, beta, n_hb, n_or, field=None):
         for kind, hit, parity, mu in sweep_schedule(self.D, n_hb, n_or):
