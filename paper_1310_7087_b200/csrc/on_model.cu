@@ -77,7 +77,11 @@ __device__ __forceinline__ uint32_t on_c2(int parity, int hit, int domain) {
 }
 // u = (k + 1/2) 2^-23, exact in both precisions; float: without an integer conversion (philox.cuh, uniform23f)
 __device__ __forceinline__ float on_uniform(uint32_t k, float) { return __uint_as_float(0x3F800000u | k) - 0.99999994f; }
-__device__ __forceinline__ double on_uniform(uint32_t k, double) { return ((double)k + 0.5) * 1.1920928955078125e-07; }
+// double: k < 2^23 placed in the low mantissa bits of 2^52 is the double 2^52 + k, and 2^52 - 1/2 is a double too, so one
+// exact subtraction gives k + 1/2 without an integer conversion (five I2F.F64 per try otherwise)
+__device__ __forceinline__ double on_uniform(uint32_t k, double) {
+  return (__hiloint2double(0x43300000, (int)k) - 4503599627370495.5) * 1.1920928955078125e-07;
+}
 
 template <int N> __device__ __forceinline__ double on_local_action(const double* p, const double* h, double kappa, double lambda) {
   double ph = 0.0, pp = 0.0;
