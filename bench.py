@@ -56,7 +56,7 @@ NCU_TRAFFIC = {"f32": {"or": 222690000, "hb": 223640000}, "f64": {"or": 65894000
                          "142 + 24 / 534 + 77 MB read + write with the caches left alone, profiles/r2_c_launch_order.md)"}
 # O(N) kernel (instruction-bound): warp-instructions of one half-sweep launch of O(4) 32^4 NHIT = 100, smsp__inst_executed.sum
 # of the same capture
-ON_WARP_INST = {"f32": 194.76e6, "f64": 257.38e6, "source": "profiles/r3_final.md (ncu --set full, commit 7d96bdb)"}
+ON_WARP_INST = {"f32": 194.76e6, "f64": 237.22e6, "source": "profiles/r3_final.md (ncu --set full; fp32 at commit 7d96bdb, fp64 at 3bb586f)"}
 N_SM, SCHEDULERS_PER_SM = 148, 4          # B200: one warp-instruction per scheduler and cycle is the issue limit
 
 
